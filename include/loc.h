@@ -1,0 +1,173 @@
+/*
+ * loc.h -- C-ABI boundary of the B200-native LOC hot path (arxiv 2009.12609, M. Juvela).
+ *
+ * The library runs the ray-tracing simulation step of accelerated lambda iteration (ALI) and the
+ * per-cell statistical-equilibrium solve on one GPU (hand-written CUDA for sm_100a).  Citations are
+ * PAPER.md:<line> of /root/reference/PAPER.md; "DESIGN Rn" are the readings listed in DESIGN.md.
+ *
+ * Conventions
+ *   - Units are CGS everywhere (cm, cm/s, K, cm^-3, 1/s).
+ *   - Every call returns an int status: LOC_OK or a negative LOC_E* code.  No exceptions, no exit().
+ *     loc_last_error() returns a static/owned message for the last failing call on that model.
+ *   - "host" pointers are ordinary CPU memory, read during the call only (the library copies what it
+ *     needs).  "device" pointers are CUDA global memory of the current device, OWNED BY THE CALLER and
+ *     kept alive by the caller until loc_destroy_model().
+ *   - The library performs NO hidden device allocation: all device scratch lives in the caller's
+ *     workspace (loc_workspace_bytes / loc_create_model).  Too small a workspace -> LOC_ENOMEM.
+ *   - All device work is enqueued on the stream given to loc_create_model and is asynchronous; only calls
+ *     that return a host scalar (loc_solve, loc_iterate, loc_get_stats) synchronise that stream.
+ *   - Channel c of NCH has velocity v_c = (c - (NCH-1)/2) dv, dv = 2 band_halfwidth / NCH (DESIGN O4).
+ *   - Doppler shift of a cell with velocity v seen along the photon direction d is v0 = -(v . d)
+ *     (radio convention, DESIGN R6); in 1D v0 = -v_r mu with mu evaluated where the ray ENTERS the step
+ *     ("the Doppler shifts are evaluated only at the beginning of each step").
+ */
+#ifndef LOC_H
+#define LOC_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LOC_OK 0
+#define LOC_EINVAL (-1) /* bad argument (non-monotone radii, nchannel<1, child index out of range, ...) */
+#define LOC_ESTATE (-2) /* call order (species / directions / populations not set)                      */
+#define LOC_ENOMEM (-3) /* workspace too small                                                          */
+#define LOC_ECUDA (-4)  /* CUDA error; text in loc_last_error()                                        */
+
+#define LOC_GRID_SHELL 1  /* 1D spherically symmetric shells   */
+#define LOC_GRID_OCTREE 2 /* 3D octree; a Cartesian grid is nlevel = 1 */
+
+#define LOC_MAX_TRANS 12  /* radiative transitions ray traced together in one pass */
+#define LOC_MAX_LEVELS 32 /* energy levels of the species                           */
+#define LOC_MAX_TREE_LEVELS 6
+
+typedef struct loc_model loc_model; /* opaque */
+
+/* Geometry (PAPER.md:87 for shells, PAPER.md:93-97 for the octree; storage format DESIGN R17). */
+typedef struct {
+    int kind; /* LOC_GRID_SHELL or LOC_GRID_OCTREE */
+    /* --- shell grid: shell k spans [r_out[k-1], r_out[k]), r_out[-1] = 0; values refer to the shell */
+    int nshell;
+    const double *r_out; /* host [nshell], strictly ascending, cm                                         */
+    int nray;
+    const double *ray_p; /* host [nray] impact parameters, 0 <= p < r_out[nshell-1]                       */
+    const double *ray_w; /* host [nray] ray weights = annulus areas pi (p_hi^2 - p_lo^2), cm^2 (Eq. 1)   */
+    /* --- octree grid: level-major cell arrays; level l holds level_offset[l+1]-level_offset[l] cells.
+     *     Root level in x-fastest raster order (ix + nx (iy + ny iz)); the 8 children of a refined cell are
+     *     contiguous in the next level in (x fastest, y, z) order.                                          */
+    int nx, ny, nz;              /* root grid dimensions                                                  */
+    double root_cell_cm;         /* edge of a root cell                                                   */
+    int nlevel;                  /* number of hierarchy levels >= 1 (<= LOC_MAX_TREE_LEVELS)              */
+    const int64_t *level_offset; /* host [nlevel+1]; level_offset[nlevel] = total number of cells         */
+    const int32_t *child;        /* DEVICE [ncell]: index WITHIN the next level of the first child, or -1 for a leaf */
+} loc_grid;
+
+/* Per-cell physical state, DEVICE float arrays over all cells (octree: leaves and refined
+ * cells alike, in the level-major order of loc_grid; values of refined cells are ignored). */
+typedef struct {
+    const float *density;   /* number density of the collision partner, cm^-3                             */
+    const float *tkin;      /* kinetic temperature, K                                                     */
+    const float *sigma;     /* turbulent 1-D velocity dispersion (std dev), cm/s; thermal part added by the
+                               library as k T / m unless species mass is 0 (DESIGN R3)                     */
+    const float *vx;        /* velocity, cm/s; shells: radial velocity (positive outward)                 */
+    const float *vy;        /* octree only                                                                */
+    const float *vz;        /* octree only                                                                */
+    const float *abundance; /* fractional abundance of the species relative to `density`                  */
+} loc_cells;
+
+typedef struct {
+    int64_t ncell;           /* cells in the model (all levels)                                           */
+    int64_t steps;           /* ray-cell steps of the last loc_simulate (one count per ray segment in a cell) */
+    int ntrans_sim;          /* transitions traced in the last loc_simulate                               */
+    int nchannel;
+    int64_t kernel_launches; /* CUDA kernels launched by the library on this model so far                  */
+    int counter_stride;      /* floats per cell in the counter / coefficient records = 2 * ntrans_padded  */
+    int64_t setup_steps;     /* octree: ray-cell steps in the precomputed step stream (all directions)      */
+    double setup_ms;         /* octree: device time of the last path set-up (loc_set_directions), ms        */
+} loc_stats;
+
+/* Bytes of device workspace loc_create_model needs for this grid and these limits.
+ * ndir_max: largest number of directions that will be set (octree; ignored for shells). */
+int64_t loc_workspace_bytes(const loc_grid *grid, int nchannel, int nlevel_species, int ntrans, int ndir_max);
+
+/* Build a model: validates the grid, precomputes the set-up tables (1D: per-ray path lengths, entry
+ * cosines, sampled shell volumes V_eff = sum_i W_i s_ik, DESIGN R12; 3D: neighbour-refinement flags) in the
+ * workspace.  `stream` is a cudaStream_t passed as void* (NULL = default stream).
+ * nchannel >= 1; band_halfwidth_cm_s > 0; t_background_K >= 0 (Planck background, Eq. 1).
+ * nlevel_species, ntrans, ndir_max: the same limits that were given to loc_workspace_bytes; later calls to
+ * loc_set_species / loc_set_directions must stay within them.                                          */
+int loc_create_model(const loc_grid *grid, const loc_cells *cells, int nchannel, double band_halfwidth_cm_s,
+                     double t_background_K, int nlevel_species, int ntrans, int ndir_max, void *workspace /* device */,
+                     int64_t workspace_bytes, void *stream, loc_model **out);
+
+/* Species: host arrays, copied.  Line frequencies follow from the level energies.  Upward
+ * collision rates by detailed balance; rate_down is [ntemp][ncoll], linear interpolation in T, clamped;
+ * ntemp = 1 -> constant.  mass_amu = 0 -> `sigma` is the total line width.  ntrans <= LOC_MAX_TRANS.     */
+int loc_set_species(loc_model *m, int nlevel, const double *energy_K, const double *g, int ntrans, const int *upper,
+                    const int *lower, const double *einstein_A, double mass_amu, int ncoll, const int *cu, const int *cl,
+                    int ntemp, const double *temps_K, const double *rate_down);
+
+/* Octree only: ray directions (unit vectors, host [ndir][3]; PAPER.md:93 uses HEALPix centres).  Each is
+ * snapped to the library's fixed-point slopes (DESIGN R7); ndir <= the ndir_max given to loc_workspace_bytes.
+ * This call also runs the path set-up: every root-grid ray and the rays born from it in refined regions
+ * are traced once with integer arithmetic and stored in the workspace as a step stream
+ * (cell index, path length) that loc_simulate replays every iteration -- the 3D counterpart of the pre-calculated
+ * per-shell path lengths of PAPER.md:87.  Synchronises the stream.  LOC_ENOMEM if the stream does not fit.      */
+int loc_set_directions(loc_model *m, int ndir, const double *dir_xyz);
+
+/* Register the caller-owned DEVICE population buffer, float [nlevel][ncell] (cm^-3), and derive the per-cell
+ * line coefficients from its current content.  Call again after writing into the buffer from outside.    */
+int loc_set_populations(loc_model *m, float *dev_pops);
+
+/* Fill the registered buffer with LTE populations at T_kin and derive the coefficients.   */
+int loc_init_lte(loc_model *m);
+
+/* Zero the counters and trace all rays (1D: all impact parameters; 3D: all directions, root rays and the
+ * rays born in refined regions) for the selected transitions (nsel = 0 -> all), evaluating
+ * per cell step and channel the Doppler-shifted Gaussian profile, the optical depth, the photon
+ * transfer of Eq. 3 and the sums of Eq. 2 (first term; the self term is handled by ALI).
+ * The selection is remembered for loc_solve / loc_iterate.  geometry_counters != 0 additionally records
+ * per-cell visit counts and integer main-axis path sums (tests).                                           */
+int loc_simulate(loc_model *m, int nsel, const int *trans_idx, int geometry_counters);
+
+/* Borrowed DEVICE pointers, valid until the next loc_simulate:
+ *   counters: float [ncell][ntrans_padded][2]; slot k of a cell belongs to the k-th selected transition:
+ *       [k][0] = SJ  = sum over ray steps of (a s / V_eff) sum_c phi_c n_c (1-e^-tau_c)/tau_c, n_c the photon
+ *                occupation number I_c c^2 / (2 h nu^3) entering the step: the profile- and path-weighted mean
+ *                radiation field.  Absorbed-photon count of Eq. 2:  ABS = k_t V_eff (4 pi dv / h c)(2 h nu^3/c^2) SJ.
+ *       [k][1] = ESC = sum over steps of (a s / V_eff) [ (1 - sum_c phi_c) + sum_c phi_c (1-e^-tau_c)/tau_c ]
+ *                = escape probability of the cell's own photons = 1 - LAMBDA* (PAPER.md:81).
+ *   visits:   uint32 [ncell] ray segments per cell        (only if geometry_counters)
+ *   pathz:    uint32 [ncell] summed main-axis path in grid units, 2^20 per root cell (octree, geometry_counters)
+ * Photon counts themselves (~1e38 per second for parsec-size cells) do not fit float32; see DESIGN.md 5.2. */
+int loc_get_counters(loc_model *m, const float **counters, int *ntrans_padded, const uint32_t **visits,
+                     const uint32_t **pathz);
+
+/* Per-cell statistical equilibrium: S_lu = (g_u/g_l) A SJ replaces B_lu I, A_ul is scaled by
+ * ESC, collisions from `density` and `tkin`; transitions that were not traced see the background only
+ * (DESIGN R23).  Writes the new populations into the registered buffer and refreshes the line coefficients.
+ * max_rel_change (host, may be NULL): largest relative change over levels holding >= 1e-10 of the molecules. */
+int loc_solve(loc_model *m, double *max_rel_change);
+
+/* niter x (loc_simulate with the remembered selection; loc_solve); no early exit.          */
+int loc_iterate(loc_model *m, int niter, double *max_rel_change);
+
+/* Spectral map: for each pixel one line of sight through the model with the current
+ * populations, T_A(c) = (c^2 / 2 k nu^2)(I_c - B_nu(T_bg)), written to dev_out float [ny][nx][nchannel] (K).
+ * Octree: lines of sight run along `dir` (host double[3]); pixel (ix,iy) starts on the upstream face at the
+ * integer grid position  (aff[0] + ix aff[2] + iy aff[3],  aff[1] + ix aff[4] + iy aff[5])  of the two transverse
+ * axes (units: 2^20 per root cell, in the ray's working frame, DESIGN 6.4).
+ * Shells: dir = NULL, ny = 1, pixel ix is the line of sight with impact parameter offsets_cm[ix] (host).   */
+int loc_spectra(loc_model *m, int trans, const double *dir, int nx, int ny, const int64_t *aff,
+                const double *offsets_cm, float *dev_out);
+
+int loc_get_stats(loc_model *m, loc_stats *out);
+void loc_destroy_model(loc_model *m);
+const char *loc_last_error(const loc_model *m); /* m may be NULL: error of the last failed loc_create_model */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LOC_H */

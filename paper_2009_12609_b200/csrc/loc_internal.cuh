@@ -1,0 +1,264 @@
+// loc_internal.cuh -- shared declarations of the CUDA implementation behind include/loc.h.
+// Hand-written for sm_100a.  Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/loc.h"
+
+#define LOC_LB 20              // log2(grid units per root cell)
+#define LOC_H0 (1 << LOC_LB)   // grid units per root cell
+#define LOC_MAXL LOC_MAX_TREE_LEVELS
+#define LOC_BUILD_BATCH 65536  // root lines traced per launch of the path builder
+#define LOC_BUILD_STACK 256    // pending rays per root line (PAPER.md:119 estimates ~7*3^(NL-1) stored rays)
+
+// physical constants (CGS, CODATA 2018) -- DESIGN R1
+#define LOC_HP 6.62607015e-27
+#define LOC_KB 1.380649e-16
+#define LOC_CL 2.99792458e10
+#define LOC_AMU 1.66053906660e-24
+#define LOC_PI 3.14159265358979323846
+
+#define LOC_LOG2E 1.4426950408889634f
+#define LOC_THICK_TAU 0.05f   // line-centre optical depth of a step above which exp() is used instead of the series
+
+// ------------------------------------------------------------------------------------------------
+// device-side species description (arrays live in the workspace)
+// ------------------------------------------------------------------------------------------------
+struct SpeciesDev {
+    int nlevel, ntrans, ncoll, ntemp;
+    const double *energy_K;  // [nlevel]
+    const double *g;         // [nlevel]
+    const int *upper, *lower;  // [ntrans]
+    const double *A;         // [ntrans]
+    const double *freq;      // [ntrans]
+    const double *bgocc;     // [ntrans] 1/(exp(h nu/k Tbg)-1)
+    const int *cu, *cl;      // [ncoll]
+    const double *temps;     // [ntemp]
+    const double *rates;     // [ntemp][ncoll]
+    double mass_amu;
+};
+
+// selection of traced transitions: slot k of the per-cell records belongs to transition sel[k]
+struct Selection {
+    int nsel, nsp;               // nsp = record stride in float2 (nsel padded to even)
+    int sel[LOC_MAX_TRANS];
+    int upper[LOC_MAX_TRANS], lower[LOC_MAX_TRANS];
+    float gratio[LOC_MAX_TRANS]; // g_u/g_l
+    float bgocc[LOC_MAX_TRANS];  // background occupation number at the line frequency (Eq. 1 in occupation units)
+    double ck[LOC_MAX_TRANS];    // c^3 A / (8 pi nu^3 dv)
+};
+
+// per-direction data of the integer ray lattice (DESIGN 6.3).  Working frame: axis 0 = main axis (zeta), 1 = p, 2 = q;
+// axes with a negative direction component are mirrored so that every ray moves towards +zeta, +p, +q.
+struct Dir3 {
+    int ax[3];              // model axis (0=x,1=y,2=z) of the working axes
+    int flip[3];            // per working axis: mirrored?
+    unsigned long long T[2];  // fixed-point inverse slopes of p, q: shift(zeta) = floor(zeta 2^32 / T); 0 = zero slope
+    int W[3];               // model extent along the working axes in grid units (2^20 per root cell)
+    int np, nq;             // root lines along p, q
+    float d[3];             // snapped unit propagation direction, model frame
+    float sf;               // cm of path per grid unit of zeta = (root_cm / 2^20) / |d_m|
+    long long task0;        // index of the direction's first root-line task
+};
+
+// one record of the precomputed step stream (8 bytes):  x = cell index (STEP) or slot (SAVE/LOAD)
+//   y = dzeta [0..20] | level [21..23] | opcode [24..26]
+#define LOC_OP_STEP 0u
+#define LOC_OP_BG 1u    // spectrum := background (model boundary / transverse wrap-around)
+#define LOC_OP_SAVE 2u  // slot[x] := spectrum   (donor duty at the upstream face of a refined cell)
+#define LOC_OP_LOAD 3u  // spectrum := slot[x]   (birth of a ray in a refined region / resume of the donor)
+#define LOC_REC(op, level, dz) (((unsigned)(op) << 24) | ((unsigned)(level) << 21) | (unsigned)(dz))
+
+struct loc_model {
+    int kind;
+    cudaStream_t stream;
+    char err[512];
+    int nch;
+    double band_half, dv, tbg;
+    int64_t ncell;
+    loc_cells cells;
+    // workspace carve-up
+    char *ws;
+    int64_t ws_bytes, ws_used;
+    float4 *kin;     // [ncell] vx,vy,vz,sigma_tot
+    float2 *coef;    // [ncell][nsp]  (kap, em)
+    float2 *cnt;     // [ncell][nsp]  (SJ, ESC)
+    uint32_t *visits, *pathz;
+    unsigned long long *d_steps;  // [1]
+    unsigned int *d_maxrel;       // [1] float bits
+    int *d_errflag;               // [1]
+    int max_trans, max_levels;    // limits given to loc_create_model
+    // species
+    bool have_species;
+    int nlevel, ntrans, ncoll, ntemp;
+    SpeciesDev sp;
+    double h_energy[LOC_MAX_LEVELS], h_g[LOC_MAX_LEVELS];
+    int *h_upper, *h_lower;
+    double *h_A, *h_freq;
+    Selection selh;
+    bool coef_valid;
+    float *pops;  // registered [nlevel][ncell]
+    // accuracy knobs (DESIGN 5.3)
+    float xmin, eps_tau;
+    // 1D
+    int nshell, nray;
+    int *d_order, *d_k0;
+    long long *d_off;
+    float *d_tabs, *d_tabmu, *d_rayw, *d_invv;
+    double *h_rout;
+    int64_t steps1d;
+    // 3D
+    int nx, ny, nz, nlev;
+    double root_cm;
+    int64_t noff[LOC_MAXL + 1];
+    const int32_t *child;
+    int ndir, ndir_max;
+    Dir3 *d_dirs;  // [ndir_max]
+    Dir3 *h_dirs;
+    unsigned int *d_queue;      // [1] task queue head
+    int64_t ntask, ntask_max;
+    long long *d_task_off;      // [ntask_max+1] record offsets of the root-line tasks
+    unsigned char *d_task_dir;  // [ntask_max]
+    uint2 *d_stream;            // precomputed step stream (S0/S2 set-up)
+    int64_t stream_cap, stream_len;
+    char *d_bstack;             // builder stacks
+    int bstack_threads;
+    int max_warps;
+    float *spec_pool;           // per resident warp: (nlev-1) spectrum slots of [nsel][nch]
+    int64_t spec_pool_floats;
+    int64_t setup_steps;
+    double setup_ms;
+    // stats
+    int64_t launches;
+    int64_t last_steps;
+};
+
+// ------------------------------------------------------------------------------------------------
+// device helpers
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ float ex2f(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// Per-transition parameters of one ray step, computed once per (step, transition)
+struct __align__(16) TParam {
+    float c0;     // thick: -kap*s*log2(e)      thin: kap*s
+    float c1;     // thick: em/kap (source)     thin: em*s
+    float scale;  // thick: w/(kap*s)           thin: w       multiplies the channel sums
+    int thick;
+};
+
+__device__ __forceinline__ TParam make_tparam(float2 ke, float s, float w, float amp)
+{
+    TParam p;
+    float ks = ke.x * s;
+    bool thick = fabsf(ks) * amp >= LOC_THICK_TAU;
+    if (thick) {
+        float inv = __fdividef(1.0f, ke.x);
+        p.c0 = -ks * LOC_LOG2E;
+        p.c1 = ke.y * inv;
+        p.scale = __fdividef(w, ks);
+    } else {
+        p.c0 = ks;
+        p.c1 = ke.y * s;
+        p.scale = w;
+    }
+    p.thick = thick;
+    return p;
+}
+
+// One channel, one transition (Eq. 3 and the two sums of Eq. 2 / PAPER.md:81 in occupation-number units).
+//   n      photon occupation number in the channel, updated
+//   phi    fraction of the profile in the channel (0 for inactive lanes)
+//   accA  += n_in * phi * f(tau)        (thick: n_in (1-e^-tau), rescaled by 1/(kap s) afterwards)
+//   accB  += phi * f(tau)               (thick: (1-e^-tau))
+__device__ __forceinline__ void channel_update(float &n, float phi, const TParam &p, float &accA, float &accB)
+{
+    if (p.thick) {
+        float e = ex2f(phi * p.c0);
+        float om = 1.0f - e;
+        accA = fmaf(n, om, accA);
+        accB += om;
+        n = fmaf(om, p.c1 - n, n);
+    } else {
+        float tau = phi * p.c0;
+        float P = fmaf(tau, fmaf(tau, fmaf(tau, -1.0f / 24.0f, 1.0f / 6.0f), -0.5f), 1.0f);  // (1-e^-tau)/tau
+        float q = phi * P;
+        float om = tau * P;
+        accA = fmaf(n, q, accA);
+        accB += q;
+        n = fmaf(p.c1, q, fmaf(-n, om, n));
+    }
+}
+
+// Reduce NV per-lane values across the warp with a halving butterfly (about NV shuffles in total instead of
+// 5 NV).  On return v[0] of lane L holds the warp total of value index *owner (or *owner = -1).
+template <int N, int OFF>
+struct MultiReduce {
+    __device__ static __forceinline__ void run(float *v, int lane, int &base, int &nvalid)
+    {
+        constexpr int C = (N + 1) / 2;  // kept by the lower half
+        constexpr int Hh = N - C;       // kept by the upper half
+        const bool up = lane & OFF;
+#pragma unroll
+        for (int i = 0; i < C; i++) {
+            if (i < Hh) {
+                float keep = up ? v[i + C] : v[i];
+                float send = up ? v[i] : v[i + C];
+                v[i] = keep + __shfl_xor_sync(0xffffffffu, send, OFF);
+            } else {  // unpaired middle value: lower half keeps it, upper half's copy becomes junk
+                float other = __shfl_xor_sync(0xffffffffu, v[i], OFF);
+                v[i] = up ? 0.0f : v[i] + other;
+            }
+        }
+        if (up) {
+            base += C;
+            nvalid = max(0, nvalid - C);
+        } else {
+            nvalid = min(nvalid, C);
+        }
+        if constexpr (OFF > 1) MultiReduce<C, OFF / 2>::run(v, lane, base, nvalid);
+    }
+};
+template <int OFF>
+struct MultiReduce<1, OFF> {
+    __device__ static __forceinline__ void run(float *v, int lane, int &base, int &nvalid)
+    {
+        // a single value left: plain butterfly over the remaining offsets
+#pragma unroll
+        for (int o = OFF; o >= 1; o >>= 1) v[0] += __shfl_xor_sync(0xffffffffu, v[0], o);
+    }
+};
+
+template <int NV>
+__device__ __forceinline__ float warp_multi_reduce(float (&v)[NV], int lane, int &owner)
+{
+    int base = 0, nvalid = NV;
+    MultiReduce<NV, 16>::run(v, lane, base, nvalid);
+    owner = (nvalid >= 1) ? base : -1;
+    return v[0];
+}
+
+// ------------------------------------------------------------------------------------------------
+// kernels / launchers implemented in the other translation units
+// ------------------------------------------------------------------------------------------------
+int loc_launch_sim1d(loc_model *m, int geom);
+int loc_launch_sim3d(loc_model *m, int geom);
+int loc_setup3d(loc_model *m);
+int loc_launch_spectra(loc_model *m, int trans, const double *dir, int nx, int ny, const int64_t *aff,
+                       const double *offsets_cm, float *dev_out);
+int loc_build_streams(loc_model *m);
+void loc_fill_dir(loc_model *m, const double *din, Dir3 *D);
+
+#define LOC_CUDA_CHECK(m, call)                                                                    \
+    do {                                                                                           \
+        cudaError_t _e = (call);                                                                   \
+        if (_e != cudaSuccess) {                                                                   \
+            snprintf((m)->err, sizeof((m)->err), "%s:%d %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(_e)); \
+            return LOC_ECUDA;                                                                      \
+        }                                                                                          \
+    } while (0)

@@ -1,0 +1,191 @@
+// loc_sim1d.cu -- 1D shell-ray simulation kernel (Eqs. 1-3).
+//
+// One thread block per ray (impact parameter), one thread per velocity channel: each thread owns its channel's
+// photon occupation numbers n[t] for all traced transitions IN REGISTERS for the whole ray (the spherical
+// symmetry makes the ray a fixed sequence of shells: in through NS-1..k0, out through k0+1..NS-1, with
+// precomputed path lengths).  Per step: one profile value per thread, one exp per (thread,
+// transition) -- only in warps that overlap the profile window --, a halving-butterfly warp reduction of the
+// 2 NT + 1 channel sums, a cross-warp reduction through shared memory that is overlapped with the next
+// step, and one float atomic per (cell, transition, counter).  The paper's kernel used one work item per ray
+// and one transition at a time.
+#include <stdio.h>
+
+#include "loc_internal.cuh"
+
+struct Sim1D {
+    int ns, nch, nsp;
+    float dv, xmin, eps_tau;
+    const int *order, *k0;
+    const long long *off;
+    const float *rayw, *invv, *tabs, *tabmu;
+    const float4 *kin;
+    const float2 *coef;
+    float2 *cnt;
+    uint32_t *visits;
+    Selection S;
+};
+
+__device__ __forceinline__ void seg1d(const Sim1D &P, int j, int nin, int k0, long long off, int &k, float &s, float &mu)
+{
+    if (j < nin) {  // inbound through shell NS-1-j
+        k = P.ns - 1 - j;
+        s = __ldg(P.tabs + off + (k - k0));
+        mu = -__ldg(P.tabmu + off + (k - k0));
+    } else if (j == nin) {  // tangent shell, one step (DESIGN R5)
+        k = k0;
+        s = __ldg(P.tabs + off);
+        mu = -__ldg(P.tabmu + off);
+    } else {  // outbound: entry cosine is that of the inner boundary r_{k-1}
+        k = k0 + (j - nin);
+        s = __ldg(P.tabs + off + (k - k0));
+        mu = __ldg(P.tabmu + off + (k - 1 - k0));
+    }
+}
+
+template <int NT, bool GEOM>
+__global__ void __launch_bounds__(1024) k_sim1d(Sim1D P)
+{
+    constexpr int NV = 2 * NT + 1;
+    __shared__ TParam s_tp[2][NT];
+    __shared__ float s_tau0[2];
+    extern __shared__ float s_part[];  // [2][nwarp*NV + 4]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
+    const int pstride = nwarp * NV + 4;
+    const int ray = P.order[blockIdx.x];
+    const int k0 = P.k0[ray];
+    const long long off = P.off[ray];
+    const float Wi = P.rayw[ray];
+    const int nin = P.ns - 1 - k0, nseg = 2 * nin + 1;
+    float n[NT];
+#pragma unroll
+    for (int t = 0; t < NT; t++) n[t] = P.S.bgocc[t];  // Eq. 1: background photons, as occupation number
+    const float cvel = ((float)tid - 0.5f * (float)(P.nch - 1)) * P.dv;
+    const float inv_dv = 1.0f / P.dv;
+
+    for (int j = 0; j <= nseg; j++) {
+        const int buf = j & 1;
+        int k = 0;
+        float s = 0.f, mu = 0.f, w = 0.f, v0 = 0.f, sig = 1.f, amp = 0.f;
+        if (j < nseg) {
+            seg1d(P, j, nin, k0, off, k, s, mu);
+            float4 kin = __ldg(P.kin + k);
+            v0 = -kin.x * mu;  // DESIGN R6, mu at the entry of the step
+            sig = kin.w;
+            w = Wi * s * __ldg(P.invv + k);  // this ray's share a s / V_eff of the shell (DESIGN R12)
+            amp = P.dv * 0.3989422804f / sig;
+            if (warp == 0) {
+                float tau0 = 0.f;
+                if (lane < NT) {
+                    float2 ke = __ldg(P.coef + (long long)k * P.nsp + lane);
+                    s_tp[buf][lane] = make_tparam(ke, s, w, amp);
+                    tau0 = fabsf(ke.x * s) * amp;
+                }
+                unsigned mx = __reduce_max_sync(0xffffffffu, __float_as_uint(tau0));
+                if (lane == 0) s_tau0[buf] = __uint_as_float(mx);
+            }
+        }
+        __syncthreads();
+        // ---- cross-warp reduction of the PREVIOUS step by the last warp (overlaps with this step's work) ----
+        if (j > 0 && warp == nwarp - 1) {
+            const float *pp = s_part + (buf ^ 1) * pstride;
+            int kp;
+            float sp_, mup;
+            seg1d(P, j - 1, nin, k0, off, kp, sp_, mup);
+            const float wprev = pp[nwarp * NV + 0];
+            const int clo = __float_as_int(pp[nwarp * NV + 1]), chi = __float_as_int(pp[nwarp * NV + 2]);
+            float tot = 0.f;
+            if (lane < NV)
+                for (int ww = 0; ww < nwarp; ww++)
+                    if (ww * 32 <= chi && ww * 32 + 31 >= clo) tot += pp[ww * NV + lane];
+            float sphi = __shfl_sync(0xffffffffu, tot, 2 * NT);
+            if (lane < NT)
+                atomicAdd(&P.cnt[(long long)kp * P.nsp + lane].x, tot);
+            else if (lane < 2 * NT)
+                atomicAdd(&P.cnt[(long long)kp * P.nsp + (lane - NT)].y, tot + (wprev - sphi));
+            if (GEOM && lane == 0) atomicAdd(&P.visits[kp], 1u);
+        }
+        if (j == nseg) break;
+        // ---- profile window of this step (DESIGN 5.3) ----
+        const float tau0m = s_tau0[buf];
+        float X = P.xmin;
+        if (tau0m > P.eps_tau) X = fmaxf(X, sqrtf(2.0f * __logf(tau0m / P.eps_tau)));
+        const float cc = v0 * inv_dv + 0.5f * (float)(P.nch - 1);
+        const float hw = X * sig * inv_dv;
+        const int c_lo = max(0, (int)ceilf(cc - hw)), c_hi = min(P.nch - 1, (int)floorf(cc + hw));
+        float *pw = s_part + buf * pstride;
+        if (tid == 0) {
+            pw[nwarp * NV + 0] = w;
+            pw[nwarp * NV + 1] = __int_as_float(c_lo);
+            pw[nwarp * NV + 2] = __int_as_float(c_hi);
+        }
+        if (warp * 32 <= c_hi && warp * 32 + 31 >= c_lo) {
+            const bool act = tid >= c_lo && tid <= c_hi;
+            const float ky = 0.8493218f / sig;  // sqrt(log2(e)/2) / sigma
+            const float y = (cvel - v0) * ky;
+            const float phi = act ? ex2f(fmaf(-y, y, __log2f(amp))) : 0.0f;
+            float v[NV];
+#pragma unroll
+            for (int t = 0; t < NT; t++) {
+                const TParam tp = s_tp[buf][t];
+                float a = 0.f, b = 0.f;
+                channel_update(n[t], phi, tp, a, b);
+                v[t] = a;
+                v[NT + t] = b;
+            }
+            v[2 * NT] = phi;
+            int owner;
+            float tot = warp_multi_reduce<NV>(v, lane, owner);
+            if (owner >= 0) {
+                float sc = (owner == 2 * NT) ? w : s_tp[buf][owner < NT ? owner : owner - NT].scale;
+                pw[warp * NV + owner] = tot * sc;
+            }
+        }
+    }
+}
+
+template <int NT>
+static int launch1d(loc_model *m, const Sim1D &P, int geom)
+{
+    int threads = (m->nch + 31) / 32 * 32;
+    int nwarp = threads / 32;
+    size_t smem = sizeof(float) * 2 * (nwarp * (2 * NT + 1) + 4);
+    if (geom)
+        k_sim1d<NT, true><<<m->nray, threads, smem, m->stream>>>(P);
+    else
+        k_sim1d<NT, false><<<m->nray, threads, smem, m->stream>>>(P);
+    m->launches++;
+    LOC_CUDA_CHECK(m, cudaGetLastError());
+    return LOC_OK;
+}
+
+int loc_launch_sim1d(loc_model *m, int geom)
+{
+    Sim1D P;
+    P.ns = m->nshell;
+    P.nch = m->nch;
+    P.nsp = m->selh.nsp;
+    P.dv = (float)m->dv;
+    P.xmin = m->xmin;
+    P.eps_tau = m->eps_tau;
+    P.order = m->d_order;
+    P.k0 = m->d_k0;
+    P.off = m->d_off;
+    P.rayw = m->d_rayw;
+    P.invv = m->d_invv;
+    P.tabs = m->d_tabs;
+    P.tabmu = m->d_tabmu;
+    P.kin = m->kin;
+    P.coef = m->coef;
+    P.cnt = m->cnt;
+    P.visits = m->visits;
+    P.S = m->selh;
+    switch (m->selh.nsel) {
+#define C1(N) \
+    case N:   \
+        return launch1d<N>(m, P, geom);
+        C1(1) C1(2) C1(3) C1(4) C1(5) C1(6) C1(7) C1(8) C1(9) C1(10) C1(11) C1(12)
+#undef C1
+    }
+    snprintf(m->err, sizeof(m->err), "unsupported number of traced transitions %d", m->selh.nsel);
+    return LOC_EINVAL;
+}

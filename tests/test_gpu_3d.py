@@ -1,0 +1,119 @@
+"""GPU parity of the 3D octree / Cartesian path (path builder + radiative kernel + solve) against the oracle."""
+import numpy as np
+import pytest
+
+import loc_workloads as W
+import oracle as O
+from parity import check_pops, f32_pops_from_oracle_lte, oracle_SJ_ESC, rel_err, tex_all
+
+pytestmark = pytest.mark.gpu
+
+TOL_SJ = 1e-4
+TOL_POP = 1e-3
+
+
+def _model(m, **kw):
+    from paper_2009_12609_b200 import LocModel
+    return LocModel(m, **kw)
+
+
+def small(which=4, nroot=4, nlev=3, nch=32, nside=1, frac=0.35, nls=4, seed=None):
+    return W.cloud_config(which, nroot=nroot, nlev=nlev, nchannel=nch, nside=nside, refine_frac=frac,
+                          nlevel_species=nls, seed_config=seed)
+
+
+GEOM_CASES = [dict(nroot=4, nlev=1, nside=2), dict(nroot=4, nlev=2, nside=2, frac=0.4), dict(nroot=4, nlev=3, nside=2),
+              dict(nroot=5, nlev=4, nside=1, frac=0.3, seed=11), dict(nroot=8, nlev=3, nside=1, frac=0.6, seed=5),
+              dict(nroot=3, nlev=3, nside=1, frac=1.0)]
+
+
+@pytest.mark.parametrize("cfg", GEOM_CASES)
+def test_geometry_bit_exact(cfg):
+    """visit counts and integer main-axis path sums per cell are bit-identical to the oracle's (north_star)."""
+    m = small(**cfg)
+    sp = O.OSpecies(m.species)
+    ref = O.sim_3d(sp, m, None, geom_only=True)
+    g = _model(m)
+    g.init_lte()
+    g.simulate(geometry_counters=True)
+    vis, pz = g.geometry_counters()
+    vis, pz = vis.cpu().numpy().astype(np.int64), pz.cpu().numpy().astype(np.int64)
+    st = g.stats()
+    g.close()
+    assert np.array_equal(vis, ref["visits"])
+    assert np.array_equal(pz, ref["pathz"])
+    assert st["steps"] == ref["visits"].sum() == st["setup_steps"]
+
+
+def test_geometry_per_direction():
+    m = small(nroot=4, nlev=3, nside=2, frac=0.45, seed=3)
+    sp = O.OSpecies(m.species)
+    g = _model(m)
+    g.init_lte()
+    for idir in (0, 7, 13, 22, 31, 40, 47):
+        ref = O.sim_3d(sp, m, None, geom_only=True, dirs=m.dirs[idir])
+        g.set_directions(m.dirs[idir:idir + 1])
+        g.simulate(geometry_counters=True)
+        vis, pz = g.geometry_counters()
+        assert np.array_equal(vis.cpu().numpy().astype(np.int64), ref["visits"]), idir
+        assert np.array_equal(pz.cpu().numpy().astype(np.int64), ref["pathz"]), idir
+    g.close()
+
+
+RAD_CASES = [dict(nroot=6, nlev=1, nside=1, nch=48), dict(nroot=4, nlev=3, nside=1, nch=40, frac=0.4),
+             dict(nroot=4, nlev=3, nside=2, nch=32, frac=0.5, seed=9), dict(which=5, nroot=4, nlev=2, nside=1, nch=64, frac=0.4, nls=10)]
+
+
+@pytest.mark.parametrize("cfg", RAD_CASES)
+def test_first_simulate_counters(cfg):
+    m = small(**cfg)
+    sp = O.OSpecies(m.species)
+    sel = np.arange(sp.ntrans, dtype=np.int32) if m.sel is None else m.sel
+    pops64, pops32 = f32_pops_from_oracle_lte(sp, m)
+    ref = O.sim_3d(sp, m, pops64, sel)
+    sj_o, esc_o = oracle_SJ_ESC(sp, m, ref, sel)
+    g = _model(m, ntrans_sim=len(sel))
+    g.set_populations(pops32)
+    g.simulate(None if m.sel is None else sel, geometry_counters=True)
+    sj, esc = g.counters()
+    sj, esc = sj.cpu().numpy(), esc.cpu().numpy()
+    vis, _ = g.geometry_counters()
+    assert np.array_equal(vis.cpu().numpy().astype(np.int64), ref["visits"])
+    g.close()
+    leaf = m.child < 0
+    assert np.all(sj[~leaf] == 0)
+    assert rel_err(sj[leaf], sj_o[leaf]).max() < TOL_SJ
+    assert np.max(np.abs(esc[leaf] - esc_o[leaf]) / (np.abs(esc_o[leaf]) + 3e-3)) < TOL_SJ
+
+
+@pytest.mark.parametrize("cfg,niter", [(dict(nroot=6, nlev=1, nside=1, nch=48), 4), (dict(nroot=4, nlev=3, nside=1, nch=40, frac=0.4), 4)])
+def test_iterate_populations_and_tex(cfg, niter):
+    m = small(**cfg)
+    sp = O.OSpecies(m.species)
+    pops_o, change_o = O.iterate(sp, m, niter)
+    g = _model(m)
+    g.init_lte()
+    g.iterate(niter)
+    pg = g.pops.cpu().numpy()
+    g.close()
+    leaf = m.child < 0
+    worst, small_abs = check_pops(pg[:, leaf], pops_o[leaf])
+    assert worst < TOL_POP and small_abs < 1e-10
+    tg, to = tex_all(sp, pg.astype(np.float64).T[leaf], m.species), tex_all(sp, pops_o[leaf], m.species)
+    assert rel_err(tg, to).max() < TOL_POP
+
+
+def test_blackbody_enclosure_gpu():
+    """pin P4 through the GPU path: T_bg = T_kin, LTE start: one iteration leaves the populations unchanged."""
+    m = small(nroot=4, nlev=3, nside=1, nch=40, frac=0.4)
+    m.tkin[:] = 12.0
+    m.t_bg = 12.0
+    g = _model(m)
+    g.init_lte()
+    p0 = g.pops.clone()
+    change = g.iterate(1)
+    leaf = np.flatnonzero(m.child < 0)
+    p1 = g.pops.cpu().numpy()[:, leaf]
+    p0 = p0.cpu().numpy()[:, leaf]
+    g.close()
+    assert np.max(np.abs(p1 - p0) / p0) < 2e-5 and change < 2e-5
