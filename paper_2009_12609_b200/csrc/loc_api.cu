@@ -69,10 +69,9 @@ static int64_t carve(loc_model *m, Carver &c, const loc_grid *g, int nch, int nl
         m->d_order = c.take<int>(g->nray);
         m->d_k0 = c.take<int>(g->nray);
         m->d_off = c.take<long long>(g->nray);
-        m->d_rayw = c.take<float>(g->nray);
-        m->d_invv = c.take<float>(g->nshell);
         m->d_tabs = c.take<float>(ntab);
         m->d_tabmu = c.take<float>(ntab);
+        m->d_tabw = c.take<float>(ntab);
     } else {
         // root-line tasks: at most max(face) lines per direction
         int64_t face = std::max((int64_t)g->nx * g->ny, std::max((int64_t)g->ny * g->nz, (int64_t)g->nx * g->nz));
@@ -370,6 +369,13 @@ extern "C" int loc_create_model(const loc_grid *g, const loc_cells *cells, int n
     m->max_levels = nlevel_max;
 
     cudaError_t e;
+    if ((e = cudaMemsetAsync(m->d_errflag, 0, sizeof(int), m->stream)) != cudaSuccess ||
+        (e = cudaMemsetAsync(m->d_maxrel, 0, sizeof(unsigned int), m->stream)) != cudaSuccess ||
+        (e = cudaMemsetAsync(m->d_steps, 0, sizeof(unsigned long long), m->stream)) != cudaSuccess) {
+        snprintf(g_create_err, 512, "cudaMemsetAsync: %s", cudaGetErrorString(e));
+        delete m;
+        return LOC_ECUDA;
+    }
     if (g->kind == LOC_GRID_SHELL) {
         m->nshell = g->nshell;
         m->nray = g->nray;
@@ -379,9 +385,8 @@ extern "C" int loc_create_model(const loc_grid *g, const loc_cells *cells, int n
         // S0 set-up tables ("The distance that a ray travels through each shell is pre-calculated")
         std::vector<int> k0(nr), order(nr);
         std::vector<long long> off(nr);
-        std::vector<float> rayw(nr), invv(ns);
         std::vector<double> veff(ns, 0.0);
-        std::vector<float> tabs, tabmu;
+        std::vector<float> tabs, tabmu, tabw;
         tabs.reserve((size_t)nr * ns / 2 + nr);
         tabmu.reserve((size_t)nr * ns / 2 + nr);
         int64_t steps = 0;
@@ -391,7 +396,6 @@ extern "C" int loc_create_model(const loc_grid *g, const loc_cells *cells, int n
             while (k < ns - 1 && p >= g->r_out[k]) k++;
             k0[i] = k;
             off[i] = (long long)tabs.size();
-            rayw[i] = (float)g->ray_w[i];
             for (int kk = k; kk < ns; kk++) {
                 double ro = g->r_out[kk], ri = (kk > 0) ? g->r_out[kk - 1] : 0.0;
                 double s = (kk == k) ? 2.0 * sqrt(ro * ro - p * p) : sqrt(ro * ro - p * p) - sqrt(ri * ri - p * p);
@@ -403,7 +407,15 @@ extern "C" int loc_create_model(const loc_grid *g, const loc_cells *cells, int n
             steps += 2 * (ns - 1 - k) + 1;
         }
         m->steps1d = steps;
-        for (int k = 0; k < ns; k++) invv[k] = veff[k] > 0.0 ? (float)(1.0 / veff[k]) : 0.0f;
+        // this ray's share W_i s_ik / V_eff,k of the shell, formed in double: the factors themselves (~1e34 cm^2,
+        // ~1e17 cm, ~1e-52 cm^-3) leave the float32 range
+        tabw.resize(tabs.size());
+        for (int i = 0; i < nr; i++)
+            for (int kk = k0[i]; kk < ns; kk++) {
+                double ro = g->r_out[kk], ri = (kk > 0) ? g->r_out[kk - 1] : 0.0, p = g->ray_p[i];
+                double sd = (kk == k0[i]) ? 2.0 * sqrt(ro * ro - p * p) : sqrt(ro * ro - p * p) - sqrt(ri * ri - p * p);
+                tabw[off[i] + (kk - k0[i])] = veff[kk] > 0.0 ? (float)(g->ray_w[i] * sd / veff[kk]) : 0.0f;
+            }
         for (int i = 0; i < nr; i++) order[i] = i;
         std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return k0[a] < k0[b]; });  // longest rays first
         if ((int64_t)tabs.size() > (int64_t)nr * ns) {
@@ -419,10 +431,9 @@ extern "C" int loc_create_model(const loc_grid *g, const loc_cells *cells, int n
         H2D(m->d_order, order.data(), sizeof(int) * nr);
         H2D(m->d_k0, k0.data(), sizeof(int) * nr);
         H2D(m->d_off, off.data(), sizeof(long long) * nr);
-        H2D(m->d_rayw, rayw.data(), sizeof(float) * nr);
-        H2D(m->d_invv, invv.data(), sizeof(float) * ns);
         H2D(m->d_tabs, tabs.data(), sizeof(float) * tabs.size());
         H2D(m->d_tabmu, tabmu.data(), sizeof(float) * tabmu.size());
+        H2D(m->d_tabw, tabw.data(), sizeof(float) * tabw.size());
         cudaStreamSynchronize(m->stream);  // host vectors go out of scope
     } else {
         m->nx = g->nx;

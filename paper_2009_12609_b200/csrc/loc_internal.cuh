@@ -105,7 +105,7 @@ struct loc_model {
     int nshell, nray;
     int *d_order, *d_k0;
     long long *d_off;
-    float *d_tabs, *d_tabmu, *d_rayw, *d_invv;
+    float *d_tabs, *d_tabmu, *d_tabw;
     double *h_rout;
     int64_t steps1d;
     // 3D
@@ -196,7 +196,8 @@ __device__ __forceinline__ void channel_update(float &n, float phi, const TParam
 }
 
 // Reduce NV per-lane values across the warp with a halving butterfly (about NV shuffles in total instead of
-// 5 NV).  On return v[0] of lane L holds the warp total of value index *owner (or *owner = -1).
+// 5 NV).  On return v[0] of lane L holds the warp total of value index *owner (or *owner = -1); every value index has
+// exactly one owner lane.
 template <int N, int OFF>
 struct MultiReduce {
     __device__ static __forceinline__ void run(float *v, int lane, int &base, int &nvalid)
@@ -231,6 +232,7 @@ struct MultiReduce<1, OFF> {
         // a single value left: plain butterfly over the remaining offsets
 #pragma unroll
         for (int o = OFF; o >= 1; o >>= 1) v[0] += __shfl_xor_sync(0xffffffffu, v[0], o);
+        if (lane & (2 * OFF - 1)) nvalid = 0;  // the 2*OFF lanes of the group hold copies: only the first one owns the total
     }
 };
 

@@ -17,7 +17,7 @@ struct Sim1D {
     float dv, xmin, eps_tau;
     const int *order, *k0;
     const long long *off;
-    const float *rayw, *invv, *tabs, *tabmu;
+    const float *tabs, *tabmu, *tabw;
     const float4 *kin;
     const float2 *coef;
     float2 *cnt;
@@ -25,19 +25,22 @@ struct Sim1D {
     Selection S;
 };
 
-__device__ __forceinline__ void seg1d(const Sim1D &P, int j, int nin, int k0, long long off, int &k, float &s, float &mu)
+__device__ __forceinline__ void seg1d(const Sim1D &P, int j, int nin, int k0, long long off, int &k, float &s, float &mu, float &w)
 {
     if (j < nin) {  // inbound through shell NS-1-j
         k = P.ns - 1 - j;
         s = __ldg(P.tabs + off + (k - k0));
+        w = __ldg(P.tabw + off + (k - k0));
         mu = -__ldg(P.tabmu + off + (k - k0));
     } else if (j == nin) {  // tangent shell, one step (DESIGN R5)
         k = k0;
         s = __ldg(P.tabs + off);
+        w = __ldg(P.tabw + off);
         mu = -__ldg(P.tabmu + off);
     } else {  // outbound: entry cosine is that of the inner boundary r_{k-1}
         k = k0 + (j - nin);
         s = __ldg(P.tabs + off + (k - k0));
+        w = __ldg(P.tabw + off + (k - k0));
         mu = __ldg(P.tabmu + off + (k - 1 - k0));
     }
 }
@@ -54,7 +57,6 @@ __global__ void __launch_bounds__(1024) k_sim1d(Sim1D P)
     const int ray = P.order[blockIdx.x];
     const int k0 = P.k0[ray];
     const long long off = P.off[ray];
-    const float Wi = P.rayw[ray];
     const int nin = P.ns - 1 - k0, nseg = 2 * nin + 1;
     float n[NT];
 #pragma unroll
@@ -67,11 +69,11 @@ __global__ void __launch_bounds__(1024) k_sim1d(Sim1D P)
         int k = 0;
         float s = 0.f, mu = 0.f, w = 0.f, v0 = 0.f, sig = 1.f, amp = 0.f;
         if (j < nseg) {
-            seg1d(P, j, nin, k0, off, k, s, mu);
+            seg1d(P, j, nin, k0, off, k, s, mu, w);
             float4 kin = __ldg(P.kin + k);
             v0 = -kin.x * mu;  // DESIGN R6, mu at the entry of the step
             sig = kin.w;
-            w = Wi * s * __ldg(P.invv + k);  // this ray's share a s / V_eff of the shell (DESIGN R12)
+            // w = this ray's share a s / V_eff of the shell (DESIGN R12), tabulated
             amp = P.dv * 0.3989422804f / sig;
             if (warp == 0) {
                 float tau0 = 0.f;
@@ -89,8 +91,8 @@ __global__ void __launch_bounds__(1024) k_sim1d(Sim1D P)
         if (j > 0 && warp == nwarp - 1) {
             const float *pp = s_part + (buf ^ 1) * pstride;
             int kp;
-            float sp_, mup;
-            seg1d(P, j - 1, nin, k0, off, kp, sp_, mup);
+            float sp_, mup, wp_;
+            seg1d(P, j - 1, nin, k0, off, kp, sp_, mup, wp_);
             const float wprev = pp[nwarp * NV + 0];
             const int clo = __float_as_int(pp[nwarp * NV + 1]), chi = __float_as_int(pp[nwarp * NV + 2]);
             float tot = 0.f;
@@ -170,8 +172,7 @@ int loc_launch_sim1d(loc_model *m, int geom)
     P.order = m->d_order;
     P.k0 = m->d_k0;
     P.off = m->d_off;
-    P.rayw = m->d_rayw;
-    P.invv = m->d_invv;
+    P.tabw = m->d_tabw;
     P.tabs = m->d_tabs;
     P.tabmu = m->d_tabmu;
     P.kin = m->kin;
