@@ -1,0 +1,351 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the LOC hot path (one ALI iteration = loc_simulate + loc_solve) on synthetic clouds.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C1|C2|C3|C4|C5] [--impl reference]
+
+One "step" is one pass of the whole hot path (ray tracing of all directions / rays for all traced transitions, then
+the per-cell statistical-equilibrium solve) over one synthetic model.  Prints ONE JSON line (rank 0).
+section 8 for the definitions of the metric, the roofline and the CPU baseline.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "ray-cell-channel updates/sec per ALI iteration"
+UNIT = "updates/s"
+DEFAULT_WORKLOAD = "C4"
+
+# ---- roofline constants -----------------------------------------------------------------------------
+N_SM = 148
+FP32_LANES_PER_SM_CLK = 128  # 4 sub-partitions x 1 warp instruction / clk
+MUFU_PER_SM_CLK = 16
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured"
+    return 6650.0, 1965.0, "fallback"
+
+
+# ---- workloads --------------------------------------------------------------------------------------------------------
+def make_workload(name: str):
+    """returns (model description, human description).  Seeded synthetic stand-ins for the paper's test models
+    (DESIGN.md section 4); the paper's own inputs are not available."""
+    import loc_workloads as W
+    if name == "C1":
+        return W.shell_config(1), "C1: 1D, 64 log shells, 64 rays, 64 channels, 5-level rotor (4 transitions)"
+    if name == "C2":
+        return W.shell_config(2), "C2: 1D, 1000 log shells, 4000 rays, 256 channels, 10-level rotor (9 transitions)"
+    if name == "C3":
+        return W.cloud_config(3), "C3: Cartesian 128^3, 48 directions, 128 channels, 10-level rotor (9 transitions)"
+    if name == "C4":
+        return W.cloud_config(4), "C4: octree root 64^3 + 3 levels (~30M leaves), 48 directions, 128 channels, 9 transitions"
+    if name == "C5":
+        return W.cloud_config(5), "C5: octree root 256^3 + 2 levels (~200M leaves), 12 directions, 256 channels, 3 transitions"
+    if name.startswith("T"):  # tiny variants for tests of bench.py itself: T3 = 16^3 Cartesian, T4 = small octree
+        if name == "T1":
+            return W.shell_config(1, ns=32), "T1: 1D test model"
+        if name == "T3":
+            return W.cloud_config(3, nroot=16, nchannel=64, nside=1), "T3: Cartesian 16^3 test model"
+        return W.cloud_config(4, nroot=8, nlev=3, nchannel=64, nside=1), "T4: octree 8^3 + 2 levels test model"
+    raise SystemExit(f"unknown workload {name}")
+
+
+def nominal_updates(steps: int, nch: int, nt: int) -> float:
+    return float(steps) * nch * nt
+
+
+# ---- clocks -----------------------------------------------------------------------------------------------------------
+class ClockSampler(threading.Thread):
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        super().__init__(daemon=True)
+        self.index, self.rows, self._stop = index, [], threading.Event()
+
+    def run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([x.strip() for x in out.split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.2)
+
+    def stop(self):
+        self._stop.set()
+        self.join(timeout=6)
+        sm = [float(r[0]) for r in self.rows if r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if r[1].replace(".", "").isdigit()]
+        reasons = []
+        for i, nm in enumerate(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")):
+            if any(len(r) > 3 + i and r[3 + i].lower().startswith("active") for r in self.rows):
+                reasons.append(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": reasons,
+                "samples": len(self.rows)}
+
+
+# ---- CPU oracle sample (cpu_baseline / --impl reference) --------------------------------------------------------------
+def oracle_sample(m, budget_updates=6e9):
+    """Runs the float64 oracle, as it stands, on a bounded sample of the workload: the ray tracing (all channels) of as
+    many transitions / directions as fit the update budget, plus the solve over all cells.  Returns
+    (nominal updates done, seconds, threads, description)."""
+    import oracle as O
+    ncores = os.cpu_count() or 1
+    O.set_threads(ncores)
+    sp = O.OSpecies(m.species)
+    nch = m.nchannel
+    dv = 2.0 * m.band_half / nch
+    dens, tk, ab = (np.asarray(x, np.float64) for x in (m.density, m.tkin, m.abundance))
+    pops = O.lte(sp, dens, tk, ab)
+    if hasattr(m, "child"):
+        r0 = O.sim_3d(sp, m, None, geom_only=True, dirs=m.dirs[0])
+        steps_dir = int(r0["visits"].sum())
+        nt = max(1, min(sp.ntrans, int(budget_updates // max(1, steps_dir * nch))))
+        sel = np.arange(nt, dtype=np.int32)
+        t0 = time.perf_counter()
+        r = O.sim_3d(sp, m, pops, sel, dirs=m.dirs[0])
+        O.solve(sp, dens, tk, ab, r["veff"], sel, r["P"], r["LAM"], dv, m.t_bg, pops)
+        dt = time.perf_counter() - t0
+        done = nominal_updates(steps_dir, nch, nt)
+        desc = f"direction 0 of {len(m.dirs)}, transitions 0..{nt - 1}, all {nch} channels, all cells; then the solve"
+        threads = ncores  # rays are distributed over OpenMP threads
+    else:
+        sel = np.arange(sp.ntrans, dtype=np.int32)
+        nray = len(m.ray_p)
+        steps_all = sum(2 * (len(m.r_out) - 1 - int(np.searchsorted(m.r_out, p, side="right"))) + 1 for p in m.ray_p)
+        frac = min(1.0, budget_updates / 8 / max(1.0, nominal_updates(steps_all, nch, len(sel))))  # 1D oracle is serial
+        if frac < 1.0:
+            import copy
+            keep = np.arange(0, nray, max(1, int(round(1 / frac))))
+            ms = copy.copy(m)
+            ms.ray_p, ms.ray_w = m.ray_p[keep], m.ray_w[keep]
+        else:
+            keep, ms = np.arange(nray), m
+        t0 = time.perf_counter()
+        r = O.sim_1d(sp, ms, pops, sel)
+        O.solve(sp, dens, tk, ab, r["veff"], sel, r["P"], r["LAM"], dv, m.t_bg, pops)
+        dt = time.perf_counter() - t0
+        done = nominal_updates(int(r["visits"].sum()), nch, len(sel))
+        desc = f"{len(keep)} of {nray} rays, all {len(sel)} transitions, all {nch} channels; then the solve"
+        threads = 1  # the 1D ray loop of the oracle is serial
+    return done, dt, threads, desc
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    m, desc = make_workload(args.workload)
+    import oracle as O
+    O.build()
+    times, done, threads, sdesc = [], 0.0, 1, ""
+    for i in range(args.warmup + args.steps):
+        d, dt, threads, sdesc = oracle_sample(m, budget_updates=args.ref_budget)
+        if i >= args.warmup:
+            times.append(dt)
+            done = d
+    t = float(np.mean(times))
+    val = done / t
+    out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": 1e3 * t, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f64", "data": "synthetic",
+           "config": {"workload": desc, "sample": sdesc},
+           "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sdesc},
+           "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out))
+
+
+# ---- own arm ------------------------------------------------------------------------------------------------------------
+def roofline(stats_geom, nt, t_sim_s, hbm_gbs, sm_mhz, peak_kind):
+    """T_roof = max(bytes / HBM, MUFU ops / MUFU rate, FP32 instructions / issue rate) for the simulation
+    kernel; `achieved`/`peak` are quoted for the binding resource."""
+    steps, act = stats_geom["steps"], stats_geom["active_channels"]
+    u_active = float(act) * nt
+    byt = float(steps) * (8 + 16 + 24 * nt)
+    mufu = u_active * (1.0 + 1.0 / nt)
+    fp32 = u_active * (8.0 + 4.0 / nt)
+    clk = sm_mhz * 1e6
+    t_hbm = byt / (hbm_gbs * 1e9)
+    t_mufu = mufu / (N_SM * MUFU_PER_SM_CLK * clk)
+    t_fp32 = fp32 / (N_SM * FP32_LANES_PER_SM_CLK * clk)
+    t_roof = max(t_hbm, t_mufu, t_fp32)
+    if t_roof == t_hbm:
+        r = {"bound": "hbm", "achieved": byt / t_sim_s / 1e9, "peak": hbm_gbs, "unit": "GB/s"}
+    elif t_roof == t_mufu:
+        r = {"bound": "alu", "achieved": mufu / t_sim_s / 1e12, "peak": N_SM * MUFU_PER_SM_CLK * clk / 1e12, "unit": "TMUFU/s"}
+    else:
+        r = {"bound": "alu", "achieved": fp32 / t_sim_s / 1e12, "peak": N_SM * FP32_LANES_PER_SM_CLK * clk / 1e12,
+             "unit": "Tinstr/s (FP32-pipe lane instructions)"}
+    r["frac"] = t_roof / t_sim_s
+    r["traffic"] = None
+    r.update({"kernel": "k_sim3d" if stats_geom.get("is3d") else "k_sim1d", "peak_source": peak_kind + " HBM copy; ALU peaks derived at sm_max clock",
+              "algorithmic_bytes_per_launch": byt, "active_updates_per_launch": u_active, "hbm_gbs_achieved": byt / t_sim_s / 1e9,
+              "hbm_frac": t_hbm / t_sim_s, "mufu_frac": t_mufu / t_sim_s, "fp32_frac": t_fp32 / t_sim_s,
+              "t_kernel_ms": 1e3 * t_sim_s})
+    return r
+
+
+def run_own(args):
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the LOC library has no CPU path; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2009_12609_b200 import LocModel
+
+    t_gen = time.perf_counter()
+    m, desc = make_workload(args.workload)
+    t_gen = time.perf_counter() - t_gen
+    is3d = hasattr(m, "child")
+    sel = None if getattr(m, "sel", None) is None else m.sel
+    nt = len(m.species.upper) if sel is None else len(sel)
+    g = LocModel(m, device=f"cuda:{local}", ntrans_sim=nt)
+    g.init_lte()
+    # one untimed pass with the geometry counters: step and active-channel counts of this workload
+    g.simulate(sel, geometry_counters=True)
+    sg = g.stats()
+    sg["is3d"] = is3d
+    g.init_lte()
+    g.simulate(sel)  # remember the selection for loc_iterate
+    g.solve()
+    g.init_lte()
+    steps_per_iter = sg["steps"]
+    u_nom = nominal_updates(steps_per_iter, m.nchannel, nt)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        g.iterate(1)
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    l0 = g.stats()["kernel_launches"]
+    barrier()
+    for k in range(args.steps):
+        ev[k][0].record()
+        g.simulate()
+        ev[k][1].record()
+        g.solve()
+        ev[k][2].record()
+    barrier()
+    clocks = sampler.stop()
+    launches = g.stats()["kernel_launches"] - l0
+    t_sim = sum(e[0].elapsed_time(e[1]) for e in ev) * 1e-3
+    t_all = sum(e[0].elapsed_time(e[2]) for e in ev) * 1e-3
+    tt = torch.tensor([t_all, t_sim], dtype=torch.float64, device=f"cuda:{local}")
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    t_all, t_sim = float(tt[0]), float(tt[1])
+    value = world * u_nom * args.steps / t_all
+
+    # ---- end to end: host buffers -> device -> one ALI iteration -> populations back to the host ----
+    names = ["density", "tkin", "sigma", "abundance"] + (["vx", "vy", "vz"] if is3d else ["vx"])
+    src = {"density": m.density, "tkin": m.tkin, "sigma": m.sigma, "abundance": m.abundance,
+           "vx": m.vx if is3d else m.vrad}
+    if is3d:
+        src.update(vy=m.vy, vz=m.vz)
+    host = {k: torch.from_numpy(np.ascontiguousarray(src[k], np.float32)).pin_memory() for k in names}
+    g.init_lte()
+    host_pops = g.pops.cpu().pin_memory()
+    host_out = torch.empty_like(host_pops).pin_memory()
+    h2d = sum(t.numel() * 4 for t in host.values()) + host_pops.numel() * 4
+    d2h = host_out.numel() * 4
+    from paper_2009_12609_b200 import binding as B
+
+    def e2e_step():
+        g.update_cells(**host)
+        g.pops.copy_(host_pops, non_blocking=True)
+        B.loc_set_populations(g.h, g.pops)
+        g.iterate(1)
+        host_out.copy_(g.pops, non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+
+    e2e_step()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n_e2e = max(1, min(args.steps, 5))
+    barrier()
+    e0.record()
+    for _ in range(n_e2e):
+        e2e_step()
+    e1.record()
+    barrier()
+    te = torch.tensor([e0.elapsed_time(e1) * 1e-3], dtype=torch.float64, device=f"cuda:{local}")
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_val = world * u_nom * n_e2e / float(te[0])
+
+    if rank == 0:
+        hbm, sm_max, kind = load_peaks()
+        roof = roofline(sg, nt, t_sim / args.steps, hbm, sm_max, kind)
+        cpu = None
+        if world == 1 and not args.no_cpu:
+            import oracle as O
+            O.build()
+            done, dt, threads, sdesc = oracle_sample(m, budget_updates=args.ref_budget)
+            cpu = {"value": done / dt, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sdesc, "seconds": dt}
+        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+               "ms_per_step": 1e3 * t_all / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+               "dtype": "f32", "data": "synthetic",
+               "config": {"workload": desc, "cells": int(g.ncell), "ray_cell_steps_per_iteration": int(steps_per_iter),
+                          "channels": int(m.nchannel), "transitions_traced": int(nt), "parallelism": "replicas" if world > 1 else "single GPU",
+                          "updates": "nominal = steps x channels x transitions (what the oracle evaluates); active = 5-sigma rule",
+                          "l2": "inputs larger than L2 (no flush)" if is3d and g.ncell > 1_000_000 else "working set fits L2 (model is small); no flush: the data is re-read from L2 by design",
+                          "setup_ms_once": sg["setup_ms"], "input_generation_s": t_gen},
+               "active_updates_per_s": world * sg["active_channels"] * nt * args.steps / t_all,
+               "ms_simulate": 1e3 * t_sim / args.steps, "ms_solve": 1e3 * (t_all - t_sim) / args.steps,
+               "clocks": clocks, "roofline": roof,
+               "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
+               "gpu_launches": int(launches)}
+        if cpu is not None:
+            out["cpu_baseline"] = cpu
+        print(json.dumps(out))
+    g.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="own", choices=["own", "reference"])
+    ap.add_argument("--workload", default=os.environ.get("LOC_BENCH_WORKLOAD", DEFAULT_WORKLOAD))
+    ap.add_argument("--ref-budget", type=float, default=6e9, help="nominal updates per oracle sample (about 10-30 s of CPU)")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_own(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -84,6 +84,9 @@ typedef struct {
     int nchannel;
     int64_t kernel_launches; /* CUDA kernels launched by the library on this model so far                  */
     int counter_stride;      /* floats per cell in the counter / coefficient records = 2 * ntrans_padded  */
+    int64_t active_channels; /* sum over the steps of the last loc_simulate(geometry_counters=1) of the number of
+                                channels with |v_c - v_0| <= 5 sigma: the counting definition of "active" ray-cell-
+                                channel updates per traced transition (DESIGN 8), independent of the kernel's window */
     int64_t setup_steps;     /* octree: ray-cell steps in the precomputed step stream (all directions)      */
     double setup_ms;         /* octree: device time of the last path set-up (loc_set_directions), ms        */
 } loc_stats;
@@ -108,6 +111,10 @@ int loc_create_model(const loc_grid *grid, const loc_cells *cells, int nchannel,
 int loc_set_species(loc_model *m, int nlevel, const double *energy_K, const double *g, int ntrans, const int *upper,
                     const int *lower, const double *einstein_A, double mass_amu, int ncoll, const int *cu, const int *cl,
                     int ntemp, const double *temps_K, const double *rate_down);
+
+/* Re-read the caller's cell arrays (same device pointers as given to loc_create_model) after their content has been
+ * changed from outside, and rebuild the derived per-cell kinematics record (velocity, total line width).     */
+int loc_refresh_cells(loc_model *m);
 
 /* Octree only: ray directions (unit vectors, host [ndir][3]; PAPER.md:93 uses HEALPix centres).  Each is
  * snapped to the library's fixed-point slopes (DESIGN R7); ndir <= the ndir_max given to loc_workspace_bytes.

@@ -17,7 +17,7 @@ from . import build as _build
 LOC_OK, LOC_EINVAL, LOC_ESTATE, LOC_ENOMEM, LOC_ECUDA = 0, -1, -2, -3, -4
 LOC_GRID_SHELL, LOC_GRID_OCTREE = 1, 2
 
-SYMBOLS = ("loc_workspace_bytes", "loc_create_model", "loc_set_species", "loc_set_directions", "loc_set_populations",
+SYMBOLS = ("loc_workspace_bytes", "loc_create_model", "loc_set_species", "loc_refresh_cells", "loc_set_directions", "loc_set_populations",
            "loc_init_lte", "loc_simulate", "loc_get_counters", "loc_solve", "loc_iterate", "loc_spectra",
            "loc_get_stats", "loc_destroy_model", "loc_last_error")
 
@@ -41,7 +41,7 @@ class loc_cells(C.Structure):
 
 class loc_stats(C.Structure):
     _fields_ = [("ncell", C.c_int64), ("steps", C.c_int64), ("ntrans_sim", C.c_int), ("nchannel", C.c_int),
-                ("kernel_launches", C.c_int64), ("counter_stride", C.c_int), ("setup_steps", C.c_int64),
+                ("kernel_launches", C.c_int64), ("counter_stride", C.c_int), ("active_channels", C.c_int64), ("setup_steps", C.c_int64),
                 ("setup_ms", C.c_double)]
 
 
@@ -68,6 +68,7 @@ def lib():
         L.loc_set_species.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p,
                                       C.c_void_p, C.c_double, C.c_int, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p,
                                       C.c_void_p]
+        L.loc_refresh_cells.argtypes = [C.c_void_p]
         L.loc_set_directions.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
         L.loc_set_populations.argtypes = [C.c_void_p, C.c_void_p]
         L.loc_init_lte.argtypes = [C.c_void_p]
@@ -148,6 +149,10 @@ def loc_set_species(h, sp):
     tk, rd = _np(sp.temps_K, np.float64), _np(sp.rate_down, np.float64)
     _check(lib().loc_set_species(h, len(e), _hp(e), _hp(g), len(up), _hp(up), _hp(lo), _hp(A), float(sp.mass_amu), len(cu),
                                  _hp(cu), _hp(cl), len(tk), _hp(tk), _hp(rd)), h)
+
+
+def loc_refresh_cells(h):
+    _check(lib().loc_refresh_cells(h), h)
 
 
 def loc_set_directions(h, dirs):

@@ -44,7 +44,7 @@ static int64_t carve(loc_model *m, Carver &c, const loc_grid *g, int nch, int nl
     m->cnt = c.take<float2>(ncell * nsp);
     m->visits = c.take<uint32_t>(ncell);
     m->pathz = c.take<uint32_t>(ncell);
-    m->d_steps = c.take<unsigned long long>(1);
+    m->d_steps = c.take<unsigned long long>(2);  // [0] steps, [1] active channels (5 sigma rule)
     m->d_maxrel = c.take<unsigned int>(1);
     m->d_errflag = c.take<int>(1);
     m->d_queue = c.take<unsigned int>(1);
@@ -371,7 +371,7 @@ extern "C" int loc_create_model(const loc_grid *g, const loc_cells *cells, int n
     cudaError_t e;
     if ((e = cudaMemsetAsync(m->d_errflag, 0, sizeof(int), m->stream)) != cudaSuccess ||
         (e = cudaMemsetAsync(m->d_maxrel, 0, sizeof(unsigned int), m->stream)) != cudaSuccess ||
-        (e = cudaMemsetAsync(m->d_steps, 0, sizeof(unsigned long long), m->stream)) != cudaSuccess) {
+        (e = cudaMemsetAsync(m->d_steps, 0, 2 * sizeof(unsigned long long), m->stream)) != cudaSuccess) {
         snprintf(g_create_err, 512, "cudaMemsetAsync: %s", cudaGetErrorString(e));
         delete m;
         return LOC_ECUDA;
@@ -455,6 +455,21 @@ extern "C" int loc_create_model(const loc_grid *g, const loc_cells *cells, int n
     return LOC_OK;
 }
 
+// kinematics record: (vx, vy, vz, total sigma) with the thermal broadening k T / m added (DESIGN R3)
+extern "C" int loc_refresh_cells(loc_model *m)
+{
+    if (!m) return LOC_EINVAL;
+    if (!m->have_species) return fail(m, LOC_ESTATE, "loc_set_species must be called first");
+    double ktm = (m->sp.mass_amu > 0.0) ? LOC_KB / (m->sp.mass_amu * LOC_AMU) : 0.0;
+    int64_t n = m->ncell;
+    k_pack_kin<<<(unsigned)((n + 255) / 256), 256, 0, m->stream>>>(n, m->cells.vx, m->kind == LOC_GRID_OCTREE ? m->cells.vy : nullptr,
+                                                                  m->kind == LOC_GRID_OCTREE ? m->cells.vz : nullptr, m->cells.sigma,
+                                                                  m->cells.tkin, ktm, m->kin);
+    m->launches++;
+    LOC_CUDA_CHECK(m, cudaGetLastError());
+    return LOC_OK;
+}
+
 extern "C" int loc_set_species(loc_model *m, int nlevel, const double *energy_K, const double *g, int ntrans, const int *upper,
                                const int *lower, const double *A, double mass_amu, int ncoll, const int *cu, const int *cl,
                                int ntemp, const double *temps_K, const double *rate_down)
@@ -512,14 +527,11 @@ extern "C" int loc_set_species(loc_model *m, int nlevel, const double *energy_K,
         LOC_CUDA_CHECK(m, cudaMemcpyAsync((void *)sp.temps, temps_K, sizeof(double) * ntemp, cudaMemcpyHostToDevice, st));
         LOC_CUDA_CHECK(m, cudaMemcpyAsync((void *)sp.rates, rate_down, sizeof(double) * ntemp * ncoll, cudaMemcpyHostToDevice, st));
     }
-    // kinematics record: thermal broadening k T / m (DESIGN R3)
-    double ktm = (mass_amu > 0.0) ? LOC_KB / (mass_amu * LOC_AMU) : 0.0;
-    int64_t n = m->ncell;
-    k_pack_kin<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, m->cells.vx, m->kind == LOC_GRID_OCTREE ? m->cells.vy : nullptr,
-                                                           m->kind == LOC_GRID_OCTREE ? m->cells.vz : nullptr, m->cells.sigma,
-                                                           m->cells.tkin, ktm, m->kin);
-    m->launches++;
-    LOC_CUDA_CHECK(m, cudaGetLastError());
+    m->have_species = true;
+    {
+        int rc = loc_refresh_cells(m);
+        if (rc) return rc;
+    }
     LOC_CUDA_CHECK(m, cudaStreamSynchronize(st));  // bg vector goes out of scope
     m->have_species = true;
     m->selh.nsel = 0;
@@ -588,7 +600,7 @@ extern "C" int loc_simulate(loc_model *m, int nsel, const int *idx, int geom)
         LOC_CUDA_CHECK(m, cudaMemsetAsync(m->visits, 0, sizeof(uint32_t) * n, m->stream));
         LOC_CUDA_CHECK(m, cudaMemsetAsync(m->pathz, 0, sizeof(uint32_t) * n, m->stream));
     }
-    LOC_CUDA_CHECK(m, cudaMemsetAsync(m->d_steps, 0, sizeof(unsigned long long), m->stream));
+    LOC_CUDA_CHECK(m, cudaMemsetAsync(m->d_steps, 0, 2 * sizeof(unsigned long long), m->stream));
     return (m->kind == LOC_GRID_SHELL) ? loc_launch_sim1d(m, geom) : loc_launch_sim3d(m, geom);
 }
 
@@ -669,11 +681,12 @@ extern "C" int loc_spectra(loc_model *m, int trans, const double *dir, int nx, i
 extern "C" int loc_get_stats(loc_model *m, loc_stats *out)
 {
     if (!m || !out) return LOC_EINVAL;
-    unsigned long long steps = 0;
-    LOC_CUDA_CHECK(m, cudaMemcpyAsync(&steps, m->d_steps, sizeof(steps), cudaMemcpyDeviceToHost, m->stream));
+    unsigned long long steps[2] = {0, 0};
+    LOC_CUDA_CHECK(m, cudaMemcpyAsync(steps, m->d_steps, sizeof(steps), cudaMemcpyDeviceToHost, m->stream));
     LOC_CUDA_CHECK(m, cudaStreamSynchronize(m->stream));
     out->ncell = m->ncell;
-    out->steps = (m->kind == LOC_GRID_SHELL) ? m->steps1d : (int64_t)steps;
+    out->steps = (m->kind == LOC_GRID_SHELL) ? m->steps1d : (int64_t)steps[0];
+    out->active_channels = (int64_t)steps[1];
     out->ntrans_sim = m->selh.nsel;
     out->nchannel = m->nch;
     out->kernel_launches = m->launches;

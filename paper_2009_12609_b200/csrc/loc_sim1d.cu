@@ -22,6 +22,7 @@ struct Sim1D {
     const float2 *coef;
     float2 *cnt;
     uint32_t *visits;
+    unsigned long long *nactive;
     Selection S;
 };
 
@@ -115,6 +116,10 @@ __global__ void __launch_bounds__(1024) k_sim1d(Sim1D P)
         const float hw = X * sig * inv_dv;
         const int c_lo = max(0, (int)ceilf(cc - hw)), c_hi = min(P.nch - 1, (int)floorf(cc + hw));
         float *pw = s_part + buf * pstride;
+        if (GEOM && tid == 0) {
+            const float h5 = 5.0f * sig * inv_dv;
+            atomicAdd(P.nactive, (unsigned long long)max(0, min(P.nch - 1, (int)floorf(cc + h5)) - max(0, (int)ceilf(cc - h5)) + 1));
+        }
         if (tid == 0) {
             pw[nwarp * NV + 0] = w;
             pw[nwarp * NV + 1] = __int_as_float(c_lo);
@@ -179,6 +184,7 @@ int loc_launch_sim1d(loc_model *m, int geom)
     P.coef = m->coef;
     P.cnt = m->cnt;
     P.visits = m->visits;
+    P.nactive = m->d_steps + 1;
     P.S = m->selh;
     switch (m->selh.nsel) {
 #define C1(N) \

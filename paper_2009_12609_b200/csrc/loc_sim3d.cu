@@ -432,7 +432,7 @@ __global__ void __launch_bounds__(128) k_sim3d(Sim3D P)
     TParam *s_tp = reinterpret_cast<TParam *>(sn + NT * nch);     // per-step transition parameters
     float *slots = P.pool + ((long long)blockIdx.x * nwarp + warp) * (long long)P.nslot * NT * nch;
     const float inv_dv = 1.0f / P.dv;
-    unsigned long long mysteps = 0;
+    unsigned long long mysteps = 0, myactive = 0;
 
     for (;;) {
         long long task = 0;
@@ -509,6 +509,8 @@ __global__ void __launch_bounds__(128) k_sim3d(Sim3D P)
                     if (GEOM && lane == 0) {
                         atomicAdd(&P.visits[cell], 1u);
                         atomicAdd(&P.pathz[cell], dz);
+                        const float h5 = 5.0f * sig * inv_dv;
+                        myactive += max(0, min(nch - 1, (int)floorf(cc + h5)) - max(0, (int)ceilf(cc - h5)) + 1);
                     }
                     mysteps++;
                     __syncwarp();
@@ -530,6 +532,7 @@ __global__ void __launch_bounds__(128) k_sim3d(Sim3D P)
         }
     }
     if (lane == 0 && mysteps) atomicAdd(P.nsteps, mysteps);
+    if (GEOM && lane == 0 && myactive) atomicAdd(P.nsteps + 1, myactive);
 }
 
 template <int NT>

@@ -71,6 +71,13 @@ class LocModel:
     def set_directions(self, dirs):
         B.loc_set_directions(self.h, dirs)
 
+    def update_cells(self, **arrays):
+        """overwrite per-cell input arrays (density, tkin, sigma, vx, vy, vz, abundance) from host or device data"""
+        for k, a in arrays.items():
+            getattr(self, k).copy_(a if isinstance(a, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(a)),
+                                   non_blocking=True)
+        B.loc_refresh_cells(self.h)
+
     def init_lte(self):
         B.loc_init_lte(self.h)
 
