@@ -32,7 +32,7 @@ struct Carver {
     }
 };
 
-static int max_resident_warps() { return 148 * 32; }  // upper bound used to size the per-warp spectrum slots
+static int max_resident_warps() { return 148 * 16; }  // upper bound used to size the per-warp spectrum slots
 
 // lays out the workspace; with dry=true only sizes are computed
 static int64_t carve(loc_model *m, Carver &c, const loc_grid *g, int nch, int nlevel, int ntrans, int ndir_max)
@@ -81,12 +81,12 @@ static int64_t carve(loc_model *m, Carver &c, const loc_grid *g, int nch, int nl
         m->d_task_dir = c.take<unsigned char>(m->ntask_max);
         // step stream: every leaf is crossed by (1 + s_p + s_q) <= 3 ray segments per direction on average;
         // control records (background / save / load) ride in the same bound
-        m->stream_cap = 3 * ncell * (int64_t)ndir_max + 4 * m->ntask_max + 1024;
+        m->stream_cap = 3 * ncell * (int64_t)ndir_max + 16 * m->ntask_max + 1024;
         m->d_stream = c.take<uint2>(m->stream_cap);
         m->bstack_threads = (int)std::min<int64_t>(m->ntask_max, LOC_BUILD_BATCH);
         m->d_bstack = c.take<char>((int64_t)m->bstack_threads * LOC_BUILD_STACK * 16);
         m->max_warps = max_resident_warps();
-        m->spec_pool_floats = (int64_t)m->max_warps * std::max(g->nlevel - 1, 1) * nsp * nch;
+        m->spec_pool_floats = (int64_t)m->max_warps * 4 * std::max(g->nlevel - 1, 1) * nsp * ((nch + 3) & ~3);  // 4 rays per warp
         m->spec_pool = c.take<float>(m->spec_pool_floats);
     }
     return align_up(c.off, 256);

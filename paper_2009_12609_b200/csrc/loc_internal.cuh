@@ -68,6 +68,8 @@ struct Dir3 {
 #define LOC_OP_BG 1u    // spectrum := background (model boundary / transverse wrap-around)
 #define LOC_OP_SAVE 2u  // slot[x] := spectrum   (donor duty at the upstream face of a refined cell)
 #define LOC_OP_LOAD 3u  // spectrum := slot[x]   (birth of a ray in a refined region / resume of the donor)
+#define LOC_OP_NOP 7u   // padding: every root-ray task is a whole number of LOC_TASK_ALIGN records
+#define LOC_TASK_ALIGN 8
 #define LOC_REC(op, level, dz) (((unsigned)(op) << 24) | ((unsigned)(level) << 21) | (unsigned)(dz))
 
 struct loc_model {

@@ -1,409 +1,30 @@
-// loc_sim3d.cu -- 3D octree / Cartesian ray tracing (Eqs. 1-3).
+// loc_sim3d.cu -- 3D radiative kernel: replays the precomputed step streams (loc_paths3d.cu) every ALI iteration and
+// evaluates, per ray step and velocity channel, the Doppler-shifted profile, the optical depth, the photon
+// transfer of Eq. 3 and the two per-cell sums (Eq. 2 first term; escape fraction of PAPER.md:81) for all traced
+// transitions at once (the "all transitions in one pass" option the paper leaves open).
 //
-// Two parts:
-//  (1) PATH BUILDER (set-up, runs when the directions are set): one thread per root-grid ray.  It walks the ray and
-//      every ray born from it in refined regions through the octree with INTEGER arithmetic only
-//      (DESIGN R7) and writes the result as a linear "step stream" of 8-byte records: STEP(cell, dzeta) plus the three
-//      spectrum operations BG / SAVE(slot) / LOAD(slot) that encode births, wrap-arounds and the return to the parent
-//      ray.  The paths depend only on the grid and the directions, not on the level populations, so -- like the
-//      per-shell path lengths of the 1D model that the paper pre-calculates -- they are computed once
-//      and kept in HBM (B200: 180 GB) instead of being recomputed by one idle-lane-surrounded work item per step
-//      (the paper's stated bottleneck).
-//  (2) RADIATIVE KERNEL (every ALI iteration): one warp per root-ray task, lanes over the velocity channels of the
-//      local profile window.  It streams the records, evaluates the Doppler-shifted profile, optical depths, Eq. 3 and
-//      the two per-cell sums (Eq. 2 first term and the escape fraction) for all traced transitions at once.
+// Work decomposition (DESIGN 6.4).  A warp carries FOUR rays at a time, one per quarter-warp ("group" of 8 lanes); a lane
+// owns 4 CONSECUTIVE channels of the ray's local profile window (8 lanes x 4 = 32 channels per pass), so that
+//   * the photon spectrum of a ray lives in shared memory and is read / written with one 128-bit access per lane and
+//     transition, conflict free for any window position (a quarter-warp is one shared-memory phase);
+//   * the sums over a lane's 4 channels are free, and the cross-lane reduction is an 8-lane halving butterfly whose every
+//     instruction serves 4 ray steps;
+//   * all per-step scalar work (record decode, Doppler shift, window, per-transition coefficients) is done lane-parallel
+//     for 8 records x 4 rays at once in a "prepare" phase, not redundantly by 32 lanes per step.
+// The four groups stay in lock step: every round each group consumes exactly one stream record (tasks are padded to
+// whole chunks of 8 records by the path builder); the rare spectrum operations (background, save, load) are executed
+// by the whole warp for the group that needs them.
 #include <stdio.h>
 
 #include <algorithm>
-#include <vector>
 
 #include "loc_internal.cuh"
 
-// ------------------------------------------------------------------------------------------------
-// direction set-up (host)
-// ------------------------------------------------------------------------------------------------
-void loc_fill_dir(loc_model *m, const double *din, Dir3 *D)
-{
-    int n[3] = {m->nx, m->ny, m->nz};
-    int mm = 0;
-    for (int a = 1; a < 3; a++)
-        if (fabs(din[a]) > fabs(din[mm])) mm = a;  // ties -> lowest axis index
-    D->ax[0] = mm;
-    D->ax[1] = (mm + 1) % 3;
-    D->ax[2] = (mm + 2) % 3;
-    double sl[2];
-    for (int k = 0; k < 2; k++) {
-        double s = fabs(din[D->ax[k + 1]]) / fabs(din[mm]);
-        unsigned long long S = (unsigned long long)nearbyint(s * (double)LOC_H0);  // round half even (DESIGN R7)
-        if (S == 0) {
-            D->T[k] = 0;
-            sl[k] = 0.0;
-        } else {
-            D->T[k] = ((1ull << 52) + S / 2) / S;
-            sl[k] = 4294967296.0 / (double)D->T[k];
-        }
-    }
-    double lenf = sqrt(1.0 + sl[0] * sl[0] + sl[1] * sl[1]);
-    for (int k = 0; k < 3; k++) {
-        D->flip[k] = din[D->ax[k]] < 0.0;
-        D->W[k] = n[D->ax[k]] * LOC_H0;
-    }
-    D->d[D->ax[0]] = (float)((D->flip[0] ? -1.0 : 1.0) / lenf);
-    D->d[D->ax[1]] = (float)((D->flip[1] ? -1.0 : 1.0) * sl[0] / lenf);
-    D->d[D->ax[2]] = (float)((D->flip[2] ? -1.0 : 1.0) * sl[1] / lenf);
-    D->sf = (float)(m->root_cm / (double)LOC_H0 * lenf);
-    D->np = n[D->ax[1]];
-    D->nq = n[D->ax[2]];
-    D->task0 = 0;
-}
+#define LOC_GROUPS 4  // rays per warp
+#define LOC_CHUNK 8   // records per group and prepare phase (= LOC_TASK_ALIGN)
 
-// ------------------------------------------------------------------------------------------------
-// integer lattice helpers (device)
-// ------------------------------------------------------------------------------------------------
-struct Tree {
-    int nx, ny, nz, nlev;
-    long long noff[LOC_MAXL + 1];
-    const int32_t *child;
-};
-
-#define LOC_ZINF (1ll << 40)
-
-__device__ __forceinline__ long long shift_of(unsigned long long T, long long z)
-{
-    return T ? (long long)(((unsigned long long)z << 32) / T) : 0ll;
-}
-
-// smallest zeta with shift_of(T, zeta) >= D
-__device__ __forceinline__ long long cross_of(unsigned long long T, long long D)
-{
-    if (D <= 0) return 0;
-    if (T == 0) return LOC_ZINF;
-    unsigned long long lo = (unsigned long long)D * T, hi = __umul64hi((unsigned long long)D, T);
-    unsigned long long lo2 = lo + 0xffffffffull;
-    if (lo2 < lo) hi++;
-    return (long long)((hi << 32) | (lo2 >> 32));
-}
-
-__device__ __forceinline__ long long floordiv(long long a, long long b) { return (a >= 0) ? a / b : -((-a + b - 1) / b); }
-
-struct LeafPos {
-    int cell[LOC_MAXL];  // global cell index of the ancestor at each level (last = the leaf)
-    int level;
-};
-
-// leaf containing the working-frame point (fz, fp, fq), all coordinates inside the model
-__device__ __forceinline__ void find_leaf(const Tree &G, const Dir3 &D, int fz, int fp, int fq, LeafPos &L)
-{
-    int X[3];
-    X[D.ax[0]] = D.flip[0] ? D.W[0] - 1 - fz : fz;
-    X[D.ax[1]] = D.flip[1] ? D.W[1] - 1 - fp : fp;
-    X[D.ax[2]] = D.flip[2] ? D.W[2] - 1 - fq : fq;
-    int g = (X[0] >> LOC_LB) + G.nx * ((X[1] >> LOC_LB) + G.ny * (X[2] >> LOC_LB));
-    int l = 0;
-    L.cell[0] = g;
-    int ch;
-    while ((ch = __ldg(G.child + g)) >= 0) {
-        int bit = LOC_LB - 1 - l;
-        g = (int)G.noff[l + 1] + ch + ((X[0] >> bit) & 1) + 2 * ((X[1] >> bit) & 1) + 4 * ((X[2] >> bit) & 1);
-        l++;
-        L.cell[l] = g;
-    }
-    L.level = l;
-}
-
-__device__ __forceinline__ int level_at(const Tree &G, const Dir3 &D, int fz, int fp, int fq)
-{
-    LeafPos L;
-    find_leaf(G, D, fz, fp, fq, L);
-    return L.level;
-}
-
-struct Pending {  // 16 bytes
-    int bp, bq, zeta;
-    unsigned char tag, src, resumed, pad;  // src: slot index, or 255 = background
-};
-#define LOC_SRC_BG 255
-
-struct BuildArgs {
-    Tree G;
-    const Dir3 *dirs;
-    const unsigned char *task_dir;
-    long long task_begin, task_end;
-    long long *task_off;  // count pass: counts written to task_off[task]; emit pass: offsets read from it
-    uint2 *stream;
-    Pending *stacks;
-    int *errflag;
-    unsigned long long *nsteps;
-    int emit;
-};
-
-// Path builder: traces root line `task` and all its descendants depth first (DESIGN 6.3).
-__global__ void __launch_bounds__(128) k_build_paths(BuildArgs A)
-{
-    long long task = A.task_begin + blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (task >= A.task_end) return;
-    const Tree &G = A.G;
-    const Dir3 D = A.dirs[A.task_dir[task]];
-    Pending *stack = A.stacks + (blockIdx.x * (long long)blockDim.x + threadIdx.x) * LOC_BUILD_STACK;
-    int sp = 0;
-    long long nrec = 0, nstep = 0;
-    uint2 *out = A.emit ? A.stream + A.task_off[task] : nullptr;
-    const int Wz = D.W[0], Wp = D.W[1], Wq = D.W[2];
-    {
-        long long lt = task - D.task0;
-        const int O_p = 25 * (LOC_H0 / 64), O_q = 41 * (LOC_H0 / 64);  // DESIGN R8
-        Pending r;
-        r.bp = O_p + (int)(lt % D.np) * LOC_H0;
-        r.bq = O_q + (int)(lt / D.np) * LOC_H0;
-        r.zeta = 0;
-        r.tag = 0;
-        r.src = LOC_SRC_BG;
-        r.resumed = 0;
-        r.pad = 0;
-        stack[sp++] = r;
-    }
-#define EMIT(x_, y_)                             \
-    do {                                         \
-        if (out) out[nrec] = make_uint2(x_, y_); \
-        nrec++;                                  \
-    } while (0)
-    while (sp > 0) {
-        const Pending cur = stack[--sp];
-        const int tag = cur.tag;
-        EMIT(cur.src == LOC_SRC_BG ? 0u : (unsigned)cur.src, LOC_REC(cur.src == LOC_SRC_BG ? LOC_OP_BG : LOC_OP_LOAD, 0, 0));
-        long long zeta = cur.zeta;
-        bool first = true;
-        long long wrp = 0, wrq = 0;
-        while (zeta < Wz) {
-            const long long Sp = shift_of(D.T[0], zeta), Sq = shift_of(D.T[1], zeta);
-            const long long up = cur.bp + Sp, uq = cur.bq + Sq;
-            const long long wp_ = up / Wp, wq_ = uq / Wq;
-            const int fp = (int)(up - wp_ * Wp), fq = (int)(uq - wq_ * Wq);
-            const bool wrapped = !first && (wp_ != wrp || wq_ != wrq);
-            wrp = wp_;
-            wrq = wq_;
-            LeafPos L;
-            find_leaf(G, D, (int)zeta, fp, fq, L);
-            if (L.level < tag) break;  // entering a region refined to less than the tag: terminated
-            if (wrapped) EMIT(0u, LOC_REC(LOC_OP_BG, 0, 0));  // left through a side, re-enters opposite
-            // ---- donor duty: upstream face of refined ancestors entered now ----
-            if (!(first && cur.resumed)) {
-                int saved = -1;
-                for (int j = tag; j < L.level; j++) {
-                    const int hj = LOC_H0 >> j, hk = hj >> 1;
-                    if (zeta & (hj - 1)) continue;
-                    const int op = fp & ~(hj - 1), oq = fq & ~(hj - 1);
-                    for (int dj = -3; dj <= 1; dj++)
-                        for (int di = -3; di <= 1; di++) {
-                            if (!((di | dj) & 1)) continue;  // member of the coarser lattice P_j
-                            const long long ap = (long long)fp + di * hk, aq = (long long)fq + dj * hk;
-                            long long zin = zeta, zout = zeta + hj, z;
-                            z = cross_of(D.T[0], Sp + op - ap); if (z > zin) zin = z;
-                            z = cross_of(D.T[1], Sq + oq - aq); if (z > zin) zin = z;
-                            z = cross_of(D.T[0], Sp + op + hj - ap); if (z < zout) zout = z;
-                            z = cross_of(D.T[1], Sq + oq + hj - aq); if (z < zout) zout = z;
-                            if (zout <= zin) continue;  // does not cross this cell
-                            int src = -1;               // -1: slot of this event
-                            if (zin == 0) {
-                                src = LOC_SRC_BG;
-                            } else {
-                                const long long zb = zin - 1;
-                                const long long pb = ap + shift_of(D.T[0], zb) - Sp, qb = aq + shift_of(D.T[1], zb) - Sq;
-                                const long long pi = ap + shift_of(D.T[0], zin) - Sp, qi = aq + shift_of(D.T[1], zin) - Sq;
-                                const long long wpb = floordiv(pb, Wp), wqb = floordiv(qb, Wq);
-                                if (level_at(G, D, (int)zb, (int)(pb - wpb * Wp), (int)(qb - wqb * Wq)) >= j + 1) continue;  // alive already
-                                if (wpb != floordiv(pi, Wp) || wqb != floordiv(qi, Wq)) src = LOC_SRC_BG;
-                            }
-                            if (saved < 0) {
-                                saved = j;
-                                EMIT((unsigned)j, LOC_REC(LOC_OP_SAVE, 0, 0));
-                                if (sp < LOC_BUILD_STACK) {
-                                    Pending c = cur;
-                                    c.zeta = (int)zeta;
-                                    c.src = (unsigned char)j;
-                                    c.resumed = 1;
-                                    stack[sp++] = c;
-                                } else
-                                    *A.errflag = 1;
-                            }
-                            if (sp < LOC_BUILD_STACK) {
-                                Pending c;
-                                long long bb = (ap - Sp) % Wp, bc = (aq - Sq) % Wq;
-                                c.bp = (int)(bb < 0 ? bb + Wp : bb);
-                                c.bq = (int)(bc < 0 ? bc + Wq : bc);
-                                c.zeta = (int)zin;
-                                c.tag = (unsigned char)(j + 1);
-                                c.src = (unsigned char)(src == LOC_SRC_BG ? LOC_SRC_BG : saved);
-                                c.resumed = 0;
-                                c.pad = 0;
-                                stack[sp++] = c;
-                            } else
-                                *A.errflag = 1;
-                        }
-                }
-                if (saved >= 0) break;  // children first; this ray resumes from the saved spectrum afterwards
-            }
-            // ---- step through the leaf ----
-            const int h = LOC_H0 >> L.level;
-            long long znext = (zeta & ~(long long)(h - 1)) + h, z;
-            z = cross_of(D.T[0], Sp + (fp & ~(h - 1)) + h - fp); if (z < znext) znext = z;
-            z = cross_of(D.T[1], Sq + (fq & ~(h - 1)) + h - fq); if (z < znext) znext = z;
-            EMIT((unsigned)L.cell[L.level], LOC_REC(LOC_OP_STEP, L.level, (unsigned)(znext - zeta)));
-            nstep++;
-            zeta = znext;
-            first = false;
-        }
-    }
-#undef EMIT
-    if (!A.emit) {
-        A.task_off[task] = nrec;
-        atomicAdd(A.nsteps, (unsigned long long)nstep);
-    }
-}
-
-// exclusive scan of counts[0..n) in place (one block), total written to counts[n]
-__global__ void __launch_bounds__(1024) k_scan_tasks(long long *counts, long long n)
-{
-    __shared__ long long part[1024];
-    const int tid = threadIdx.x;
-    const long long per = (n + 1023) / 1024;
-    const long long b = tid * per, e = (b + per < n) ? b + per : n;
-    long long s = 0;
-    for (long long i = b; i < e; i++) s += counts[i];
-    part[tid] = s;
-    __syncthreads();
-    for (int o = 1; o < 1024; o <<= 1) {
-        long long v = (tid >= o) ? part[tid - o] : 0;
-        __syncthreads();
-        part[tid] += v;
-        __syncthreads();
-    }
-    long long run = part[tid] - s;
-    for (long long i = b; i < e; i++) {
-        long long c = counts[i];
-        counts[i] = run;
-        run += c;
-    }
-    if (tid == 1023) counts[n] = part[1023];
-}
-
-__global__ void k_check_tree(Tree G, int *errflag)
-{
-    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    long long n = G.noff[G.nlev];
-    if (i >= n) return;
-    int l = 0;
-    while (i >= G.noff[l + 1]) l++;
-    int ch = G.child[i];
-    if (ch < 0) return;
-    if (l + 1 >= G.nlev || (ch & 7) || (long long)ch + 8 > G.noff[l + 2] - G.noff[l + 1]) *errflag = 2;
-}
-
-static Tree make_tree(const loc_model *m)
-{
-    Tree G;
-    G.nx = m->nx;
-    G.ny = m->ny;
-    G.nz = m->nz;
-    G.nlev = m->nlev;
-    for (int l = 0; l <= LOC_MAXL; l++) G.noff[l] = (l <= m->nlev) ? m->noff[l] : m->noff[m->nlev];
-    G.child = m->child;
-    return G;
-}
-
-int loc_setup3d(loc_model *m)
-{
-    Tree G = make_tree(m);
-    LOC_CUDA_CHECK(m, cudaMemsetAsync(m->d_errflag, 0, sizeof(int), m->stream));
-    int64_t n = m->ncell;
-    k_check_tree<<<(unsigned)((n + 255) / 256), 256, 0, m->stream>>>(G, m->d_errflag);
-    m->launches++;
-    LOC_CUDA_CHECK(m, cudaGetLastError());
-    int err = 0;
-    LOC_CUDA_CHECK(m, cudaMemcpyAsync(&err, m->d_errflag, sizeof(int), cudaMemcpyDeviceToHost, m->stream));
-    LOC_CUDA_CHECK(m, cudaStreamSynchronize(m->stream));
-    if (err) {
-        snprintf(m->err, sizeof(m->err), "octree child index out of range or not a multiple of 8");
-        return LOC_EINVAL;
-    }
-    return LOC_OK;
-}
-
-int loc_build_streams(loc_model *m)
-{
-    cudaEvent_t e0, e1;
-    LOC_CUDA_CHECK(m, cudaEventCreate(&e0));
-    LOC_CUDA_CHECK(m, cudaEventCreate(&e1));
-    LOC_CUDA_CHECK(m, cudaEventRecord(e0, m->stream));
-    // task -> direction table
-    {
-        std::vector<unsigned char> td((size_t)m->ntask);
-        for (int i = 0; i < m->ndir; i++) {
-            int64_t n = (int64_t)m->h_dirs[i].np * m->h_dirs[i].nq;
-            std::fill(td.begin() + m->h_dirs[i].task0, td.begin() + m->h_dirs[i].task0 + n, (unsigned char)i);
-        }
-        LOC_CUDA_CHECK(m, cudaMemcpyAsync(m->d_task_dir, td.data(), td.size(), cudaMemcpyHostToDevice, m->stream));
-        LOC_CUDA_CHECK(m, cudaStreamSynchronize(m->stream));
-    }
-    BuildArgs A;
-    A.G = make_tree(m);
-    A.dirs = m->d_dirs;
-    A.task_dir = m->d_task_dir;
-    A.task_off = m->d_task_off;
-    A.stream = m->d_stream;
-    A.stacks = (Pending *)m->d_bstack;
-    A.errflag = m->d_errflag;
-    A.nsteps = m->d_steps;
-    LOC_CUDA_CHECK(m, cudaMemsetAsync(m->d_errflag, 0, sizeof(int), m->stream));
-    LOC_CUDA_CHECK(m, cudaMemsetAsync(m->d_steps, 0, sizeof(unsigned long long), m->stream));
-    for (int pass = 0; pass < 2; pass++) {
-        A.emit = pass;
-        for (int64_t b = 0; b < m->ntask; b += m->bstack_threads) {
-            A.task_begin = b;
-            A.task_end = std::min<int64_t>(m->ntask, b + m->bstack_threads);
-            unsigned nb = (unsigned)((A.task_end - A.task_begin + 127) / 128);
-            k_build_paths<<<nb, 128, 0, m->stream>>>(A);
-            m->launches++;
-            LOC_CUDA_CHECK(m, cudaGetLastError());
-        }
-        if (pass == 0) {
-            k_scan_tasks<<<1, 1024, 0, m->stream>>>(m->d_task_off, m->ntask);
-            m->launches++;
-            LOC_CUDA_CHECK(m, cudaGetLastError());
-            long long total = 0;
-            unsigned long long steps = 0;
-            int err = 0;
-            LOC_CUDA_CHECK(m, cudaMemcpyAsync(&total, m->d_task_off + m->ntask, sizeof(total), cudaMemcpyDeviceToHost, m->stream));
-            LOC_CUDA_CHECK(m, cudaMemcpyAsync(&steps, m->d_steps, sizeof(steps), cudaMemcpyDeviceToHost, m->stream));
-            LOC_CUDA_CHECK(m, cudaMemcpyAsync(&err, m->d_errflag, sizeof(err), cudaMemcpyDeviceToHost, m->stream));
-            LOC_CUDA_CHECK(m, cudaStreamSynchronize(m->stream));
-            if (err) {
-                snprintf(m->err, sizeof(m->err), "path builder: more than %d pending rays on one root ray", LOC_BUILD_STACK);
-                return LOC_ENOMEM;
-            }
-            if (total > m->stream_cap) {
-                snprintf(m->err, sizeof(m->err), "step stream needs %lld records, workspace holds %lld", total, (long long)m->stream_cap);
-                return LOC_ENOMEM;
-            }
-            m->stream_len = total;
-            m->setup_steps = (int64_t)steps;
-        }
-    }
-    LOC_CUDA_CHECK(m, cudaEventRecord(e1, m->stream));
-    LOC_CUDA_CHECK(m, cudaEventSynchronize(e1));
-    float ms = 0.f;
-    cudaEventElapsedTime(&ms, e0, e1);
-    m->setup_ms = ms;
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    return LOC_OK;
-}
-
-// ------------------------------------------------------------------------------------------------
-// radiative kernel
-// ------------------------------------------------------------------------------------------------
 struct Sim3D {
-    int nch, nsp, nslot;
+    int nch, nchp, nsp, nslot;
     float dv, xmin, eps_tau, inv_ndir;
     const Dir3 *dirs;
     const unsigned char *task_dir;
@@ -420,116 +41,299 @@ struct Sim3D {
     Selection S;
 };
 
-template <int NT, bool GEOM>
-__global__ void __launch_bounds__(128) k_sim3d(Sim3D P)
+// per-record scalars written by the prepare phase (32 bytes)
+struct __align__(16) RecPrep {
+    float cc;        // profile centre in channel units: v0 / dv + (nch - 1) / 2
+    float ky;        // dv sqrt(log2(e) / 2) / sigma :  phi = 2^(lamp - ((c - cc) ky)^2)
+    float lamp;      // log2(dv / (sigma sqrt(2 pi)))
+    float w;         // a s / V_eff = dzeta / (h NDIR)
+    unsigned cell;   // STEP: cell index; SAVE / LOAD: slot
+    unsigned opdz;   // opcode | level | dzeta (stream word)
+    int clo, chi;    // channel window of the step
+};
+
+// per (record, transition) coefficients (16 bytes): X_c = thin ? phi + c0 (B2 + c0 (B3 + c0 B4)) : 1 - 2^(c0 phi)
+//   n' = n + X (c1 + alpha n);  SJ += scale sum n X;  ESC += scale sum X
+struct __align__(16) TPrep {
+    float c0, c1, alpha, scale;
+};
+
+#define LOC_THIN_TAU 0.03f  // line-centre optical depth of a step below which the cubic series of (1-e^-t)/t is used
+
+template <int NT>
+__device__ __forceinline__ void prepare_record(const Sim3D &P, uint2 rec, float d0, float d1, float d2, float sf, RecPrep *rp, TPrep *tp,
+                                               unsigned &thickmask)
 {
-    constexpr int NV = 2 * NT + 1;
-    extern __shared__ float smem[];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
-    const int nch = P.nch;
-    const int per_warp = NT * nch + 4 * NT;
-    float *sn = smem + warp * per_warp;                           // photon occupation numbers [NT][nch]
-    TParam *s_tp = reinterpret_cast<TParam *>(sn + NT * nch);     // per-step transition parameters
-    float *slots = P.pool + ((long long)blockIdx.x * nwarp + warp) * (long long)P.nslot * NT * nch;
-    const float inv_dv = 1.0f / P.dv;
+    RecPrep r;
+    r.cell = rec.x;
+    r.opdz = rec.y;
+    r.cc = 0.f;
+    r.ky = 0.f;
+    r.lamp = 0.f;
+    r.w = 0.f;
+    r.clo = 0;
+    r.chi = -1;
+    thickmask = 0;
+    if ((rec.y >> 24) == LOC_OP_STEP) {
+        const float4 k = __ldg(P.kin + rec.x);
+        const float v0 = -(k.x * d0 + k.y * d1 + k.z * d2);  // DESIGN R6
+        const float sig = k.w;
+        const unsigned dz = rec.y & 0x1fffffu;
+        const int lev = (rec.y >> 21) & 7;
+        const float s = (float)dz * sf;
+        const float w = (float)dz * P.inv_ndir * __int_as_float((127 - LOC_LB + lev) << 23);
+        const float inv_sig = __fdividef(1.0f, sig);
+        const float amp = P.dv * 0.3989422804f * inv_sig;
+        const float2 *cf = P.coef + (long long)rec.x * P.nsp;
+        float tau0m = 0.f;
+#pragma unroll
+        for (int t = 0; t < NT; t++) {
+            const float2 ke = __ldg(cf + t);
+            const float ks = ke.x * s;
+            const float tau0 = fabsf(ks) * amp;
+            tau0m = fmaxf(tau0m, tau0);
+            TPrep q;
+            if (tau0 >= LOC_THIN_TAU) {
+                thickmask |= 1u << t;
+                q.c0 = -ks * LOC_LOG2E;
+                q.c1 = __fdividef(ke.y, ke.x);  // source function in occupation-number units
+                q.alpha = -1.0f;
+                q.scale = __fdividef(w, ks);
+            } else {
+                q.c0 = ks;
+                q.c1 = ke.y * s;
+                q.alpha = -ks;
+                q.scale = w;
+            }
+            tp[t] = q;
+        }
+        float X = P.xmin;
+        if (tau0m > P.eps_tau) X = fmaxf(X, sqrtf(2.0f * __logf(tau0m / P.eps_tau)));
+        const float inv_dv = __fdividef(1.0f, P.dv);
+        r.cc = fmaf(v0, inv_dv, 0.5f * (float)(P.nch - 1));
+        const float hw = X * sig * inv_dv;
+        r.clo = max(0, (int)ceilf(r.cc - hw));
+        r.chi = min(P.nch - 1, (int)floorf(r.cc + hw));
+        r.ky = P.dv * 0.8493218f * inv_sig;
+        r.lamp = __log2f(amp);
+        r.w = w;
+    }
+    *rp = r;
+}
+
+template <int NT, bool GEOM>
+__global__ void __launch_bounds__(32) k_sim3d(Sim3D P)
+{
+    constexpr int NV = 2 * NT;                 // reduced values per step: a[t], b[t]
+    constexpr int NPASS = (NV + 7) / 8;        // 8-lane butterflies of up to 8 values
+    extern __shared__ __align__(16) float smem[];
+    const int lane = threadIdx.x, grp = lane >> 3, l8 = lane & 7;
+    const int nchp = P.nchp;
+    const int spec = NT * nchp;                // floats per ray spectrum
+    float *sn_all = smem;                                                 // [4][NT][nchp]
+    TPrep *tp_all = reinterpret_cast<TPrep *>(smem + LOC_GROUPS * spec);  // [4][8][NT]
+    RecPrep *rp_all = reinterpret_cast<RecPrep *>(tp_all + LOC_GROUPS * LOC_CHUNK * NT);  // [4][8]
+    float *sn = sn_all + grp * spec;
+    TPrep *tpg = tp_all + grp * LOC_CHUNK * NT;
+    RecPrep *rpg = rp_all + grp * LOC_CHUNK;
+    float *slots_warp = P.pool + (long long)blockIdx.x * LOC_GROUPS * P.nslot * spec;
+
+    long long off = 0, end = 0;  // this group's position in the stream
+    bool done = false;
+    float d0 = 0.f, d1 = 0.f, d2 = 0.f, sf = 0.f;
     unsigned long long mysteps = 0, myactive = 0;
 
     for (;;) {
-        long long task = 0;
-        if (lane == 0) task = atomicAdd(P.queue, 1u);
-        task = __shfl_sync(0xffffffffu, task, 0);
-        if (task >= P.ntask) break;
-        const Dir3 *Dp = P.dirs + P.task_dir[task];
-        const float d0 = __ldg(&Dp->d[0]), d1 = __ldg(&Dp->d[1]), d2 = __ldg(&Dp->d[2]), sf = __ldg(&Dp->sf);
-        const long long off0 = __ldg(P.task_off + task), off1 = __ldg(P.task_off + task + 1);
-        for (long long base = off0; base < off1; base += 32) {
-            const long long idx = base + lane;
-            uint2 rec = make_uint2(0u, 7u << 24);
-            if (idx < off1) rec = __ldg(P.stream + idx);
-            float v0l = 0.f, sigl = 1.f;
-            if ((rec.y >> 24) == LOC_OP_STEP) {
-                const float4 k = __ldg(P.kin + rec.x);
-                v0l = -(k.x * d0 + k.y * d1 + k.z * d2);  // DESIGN R6
-                sigl = k.w;
-            }
-            const int cntr = (int)min(32ll, off1 - base);
-            for (int r = 0; r < cntr; r++) {
-                const unsigned x = __shfl_sync(0xffffffffu, rec.x, r), y = __shfl_sync(0xffffffffu, rec.y, r);
-                const unsigned op = y >> 24;
-                if (op == LOC_OP_STEP) {
-                    const long long cell = x;
-                    const unsigned dz = y & 0x1fffffu;
-                    const int lev = (y >> 21) & 7;
-                    const float v0 = __shfl_sync(0xffffffffu, v0l, r), sig = __shfl_sync(0xffffffffu, sigl, r);
-                    const float s = (float)dz * sf;
-                    const float w = (float)dz * P.inv_ndir * __int_as_float((127 - LOC_LB + lev) << 23);  // a s / V = dzeta / (h NDIR)
-                    const float amp = P.dv * 0.3989422804f / sig;
-                    float tau0 = 0.f;
-                    if (lane < NT) {
-                        const float2 ke = __ldg(P.coef + cell * P.nsp + lane);
-                        s_tp[lane] = make_tparam(ke, s, w, amp);
-                        tau0 = fabsf(ke.x * s) * amp;
-                    }
-                    const float tau0m = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(tau0)));
-                    __syncwarp();
-                    float X = P.xmin;
-                    if (tau0m > P.eps_tau) X = fmaxf(X, sqrtf(2.0f * __logf(tau0m / P.eps_tau)));
-                    const float cc = v0 * inv_dv + 0.5f * (float)(nch - 1);
-                    const float hw = X * sig * inv_dv;
-                    const int c_lo = max(0, (int)ceilf(cc - hw)), c_hi = min(nch - 1, (int)floorf(cc + hw));
-                    const float ky = 0.8493218f / sig;  // sqrt(log2(e)/2) / sigma
-                    const float lamp = __log2f(amp);
-                    float v[NV];
-#pragma unroll
-                    for (int i = 0; i < NV; i++) v[i] = 0.f;
-                    for (int cb = c_lo; cb <= c_hi; cb += 32) {
-                        const int c = cb + lane;
-                        const bool act = c <= c_hi;
-                        const float yv = (((float)c - 0.5f * (float)(nch - 1)) * P.dv - v0) * ky;
-                        const float phi = act ? ex2f(fmaf(-yv, yv, lamp)) : 0.0f;
-                        if (act) {
-#pragma unroll
-                            for (int t = 0; t < NT; t++) {
-                                const TParam tp = s_tp[t];
-                                float n = sn[t * nch + c];
-                                channel_update(n, phi, tp, v[t], v[NT + t]);
-                                sn[t * nch + c] = n;
-                            }
-                        }
-                        v[2 * NT] += phi;
-                    }
-                    int owner;
-                    const float tot = warp_multi_reduce<NV>(v, lane, owner);
-                    const unsigned mphi = __ballot_sync(0xffffffffu, owner == 2 * NT);
-                    const float sphi = __shfl_sync(0xffffffffu, tot, __ffs(mphi) - 1);
-                    if (owner >= 0 && owner < NT)
-                        atomicAdd(&P.cnt[cell * P.nsp + owner].x, tot * s_tp[owner].scale);
-                    else if (owner >= NT && owner < 2 * NT)
-                        atomicAdd(&P.cnt[cell * P.nsp + (owner - NT)].y, fmaf(tot, s_tp[owner - NT].scale, w - w * sphi));
-                    if (GEOM && lane == 0) {
-                        atomicAdd(&P.visits[cell], 1u);
-                        atomicAdd(&P.pathz[cell], dz);
-                        const float h5 = 5.0f * sig * inv_dv;
-                        myactive += max(0, min(nch - 1, (int)floorf(cc + h5)) - max(0, (int)ceilf(cc - h5)) + 1);
-                    }
-                    mysteps++;
-                    __syncwarp();
-                } else if (op == LOC_OP_BG) {
-#pragma unroll
-                    for (int t = 0; t < NT; t++)
-                        for (int c = lane; c < nch; c += 32) sn[t * nch + c] = P.S.bgocc[t];
-                    __syncwarp();
-                } else if (op == LOC_OP_SAVE) {
-                    float *dst = slots + (long long)x * NT * nch;
-                    for (int i = lane; i < NT * nch; i += 32) dst[i] = sn[i];
-                    __syncwarp();
-                } else if (op == LOC_OP_LOAD) {
-                    const float *src = slots + (long long)x * NT * nch;
-                    for (int i = lane; i < NT * nch; i += 32) sn[i] = src[i];
-                    __syncwarp();
+        // ---- refill: groups whose task is exhausted take the next root ray from the queue ----
+        {
+            const bool need = !done && off >= end;
+            long long task = 0;
+            if (need && l8 == 0) task = atomicAdd(P.queue, 1u);
+            task = __shfl_sync(0xffffffffu, task, grp * 8);
+            if (need) {
+                if (task >= P.ntask) {
+                    done = true;
+                } else {
+                    const Dir3 *Dp = P.dirs + P.task_dir[task];
+                    d0 = __ldg(&Dp->d[0]);
+                    d1 = __ldg(&Dp->d[1]);
+                    d2 = __ldg(&Dp->d[2]);
+                    sf = __ldg(&Dp->sf);
+                    off = __ldg(P.task_off + task);
+                    end = __ldg(P.task_off + task + 1);
                 }
             }
         }
+        __syncwarp();
+        if (__all_sync(0xffffffffu, done)) break;
+        // ---- prepare: lane l8 of each group decodes record off + l8 of its ray ----
+        uint2 rec = make_uint2(0u, LOC_OP_NOP << 24);
+        if (!done && off + l8 < end) rec = __ldg(P.stream + off + l8);
+        unsigned thick_l;
+        prepare_record<NT>(P, rec, d0, d1, d2, sf, rpg + l8, tpg + l8 * NT, thick_l);
+        off += LOC_CHUNK;
+        __syncwarp();
+
+        // ---- 8 rounds: every group consumes one record per round ----
+        for (int r = 0; r < LOC_CHUNK; r++) {
+            const RecPrep rp = rpg[r];
+            const unsigned op = rp.opdz >> 24;
+            const unsigned thick = __shfl_sync(0xffffffffu, thick_l, grp * 8 + r);
+            // spectrum operations, executed by the whole warp for one group at a time
+            unsigned ctrl = __ballot_sync(0xffffffffu, op == LOC_OP_BG || op == LOC_OP_SAVE || op == LOC_OP_LOAD) & 0x01010101u;
+            while (ctrl) {
+                const int g = (__ffs(ctrl) - 1) >> 3;
+                ctrl &= ctrl - 1;
+                const unsigned gop = __shfl_sync(0xffffffffu, op, g * 8), gx = __shfl_sync(0xffffffffu, rp.cell, g * 8);
+                float *gs = sn_all + g * spec;
+                float *slot = slots_warp + ((long long)g * P.nslot + gx) * spec;
+                if (gop == LOC_OP_BG) {
+#pragma unroll
+                    for (int t = 0; t < NT; t++) {
+                        const float b = P.S.bgocc[t];
+                        for (int c = lane; c < nchp; c += 32) gs[t * nchp + c] = b;
+                    }
+                } else if (gop == LOC_OP_SAVE) {
+                    for (int i = lane * 4; i < spec; i += 128) *reinterpret_cast<float4 *>(slot + i) = *reinterpret_cast<const float4 *>(gs + i);
+                } else {
+                    for (int i = lane * 4; i < spec; i += 128) *reinterpret_cast<float4 *>(gs + i) = *reinterpret_cast<const float4 *>(slot + i);
+                }
+                __syncwarp();
+            }
+            const bool step = op == LOC_OP_STEP;
+            const unsigned anystep = __ballot_sync(0xffffffffu, step);
+            if (!anystep) continue;
+            const unsigned any_thick = __reduce_or_sync(0xffffffffu, step ? thick : 0u);
+            const unsigned any_thin = __reduce_or_sync(0xffffffffu, step ? ~thick : 0u);
+
+            float a[NT], b[NT];
+#pragma unroll
+            for (int t = 0; t < NT; t++) a[t] = b[t] = 0.f;
+            float sphi = 0.f;
+            const TPrep *tpr = tpg + r * NT;
+            // passes of 32 channels over the window (one pass unless the window is wider than 32 - alignment)
+            int cb = (rp.clo & ~3) + 4 * l8;
+            int chi = step ? rp.chi : -1;
+            while (__any_sync(0xffffffffu, cb - 4 * l8 <= chi)) {
+                float phi[4], B2[4], B3[4], B4[4];
+#pragma unroll
+                for (int k = 0; k < 4; k++) {
+                    const int c = cb + k;
+                    const float y = ((float)c - rp.cc) * rp.ky;
+                    const float e = ex2f(fmaf(-y, y, rp.lamp));
+                    phi[k] = (c >= rp.clo && c <= chi) ? e : 0.0f;
+                    sphi += phi[k];
+                    const float p2 = phi[k] * phi[k];
+                    B2[k] = -0.5f * p2;
+                    B3[k] = (1.0f / 6.0f) * p2 * phi[k];
+                    B4[k] = (-1.0f / 24.0f) * p2 * p2;
+                }
+                const bool inb = cb < nchp && cb <= chi;
+#pragma unroll
+                for (int t = 0; t < NT; t++) {
+                    const TPrep q = tpr[t];
+                    float4 n4 = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (inb) n4 = *reinterpret_cast<const float4 *>(sn + t * nchp + cb);
+                    float nn[4] = {n4.x, n4.y, n4.z, n4.w};
+                    const bool tk = (thick >> t) & 1u;
+                    if (!((any_thick >> t) & 1u)) {  // every ray of the warp is thin in this transition
+#pragma unroll
+                        for (int k = 0; k < 4; k++) {
+                            const float X = fmaf(q.c0, fmaf(q.c0, fmaf(q.c0, B4[k], B3[k]), B2[k]), phi[k]);
+                            a[t] = fmaf(nn[k], X, a[t]);
+                            b[t] += X;
+                            nn[k] = fmaf(X, fmaf(q.alpha, nn[k], q.c1), nn[k]);
+                        }
+                    } else if (!((any_thin >> t) & 1u)) {  // every ray is thick
+#pragma unroll
+                        for (int k = 0; k < 4; k++) {
+                            const float X = 1.0f - ex2f(q.c0 * phi[k]);
+                            a[t] = fmaf(nn[k], X, a[t]);
+                            b[t] += X;
+                            nn[k] = fmaf(X, fmaf(q.alpha, nn[k], q.c1), nn[k]);
+                        }
+                    } else {  // mixed: both forms, selected per ray
+#pragma unroll
+                        for (int k = 0; k < 4; k++) {
+                            const float Xs = fmaf(q.c0, fmaf(q.c0, fmaf(q.c0, B4[k], B3[k]), B2[k]), phi[k]);
+                            const float Xe = 1.0f - ex2f(q.c0 * phi[k]);
+                            const float X = tk ? Xe : Xs;
+                            a[t] = fmaf(nn[k], X, a[t]);
+                            b[t] += X;
+                            nn[k] = fmaf(X, fmaf(q.alpha, nn[k], q.c1), nn[k]);
+                        }
+                    }
+                    if (inb) *reinterpret_cast<float4 *>(sn + t * nchp + cb) = make_float4(nn[0], nn[1], nn[2], nn[3]);
+                }
+                cb += 32;
+            }
+            // ---- reductions over the 8 lanes of each group ----
+            sphi += __shfl_xor_sync(0xffffffffu, sphi, 4);
+            sphi += __shfl_xor_sync(0xffffffffu, sphi, 2);
+            sphi += __shfl_xor_sync(0xffffffffu, sphi, 1);
+            float v[NPASS * 8];
+#pragma unroll
+            for (int i = 0; i < NPASS * 8; i++) v[i] = 0.f;
+#pragma unroll
+            for (int t = 0; t < NT; t++) {
+                v[t] = a[t];
+                v[NT + t] = b[t];
+            }
+            float tot[NPASS];
+#pragma unroll
+            for (int p = 0; p < NPASS; p++) {
+                float *u = v + 8 * p;
+                {
+                    const bool up = l8 & 4;
+#pragma unroll
+                    for (int i = 0; i < 4; i++) {
+                        const float keep = up ? u[i + 4] : u[i], send = up ? u[i] : u[i + 4];
+                        u[i] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+                    }
+                }
+                {
+                    const bool up = l8 & 2;
+#pragma unroll
+                    for (int i = 0; i < 2; i++) {
+                        const float keep = up ? u[i + 2] : u[i], send = up ? u[i] : u[i + 2];
+                        u[i] = keep + __shfl_xor_sync(0xffffffffu, send, 2);
+                    }
+                }
+                {
+                    const bool up = l8 & 1;
+                    const float keep = up ? u[1] : u[0], send = up ? u[0] : u[1];
+                    tot[p] = keep + __shfl_xor_sync(0xffffffffu, send, 1);
+                }
+            }
+            // lane l8 of a group now holds the group totals of values 4*bit2 + 2*bit1 + bit0 ... = l8, 8 + l8, 16 + l8
+            if (step) {
+                float2 *cn = P.cnt + (long long)rp.cell * P.nsp;
+                const float wesc = rp.w - rp.w * sphi;  // photons emitted outside the window escape (DESIGN 5.3)
+#pragma unroll
+                for (int p = 0; p < NPASS; p++) {
+                    const int i = 8 * p + l8;
+                    if (i < NT)
+                        atomicAdd(&cn[i].x, tot[p] * tpr[i].scale);
+                    else if (i < NV)
+                        atomicAdd(&cn[i - NT].y, fmaf(tot[p], tpr[i - NT].scale, wesc));
+                }
+                if (l8 == 0) {
+                    mysteps++;
+                    if (GEOM) {
+                        atomicAdd(&P.visits[rp.cell], 1u);
+                        atomicAdd(&P.pathz[rp.cell], rp.opdz & 0x1fffffu);
+                        const float h5 = 5.0f * 0.8493218f / rp.ky;  // 5 sigma in channels
+                        myactive += max(0, min(P.nch - 1, (int)floorf(rp.cc + h5)) - max(0, (int)ceilf(rp.cc - h5)) + 1);
+                    }
+                }
+            }
+            __syncwarp();
+        }
+    }
+    // per-warp totals
+    for (int o = 16; o >= 1; o >>= 1) {
+        mysteps += __shfl_xor_sync(0xffffffffu, mysteps, o);
+        myactive += __shfl_xor_sync(0xffffffffu, myactive, o);
     }
     if (lane == 0 && mysteps) atomicAdd(P.nsteps, mysteps);
     if (GEOM && lane == 0 && myactive) atomicAdd(P.nsteps + 1, myactive);
@@ -538,28 +342,25 @@ __global__ void __launch_bounds__(128) k_sim3d(Sim3D P)
 template <int NT>
 static int launch3d(loc_model *m, Sim3D &P, int geom)
 {
-    // warps per block so that the per-warp spectra fit comfortably in shared memory
-    const size_t per_warp = sizeof(float) * ((size_t)NT * m->nch + 4 * NT);
-    int nwarp = 4;
-    while (nwarp > 1 && per_warp * nwarp > 96 * 1024) nwarp >>= 1;
-    const size_t smem = per_warp * nwarp;
-    if (smem > 200 * 1024) {
-        snprintf(m->err, sizeof(m->err), "nchannel * ntrans too large for the shared-memory spectrum (%zu bytes)", smem);
+    const size_t smem = sizeof(float) * LOC_GROUPS * NT * P.nchp + sizeof(TPrep) * LOC_GROUPS * LOC_CHUNK * NT +
+                        sizeof(RecPrep) * LOC_GROUPS * LOC_CHUNK;
+    if (smem > 220 * 1024) {
+        snprintf(m->err, sizeof(m->err), "nchannel * ntrans too large for the shared-memory spectra (%zu bytes per warp)", smem);
         return LOC_EINVAL;
     }
     auto kern = geom ? k_sim3d<NT, true> : k_sim3d<NT, false>;
     LOC_CUDA_CHECK(m, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int bps = 0;
-    LOC_CUDA_CHECK(m, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kern, nwarp * 32, smem));
+    LOC_CUDA_CHECK(m, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kern, 32, smem));
     if (bps < 1) bps = 1;
     int nsm = 148;
     cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, 0);
     long long blocks = (long long)nsm * bps;
-    blocks = std::min<long long>(blocks, (m->ntask + nwarp - 1) / nwarp);
-    blocks = std::min<long long>(blocks, m->max_warps / nwarp);
+    blocks = std::min<long long>(blocks, (m->ntask + LOC_GROUPS - 1) / LOC_GROUPS);
+    blocks = std::min<long long>(blocks, m->max_warps);
     if (blocks < 1) blocks = 1;
     LOC_CUDA_CHECK(m, cudaMemsetAsync(m->d_queue, 0, sizeof(unsigned int), m->stream));
-    kern<<<(unsigned)blocks, nwarp * 32, smem, m->stream>>>(P);
+    kern<<<(unsigned)blocks, 32, smem, m->stream>>>(P);
     m->launches++;
     LOC_CUDA_CHECK(m, cudaGetLastError());
     return LOC_OK;
@@ -569,6 +370,7 @@ int loc_launch_sim3d(loc_model *m, int geom)
 {
     Sim3D P;
     P.nch = m->nch;
+    P.nchp = (m->nch + 3) & ~3;
     P.nsp = m->selh.nsp;
     P.nslot = std::max(m->nlev - 1, 1);
     P.dv = (float)m->dv;
