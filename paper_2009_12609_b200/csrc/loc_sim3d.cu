@@ -22,6 +22,7 @@
 
 #define LOC_GROUPS 4  // rays per warp
 #define LOC_CHUNK 8   // records per group and prepare phase (= LOC_TASK_ALIGN)
+#define LOC_PASS 40   // channels per pass: 8 lanes x (one aligned float4 + one scalar)
 
 struct Sim3D {
     int nch, nchp, nsp, nslot;
@@ -58,6 +59,7 @@ struct __align__(16) TPrep {
     float c0, c1, alpha, scale;
 };
 
+#define LOC_XCLIP 4.0f       // the window may be clipped to one 32-channel pass only outside +-4 sigma
 #define LOC_THIN_TAU 0.03f  // line-centre optical depth of a step below which the cubic series of (1-e^-t)/t is used
 
 template <int NT>
@@ -107,13 +109,33 @@ __device__ __forceinline__ void prepare_record(const Sim3D &P, uint2 rec, float 
             }
             tp[t] = q;
         }
+        // window half-width in sigma: the profile mass left outside stays a fixed fraction (that of xmin at tau0 <= 1) of
+        // the escape sum  sum_c phi_c f(tau_c) ~ 1/tau0  of an optically thick step (DESIGN 5.3)
         float X = P.xmin;
-        if (tau0m > P.eps_tau) X = fmaxf(X, sqrtf(2.0f * __logf(tau0m / P.eps_tau)));
+        if (tau0m > 1.0f) X = sqrtf(fmaf(2.0f, __logf(tau0m), X * X));
         const float inv_dv = __fdividef(1.0f, P.dv);
         r.cc = fmaf(v0, inv_dv, 0.5f * (float)(P.nch - 1));
         const float hw = X * sig * inv_dv;
-        r.clo = max(0, (int)ceilf(r.cc - hw));
-        r.chi = min(P.nch - 1, (int)floorf(r.cc + hw));
+        int clo = max(0, (int)ceilf(r.cc - hw)), chi = min(P.nch - 1, (int)floorf(r.cc + hw));
+        // One pass of the kernel covers LOC_PASS = 40 channels starting at a multiple of 4.  If the window overshoots that by a few
+        // channels, drop the outermost ones (never closer than LOC_XCLIP sigma to the line centre) instead of paying a
+        // second pass; their profile mass is booked as escaping like everything outside the window (DESIGN 5.3).
+        {
+            const float lim = LOC_XCLIP * sig * inv_dv;
+            int lo = clo, hi = chi;
+#pragma unroll
+            for (int i = 0; i < 3; i++) {
+                if ((lo & 3) + (hi - lo + 1) <= LOC_PASS) break;
+                if (r.cc - (float)lo > (float)hi - r.cc) lo++;
+                else hi--;
+            }
+            if ((lo & 3) + (hi - lo + 1) <= LOC_PASS && r.cc - (float)lo >= lim && (float)hi - r.cc >= lim) {
+                clo = lo;
+                chi = hi;
+            }
+        }
+        r.clo = clo;
+        r.chi = chi;
         r.ky = P.dv * 0.8493218f * inv_sig;
         r.lamp = __log2f(amp);
         r.w = w;
@@ -130,9 +152,9 @@ __global__ void __launch_bounds__(32) k_sim3d(Sim3D P)
     const int lane = threadIdx.x, grp = lane >> 3, l8 = lane & 7;
     const int nchp = P.nchp;
     const int spec = NT * nchp;                // floats per ray spectrum
-    float *sn_all = smem;                                                 // [4][NT][nchp]
-    TPrep *tp_all = reinterpret_cast<TPrep *>(smem + LOC_GROUPS * spec);  // [4][8][NT]
-    RecPrep *rp_all = reinterpret_cast<RecPrep *>(tp_all + LOC_GROUPS * LOC_CHUNK * NT);  // [4][8]
+    float *sn_all = smem;                                  // [4][NT][nchp]
+    __shared__ TPrep tp_all[LOC_GROUPS * LOC_CHUNK * NT];    // [4][8][NT]   (separate objects: no aliasing with the spectra)
+    __shared__ RecPrep rp_all[LOC_GROUPS * LOC_CHUNK];       // [4][8]
     float *sn = sn_all + grp * spec;
     TPrep *tpg = tp_all + grp * LOC_CHUNK * NT;
     RecPrep *rpg = rp_all + grp * LOC_CHUNK;
@@ -211,14 +233,16 @@ __global__ void __launch_bounds__(32) k_sim3d(Sim3D P)
             for (int t = 0; t < NT; t++) a[t] = b[t] = 0.f;
             float sphi = 0.f;
             const TPrep *tpr = tpg + r * NT;
-            // passes of 32 channels over the window (one pass unless the window is wider than 32 - alignment)
-            int cb = (rp.clo & ~3) + 4 * l8;
-            int chi = step ? rp.chi : -1;
-            while (__any_sync(0xffffffffu, cb - 4 * l8 <= chi)) {
-                float phi[4], B2[4], B3[4], B4[4];
+            // passes of 40 channels over the window (one pass unless the line is very thick): lane l8 owns the aligned
+            // float4 at wb + 4 l8 and the single channel wb + 32 + l8
+            int wb = rp.clo & ~3;
+            const int chi = step ? rp.chi : -1;
+            while (__any_sync(0xffffffffu, wb <= chi)) {
+                const int cb = wb + 4 * l8, ce = wb + 32 + l8;
+                float phi[5], B2[5], B3[5], B4[5];
 #pragma unroll
-                for (int k = 0; k < 4; k++) {
-                    const int c = cb + k;
+                for (int k = 0; k < 5; k++) {
+                    const int c = (k < 4) ? cb + k : ce;
                     const float y = ((float)c - rp.cc) * rp.ky;
                     const float e = ex2f(fmaf(-y, y, rp.lamp));
                     phi[k] = (c >= rp.clo && c <= chi) ? e : 0.0f;
@@ -228,44 +252,57 @@ __global__ void __launch_bounds__(32) k_sim3d(Sim3D P)
                     B3[k] = (1.0f / 6.0f) * p2 * phi[k];
                     B4[k] = (-1.0f / 24.0f) * p2 * p2;
                 }
-                const bool inb = cb < nchp && cb <= chi;
+                const bool inb = cb <= chi;            // chi < nch <= nchp and cb is a multiple of 4: the float4 is in range
+                const bool ine = ce <= chi;
+                float nn[NT][5];
+#pragma unroll
+                for (int t = 0; t < NT; t++) {
+                    float4 n4 = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (inb) n4 = *reinterpret_cast<const float4 *>(sn + t * nchp + cb);
+                    nn[t][0] = n4.x;
+                    nn[t][1] = n4.y;
+                    nn[t][2] = n4.z;
+                    nn[t][3] = n4.w;
+                    nn[t][4] = ine ? sn[t * nchp + ce] : 0.f;
+                }
 #pragma unroll
                 for (int t = 0; t < NT; t++) {
                     const TPrep q = tpr[t];
-                    float4 n4 = make_float4(0.f, 0.f, 0.f, 0.f);
-                    if (inb) n4 = *reinterpret_cast<const float4 *>(sn + t * nchp + cb);
-                    float nn[4] = {n4.x, n4.y, n4.z, n4.w};
                     const bool tk = (thick >> t) & 1u;
                     if (!((any_thick >> t) & 1u)) {  // every ray of the warp is thin in this transition
 #pragma unroll
-                        for (int k = 0; k < 4; k++) {
+                        for (int k = 0; k < 5; k++) {
                             const float X = fmaf(q.c0, fmaf(q.c0, fmaf(q.c0, B4[k], B3[k]), B2[k]), phi[k]);
-                            a[t] = fmaf(nn[k], X, a[t]);
+                            a[t] = fmaf(nn[t][k], X, a[t]);
                             b[t] += X;
-                            nn[k] = fmaf(X, fmaf(q.alpha, nn[k], q.c1), nn[k]);
+                            nn[t][k] = fmaf(X, fmaf(q.alpha, nn[t][k], q.c1), nn[t][k]);
                         }
                     } else if (!((any_thin >> t) & 1u)) {  // every ray is thick
 #pragma unroll
-                        for (int k = 0; k < 4; k++) {
+                        for (int k = 0; k < 5; k++) {
                             const float X = 1.0f - ex2f(q.c0 * phi[k]);
-                            a[t] = fmaf(nn[k], X, a[t]);
+                            a[t] = fmaf(nn[t][k], X, a[t]);
                             b[t] += X;
-                            nn[k] = fmaf(X, fmaf(q.alpha, nn[k], q.c1), nn[k]);
+                            nn[t][k] = fmaf(X, fmaf(q.alpha, nn[t][k], q.c1), nn[t][k]);
                         }
                     } else {  // mixed: both forms, selected per ray
 #pragma unroll
-                        for (int k = 0; k < 4; k++) {
+                        for (int k = 0; k < 5; k++) {
                             const float Xs = fmaf(q.c0, fmaf(q.c0, fmaf(q.c0, B4[k], B3[k]), B2[k]), phi[k]);
                             const float Xe = 1.0f - ex2f(q.c0 * phi[k]);
                             const float X = tk ? Xe : Xs;
-                            a[t] = fmaf(nn[k], X, a[t]);
+                            a[t] = fmaf(nn[t][k], X, a[t]);
                             b[t] += X;
-                            nn[k] = fmaf(X, fmaf(q.alpha, nn[k], q.c1), nn[k]);
+                            nn[t][k] = fmaf(X, fmaf(q.alpha, nn[t][k], q.c1), nn[t][k]);
                         }
                     }
-                    if (inb) *reinterpret_cast<float4 *>(sn + t * nchp + cb) = make_float4(nn[0], nn[1], nn[2], nn[3]);
                 }
-                cb += 32;
+#pragma unroll
+                for (int t = 0; t < NT; t++) {
+                    if (inb) *reinterpret_cast<float4 *>(sn + t * nchp + cb) = make_float4(nn[t][0], nn[t][1], nn[t][2], nn[t][3]);
+                    if (ine) sn[t * nchp + ce] = nn[t][4];
+                }
+                wb += LOC_PASS;
             }
             // ---- reductions over the 8 lanes of each group ----
             sphi += __shfl_xor_sync(0xffffffffu, sphi, 4);
@@ -342,8 +379,7 @@ __global__ void __launch_bounds__(32) k_sim3d(Sim3D P)
 template <int NT>
 static int launch3d(loc_model *m, Sim3D &P, int geom)
 {
-    const size_t smem = sizeof(float) * LOC_GROUPS * NT * P.nchp + sizeof(TPrep) * LOC_GROUPS * LOC_CHUNK * NT +
-                        sizeof(RecPrep) * LOC_GROUPS * LOC_CHUNK;
+    const size_t smem = sizeof(float) * LOC_GROUPS * NT * P.nchp;  // + static: TPrep / RecPrep tables
     if (smem > 220 * 1024) {
         snprintf(m->err, sizeof(m->err), "nchannel * ntrans too large for the shared-memory spectra (%zu bytes per warp)", smem);
         return LOC_EINVAL;
