@@ -44,7 +44,7 @@ static int64_t carve(loc_model *m, Carver &c, const loc_grid *g, int nch, int nl
     m->cnt = c.take<float2>(ncell * nsp);
     m->visits = c.take<uint32_t>(ncell);
     m->pathz = c.take<uint32_t>(ncell);
-    m->d_steps = c.take<unsigned long long>(2);  // [0] steps, [1] active channels (5 sigma rule)
+    m->d_steps = c.take<unsigned long long>(4);  // [0] steps, [1] active channels (5 sigma rule), [2..3] scratch
     m->d_maxrel = c.take<unsigned int>(1);
     m->d_errflag = c.take<int>(1);
     m->d_queue = c.take<unsigned int>(1);

@@ -15,6 +15,7 @@
 // whole chunks of 8 records by the path builder); the rare spectrum operations (background, save, load) are executed
 // by the whole warp for the group that needs them.
 #include <stdio.h>
+#include <stdlib.h>
 
 #include <algorithm>
 
@@ -26,6 +27,7 @@
 
 struct Sim3D {
     int nch, nchp, nsp, nslot;
+    int slot0;  // first counter / coefficient slot handled by this launch (transitions may be split over launches)
     float dv, xmin, eps_tau, inv_ndir;
     const Dir3 *dirs;
     const unsigned char *task_dir;
@@ -86,7 +88,7 @@ __device__ __forceinline__ void prepare_record(const Sim3D &P, uint2 rec, float 
         const float w = (float)dz * P.inv_ndir * __int_as_float((127 - LOC_LB + lev) << 23);
         const float inv_sig = __fdividef(1.0f, sig);
         const float amp = P.dv * 0.3989422804f * inv_sig;
-        const float2 *cf = P.coef + (long long)rec.x * P.nsp;
+        const float2 *cf = P.coef + (long long)rec.x * P.nsp + P.slot0;
         float tau0m = 0.f;
 #pragma unroll
         for (int t = 0; t < NT; t++) {
@@ -212,7 +214,7 @@ __global__ void __launch_bounds__(32) k_sim3d(Sim3D P)
                 if (gop == LOC_OP_BG) {
 #pragma unroll
                     for (int t = 0; t < NT; t++) {
-                        const float b = P.S.bgocc[t];
+                        const float b = P.S.bgocc[P.slot0 + t];
                         for (int c = lane; c < nchp; c += 32) gs[t * nchp + c] = b;
                     }
                 } else if (gop == LOC_OP_SAVE) {
@@ -344,7 +346,7 @@ __global__ void __launch_bounds__(32) k_sim3d(Sim3D P)
             }
             // lane l8 of a group now holds the group totals of values 4*bit2 + 2*bit1 + bit0 ... = l8, 8 + l8, 16 + l8
             if (step) {
-                float2 *cn = P.cnt + (long long)rp.cell * P.nsp;
+                float2 *cn = P.cnt + (long long)rp.cell * P.nsp + P.slot0;
                 const float wesc = rp.w - rp.w * sphi;  // photons emitted outside the window escape (DESIGN 5.3)
 #pragma unroll
                 for (int p = 0; p < NPASS; p++) {
@@ -427,13 +429,32 @@ int loc_launch_sim3d(loc_model *m, int geom)
     P.queue = m->d_queue;
     P.pool = m->spec_pool;
     P.S = m->selh;
-    switch (m->selh.nsel) {
-#define C3(N) \
-    case N:   \
-        return launch3d<N>(m, P, geom);
-        C3(1) C3(2) C3(3) C3(4) C3(5) C3(6) C3(7) C3(8) C3(9) C3(10) C3(11) C3(12)
+    // Transitions are traced in `npart` launches of nearly equal size: the per-ray spectra of one launch then need less
+    // shared memory, so more rays are in flight per SM (latency hiding), at the price of repeating the per-step scalar
+    // work once per launch.  Default: parts of at most 5 transitions.
+    int nsel = m->selh.nsel;
+    int npart = (nsel + 4) / 5;
+    if (getenv("LOC_SIM3D_PARTS")) npart = std::max(1, std::min(nsel, atoi(getenv("LOC_SIM3D_PARTS"))));
+    int slot = 0;
+    for (int part = 0; part < npart; part++) {
+        int n = (nsel - slot + (npart - part) - 1) / (npart - part);
+        P.slot0 = slot;
+        int rc = LOC_EINVAL;
+        // the step / active-channel statistics are taken by the first part only
+        int g = geom && part == 0;
+        unsigned long long *keep = P.nsteps;
+        if (part > 0) P.nsteps = m->d_steps + 2;  // scratch slot
+        switch (n) {
+#define C3(N)                        \
+    case N:                          \
+        rc = launch3d<N>(m, P, g);   \
+        break;
+            C3(1) C3(2) C3(3) C3(4) C3(5) C3(6) C3(7) C3(8) C3(9) C3(10) C3(11) C3(12)
 #undef C3
+        }
+        P.nsteps = keep;
+        if (rc != LOC_OK) return rc;
+        slot += n;
     }
-    snprintf(m->err, sizeof(m->err), "unsupported number of traced transitions %d", m->selh.nsel);
-    return LOC_EINVAL;
+    return LOC_OK;
 }
