@@ -72,6 +72,7 @@ static int64_t carve(loc_model *m, Carver &c, const loc_grid *g, int nch, int nl
         m->d_tabs = c.take<float>(ntab);
         m->d_tabmu = c.take<float>(ntab);
         m->d_tabw = c.take<float>(ntab);
+        m->d_rout = c.take<double>(g->nshell);
     } else {
         // root-line tasks: at most max(face) lines per direction
         int64_t face = std::max((int64_t)g->nx * g->ny, std::max((int64_t)g->ny * g->nz, (int64_t)g->nx * g->nz));
@@ -434,6 +435,7 @@ extern "C" int loc_create_model(const loc_grid *g, const loc_cells *cells, int n
         H2D(m->d_tabs, tabs.data(), sizeof(float) * tabs.size());
         H2D(m->d_tabmu, tabmu.data(), sizeof(float) * tabmu.size());
         H2D(m->d_tabw, tabw.data(), sizeof(float) * tabw.size());
+        H2D(m->d_rout, g->r_out, sizeof(double) * ns);
         cudaStreamSynchronize(m->stream);  // host vectors go out of scope
     } else {
         m->nx = g->nx;

@@ -109,6 +109,7 @@ struct loc_model {
     long long *d_off;
     float *d_tabs, *d_tabmu, *d_tabw;
     double *h_rout;
+    double *d_rout;  // device copy of the shell radii (1D spectra)
     int64_t steps1d;
     // 3D
     int nx, ny, nz, nlev;
@@ -245,6 +246,79 @@ __device__ __forceinline__ float warp_multi_reduce(float (&v)[NV], int lane, int
     MultiReduce<NV, 16>::run(v, lane, base, nvalid);
     owner = (nvalid >= 1) ? base : -1;
     return v[0];
+}
+
+// ------------------------------------------------------------------------------------------------
+// integer lattice helpers (device)
+// ------------------------------------------------------------------------------------------------
+struct Tree {
+    int nx, ny, nz, nlev;
+    long long noff[LOC_MAXL + 1];
+    const int32_t *child;
+};
+
+#define LOC_ZINF (1ll << 40)
+
+__device__ __forceinline__ long long shift_of(unsigned long long T, long long z)
+{
+    return T ? (long long)(((unsigned long long)z << 32) / T) : 0ll;
+}
+
+// smallest zeta with shift_of(T, zeta) >= D
+__device__ __forceinline__ long long cross_of(unsigned long long T, long long D)
+{
+    if (D <= 0) return 0;
+    if (T == 0) return LOC_ZINF;
+    unsigned long long lo = (unsigned long long)D * T, hi = __umul64hi((unsigned long long)D, T);
+    unsigned long long lo2 = lo + 0xffffffffull;
+    if (lo2 < lo) hi++;
+    return (long long)((hi << 32) | (lo2 >> 32));
+}
+
+__device__ __forceinline__ long long floordiv(long long a, long long b) { return (a >= 0) ? a / b : -((-a + b - 1) / b); }
+
+struct LeafPos {
+    int cell[LOC_MAXL];  // global cell index of the ancestor at each level (last = the leaf)
+    int level;
+};
+
+// leaf containing the working-frame point (fz, fp, fq), all coordinates inside the model
+__device__ __forceinline__ void find_leaf(const Tree &G, const Dir3 &D, int fz, int fp, int fq, LeafPos &L)
+{
+    int X[3];
+    X[D.ax[0]] = D.flip[0] ? D.W[0] - 1 - fz : fz;
+    X[D.ax[1]] = D.flip[1] ? D.W[1] - 1 - fp : fp;
+    X[D.ax[2]] = D.flip[2] ? D.W[2] - 1 - fq : fq;
+    int g = (X[0] >> LOC_LB) + G.nx * ((X[1] >> LOC_LB) + G.ny * (X[2] >> LOC_LB));
+    int l = 0;
+    L.cell[0] = g;
+    int ch;
+    while ((ch = __ldg(G.child + g)) >= 0) {
+        int bit = LOC_LB - 1 - l;
+        g = (int)G.noff[l + 1] + ch + ((X[0] >> bit) & 1) + 2 * ((X[1] >> bit) & 1) + 4 * ((X[2] >> bit) & 1);
+        l++;
+        L.cell[l] = g;
+    }
+    L.level = l;
+}
+
+__device__ __forceinline__ int level_at(const Tree &G, const Dir3 &D, int fz, int fp, int fq)
+{
+    LeafPos L;
+    find_leaf(G, D, fz, fp, fq, L);
+    return L.level;
+}
+
+static inline Tree make_tree(const loc_model *m)
+{
+    Tree G;
+    G.nx = m->nx;
+    G.ny = m->ny;
+    G.nz = m->nz;
+    G.nlev = m->nlev;
+    for (int l = 0; l <= LOC_MAXL; l++) G.noff[l] = (l <= m->nlev) ? m->noff[l] : m->noff[m->nlev];
+    G.child = m->child;
+    return G;
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -1,11 +1,222 @@
-// loc_spectra.cu -- spectral-line map kernel.  Placeholder until the map kernels land.
+// loc_spectra.cu -- spectral-line map kernels (S10; "spectral line maps ... are calculated for selected
+// transitions by a final line-of-sight integration through the model", "simple tracing of individual rays
+// through an octree", PAPER.md:203 pixel = smallest cell).
+//
+// One warp per line of sight (map pixel).  The pixel's spectrum lives in shared memory as the EXCESS photon occupation
+// number over the background, D_c = n_c - n_bg, so that the output T_A(c) = (h nu / k) D_c (= (c^2/2k nu^2)(I_c - B_nu(T_bg)))
+// carries no cancellation:
+//     D_c <- D_c + X_c (S - n_bg - D_c),   X_c = 1 - exp(-tau_c),   tau_c = kap s phi_c,   S = n_u / (n_l g_u/g_l - n_u)
+// (the formal solution I <- I e^-tau + S_nu (1 - e^-tau) in occupation-number units, DESIGN 5.2).  The path is walked by all
+// lanes in lock step with the integer lattice arithmetic of the path builder (DESIGN R7) -- no births, no wrap-around: a line
+// of sight starts where it enters the model and ends where it leaves it -- and the lanes then split the channels of the
+// step's profile window (DESIGN R13).  kap and S are formed in double from the float32 populations (n_l g_u/g_l - n_u cancels).
+#include <math.h>
 #include <stdio.h>
 
+#include <algorithm>
+
 #include "loc_internal.cuh"
+
+#define LOC_SPEC_WARPS 4       // lines of sight per block
+#define LOC_SPEC_BATCH1D 256   // 1D lines of sight per launch (their impact parameters travel as kernel arguments)
+
+struct SpecCommon {
+    int nch, nchp;
+    float dv, xmin;
+    float tk_per_occ;  // h nu / k: antenna temperature per unit of occupation number
+    float bgocc;       // background occupation number at the line frequency
+    double ck, gratio; // c^3 A / (8 pi nu^3 dv), g_u / g_l
+    int64_t ncell;
+    const float *pop_u, *pop_l;
+    const float4 *kin;
+    float *out;
+};
+
+// one cell step of a line of sight: all lanes of the warp, channels of the window split over the lanes
+__device__ __forceinline__ void spectrum_step(const SpecCommon &C, float *D, int lane, long long cell, float s, float v0, float sig)
+{
+    const double nu_ = (double)__ldg(C.pop_u + cell), nl_ = (double)__ldg(C.pop_l + cell);
+    const double den = nl_ * C.gratio - nu_;
+    if (den == 0.0) return;  // no molecules (or exactly saturated): tau = 0
+    const float kap = (float)(C.ck * den);
+    const float src = (float)(nu_ / den) - C.bgocc;
+    const float inv_sig = __fdividef(1.0f, sig);
+    const float amp = C.dv * 0.3989422804f * inv_sig;
+    const float ks = kap * s;
+    const float tau0 = fabsf(ks) * amp;
+    float X = C.xmin;
+    if (tau0 > 1.0f) X = sqrtf(fmaf(2.0f, __logf(tau0), X * X));
+    const float inv_dv = __fdividef(1.0f, C.dv);
+    const float cc = fmaf(v0, inv_dv, 0.5f * (float)(C.nch - 1));
+    const float hw = X * sig * inv_dv;
+    const int clo = max(0, (int)ceilf(cc - hw)), chi = min(C.nch - 1, (int)floorf(cc + hw));
+    const float ky = C.dv * 0.8493218f * inv_sig, lamp = __log2f(amp);
+    const bool thick = tau0 >= 0.03f;
+    for (int c = clo + lane; c <= chi; c += 32) {
+        const float y = ((float)c - cc) * ky;
+        const float phi = ex2f(fmaf(-y, y, lamp));
+        const float tau = ks * phi;
+        float Xc;
+        if (thick)
+            Xc = 1.0f - ex2f(-tau * LOC_LOG2E);
+        else
+            Xc = tau * fmaf(tau, fmaf(tau, fmaf(tau, -1.0f / 24.0f, 1.0f / 6.0f), -0.5f), 1.0f);
+        const float d = D[c];
+        D[c] = fmaf(Xc, src - d, d);
+    }
+}
+
+struct Spec3D {
+    SpecCommon C;
+    Tree G;
+    Dir3 D;
+    int nx, ny;
+    long long aff[6];
+};
+
+__global__ void __launch_bounds__(32 * LOC_SPEC_WARPS) k_spectra3d(Spec3D P)
+{
+    extern __shared__ __align__(16) float smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const long long pix = (long long)blockIdx.x * LOC_SPEC_WARPS + warp;
+    if (pix >= (long long)P.nx * P.ny) return;
+    float *Dc = smem + warp * P.C.nchp;
+    for (int c = lane; c < P.C.nchp; c += 32) Dc[c] = 0.f;
+    __syncwarp();
+    const int ix = (int)(pix % P.nx), iy = (int)(pix / P.nx);
+    const long long bp = P.aff[0] + ix * P.aff[2] + iy * P.aff[3], bq = P.aff[1] + ix * P.aff[4] + iy * P.aff[5];
+    const Dir3 &D = P.D;
+    const long long Wz = D.W[0], Wp = D.W[1], Wq = D.W[2];
+    long long zeta = 0;
+    // a line that starts beside the model enters through a side face: advance to the first zeta at which it is inside
+    if (bp < 0) zeta = max(zeta, cross_of(D.T[0], -bp));
+    if (bq < 0) zeta = max(zeta, cross_of(D.T[1], -bq));
+    while (zeta < Wz) {
+        const long long up = bp + shift_of(D.T[0], zeta), uq = bq + shift_of(D.T[1], zeta);
+        if (up < 0 || uq < 0 || up >= Wp || uq >= Wq) break;  // left through a side face
+        LeafPos L;
+        find_leaf(P.G, D, (int)zeta, (int)up, (int)uq, L);
+        const long long h = LOC_H0 >> L.level;
+        long long znext = (zeta & ~(h - 1)) + h, z;
+        z = cross_of(D.T[0], (up & ~(h - 1)) + h - bp); if (z < znext) znext = z;
+        z = cross_of(D.T[1], (uq & ~(h - 1)) + h - bq); if (z < znext) znext = z;
+        const long long cell = L.cell[L.level];
+        const float4 k = __ldg(P.C.kin + cell);
+        const float v0 = -(k.x * D.d[0] + k.y * D.d[1] + k.z * D.d[2]);  // DESIGN R6
+        spectrum_step(P.C, Dc, lane, cell, (float)(znext - zeta) * D.sf, v0, k.w);
+        zeta = znext;
+    }
+    __syncwarp();
+    float *o = P.C.out + pix * P.C.nch;
+    for (int c = lane; c < P.C.nch; c += 32) o[c] = P.C.tk_per_occ * Dc[c];
+}
+
+struct Spec1D {
+    SpecCommon C;
+    int ns, nlos;
+    const double *r_out;  // device [ns]
+    double b[LOC_SPEC_BATCH1D];
+};
+
+// 1D: line of sight at impact parameter b through the shells: in through NS-1 .. k0+1, the tangent shell k0 as one step
+// (DESIGN R5), out through k0+1 .. NS-1; Doppler shift from the direction cosine at the ENTRY of each step.
+__global__ void __launch_bounds__(32 * LOC_SPEC_WARPS) k_spectra1d(Spec1D P)
+{
+    extern __shared__ __align__(16) float smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int los = blockIdx.x * LOC_SPEC_WARPS + warp;
+    if (los >= P.nlos) return;
+    float *Dc = smem + warp * P.C.nchp;
+    for (int c = lane; c < P.C.nchp; c += 32) Dc[c] = 0.f;
+    __syncwarp();
+    const double b = fabs(P.b[los]);
+    const int ns = P.ns;
+    if (b < P.r_out[ns - 1]) {
+        int k0 = 0;
+        while (k0 < ns - 1 && b >= P.r_out[k0]) k0++;
+        const double b2 = b * b;
+        for (int j = 0; j < 2 * (ns - 1 - k0) + 1; j++) {
+            const int nin = ns - 1 - k0;
+            const int k = (j < nin) ? ns - 1 - j : k0 + (j - nin);
+            const double ro = P.r_out[k], ri = (k > 0) ? P.r_out[k - 1] : 0.0;
+            double s, mu;
+            if (j < nin) {
+                s = sqrt(ro * ro - b2) - sqrt(ri * ri - b2);
+                mu = -sqrt(1.0 - b2 / (ro * ro));
+            } else if (j == nin) {
+                s = 2.0 * sqrt(ro * ro - b2);
+                mu = -sqrt(1.0 - b2 / (ro * ro));
+            } else {
+                s = sqrt(ro * ro - b2) - sqrt(ri * ri - b2);
+                mu = sqrt(1.0 - b2 / (ri * ri));
+            }
+            const float4 kk = __ldg(P.C.kin + k);
+            spectrum_step(P.C, Dc, lane, k, (float)s, -kk.x * (float)mu, kk.w);
+        }
+    }
+    __syncwarp();
+    float *o = P.C.out + (long long)los * P.C.nch;
+    for (int c = lane; c < P.C.nch; c += 32) o[c] = P.C.tk_per_occ * Dc[c];
+}
 
 int loc_launch_spectra(loc_model *m, int trans, const double *dir, int nx, int ny, const int64_t *aff, const double *offsets_cm,
                        float *dev_out)
 {
-    snprintf(m->err, sizeof(m->err), "loc_spectra: not implemented yet");
-    return LOC_ESTATE;
+    SpecCommon C;
+    const int u = m->h_upper[trans], l = m->h_lower[trans];
+    const double nu = m->h_freq[trans];
+    C.nch = m->nch;
+    C.nchp = (m->nch + 3) & ~3;
+    C.dv = (float)m->dv;
+    C.xmin = m->xmin;
+    C.tk_per_occ = (float)(LOC_HP * nu / LOC_KB);
+    C.bgocc = (m->tbg > 0.0) ? (float)(1.0 / expm1(LOC_HP * nu / (LOC_KB * m->tbg))) : 0.0f;
+    C.ck = LOC_CL * LOC_CL * LOC_CL * m->h_A[trans] / (8.0 * LOC_PI * nu * nu * nu * m->dv);
+    C.gratio = m->h_g[u] / m->h_g[l];
+    C.ncell = m->ncell;
+    C.pop_u = m->pops + (int64_t)u * m->ncell;
+    C.pop_l = m->pops + (int64_t)l * m->ncell;
+    C.kin = m->kin;
+    const size_t smem = sizeof(float) * LOC_SPEC_WARPS * C.nchp;
+    if (m->kind == LOC_GRID_OCTREE) {
+        if (!dir || !aff) {
+            snprintf(m->err, sizeof(m->err), "loc_spectra: octree models need dir and aff");
+            return LOC_EINVAL;
+        }
+        const double nn = dir[0] * dir[0] + dir[1] * dir[1] + dir[2] * dir[2];
+        if (!(fabs(nn - 1.0) < 1e-9)) {
+            snprintf(m->err, sizeof(m->err), "loc_spectra: direction is not a unit vector");
+            return LOC_EINVAL;
+        }
+        Spec3D P;
+        P.C = C;
+        P.C.out = dev_out;
+        P.G = make_tree(m);
+        loc_fill_dir(m, dir, &P.D);
+        P.nx = nx;
+        P.ny = ny;
+        for (int i = 0; i < 6; i++) P.aff[i] = aff[i];
+        const long long npix = (long long)nx * ny;
+        k_spectra3d<<<(unsigned)((npix + LOC_SPEC_WARPS - 1) / LOC_SPEC_WARPS), 32 * LOC_SPEC_WARPS, smem, m->stream>>>(P);
+        m->launches++;
+        LOC_CUDA_CHECK(m, cudaGetLastError());
+        return LOC_OK;
+    }
+    if (ny != 1 || !offsets_cm) {
+        snprintf(m->err, sizeof(m->err), "loc_spectra: shell models need ny = 1 and offsets_cm");
+        return LOC_EINVAL;
+    }
+    for (int b0 = 0; b0 < nx; b0 += LOC_SPEC_BATCH1D) {
+        Spec1D P;
+        P.C = C;
+        P.C.out = dev_out + (int64_t)b0 * m->nch;
+        P.ns = m->nshell;
+        P.nlos = std::min(nx - b0, LOC_SPEC_BATCH1D);
+        P.r_out = m->d_rout;
+        for (int i = 0; i < LOC_SPEC_BATCH1D; i++) P.b[i] = (i < P.nlos) ? offsets_cm[b0 + i] : 0.0;
+        k_spectra1d<<<(P.nlos + LOC_SPEC_WARPS - 1) / LOC_SPEC_WARPS, 32 * LOC_SPEC_WARPS, smem, m->stream>>>(P);
+        m->launches++;
+        LOC_CUDA_CHECK(m, cudaGetLastError());
+    }
+    return LOC_OK;
 }

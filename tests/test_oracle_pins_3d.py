@@ -191,3 +191,89 @@ def test_cartesian_wraparound_photon_balance():
     expect = (d.sum(axis=1) / d.max(axis=1)).mean()
     assert abs(expect - 1.9415) < 1e-3
     assert abs(r["visits"].mean() / 48 / expect - 1) < 0.02
+
+
+# ----------------------------------------------------------------------------------------------------------------------
+# O11 spectral map (orc_spectra_3d): closed forms and per-column sums
+# ----------------------------------------------------------------------------------------------------------------------
+_H, _K, _C = 6.62607015e-27, 1.380649e-16, 2.99792458e10
+
+
+def _map_aff(pix_units, x0=None):
+    """affine pixel map of a map seen along a main axis: pixel (ix, iy) -> (x0 + ix pix, x0 + iy pix)"""
+    x0 = pix_units // 2 if x0 is None else x0
+    return np.array([x0, x0, pix_units, 0, 0, pix_units], np.int64)
+
+
+def test_spectra_3d_uniform_slab_closed_form():
+    """P1 for the map: a uniform model (two levels of full refinement) seen along +z and along an oblique direction
+    is a homogeneous slab of length L / |d_m|: T_A(c) = (h nu / k)(S - n_bg)(1 - e^{-tau_c}), tau_c = kappa phi_c L / |d_m|
+    (S, n_bg photon occupation numbers), written out here with numpy from the textbook formulae."""
+    sp_ = W.rotor_species(3, 4)
+    root_cm, nroot = 1.0e17, 4
+    dens, tk, sig, ab, tbg = 3.0e3, 12.0, 2.0e4, 1e-6, 2.73
+    nch, band = 48, 1.5e5
+    m = W.uniform_octree(nroot, 3, root_cm, dens, tk, sig, (0.0, 0.0, 0.0), ab, sp_, W.healpix_dirs(1), nch, band, tbg)
+    os_ = O.OSpecies(sp_)
+    pops = O.lte(os_, m.density, m.tkin, m.abundance)
+    t = 1
+    u, l = sp_.upper[t], sp_.lower[t]
+    nu = (sp_.energy_K[u] - sp_.energy_K[l]) * _K / _H
+    dv = 2 * band / nch
+    sigma = math.sqrt(sig ** 2 + _K * tk / (sp_.mass_amu * 1.66053906660e-24))
+    v = (np.arange(nch) - (nch - 1) / 2) * dv
+    phi = dv / (sigma * math.sqrt(2 * math.pi)) * np.exp(-v ** 2 / (2 * sigma ** 2))
+    n_u, n_l = pops[-1, u], pops[-1, l]
+    gr = sp_.g[u] / sp_.g[l]
+    kap = _C ** 3 * sp_.einstein_A[t] / (8 * math.pi * nu ** 3 * dv) * (n_l * gr - n_u)
+    S_occ, bg_occ = 1.0 / (n_l * gr / n_u - 1.0), 1.0 / math.expm1(_H * nu / (_K * tbg))
+    L = nroot * root_cm
+    # along +z: every pixel sees the full depth
+    TA = O.spectra_3d(os_, m, pops, t, np.array([0.0, 0.0, 1.0]), 3, 2, _map_aff(H0))
+    expect = _H * nu / _K * (S_occ - bg_occ) * -np.expm1(-kap * phi * L)
+    assert np.max(np.abs(TA - expect[None, None, :])) < 1e-12 * np.max(np.abs(expect))
+    assert np.max(np.abs(expect)) > 1e-3  # the line is there
+    # oblique, pixel that stays inside the model over the whole depth: path L / |d_m|
+    d = np.array([0.1, -0.2, 1.0])
+    d /= np.linalg.norm(d)
+    _, _, _, sl = _snapped(d)
+    lenf = math.sqrt(1.0 + sl[0] ** 2 + sl[1] ** 2)
+    TA = O.spectra_3d(os_, m, pops, t, d, 1, 1, np.array([H0 // 3, H0 // 5, 0, 0, 0, 0], np.int64))
+    expect = _H * nu / _K * (S_occ - bg_occ) * -np.expm1(-kap * phi * L * lenf)
+    assert np.max(np.abs(TA[0, 0] - expect)) < 1e-9 * np.max(np.abs(expect))
+    # a pixel beside the model that never enters it: no line
+    TA = O.spectra_3d(os_, m, pops, t, np.array([0.0, 0.0, 1.0]), 1, 1, np.array([-5, 7, 0, 0, 0, 0], np.int64))
+    assert np.all(TA == 0.0)
+
+
+def test_spectra_3d_thin_limit_column_density():
+    """P2 for the map: tau << 1, T_bg = 0: integral T_A dv = (h c^3 A / 8 pi k nu^2) N_u, with the upper-level column
+    N_u summed here, pixel by pixel, over the cells of the column (x, y fixed) of an octree with two refinement levels:
+    pins which cells a pixel sees (orientation, refinement descent) and the path lengths."""
+    m, os_ = small_cloud(nroot=4, nlev=3, nch=32, nlevel_species=3)
+    m.t_bg = 0.0
+    m.abundance[:] = 1e-13
+    for a in (m.vx, m.vy, m.vz):
+        a[:] = 0
+    pops = O.lte(os_, m.density, m.tkin, m.abundance)
+    t = 0
+    u = m.species.upper[t]
+    nu = os_.freq(t)
+    dv = 2 * m.band_half / m.nchannel
+    nfine = m.nx << (m.nlev - 1)
+    pix = H0 >> (m.nlev - 1)
+    # column density on the finest grid: every leaf contributes n_u h_leaf to each finest-grid column it covers
+    Nu = np.zeros((nfine, nfine))
+    leaf = np.flatnonzero(m.child < 0)
+    for c in leaf:
+        lv = int(m.level[c])
+        f = 1 << (m.nlev - 1 - lv)
+        x, y = int(m.coords[c][0]) * f, int(m.coords[c][1]) * f
+        Nu[y:y + f, x:x + f] += pops[c, u] * m.root_cm / (1 << lv)
+    for dirz in (1.0, -1.0):  # from the other side the same column is seen
+        TA = O.spectra_3d(os_, m, pops, t, np.array([0.0, 0.0, dirz]), nfine, nfine, _map_aff(pix))
+        W_int = TA.sum(axis=2) * dv
+        expect = _H * _C ** 3 * m.species.einstein_A[t] / (8 * math.pi * _K * nu ** 2) * Nu
+        assert np.max(np.abs(W_int / expect - 1)) < 1e-5  # O(tau) terms
+    assert Nu.std() / Nu.mean() > 0.05  # the columns differ: a transposed map would fail
+    assert np.max(np.abs(Nu - Nu.T)) / Nu.mean() > 0.05
