@@ -168,7 +168,7 @@ int loc_launch_spectra(loc_model *m, int trans, const double *dir, int nx, int n
     C.nch = m->nch;
     C.nchp = (m->nch + 3) & ~3;
     C.dv = (float)m->dv;
-    C.xmin = m->xmin;
+    C.xmin = 6.0f;  // wider than the simulation's window: the map is cheap, and tau_edge = e^-18 tau-independent (DESIGN R13)
     C.tk_per_occ = (float)(LOC_HP * nu / LOC_KB);
     C.bgocc = (m->tbg > 0.0) ? (float)(1.0 / expm1(LOC_HP * nu / (LOC_KB * m->tbg))) : 0.0f;
     C.ck = LOC_CL * LOC_CL * LOC_CL * m->h_A[trans] / (8.0 * LOC_PI * nu * nu * nu * m->dv);

@@ -18,7 +18,10 @@ def _close(ta, ref):
     ta = np.asarray(ta, np.float64)
     tol = 1e-3 * np.abs(ref) + 2e-5 * np.max(np.abs(ref))
     bad = np.abs(ta - ref) > tol
-    assert not bad.any(), f"{bad.sum()} of {bad.size} channels off; worst {np.max(np.abs(ta - ref) / tol):.2f} x tolerance"
+    if bad.any():
+        i = np.unravel_index(np.argmax(np.abs(ta - ref) / tol), ref.shape)
+        raise AssertionError(f"{bad.sum()} of {bad.size} channels off; worst {np.max(np.abs(ta - ref) / tol):.2f} x tolerance at {i}: "
+                             f"{ta[i]} vs {ref[i]} (peak {np.max(np.abs(ref))}); spectrum there: {ta[i[:-1]]} vs {ref[i[:-1]]}")
 
 
 @pytest.mark.parametrize("ns,nch", [(12, 64), (64, 67)])
