@@ -147,6 +147,36 @@ __device__ __forceinline__ float ex2f(float x)
     return y;
 }
 
+// Packed float32 pairs (sm_100a `*.f32x2`): one instruction updates two channels.  On B200 an FFMA2 holds the FMA pipe
+// for two cycles like two FFMA, but takes ONE issue slot (measured, profiles/r1_pipe_microbench.md) -- the 3D kernel is
+// issue bound, so the bulk per-channel arithmetic is written in pairs.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float lo, float hi)
+{
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void upk2(f32x2 v, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c)
+{
+    f32x2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
+{
+    f32x2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b)
+{
+    f32x2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+
 // Per-transition parameters of one ray step, computed once per (step, transition)
 struct __align__(16) TParam {
     float c0;     // thick: -kap*s*log2(e)      thin: kap*s

@@ -3,17 +3,24 @@
 // transfer of Eq. 3 and the two per-cell sums (Eq. 2 first term; escape fraction of PAPER.md:81) for all traced
 // transitions at once (the "all transitions in one pass" option the paper leaves open).
 //
-// Work decomposition (DESIGN 6.4).  A warp carries FOUR rays at a time, one per quarter-warp ("group" of 8 lanes); a lane
-// owns 4 CONSECUTIVE channels of the ray's local profile window (8 lanes x 4 = 32 channels per pass), so that
+// Work decomposition (DESIGN 6.4).  A warp carries FOUR rays at a time, one per quarter-warp ("group" of 8 lanes).  Every
+// step touches a SPAN of 32 consecutive channels that starts at a multiple of 4 and is centred on the Doppler-shifted
+// line; lane l8 of the group owns the aligned quad  span + 4 l8 .. + 3, so that
 //   * the photon spectrum of a ray lives in shared memory and is read / written with one 128-bit access per lane and
-//     transition, conflict free for any window position (a quarter-warp is one shared-memory phase);
+//     transition, conflict free for any span position (a quarter-warp is one shared-memory phase);
+//   * the per-channel arithmetic is done on packed pairs (fma.rn.f32x2): the kernel is bound by instruction issue and by
+//     the 16-lane ALU pipe (selects, compares, logic: 2 cycles each), not by FP32 throughput, so the common path has no
+//     masks and no selects at all -- a span always lies inside the band, and channels of the span outside the nominal
+//     window are simply updated too;
 //   * the sums over a lane's 4 channels are free, and the cross-lane reduction is an 8-lane halving butterfly whose every
 //     instruction serves 4 ray steps;
-//   * all per-step scalar work (record decode, Doppler shift, window, per-transition coefficients) is done lane-parallel
-//     for 8 records x 4 rays at once in a "prepare" phase, not redundantly by 32 lanes per step.
-// The four groups stay in lock step: every round each group consumes exactly one stream record (tasks are padded to
-// whole chunks of 8 records by the path builder); the rare spectrum operations (background, save, load) are executed
+//   * all per-step scalar work (record decode, Doppler shift, window, per-transition coefficients, classification of the
+//     round) is done lane-parallel for 8 records x 4 rays at once in a "prepare" phase.
+// Steps whose window does not fit one span (very thick lines, bands narrower than 32 channels) take a masked multi-pass
+// path.  The four groups stay in lock step: every round each group consumes exactly one stream record (tasks are padded
+// to whole chunks of 8 records by the path builder); the rare spectrum operations (background, save, load) are executed
 // by the whole warp for the group that needs them.
+#include <math.h>
 #include <stdio.h>
 #include <stdlib.h>
 
@@ -23,7 +30,7 @@
 
 #define LOC_GROUPS 4  // rays per warp
 #define LOC_CHUNK 8   // records per group and prepare phase (= LOC_TASK_ALIGN)
-#define LOC_PASS 40   // channels per pass: 8 lanes x (one aligned float4 + one scalar)
+#define LOC_SPAN 32   // channels per pass: 8 lanes x one aligned float4
 
 struct Sim3D {
     int nch, nchp, nsp, nslot;
@@ -44,41 +51,60 @@ struct Sim3D {
     Selection S;
 };
 
-// per-record scalars written by the prepare phase (32 bytes)
-struct __align__(16) RecPrep {
-    float cc;        // profile centre in channel units: v0 / dv + (nch - 1) / 2
-    float ky;        // dv sqrt(log2(e) / 2) / sigma :  phi = 2^(lamp - ((c - cc) ky)^2)
-    float lamp;      // log2(dv / (sigma sqrt(2 pi)))
-    float w;         // a s / V_eff = dzeta / (h NDIR)
-    unsigned cell;   // STEP: cell index; SAVE / LOAD: slot
-    unsigned opdz;   // opcode | level | dzeta (stream word)
-    int clo, chi;    // channel window of the step
+// Per-record scalars every lane of the group reads each round (16 bytes, one broadcast LDS.128).
+//   y(channel wb + j) = A + j ky ;  phi = 2^(lamp - y^2)
+// wbop: bits 0..9 first channel of the span, bits 10..21 per-transition "thick" flags, bit 31 = the record is a STEP
+struct __align__(16) RecS {
+    float A, ky, lamp;
+    unsigned wbop;
 };
+#define LOC_WB_MASK 0x3ffu
+#define LOC_THICK_SHIFT 10
+#define LOC_RS_STEP 0x80000000u
 
-// per (record, transition) coefficients (16 bytes): X_c = thin ? phi + c0 (B2 + c0 (B3 + c0 B4)) : 1 - 2^(c0 phi)
-//   n' = n + X (c1 + alpha n);  SJ += scale sum n X;  ESC += scale sum X
-struct __align__(16) TPrep {
-    float c0, c1, alpha, scale;
-};
+// Class word of a round (one per chunk record index, OR over the four groups):
+//   bits 0..11 some stepping ray is thick in transition t, bits 12..23 some stepping ray is thin in t,
+//   bit 24 a spectrum operation is due, bit 25 some group steps, bit 26 some stepping group needs the masked path
+#define LOC_CLS_THIN_SHIFT 12
+#define LOC_CLS_CTRL (1u << 24)
+#define LOC_CLS_STEP (1u << 25)
+#define LOC_CLS_SLOW (1u << 26)
 
-#define LOC_XCLIP 4.0f       // the window may be clipped to one 32-channel pass only outside +-4 sigma
+#define LOC_XCLIP 3.9f      // a span may cut the nominal window, but never closer than this many sigma to the line centre
 #define LOC_THIN_TAU 0.03f  // line-centre optical depth of a step below which the cubic series of (1-e^-t)/t is used
 
+// shared-memory tables of one warp, written by the prepare phase
 template <int NT>
-__device__ __forceinline__ void prepare_record(const Sim3D &P, uint2 rec, float d0, float d1, float d2, float sf, RecPrep *rp, TPrep *tp,
-                                               unsigned &thickmask)
+struct WarpTables {
+    RecS rs[LOC_GROUPS][LOC_CHUNK];
+    float2 tp[LOC_GROUPS][LOC_CHUNK][NT];   // (c0, c1):  X_c = thin ? phi + c0 (B2 + c0 (B3 + c0 B4)) : 1 - 2^(c0 phi)
+                                            //            n' = n + X (c1 + alpha n),  alpha = thin ? -c0 : -1
+    float sc[LOC_GROUPS][LOC_CHUNK][NT];    // SJ += sc sum n X;  ESC += sc sum X
+    unsigned cell[LOC_GROUPS][LOC_CHUNK];   // STEP: cell index; SAVE / LOAD: slot
+    unsigned opdz[LOC_GROUPS][LOC_CHUNK];   // opcode | level | dzeta (stream word)
+    float w[LOC_GROUPS][LOC_CHUNK];         // a s / V_eff = dzeta / (h NDIR)
+    float h5[LOC_GROUPS][LOC_CHUNK];        // 5 sigma in channels (statistics only)
+    float cc[LOC_GROUPS][LOC_CHUNK];        // line centre in channels (statistics, masked path)
+    int2 win[LOC_GROUPS][LOC_CHUNK];        // nominal channel window [clo, chi] (masked path)
+    unsigned cls[LOC_CHUNK];
+};
+
+// Prepare phase: lane (g, j) decodes record j of the chunk of group g, loads the cell's kinematics and line coefficients
+// and fills the tables.  Returns the lane's contribution to the class word of round j.
+template <int NT>
+__device__ __forceinline__ unsigned prepare_record(const Sim3D &P, uint2 rec, float d0, float d1, float d2, float sf, WarpTables<NT> &T, int g,
+                                                   int j)
 {
-    RecPrep r;
-    r.cell = rec.x;
-    r.opdz = rec.y;
-    r.cc = 0.f;
+    RecS r;
+    r.A = 0.f;
     r.ky = 0.f;
-    r.lamp = 0.f;
-    r.w = 0.f;
-    r.clo = 0;
-    r.chi = -1;
-    thickmask = 0;
-    if ((rec.y >> 24) == LOC_OP_STEP) {
+    r.lamp = -INFINITY;  // phi = 2^(-inf) = 0 for records that are not steps: the round leaves their spectra untouched
+    r.wbop = 0u;
+    T.cell[g][j] = rec.x;
+    T.opdz[g][j] = rec.y;
+    const unsigned op = rec.y >> 24;
+    unsigned cls = (op == LOC_OP_BG || op == LOC_OP_SAVE || op == LOC_OP_LOAD) ? LOC_CLS_CTRL : 0u;
+    if (op == LOC_OP_STEP) {
         const float4 k = __ldg(P.kin + rec.x);
         const float v0 = -(k.x * d0 + k.y * d1 + k.z * d2);  // DESIGN R6
         const float sig = k.w;
@@ -90,59 +116,140 @@ __device__ __forceinline__ void prepare_record(const Sim3D &P, uint2 rec, float 
         const float amp = P.dv * 0.3989422804f * inv_sig;
         const float2 *cf = P.coef + (long long)rec.x * P.nsp + P.slot0;
         float tau0m = 0.f;
+        unsigned thick = 0u;
 #pragma unroll
         for (int t = 0; t < NT; t++) {
             const float2 ke = __ldg(cf + t);
             const float ks = ke.x * s;
             const float tau0 = fabsf(ks) * amp;
             tau0m = fmaxf(tau0m, tau0);
-            TPrep q;
+            float2 q;
+            float scale;
             if (tau0 >= LOC_THIN_TAU) {
-                thickmask |= 1u << t;
-                q.c0 = -ks * LOC_LOG2E;
-                q.c1 = __fdividef(ke.y, ke.x);  // source function in occupation-number units
-                q.alpha = -1.0f;
-                q.scale = __fdividef(w, ks);
+                thick |= 1u << t;
+                q.x = -ks * LOC_LOG2E;
+                q.y = __fdividef(ke.y, ke.x);  // source function in occupation-number units
+                scale = __fdividef(w, ks);
             } else {
-                q.c0 = ks;
-                q.c1 = ke.y * s;
-                q.alpha = -ks;
-                q.scale = w;
+                q.x = ks;
+                q.y = ke.y * s;
+                scale = w;
             }
-            tp[t] = q;
+            T.tp[g][j][t] = q;
+            T.sc[g][j][t] = scale;
         }
         // window half-width in sigma: the profile mass left outside stays a fixed fraction (that of xmin at tau0 <= 1) of
         // the escape sum  sum_c phi_c f(tau_c) ~ 1/tau0  of an optically thick step (DESIGN 5.3)
         float X = P.xmin;
         if (tau0m > 1.0f) X = sqrtf(fmaf(2.0f, __logf(tau0m), X * X));
         const float inv_dv = __fdividef(1.0f, P.dv);
-        r.cc = fmaf(v0, inv_dv, 0.5f * (float)(P.nch - 1));
-        const float hw = X * sig * inv_dv;
-        int clo = max(0, (int)ceilf(r.cc - hw)), chi = min(P.nch - 1, (int)floorf(r.cc + hw));
-        // One pass of the kernel covers LOC_PASS = 40 channels starting at a multiple of 4.  If the window overshoots that by a few
-        // channels, drop the outermost ones (never closer than LOC_XCLIP sigma to the line centre) instead of paying a
-        // second pass; their profile mass is booked as escaping like everything outside the window (DESIGN 5.3).
-        {
-            const float lim = LOC_XCLIP * sig * inv_dv;
-            int lo = clo, hi = chi;
+        const float cc = fmaf(v0, inv_dv, 0.5f * (float)(P.nch - 1));
+        const float sigch = sig * inv_dv;
+        const float hw = X * sigch;
+        const int clo = max(0, (int)ceilf(cc - hw)), chi = min(P.nch - 1, (int)floorf(cc + hw));
+        // the span: 32 channels from a multiple of 4, centred on the line, inside the band
+        const int wbmax = (P.nch - LOC_SPAN) & ~3;
+        int wb = 4 * (int)rintf((cc - 15.5f) * 0.25f);
+        wb = max(0, min(wb, wbmax));
+        const float lim = LOC_XCLIP * sigch;
+        const bool fast = P.nch >= LOC_SPAN && (clo >= wb || cc - (float)wb >= lim) && (chi <= wb + LOC_SPAN - 1 || (float)(wb + LOC_SPAN - 1) - cc >= lim);
+        if (P.nch < LOC_SPAN) wb = 0;
+        r.ky = P.dv * 0.8493218f * inv_sig;  // sqrt(log2(e) / 2) in channel units
+        r.A = ((float)wb - cc) * r.ky;
+        r.lamp = __log2f(amp);
+        r.wbop = (unsigned)wb | (thick << LOC_THICK_SHIFT) | LOC_RS_STEP;
+        T.w[g][j] = w;
+        T.h5[g][j] = 5.0f * sigch;
+        T.cc[g][j] = cc;
+        T.win[g][j] = make_int2(clo, chi);
+        cls |= LOC_CLS_STEP | thick | ((~thick & ((1u << NT) - 1u)) << LOC_CLS_THIN_SHIFT) | (fast ? 0u : LOC_CLS_SLOW);
+    } else {
 #pragma unroll
-            for (int i = 0; i < 3; i++) {
-                if ((lo & 3) + (hi - lo + 1) <= LOC_PASS) break;
-                if (r.cc - (float)lo > (float)hi - r.cc) lo++;
-                else hi--;
-            }
-            if ((lo & 3) + (hi - lo + 1) <= LOC_PASS && r.cc - (float)lo >= lim && (float)hi - r.cc >= lim) {
-                clo = lo;
-                chi = hi;
+        for (int t = 0; t < NT; t++) {
+            T.tp[g][j][t] = make_float2(0.f, 0.f);
+            T.sc[g][j][t] = 0.f;
+        }
+        T.w[g][j] = 0.f;
+        T.win[g][j] = make_int2(0, -1);
+    }
+    T.rs[g][j] = r;
+    return cls;
+}
+
+// One pass over a span of 32 channels for the four ray steps of a round: lane l8 of a group updates the quad at `sq`
+// (its channels have the offsets jf[0..3] from the span start of RecS) for all NT transitions.
+//   MASK = false: the common path -- no masks, the quad is known to lie inside the spectrum
+//   MASK = true : channel k takes part iff m[k]; the quad is loaded / stored iff `inq`
+// Accumulates the lane's partial sums a[t] += sum_k n_k X_k, b[t] += sum_k X_k, sphi += sum_k phi_k.
+template <int NT, bool MASK>
+__device__ __forceinline__ void span_pass(float *sq, int nchp, const float2 *tpr, const RecS &rs, const float (&jf)[4], unsigned thick,
+                                          unsigned any_thick, unsigned any_thin, bool inq, const bool (&m)[4], float (&a)[NT], float (&b)[NT],
+                                          float &sphi)
+{
+    float e[4];
+#pragma unroll
+    for (int k = 0; k < 4; k++) {
+        const float y = fmaf(jf[k], rs.ky, rs.A);
+        e[k] = ex2f(fmaf(-y, y, rs.lamp));
+        if (MASK) e[k] = m[k] ? e[k] : 0.0f;
+    }
+    sphi += (e[0] + e[1]) + (e[2] + e[3]);
+    const f32x2 P01 = pk2(e[0], e[1]), P23 = pk2(e[2], e[3]);
+    const f32x2 ONE2 = pk2(1.0f, 1.0f), MONE2 = pk2(-1.0f, -1.0f);
+    f32x2 B2a = 0ull, B2b = 0ull, B3a = 0ull, B3b = 0ull, B4a = 0ull, B4b = 0ull;
+    if (any_thin) {  // powers of phi for the series, shared by all thin transitions of the round
+        const f32x2 K2 = pk2(-0.5f, -0.5f), K3 = pk2(1.0f / 6.0f, 1.0f / 6.0f), K4 = pk2(-1.0f / 24.0f, -1.0f / 24.0f);
+        const f32x2 s01 = mul2(P01, P01), s23 = mul2(P23, P23);
+        B2a = mul2(s01, K2);
+        B2b = mul2(s23, K2);
+        B3a = mul2(mul2(s01, P01), K3);
+        B3b = mul2(mul2(s23, P23), K3);
+        B4a = mul2(mul2(s01, s01), K4);
+        B4b = mul2(mul2(s23, s23), K4);
+    }
+#pragma unroll
+    for (int t = 0; t < NT; t++) {
+        const float2 q = tpr[t];
+        float4 n4 = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (!MASK || inq) n4 = *reinterpret_cast<const float4 *>(sq + t * nchp);
+        const f32x2 N01 = pk2(n4.x, n4.y), N23 = pk2(n4.z, n4.w);
+        const f32x2 C0 = pk2(q.x, q.x), C1 = pk2(q.y, q.y);
+        f32x2 X01, X23, AL;
+        if (!((any_thick >> t) & 1u)) {  // every stepping ray of the warp is thin in this transition
+            X01 = fma2(C0, fma2(C0, fma2(C0, B4a, B3a), B2a), P01);
+            X23 = fma2(C0, fma2(C0, fma2(C0, B4b, B3b), B2b), P23);
+            AL = pk2(-q.x, -q.x);
+        } else {
+            float z0, z1, z2, z3;
+            upk2(mul2(C0, P01), z0, z1);
+            upk2(mul2(C0, P23), z2, z3);
+            const f32x2 E01 = pk2(ex2f(z0), ex2f(z1)), E23 = pk2(ex2f(z2), ex2f(z3));
+            X01 = fma2(E01, MONE2, ONE2);
+            X23 = fma2(E23, MONE2, ONE2);
+            AL = MONE2;
+            if ((any_thin >> t) & 1u) {  // mixed: both forms, selected per ray
+                const bool tk = (thick >> t) & 1u;
+                float x0, x1, x2, x3, s0, s1, s2, s3;
+                upk2(X01, x0, x1);
+                upk2(X23, x2, x3);
+                upk2(fma2(C0, fma2(C0, fma2(C0, B4a, B3a), B2a), P01), s0, s1);
+                upk2(fma2(C0, fma2(C0, fma2(C0, B4b, B3b), B2b), P23), s2, s3);
+                X01 = pk2(tk ? x0 : s0, tk ? x1 : s1);
+                X23 = pk2(tk ? x2 : s2, tk ? x3 : s3);
+                const float al = tk ? -1.0f : -q.x;
+                AL = pk2(al, al);
             }
         }
-        r.clo = clo;
-        r.chi = chi;
-        r.ky = P.dv * 0.8493218f * inv_sig;
-        r.lamp = __log2f(amp);
-        r.w = w;
+        float a0, a1, b0, b1;
+        upk2(fma2(N01, X01, mul2(N23, X23)), a0, a1);
+        upk2(add2(X01, X23), b0, b1);
+        a[t] += a0 + a1;
+        b[t] += b0 + b1;
+        float r0, r1, r2, r3;
+        upk2(fma2(X01, fma2(AL, N01, C1), N01), r0, r1);
+        upk2(fma2(X23, fma2(AL, N23, C1), N23), r2, r3);
+        if (!MASK || inq) *reinterpret_cast<float4 *>(sq + t * nchp) = make_float4(r0, r1, r2, r3);
     }
-    *rp = r;
 }
 
 template <int NT, bool GEOM>
@@ -151,21 +258,21 @@ __global__ void __launch_bounds__(32) k_sim3d(Sim3D P)
     constexpr int NV = 2 * NT;                 // reduced values per step: a[t], b[t]
     constexpr int NPASS = (NV + 7) / 8;        // 8-lane butterflies of up to 8 values
     extern __shared__ __align__(16) float smem[];
+    __shared__ WarpTables<NT> T;               // separate object: no aliasing with the spectra
     const int lane = threadIdx.x, grp = lane >> 3, l8 = lane & 7;
     const int nchp = P.nchp;
     const int spec = NT * nchp;                // floats per ray spectrum
-    float *sn_all = smem;                                  // [4][NT][nchp]
-    __shared__ TPrep tp_all[LOC_GROUPS * LOC_CHUNK * NT];    // [4][8][NT]   (separate objects: no aliasing with the spectra)
-    __shared__ RecPrep rp_all[LOC_GROUPS * LOC_CHUNK];       // [4][8]
+    float *sn_all = smem;                      // [4][NT][nchp]
     float *sn = sn_all + grp * spec;
-    TPrep *tpg = tp_all + grp * LOC_CHUNK * NT;
-    RecPrep *rpg = rp_all + grp * LOC_CHUNK;
     float *slots_warp = P.pool + (long long)blockIdx.x * LOC_GROUPS * P.nslot * spec;
+    const float jf[4] = {(float)(4 * l8), (float)(4 * l8 + 1), (float)(4 * l8 + 2), (float)(4 * l8 + 3)};
 
     long long off = 0, end = 0;  // this group's position in the stream
     bool done = false;
     float d0 = 0.f, d1 = 0.f, d2 = 0.f, sf = 0.f;
     unsigned long long mysteps = 0, myactive = 0;
+    uint2 nrec = make_uint2(0u, LOC_OP_NOP << 24);  // record of the next chunk, fetched one chunk ahead
+    bool have_next = false;
 
     for (;;) {
         // ---- refill: groups whose task is exhausted take the next root ray from the queue ----
@@ -175,6 +282,7 @@ __global__ void __launch_bounds__(32) k_sim3d(Sim3D P)
             if (need && l8 == 0) task = atomicAdd(P.queue, 1u);
             task = __shfl_sync(0xffffffffu, task, grp * 8);
             if (need) {
+                have_next = false;
                 if (task >= P.ntask) {
                     done = true;
                 } else {
@@ -188,123 +296,75 @@ __global__ void __launch_bounds__(32) k_sim3d(Sim3D P)
                 }
             }
         }
-        __syncwarp();
         if (__all_sync(0xffffffffu, done)) break;
         // ---- prepare: lane l8 of each group decodes record off + l8 of its ray ----
         uint2 rec = make_uint2(0u, LOC_OP_NOP << 24);
-        if (!done && off + l8 < end) rec = __ldg(P.stream + off + l8);
-        unsigned thick_l;
-        prepare_record<NT>(P, rec, d0, d1, d2, sf, rpg + l8, tpg + l8 * NT, thick_l);
+        if (have_next)
+            rec = nrec;
+        else if (!done && off + l8 < end)
+            rec = __ldg(P.stream + off + l8);
         off += LOC_CHUNK;
+        have_next = !done && off < end;
+        nrec = make_uint2(0u, LOC_OP_NOP << 24);
+        if (have_next && off + l8 < end) nrec = __ldg(P.stream + off + l8);
+        {
+            unsigned c = prepare_record<NT>(P, rec, d0, d1, d2, sf, T, grp, l8);
+            c |= __shfl_xor_sync(0xffffffffu, c, 8);
+            c |= __shfl_xor_sync(0xffffffffu, c, 16);
+            if (lane < LOC_CHUNK) T.cls[lane] = c;
+        }
         __syncwarp();
 
         // ---- 8 rounds: every group consumes one record per round ----
         for (int r = 0; r < LOC_CHUNK; r++) {
-            const RecPrep rp = rpg[r];
-            const unsigned op = rp.opdz >> 24;
-            const unsigned thick = __shfl_sync(0xffffffffu, thick_l, grp * 8 + r);
-            // spectrum operations, executed by the whole warp for one group at a time
-            unsigned ctrl = __ballot_sync(0xffffffffu, op == LOC_OP_BG || op == LOC_OP_SAVE || op == LOC_OP_LOAD) & 0x01010101u;
-            while (ctrl) {
-                const int g = (__ffs(ctrl) - 1) >> 3;
-                ctrl &= ctrl - 1;
-                const unsigned gop = __shfl_sync(0xffffffffu, op, g * 8), gx = __shfl_sync(0xffffffffu, rp.cell, g * 8);
-                float *gs = sn_all + g * spec;
-                float *slot = slots_warp + ((long long)g * P.nslot + gx) * spec;
-                if (gop == LOC_OP_BG) {
+            const unsigned cls = T.cls[r];
+            if (cls & LOC_CLS_CTRL) {
+                // spectrum operations, executed by the whole warp for one group at a time
+                for (int g = 0; g < LOC_GROUPS; g++) {
+                    const unsigned gop = T.opdz[g][r] >> 24, gx = T.cell[g][r];
+                    float *gs = sn_all + g * spec;
+                    float *slot = slots_warp + ((long long)g * P.nslot + gx) * spec;
+                    if (gop == LOC_OP_BG) {
 #pragma unroll
-                    for (int t = 0; t < NT; t++) {
-                        const float b = P.S.bgocc[P.slot0 + t];
-                        for (int c = lane; c < nchp; c += 32) gs[t * nchp + c] = b;
+                        for (int t = 0; t < NT; t++) {
+                            const float bg = P.S.bgocc[P.slot0 + t];
+                            for (int c = lane; c < nchp; c += 32) gs[t * nchp + c] = bg;
+                        }
+                    } else if (gop == LOC_OP_SAVE) {
+                        for (int i = lane * 4; i < spec; i += 128) *reinterpret_cast<float4 *>(slot + i) = *reinterpret_cast<const float4 *>(gs + i);
+                    } else if (gop == LOC_OP_LOAD) {
+                        for (int i = lane * 4; i < spec; i += 128) *reinterpret_cast<float4 *>(gs + i) = *reinterpret_cast<const float4 *>(slot + i);
                     }
-                } else if (gop == LOC_OP_SAVE) {
-                    for (int i = lane * 4; i < spec; i += 128) *reinterpret_cast<float4 *>(slot + i) = *reinterpret_cast<const float4 *>(gs + i);
-                } else {
-                    for (int i = lane * 4; i < spec; i += 128) *reinterpret_cast<float4 *>(gs + i) = *reinterpret_cast<const float4 *>(slot + i);
                 }
                 __syncwarp();
             }
-            const bool step = op == LOC_OP_STEP;
-            const unsigned anystep = __ballot_sync(0xffffffffu, step);
-            if (!anystep) continue;
-            const unsigned any_thick = __reduce_or_sync(0xffffffffu, step ? thick : 0u);
-            const unsigned any_thin = __reduce_or_sync(0xffffffffu, step ? ~thick : 0u);
+            if (!(cls & LOC_CLS_STEP)) continue;
+            const unsigned any_thick = cls & 0xfffu, any_thin = (cls >> LOC_CLS_THIN_SHIFT) & 0xfffu;
+            const RecS rs = T.rs[grp][r];
+            const unsigned thick = (rs.wbop >> LOC_THICK_SHIFT) & 0xfffu;
+            const int wb = (int)(rs.wbop & LOC_WB_MASK);
+            const float2 *tpr = T.tp[grp][r];
 
             float a[NT], b[NT];
 #pragma unroll
             for (int t = 0; t < NT; t++) a[t] = b[t] = 0.f;
             float sphi = 0.f;
-            const TPrep *tpr = tpg + r * NT;
-            // passes of 40 channels over the window (one pass unless the line is very thick): lane l8 owns the aligned
-            // float4 at wb + 4 l8 and the single channel wb + 32 + l8
-            int wb = rp.clo & ~3;
-            const int chi = step ? rp.chi : -1;
-            while (__any_sync(0xffffffffu, wb <= chi)) {
-                const int cb = wb + 4 * l8, ce = wb + 32 + l8;
-                float phi[5], B2[5], B3[5], B4[5];
-#pragma unroll
-                for (int k = 0; k < 5; k++) {
-                    const int c = (k < 4) ? cb + k : ce;
-                    const float y = ((float)c - rp.cc) * rp.ky;
-                    const float e = ex2f(fmaf(-y, y, rp.lamp));
-                    phi[k] = (c >= rp.clo && c <= chi) ? e : 0.0f;
-                    sphi += phi[k];
-                    const float p2 = phi[k] * phi[k];
-                    B2[k] = -0.5f * p2;
-                    B3[k] = (1.0f / 6.0f) * p2 * phi[k];
-                    B4[k] = (-1.0f / 24.0f) * p2 * p2;
+            if (!(cls & LOC_CLS_SLOW)) {
+                const bool nomask[4] = {true, true, true, true};
+                span_pass<NT, false>(sn + wb + 4 * l8, nchp, tpr, rs, jf, thick, any_thick, any_thin, true, nomask, a, b, sphi);
+            } else {
+                // masked passes of 32 channels over the nominal window (several when the line is very thick)
+                const int2 win = T.win[grp][r];
+                int base = win.x & ~3;
+                while (__any_sync(0xffffffffu, base <= win.y)) {
+                    const int cb = base + 4 * l8;  // the lane's quad in this pass (win.y < nch <= nchp: in range if cb <= win.y)
+                    const float ob = (float)(base - wb);
+                    const float jo[4] = {jf[0] + ob, jf[1] + ob, jf[2] + ob, jf[3] + ob};
+                    const bool m[4] = {cb >= win.x && cb <= win.y, cb + 1 >= win.x && cb + 1 <= win.y, cb + 2 >= win.x && cb + 2 <= win.y,
+                                       cb + 3 >= win.x && cb + 3 <= win.y};
+                    span_pass<NT, true>(sn + cb, nchp, tpr, rs, jo, thick, any_thick, any_thin, cb <= win.y, m, a, b, sphi);
+                    base += LOC_SPAN;
                 }
-                const bool inb = cb <= chi;            // chi < nch <= nchp and cb is a multiple of 4: the float4 is in range
-                const bool ine = ce <= chi;
-                float nn[NT][5];
-#pragma unroll
-                for (int t = 0; t < NT; t++) {
-                    float4 n4 = make_float4(0.f, 0.f, 0.f, 0.f);
-                    if (inb) n4 = *reinterpret_cast<const float4 *>(sn + t * nchp + cb);
-                    nn[t][0] = n4.x;
-                    nn[t][1] = n4.y;
-                    nn[t][2] = n4.z;
-                    nn[t][3] = n4.w;
-                    nn[t][4] = ine ? sn[t * nchp + ce] : 0.f;
-                }
-#pragma unroll
-                for (int t = 0; t < NT; t++) {
-                    const TPrep q = tpr[t];
-                    const bool tk = (thick >> t) & 1u;
-                    if (!((any_thick >> t) & 1u)) {  // every ray of the warp is thin in this transition
-#pragma unroll
-                        for (int k = 0; k < 5; k++) {
-                            const float X = fmaf(q.c0, fmaf(q.c0, fmaf(q.c0, B4[k], B3[k]), B2[k]), phi[k]);
-                            a[t] = fmaf(nn[t][k], X, a[t]);
-                            b[t] += X;
-                            nn[t][k] = fmaf(X, fmaf(q.alpha, nn[t][k], q.c1), nn[t][k]);
-                        }
-                    } else if (!((any_thin >> t) & 1u)) {  // every ray is thick
-#pragma unroll
-                        for (int k = 0; k < 5; k++) {
-                            const float X = 1.0f - ex2f(q.c0 * phi[k]);
-                            a[t] = fmaf(nn[t][k], X, a[t]);
-                            b[t] += X;
-                            nn[t][k] = fmaf(X, fmaf(q.alpha, nn[t][k], q.c1), nn[t][k]);
-                        }
-                    } else {  // mixed: both forms, selected per ray
-#pragma unroll
-                        for (int k = 0; k < 5; k++) {
-                            const float Xs = fmaf(q.c0, fmaf(q.c0, fmaf(q.c0, B4[k], B3[k]), B2[k]), phi[k]);
-                            const float Xe = 1.0f - ex2f(q.c0 * phi[k]);
-                            const float X = tk ? Xe : Xs;
-                            a[t] = fmaf(nn[t][k], X, a[t]);
-                            b[t] += X;
-                            nn[t][k] = fmaf(X, fmaf(q.alpha, nn[t][k], q.c1), nn[t][k]);
-                        }
-                    }
-                }
-#pragma unroll
-                for (int t = 0; t < NT; t++) {
-                    if (inb) *reinterpret_cast<float4 *>(sn + t * nchp + cb) = make_float4(nn[t][0], nn[t][1], nn[t][2], nn[t][3]);
-                    if (ine) sn[t * nchp + ce] = nn[t][4];
-                }
-                wb += LOC_PASS;
             }
             // ---- reductions over the 8 lanes of each group ----
             sphi += __shfl_xor_sync(0xffffffffu, sphi, 4);
@@ -344,29 +404,32 @@ __global__ void __launch_bounds__(32) k_sim3d(Sim3D P)
                     tot[p] = keep + __shfl_xor_sync(0xffffffffu, send, 1);
                 }
             }
-            // lane l8 of a group now holds the group totals of values 4*bit2 + 2*bit1 + bit0 ... = l8, 8 + l8, 16 + l8
-            if (step) {
-                float2 *cn = P.cnt + (long long)rp.cell * P.nsp + P.slot0;
-                const float wesc = rp.w - rp.w * sphi;  // photons emitted outside the window escape (DESIGN 5.3)
+            // lane l8 of a group now holds the group totals of values l8, 8 + l8, 16 + l8
+            if (rs.wbop & LOC_RS_STEP) {
+                const unsigned cell = T.cell[grp][r];
+                const float w = T.w[grp][r];
+                float2 *cn = P.cnt + (long long)cell * P.nsp + P.slot0;
+                const float wesc = w - w * sphi;  // photons emitted outside the updated channels escape (DESIGN 5.3)
+                const float *scr = T.sc[grp][r];
 #pragma unroll
                 for (int p = 0; p < NPASS; p++) {
                     const int i = 8 * p + l8;
                     if (i < NT)
-                        atomicAdd(&cn[i].x, tot[p] * tpr[i].scale);
+                        atomicAdd(&cn[i].x, tot[p] * scr[i]);
                     else if (i < NV)
-                        atomicAdd(&cn[i - NT].y, fmaf(tot[p], tpr[i - NT].scale, wesc));
+                        atomicAdd(&cn[i - NT].y, fmaf(tot[p], scr[i - NT], wesc));
                 }
                 if (l8 == 0) {
                     mysteps++;
                     if (GEOM) {
-                        atomicAdd(&P.visits[rp.cell], 1u);
-                        atomicAdd(&P.pathz[rp.cell], rp.opdz & 0x1fffffu);
-                        const float h5 = 5.0f * 0.8493218f / rp.ky;  // 5 sigma in channels
-                        myactive += max(0, min(P.nch - 1, (int)floorf(rp.cc + h5)) - max(0, (int)ceilf(rp.cc - h5)) + 1);
+                        atomicAdd(&P.visits[cell], 1u);
+                        atomicAdd(&P.pathz[cell], T.opdz[grp][r] & 0x1fffffu);
+                        const float h5 = T.h5[grp][r], cc = T.cc[grp][r];  // 5 sigma in channels
+                        myactive += max(0, min(P.nch - 1, (int)floorf(cc + h5)) - max(0, (int)ceilf(cc - h5)) + 1);
                     }
                 }
             }
-            __syncwarp();
+            __syncwarp();  // the next round's quads were written by other lanes
         }
     }
     // per-warp totals
@@ -381,8 +444,8 @@ __global__ void __launch_bounds__(32) k_sim3d(Sim3D P)
 template <int NT>
 static int launch3d(loc_model *m, Sim3D &P, int geom)
 {
-    const size_t smem = sizeof(float) * LOC_GROUPS * NT * P.nchp;  // + static: TPrep / RecPrep tables
-    if (smem > 220 * 1024) {
+    const size_t smem = sizeof(float) * LOC_GROUPS * NT * P.nchp;  // + static: the prepare tables
+    if (smem > 200 * 1024 || P.nch > (int)LOC_WB_MASK) {
         snprintf(m->err, sizeof(m->err), "nchannel * ntrans too large for the shared-memory spectra (%zu bytes per warp)", smem);
         return LOC_EINVAL;
     }
