@@ -63,37 +63,44 @@ struct __align__(16) RecS {
 #define LOC_RS_STEP 0x80000000u
 
 // Class word of a round (one per chunk record index, OR over the four groups):
-//   bits 0..11 some stepping ray is thick in transition t, bits 12..23 some stepping ray is thin in t,
+//   bits 0..11 some stepping ray MUST use the exponential form in transition t (tau0 > LOC_SER_TAU),
+//   bits 12..23 some stepping ray MUST use the series (tau0 < LOC_EXP_TAU),
 //   bit 24 a spectrum operation is due, bit 25 some group steps, bit 26 some stepping group needs the masked path
 #define LOC_CLS_THIN_SHIFT 12
 #define LOC_CLS_CTRL (1u << 24)
 #define LOC_CLS_STEP (1u << 25)
 #define LOC_CLS_SLOW (1u << 26)
 
-#define LOC_XCLIP 3.9f      // a span may cut the nominal window, but never closer than this many sigma to the line centre
-#define LOC_THIN_TAU 0.03f  // line-centre optical depth of a step below which the cubic series of (1-e^-t)/t is used
+#define LOC_XCLIP 3.9f     // a span may cut the nominal window, but never closer than this many sigma to the line centre
+// Two forms of the per-channel factor (DESIGN 5.3).  Exponential: X = 1 - 2^(c0 phi), accurate (ex2.approx plus the
+// subtraction) only while the line-centre optical depth of the step is >= LOC_EXP_TAU.  Series: X = phi f(tau) with
+// f = 1 - tau/2 + tau^2/6 - tau^3/24 + tau^4/120, truncation < 2e-6 while tau0 <= LOC_SER_TAU.  In between either form
+// will do, so a round whose four steps do not hold both extremes runs ONE form for the transition.
+#define LOC_EXP_TAU 0.03f
+#define LOC_SER_TAU 0.3f
 
 // shared-memory tables of one warp, written by the prepare phase
 template <int NT>
 struct WarpTables {
+    static constexpr int ROW = 10;                                  // float2 per row of partial sums (8 used): 80 bytes
+    static constexpr int PGW = NT * ROW * 2;                        // words per group ...
+    static constexpr int PG = (PGW + ((48 - PGW % 32) % 32)) / 2;   // ... padded to 16 mod 32 words (float2 units)
     RecS rs[LOC_GROUPS][LOC_CHUNK];
-    float2 tp[LOC_GROUPS][LOC_CHUNK][NT];   // (c0, c1):  X_c = thin ? phi + c0 (B2 + c0 (B3 + c0 B4)) : 1 - 2^(c0 phi)
-                                            //            n' = n + X (c1 + alpha n),  alpha = thin ? -c0 : -1
-    float sc[LOC_GROUPS][LOC_CHUNK][NT];    // SJ += sc sum n X;  ESC += sc sum X
+    float2 tp[LOC_GROUPS][LOC_CHUNK][NT];   // (c0, c1):  X_c = series ? phi + c0 (B2 + c0 (B3 + c0 (B4 + c0 B5))) : 1 - 2^(c0 phi)
+                                            //            n' = n + X (c1 + alpha n),  alpha = series ? -c0 : -1
     unsigned cell[LOC_GROUPS][LOC_CHUNK];   // STEP: cell index; SAVE / LOAD: slot
     unsigned opdz[LOC_GROUPS][LOC_CHUNK];   // opcode | level | dzeta (stream word)
     float w[LOC_GROUPS][LOC_CHUNK];         // a s / V_eff = dzeta / (h NDIR)
-    float h5[LOC_GROUPS][LOC_CHUNK];        // 5 sigma in channels (statistics only)
-    float cc[LOC_GROUPS][LOC_CHUNK];        // line centre in channels (statistics, masked path)
     int2 win[LOC_GROUPS][LOC_CHUNK];        // nominal channel window [clo, chi] (masked path)
     unsigned cls[LOC_CHUNK];
+    float2 part[LOC_GROUPS][PG];            // per-lane partial sums (a_t, b_t) of the round: [group][t][lane] (rows of 10)
 };
 
 // Prepare phase: lane (g, j) decodes record j of the chunk of group g, loads the cell's kinematics and line coefficients
-// and fills the tables.  Returns the lane's contribution to the class word of round j.
+// and fills the tables, including the class word of round j (the same for the four groups).
 template <int NT>
-__device__ __forceinline__ unsigned prepare_record(const Sim3D &P, uint2 rec, float d0, float d1, float d2, float sf, WarpTables<NT> &T, int g,
-                                                   int j)
+__device__ __forceinline__ void prepare_record(const Sim3D &P, uint2 rec, float d0, float d1, float d2, float sf, WarpTables<NT> &T, int g,
+                                               int j)
 {
     RecS r;
     r.A = 0.f;
@@ -103,48 +110,43 @@ __device__ __forceinline__ unsigned prepare_record(const Sim3D &P, uint2 rec, fl
     T.cell[g][j] = rec.x;
     T.opdz[g][j] = rec.y;
     const unsigned op = rec.y >> 24;
+    const bool step = op == LOC_OP_STEP;
     unsigned cls = (op == LOC_OP_BG || op == LOC_OP_SAVE || op == LOC_OP_LOAD) ? LOC_CLS_CTRL : 0u;
-    if (op == LOC_OP_STEP) {
-        const float4 k = __ldg(P.kin + rec.x);
-        const float v0 = -(k.x * d0 + k.y * d1 + k.z * d2);  // DESIGN R6
-        const float sig = k.w;
+    float2 ke[NT];
+    float s = 0.f, w = 0.f, amp = 0.f, tau0m = 0.f;
+    float4 k = make_float4(0.f, 0.f, 0.f, 1.f);
+    unsigned mexp = 0u, mser = 0u;
+    if (step) {
+        k = __ldg(P.kin + rec.x);
         const unsigned dz = rec.y & 0x1fffffu;
         const int lev = (rec.y >> 21) & 7;
-        const float s = (float)dz * sf;
-        const float w = (float)dz * P.inv_ndir * __int_as_float((127 - LOC_LB + lev) << 23);
-        const float inv_sig = __fdividef(1.0f, sig);
-        const float amp = P.dv * 0.3989422804f * inv_sig;
+        s = (float)dz * sf;
+        w = (float)dz * P.inv_ndir * __int_as_float((127 - LOC_LB + lev) << 23);
+        amp = P.dv * 0.3989422804f * __fdividef(1.0f, k.w);
         const float2 *cf = P.coef + (long long)rec.x * P.nsp + P.slot0;
-        float tau0m = 0.f;
-        unsigned thick = 0u;
 #pragma unroll
         for (int t = 0; t < NT; t++) {
-            const float2 ke = __ldg(cf + t);
-            const float ks = ke.x * s;
-            const float tau0 = fabsf(ks) * amp;
+            ke[t] = __ldg(cf + t);
+            const float tau0 = fabsf(ke[t].x * s) * amp;
             tau0m = fmaxf(tau0m, tau0);
-            float2 q;
-            float scale;
-            if (tau0 >= LOC_THIN_TAU) {
-                thick |= 1u << t;
-                q.x = -ks * LOC_LOG2E;
-                q.y = __fdividef(ke.y, ke.x);  // source function in occupation-number units
-                scale = __fdividef(w, ks);
-            } else {
-                q.x = ks;
-                q.y = ke.y * s;
-                scale = w;
-            }
-            T.tp[g][j][t] = q;
-            T.sc[g][j][t] = scale;
+            if (tau0 > LOC_SER_TAU) mexp |= 1u << t;
+            if (tau0 < LOC_EXP_TAU) mser |= 1u << t;
         }
+        cls |= LOC_CLS_STEP | mexp | (mser << LOC_CLS_THIN_SHIFT);
+    } else {
+#pragma unroll
+        for (int t = 0; t < NT; t++) ke[t] = make_float2(0.f, 0.f);
+    }
+    unsigned thick = 0u;
+    if (step) {
         // window half-width in sigma: the profile mass left outside stays a fixed fraction (that of xmin at tau0 <= 1) of
         // the escape sum  sum_c phi_c f(tau_c) ~ 1/tau0  of an optically thick step (DESIGN 5.3)
+        const float v0 = -(k.x * d0 + k.y * d1 + k.z * d2);  // DESIGN R6
         float X = P.xmin;
         if (tau0m > 1.0f) X = sqrtf(fmaf(2.0f, __logf(tau0m), X * X));
         const float inv_dv = __fdividef(1.0f, P.dv);
         const float cc = fmaf(v0, inv_dv, 0.5f * (float)(P.nch - 1));
-        const float sigch = sig * inv_dv;
+        const float sigch = k.w * inv_dv;
         const float hw = X * sigch;
         const int clo = max(0, (int)ceilf(cc - hw)), chi = min(P.nch - 1, (int)floorf(cc + hw));
         // the span: 32 channels from a multiple of 4, centred on the line, inside the band
@@ -154,26 +156,41 @@ __device__ __forceinline__ unsigned prepare_record(const Sim3D &P, uint2 rec, fl
         const float lim = LOC_XCLIP * sigch;
         const bool fast = P.nch >= LOC_SPAN && (clo >= wb || cc - (float)wb >= lim) && (chi <= wb + LOC_SPAN - 1 || (float)(wb + LOC_SPAN - 1) - cc >= lim);
         if (P.nch < LOC_SPAN) wb = 0;
-        r.ky = P.dv * 0.8493218f * inv_sig;  // sqrt(log2(e) / 2) in channel units
+        if (!fast) {
+            cls |= LOC_CLS_SLOW;
+            T.win[g][j] = make_int2(clo, chi);
+        }
+        r.ky = 0.8493218f * __fdividef(1.0f, sigch);  // sqrt(log2(e) / 2) in channel units
         r.A = ((float)wb - cc) * r.ky;
         r.lamp = __log2f(amp);
-        r.wbop = (unsigned)wb | (thick << LOC_THICK_SHIFT) | LOC_RS_STEP;
-        T.w[g][j] = w;
-        T.h5[g][j] = 5.0f * sigch;
-        T.cc[g][j] = cc;
-        T.win[g][j] = make_int2(clo, chi);
-        cls |= LOC_CLS_STEP | thick | ((~thick & ((1u << NT) - 1u)) << LOC_CLS_THIN_SHIFT) | (fast ? 0u : LOC_CLS_SLOW);
+        r.wbop = (unsigned)wb | LOC_RS_STEP;
     } else {
-#pragma unroll
-        for (int t = 0; t < NT; t++) {
-            T.tp[g][j][t] = make_float2(0.f, 0.f);
-            T.sc[g][j][t] = 0.f;
-        }
-        T.w[g][j] = 0.f;
         T.win[g][j] = make_int2(0, -1);
     }
+    T.w[g][j] = w;
+    // class of the round: OR over the four groups (lanes j, 8 + j, 16 + j, 24 + j)
+    cls |= __shfl_xor_sync(0xffffffffu, cls, 8);
+    cls |= __shfl_xor_sync(0xffffffffu, cls, 16);
+    if (g == 0) T.cls[j] = cls;
+    const unsigned any_exp = cls & 0xfffu, any_ser = (cls >> LOC_CLS_THIN_SHIFT) & 0xfffu;
+    // form per transition: the series unless some ray of the round must use the exponential; in a round that holds both
+    // extremes every ray takes the form its own tau0 prefers
+    thick = (any_exp & ~any_ser) | (any_exp & any_ser & ~mser);
+#pragma unroll
+    for (int t = 0; t < NT; t++) {
+        const float ks = ke[t].x * s;
+        float2 q;
+        if ((thick >> t) & 1u) {
+            q.x = -ks * LOC_LOG2E;
+            q.y = __fdividef(ke[t].y, ke[t].x);  // source function in occupation-number units
+        } else {
+            q.x = ks;
+            q.y = ke[t].y * s;
+        }
+        T.tp[g][j][t] = step ? q : make_float2(0.f, 0.f);
+    }
+    r.wbop |= (step ? thick : 0u) << LOC_THICK_SHIFT;
     T.rs[g][j] = r;
-    return cls;
 }
 
 // One pass over a span of 32 channels for the four ray steps of a round: lane l8 of a group updates the quad at `sq`
@@ -181,6 +198,7 @@ __device__ __forceinline__ unsigned prepare_record(const Sim3D &P, uint2 rec, fl
 //   MASK = false: the common path -- no masks, the quad is known to lie inside the spectrum
 //   MASK = true : channel k takes part iff m[k]; the quad is loaded / stored iff `inq`
 // Accumulates the lane's partial sums a[t] += sum_k n_k X_k, b[t] += sum_k X_k, sphi += sum_k phi_k.
+#define LOC_SERIES(C0, P, B2, B3, B4, B5) fma2(C0, fma2(C0, fma2(C0, fma2(C0, B5, B4), B3), B2), P)
 template <int NT, bool MASK>
 __device__ __forceinline__ void span_pass(float *sq, int nchp, const float2 *tpr, const RecS &rs, const float (&jf)[4], unsigned thick,
                                           unsigned any_thick, unsigned any_thin, bool inq, const bool (&m)[4], float (&a)[NT], float (&b)[NT],
@@ -196,8 +214,9 @@ __device__ __forceinline__ void span_pass(float *sq, int nchp, const float2 *tpr
     sphi += (e[0] + e[1]) + (e[2] + e[3]);
     const f32x2 P01 = pk2(e[0], e[1]), P23 = pk2(e[2], e[3]);
     const f32x2 ONE2 = pk2(1.0f, 1.0f), MONE2 = pk2(-1.0f, -1.0f);
-    f32x2 B2a = 0ull, B2b = 0ull, B3a = 0ull, B3b = 0ull, B4a = 0ull, B4b = 0ull;
-    if (any_thin) {  // powers of phi for the series, shared by all thin transitions of the round
+    f32x2 B2a = 0ull, B2b = 0ull, B3a = 0ull, B3b = 0ull, B4a = 0ull, B4b = 0ull, B5a = 0ull, B5b = 0ull;
+    // powers of phi for the series, shared by the transitions of the round that use it (all rays thin, or mixed)
+    if ((~any_thick | any_thin) & ((1u << NT) - 1u)) {
         const f32x2 K2 = pk2(-0.5f, -0.5f), K3 = pk2(1.0f / 6.0f, 1.0f / 6.0f), K4 = pk2(-1.0f / 24.0f, -1.0f / 24.0f);
         const f32x2 s01 = mul2(P01, P01), s23 = mul2(P23, P23);
         B2a = mul2(s01, K2);
@@ -206,48 +225,67 @@ __device__ __forceinline__ void span_pass(float *sq, int nchp, const float2 *tpr
         B3b = mul2(mul2(s23, P23), K3);
         B4a = mul2(mul2(s01, s01), K4);
         B4b = mul2(mul2(s23, s23), K4);
+        const f32x2 K5 = pk2(-0.2f, -0.2f);
+        B5a = mul2(mul2(B4a, P01), K5);
+        B5b = mul2(mul2(B4b, P23), K5);
     }
+    // Three phases, so that the loads and the common tail of all transitions are straight-line code the scheduler can
+    // interleave (the form of X is chosen by warp-uniform branches per transition).
+    float2 q[NT];
+    float4 n4[NT];
 #pragma unroll
     for (int t = 0; t < NT; t++) {
-        const float2 q = tpr[t];
-        float4 n4 = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (!MASK || inq) n4 = *reinterpret_cast<const float4 *>(sq + t * nchp);
-        const f32x2 N01 = pk2(n4.x, n4.y), N23 = pk2(n4.z, n4.w);
-        const f32x2 C0 = pk2(q.x, q.x), C1 = pk2(q.y, q.y);
-        f32x2 X01, X23, AL;
-        if (!((any_thick >> t) & 1u)) {  // every stepping ray of the warp is thin in this transition
-            X01 = fma2(C0, fma2(C0, fma2(C0, B4a, B3a), B2a), P01);
-            X23 = fma2(C0, fma2(C0, fma2(C0, B4b, B3b), B2b), P23);
-            AL = pk2(-q.x, -q.x);
+        q[t] = tpr[t];
+        n4[t] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (!MASK || inq) n4[t] = *reinterpret_cast<const float4 *>(sq + t * nchp);
+    }
+    f32x2 X01[NT], X23[NT];
+    float al[NT];
+#pragma unroll
+    for (int t = 0; t < NT; t++) {
+        const f32x2 C0 = pk2(q[t].x, q[t].x);
+        if (!((any_thick >> t) & 1u)) {  // every stepping ray of the warp uses the series in this transition
+            X01[t] = LOC_SERIES(C0, P01, B2a, B3a, B4a, B5a);
+            X23[t] = LOC_SERIES(C0, P23, B2b, B3b, B4b, B5b);
+            al[t] = -q[t].x;
         } else {
             float z0, z1, z2, z3;
             upk2(mul2(C0, P01), z0, z1);
             upk2(mul2(C0, P23), z2, z3);
             const f32x2 E01 = pk2(ex2f(z0), ex2f(z1)), E23 = pk2(ex2f(z2), ex2f(z3));
-            X01 = fma2(E01, MONE2, ONE2);
-            X23 = fma2(E23, MONE2, ONE2);
-            AL = MONE2;
+            X01[t] = fma2(E01, MONE2, ONE2);
+            X23[t] = fma2(E23, MONE2, ONE2);
+            al[t] = -1.0f;
             if ((any_thin >> t) & 1u) {  // mixed: both forms, selected per ray
                 const bool tk = (thick >> t) & 1u;
                 float x0, x1, x2, x3, s0, s1, s2, s3;
-                upk2(X01, x0, x1);
-                upk2(X23, x2, x3);
-                upk2(fma2(C0, fma2(C0, fma2(C0, B4a, B3a), B2a), P01), s0, s1);
-                upk2(fma2(C0, fma2(C0, fma2(C0, B4b, B3b), B2b), P23), s2, s3);
-                X01 = pk2(tk ? x0 : s0, tk ? x1 : s1);
-                X23 = pk2(tk ? x2 : s2, tk ? x3 : s3);
-                const float al = tk ? -1.0f : -q.x;
-                AL = pk2(al, al);
+                upk2(X01[t], x0, x1);
+                upk2(X23[t], x2, x3);
+                upk2(LOC_SERIES(C0, P01, B2a, B3a, B4a, B5a), s0, s1);
+                upk2(LOC_SERIES(C0, P23, B2b, B3b, B4b, B5b), s2, s3);
+                X01[t] = pk2(tk ? x0 : s0, tk ? x1 : s1);
+                X23[t] = pk2(tk ? x2 : s2, tk ? x3 : s3);
+                al[t] = tk ? -1.0f : -q[t].x;
             }
         }
+    }
+#pragma unroll
+    for (int t = 0; t < NT; t++) {
+        const f32x2 N01 = pk2(n4[t].x, n4[t].y), N23 = pk2(n4[t].z, n4[t].w);
+        const f32x2 C1 = pk2(q[t].y, q[t].y), AL = pk2(al[t], al[t]);
         float a0, a1, b0, b1;
-        upk2(fma2(N01, X01, mul2(N23, X23)), a0, a1);
-        upk2(add2(X01, X23), b0, b1);
-        a[t] += a0 + a1;
-        b[t] += b0 + b1;
+        upk2(fma2(N01, X01[t], mul2(N23, X23[t])), a0, a1);
+        upk2(add2(X01[t], X23[t]), b0, b1);
+        if (MASK) {  // several passes may follow one another
+            a[t] += a0 + a1;
+            b[t] += b0 + b1;
+        } else {
+            a[t] = a0 + a1;
+            b[t] = b0 + b1;
+        }
         float r0, r1, r2, r3;
-        upk2(fma2(X01, fma2(AL, N01, C1), N01), r0, r1);
-        upk2(fma2(X23, fma2(AL, N23, C1), N23), r2, r3);
+        upk2(fma2(X01[t], fma2(AL, N01, C1), N01), r0, r1);
+        upk2(fma2(X23[t], fma2(AL, N23, C1), N23), r2, r3);
         if (!MASK || inq) *reinterpret_cast<float4 *>(sq + t * nchp) = make_float4(r0, r1, r2, r3);
     }
 }
@@ -255,8 +293,6 @@ __device__ __forceinline__ void span_pass(float *sq, int nchp, const float2 *tpr
 template <int NT, bool GEOM>
 __global__ void __launch_bounds__(32) k_sim3d(Sim3D P)
 {
-    constexpr int NV = 2 * NT;                 // reduced values per step: a[t], b[t]
-    constexpr int NPASS = (NV + 7) / 8;        // 8-lane butterflies of up to 8 values
     extern __shared__ __align__(16) float smem[];
     __shared__ WarpTables<NT> T;               // separate object: no aliasing with the spectra
     const int lane = threadIdx.x, grp = lane >> 3, l8 = lane & 7;
@@ -307,12 +343,7 @@ __global__ void __launch_bounds__(32) k_sim3d(Sim3D P)
         have_next = !done && off < end;
         nrec = make_uint2(0u, LOC_OP_NOP << 24);
         if (have_next && off + l8 < end) nrec = __ldg(P.stream + off + l8);
-        {
-            unsigned c = prepare_record<NT>(P, rec, d0, d1, d2, sf, T, grp, l8);
-            c |= __shfl_xor_sync(0xffffffffu, c, 8);
-            c |= __shfl_xor_sync(0xffffffffu, c, 16);
-            if (lane < LOC_CHUNK) T.cls[lane] = c;
-        }
+        prepare_record<NT>(P, rec, d0, d1, d2, sf, T, grp, l8);
         __syncwarp();
 
         // ---- 8 rounds: every group consumes one record per round ----
@@ -366,67 +397,42 @@ __global__ void __launch_bounds__(32) k_sim3d(Sim3D P)
                     base += LOC_SPAN;
                 }
             }
-            // ---- reductions over the 8 lanes of each group ----
+            // ---- reduction over the 8 lanes of each group, through shared memory (no selects, DESIGN 6.4) ----
             sphi += __shfl_xor_sync(0xffffffffu, sphi, 4);
             sphi += __shfl_xor_sync(0xffffffffu, sphi, 2);
             sphi += __shfl_xor_sync(0xffffffffu, sphi, 1);
-            float v[NPASS * 8];
+            float2 *pg = T.part[grp];
 #pragma unroll
-            for (int i = 0; i < NPASS * 8; i++) v[i] = 0.f;
+            for (int t = 0; t < NT; t++) pg[t * WarpTables<NT>::ROW + l8] = make_float2(a[t], b[t]);
+            __syncwarp();
+            // lane t of a group adds up row t and issues the two float atomics of (cell, transition t) as one 64-bit RED
+            const bool step = rs.wbop & LOC_RS_STEP;
+            const unsigned cell = T.cell[grp][r];
+            const float w = T.w[grp][r];
+            const float wesc = w - w * sphi;  // photons emitted outside the updated channels escape (DESIGN 5.3)
 #pragma unroll
-            for (int t = 0; t < NT; t++) {
-                v[t] = a[t];
-                v[NT + t] = b[t];
-            }
-            float tot[NPASS];
-#pragma unroll
-            for (int p = 0; p < NPASS; p++) {
-                float *u = v + 8 * p;
-                {
-                    const bool up = l8 & 4;
-#pragma unroll
-                    for (int i = 0; i < 4; i++) {
-                        const float keep = up ? u[i + 4] : u[i], send = up ? u[i] : u[i + 4];
-                        u[i] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
-                    }
-                }
-                {
-                    const bool up = l8 & 2;
-#pragma unroll
-                    for (int i = 0; i < 2; i++) {
-                        const float keep = up ? u[i + 2] : u[i], send = up ? u[i] : u[i + 2];
-                        u[i] = keep + __shfl_xor_sync(0xffffffffu, send, 2);
-                    }
-                }
-                {
-                    const bool up = l8 & 1;
-                    const float keep = up ? u[1] : u[0], send = up ? u[0] : u[1];
-                    tot[p] = keep + __shfl_xor_sync(0xffffffffu, send, 1);
+            for (int t0 = 0; t0 < NT; t0 += 8) {
+                const int t = t0 + l8;
+                if (step && t < NT) {
+                    const float4 *row = reinterpret_cast<const float4 *>(pg + t * WarpTables<NT>::ROW);
+                    const float4 r0 = row[0], r1 = row[1], r2 = row[2], r3 = row[3];
+                    const f32x2 s01 = add2(add2(pk2(r0.x, r0.y), pk2(r0.z, r0.w)), add2(pk2(r1.x, r1.y), pk2(r1.z, r1.w)));
+                    const f32x2 s23 = add2(add2(pk2(r2.x, r2.y), pk2(r2.z, r2.w)), add2(pk2(r3.x, r3.y), pk2(r3.z, r3.w)));
+                    float A, B;
+                    upk2(add2(s01, s23), A, B);
+                    // scale of the sums: w for the series form, w / (kappa s) for the exponential form (c0 = -kappa s log2 e)
+                    const float sc = ((thick >> t) & 1u) ? __fdividef(-LOC_LOG2E * w, tpr[t].x) : w;
+                    float2 *cn = P.cnt + (long long)cell * P.nsp + P.slot0 + t;
+                    asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(cn), "f"(A * sc), "f"(fmaf(B, sc, wesc)) : "memory");
                 }
             }
-            // lane l8 of a group now holds the group totals of values l8, 8 + l8, 16 + l8
-            if (rs.wbop & LOC_RS_STEP) {
-                const unsigned cell = T.cell[grp][r];
-                const float w = T.w[grp][r];
-                float2 *cn = P.cnt + (long long)cell * P.nsp + P.slot0;
-                const float wesc = w - w * sphi;  // photons emitted outside the updated channels escape (DESIGN 5.3)
-                const float *scr = T.sc[grp][r];
-#pragma unroll
-                for (int p = 0; p < NPASS; p++) {
-                    const int i = 8 * p + l8;
-                    if (i < NT)
-                        atomicAdd(&cn[i].x, tot[p] * scr[i]);
-                    else if (i < NV)
-                        atomicAdd(&cn[i - NT].y, fmaf(tot[p], scr[i - NT], wesc));
-                }
-                if (l8 == 0) {
-                    mysteps++;
-                    if (GEOM) {
-                        atomicAdd(&P.visits[cell], 1u);
-                        atomicAdd(&P.pathz[cell], T.opdz[grp][r] & 0x1fffffu);
-                        const float h5 = T.h5[grp][r], cc = T.cc[grp][r];  // 5 sigma in channels
-                        myactive += max(0, min(P.nch - 1, (int)floorf(cc + h5)) - max(0, (int)ceilf(cc - h5)) + 1);
-                    }
+            if (step && l8 == 0) {
+                mysteps++;
+                if (GEOM) {
+                    atomicAdd(&P.visits[cell], 1u);
+                    atomicAdd(&P.pathz[cell], T.opdz[grp][r] & 0x1fffffu);
+                    const float h5 = 5.0f * 0.8493218f / rs.ky, cc = (float)wb - rs.A / rs.ky;  // 5 sigma in channels, line centre
+                    myactive += max(0, min(P.nch - 1, (int)floorf(cc + h5)) - max(0, (int)ceilf(cc - h5)) + 1);
                 }
             }
             __syncwarp();  // the next round's quads were written by other lanes
