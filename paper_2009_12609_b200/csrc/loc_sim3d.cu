@@ -8,18 +8,30 @@
 // line; lane l8 of the group owns the aligned quad  span + 4 l8 .. + 3, so that
 //   * the photon spectrum of a ray lives in shared memory and is read / written with one 128-bit access per lane and
 //     transition, conflict free for any span position (a quarter-warp is one shared-memory phase);
-//   * the per-channel arithmetic is done on packed pairs (fma.rn.f32x2): the kernel is bound by instruction issue and by
-//     the 16-lane ALU pipe (selects, compares, logic: 2 cycles each), not by FP32 throughput, so the common path has no
-//     masks and no selects at all -- a span always lies inside the band, and channels of the span outside the nominal
-//     window are simply updated too;
-//   * the sums over a lane's 4 channels are free, and the cross-lane reduction is an 8-lane halving butterfly whose every
-//     instruction serves 4 ray steps;
-//   * all per-step scalar work (record decode, Doppler shift, window, per-transition coefficients, classification of the
-//     round) is done lane-parallel for 8 records x 4 rays at once in a "prepare" phase.
-// Steps whose window does not fit one span (very thick lines, bands narrower than 32 channels) take a masked multi-pass
-// path.  The four groups stay in lock step: every round each group consumes exactly one stream record (tasks are padded
-// to whole chunks of 8 records by the path builder); the rare spectrum operations (background, save, load) are executed
-// by the whole warp for the group that needs them.
+//   * the per-channel arithmetic is done on packed pairs (fma.rn.f32x2) and is ONE straight-line expression for both
+//     regimes of the optical depth (below): no masks, no selects, no branches per transition, so that the 2 NT
+//     independent chains of a round give the instruction-level parallelism that ~2 warps per scheduler need;
+//   * the sums over a lane's 4 channels are free, and the cross-lane reduction goes through shared memory: lane t of
+//     the group adds up the 8 partial sums of transition t and issues ONE 64-bit RED for the cell's (SJ, ESC) pair;
+//   * all per-step scalar work (record decode, Doppler shift, window, per-transition coefficients, scale of the sums,
+//     counter offset) is done in a "prepare" phase, two lanes per record for 4 records x 4 rays at once, from cell data
+//     prefetched into registers one chunk ahead, and left in one shared-memory record per (ray, round): the round
+//     addresses everything with immediate offsets from one register.
+// All traced transitions (up to the shared-memory limit) go through ONE launch: the per-step overhead is paid once
+// (profiles/r1_v5_sim3d_C3.md: splitting 9 transitions over 2 launches cost ~10 ms per launch on C3).
+//
+// Unified per-channel factor (DESIGN 5.3).  With phi the profile value of the channel,
+//     X = (1 - 2^(Ce phi)) + U phi + C0 (B2 + C0 B3),   B2 = -phi^2 / 2,  B3 = phi^3 / 6
+//     n' = n + X (c1 + alpha n),     a += n X,   b += X
+// a ray step whose line-centre optical depth tau0 = kappa s phi_max is >= LOC_EXP_TAU uses the exponential form
+// (Ce = -kappa s log2 e, U = C0 = 0, c1 = S = eps / kappa, alpha = -1: X = 1 - e^-tau), a thinner one the series
+// (Ce = 0, U = 1, C0 = kappa s, c1 = eps s, alpha = -C0: X = phi f(tau), f = 1 - tau/2 + tau^2/6, truncation
+// tau^3/24 < 1.2e-6; ex2(0) = 1 exactly, so the first bracket vanishes).  1 - e^-tau by ex2.approx and a subtraction
+// has an absolute error of ~1e-7 per channel, i.e. < 1e-5 of the channel sums for tau0 >= 0.03.
+// Steps whose window does not fit one span (bands narrower than 32 channels, lines cut by the band edge, very wide
+// lines) take a masked multi-pass path written as a rolled loop.  The four groups stay in lock step: every round each
+// group consumes exactly one stream record (tasks are padded to whole chunks by the path builder); the rare spectrum
+// operations (background, save, load) are executed by the whole warp for the group that needs them.
 #include <math.h>
 #include <stdio.h>
 #include <stdlib.h>
@@ -29,12 +41,13 @@
 #include "loc_internal.cuh"
 
 #define LOC_GROUPS 4  // rays per warp
-#define LOC_CHUNK 8   // records per group and prepare phase (= LOC_TASK_ALIGN)
+#define LOC_CHUNK 4   // records per group and prepare phase (LOC_TASK_ALIGN is a multiple)
 #define LOC_SPAN 32   // channels per pass: 8 lanes x one aligned float4
 
 struct Sim3D {
     int nch, nchp, nsp, nslot;
     int slot0;  // first counter / coefficient slot handled by this launch (transitions may be split over launches)
+    int geom;   // also accumulate the geometry counters (visits, path sums, active channels)
     float dv, xmin, eps_tau, inv_ndir;
     const Dir3 *dirs;
     const unsigned char *task_dir;
@@ -51,312 +64,457 @@ struct Sim3D {
     Selection S;
 };
 
-// Per-record scalars every lane of the group reads each round (16 bytes, one broadcast LDS.128).
-//   y(channel wb + j) = A + j ky ;  phi = 2^(lamp - y^2)
-// wbop: bits 0..9 first channel of the span, bits 10..21 per-transition "thick" flags, bit 31 = the record is a STEP
-struct __align__(16) RecS {
-    float A, ky, lamp;
-    unsigned wbop;
-};
+// ---- shared-memory record of one (ray, round), written by the prepare phase --------------------------------------
+//   +0   float q0, q1, q2     log2 phi(channel wb + 16 + j) = q0 + j (q1 + j q2)      (j = -16 .. 15 inside the span)
+//   +12  uint  wbop           bits 0..9 first channel of the span, bit 29 = needs the masked path,
+//                             bit 30 = spectrum operation (BG / SAVE / LOAD), bit 31 = the record is a STEP
+//   +16  uint  coff           cell * nsp + slot0 : element offset of the cell's counter record (STEP); slot (SAVE / LOAD)
+//   +20  float w              a s / V_eff = dzeta / (h NDIR)
+//   +24  uint  opdz           opcode | level | dzeta (stream word)
+//   +28  uint  win            nominal channel window clo | chi << 16 (masked path; chi < clo = empty)
+//   +32  float4 tp[NT]        (C0, Ce, c1, alpha) per transition (header comment)
+//   +32 + 16 NT   float U[NT4]    1 = series, 0 = exponential; NT4 = NT rounded up to 4
+//   then          float sc[NT4]   scale of the channel sums: w (series) or w / (kappa s) (exponential)
 #define LOC_WB_MASK 0x3ffu
-#define LOC_THICK_SHIFT 10
+#define LOC_RS_SLOW 0x20000000u
+#define LOC_RS_CTRL 0x40000000u
 #define LOC_RS_STEP 0x80000000u
 
-// Class word of a round (one per chunk record index, OR over the four groups):
-//   bits 0..11 some stepping ray MUST use the exponential form in transition t (tau0 > LOC_SER_TAU),
-//   bits 12..23 some stepping ray MUST use the series (tau0 < LOC_EXP_TAU),
-//   bit 24 a spectrum operation is due, bit 25 some group steps, bit 26 some stepping group needs the masked path
-#define LOC_CLS_THIN_SHIFT 12
-#define LOC_CLS_CTRL (1u << 24)
-#define LOC_CLS_STEP (1u << 25)
-#define LOC_CLS_SLOW (1u << 26)
-
 #define LOC_XCLIP 3.9f     // a span may cut the nominal window, but never closer than this many sigma to the line centre
-// Two forms of the per-channel factor (DESIGN 5.3).  Exponential: X = 1 - 2^(c0 phi), accurate (ex2.approx plus the
-// subtraction) only while the line-centre optical depth of the step is >= LOC_EXP_TAU.  Series: X = phi f(tau) with
-// f = 1 - tau/2 + tau^2/6 - tau^3/24 + tau^4/120, truncation < 2e-6 while tau0 <= LOC_SER_TAU.  In between either form
-// will do, so a round whose four steps do not hold both extremes runs ONE form for the transition.
-#define LOC_EXP_TAU 0.03f
-#define LOC_SER_TAU 0.3f
+#define LOC_EXP_TAU 0.03f  // line-centre optical depth of a step from which the exponential form is used
 
-// shared-memory tables of one warp, written by the prepare phase
 template <int NT>
-struct WarpTables {
-    static constexpr int ROW = 10;                                  // float2 per row of partial sums (8 used): 80 bytes
-    static constexpr int PGW = NT * ROW * 2;                        // words per group ...
-    static constexpr int PG = (PGW + ((48 - PGW % 32) % 32)) / 2;   // ... padded to 16 mod 32 words (float2 units)
-    RecS rs[LOC_GROUPS][LOC_CHUNK];
-    float2 tp[LOC_GROUPS][LOC_CHUNK][NT];   // (c0, c1):  X_c = series ? phi + c0 (B2 + c0 (B3 + c0 (B4 + c0 B5))) : 1 - 2^(c0 phi)
-                                            //            n' = n + X (c1 + alpha n),  alpha = series ? -c0 : -1
-    unsigned cell[LOC_GROUPS][LOC_CHUNK];   // STEP: cell index; SAVE / LOAD: slot
-    unsigned opdz[LOC_GROUPS][LOC_CHUNK];   // opcode | level | dzeta (stream word)
-    float w[LOC_GROUPS][LOC_CHUNK];         // a s / V_eff = dzeta / (h NDIR)
-    int2 win[LOC_GROUPS][LOC_CHUNK];        // nominal channel window [clo, chi] (masked path)
-    unsigned cls[LOC_CHUNK];
-    float2 part[LOC_GROUPS][PG];            // per-lane partial sums (a_t, b_t) of the round: [group][t][lane] (rows of 10)
+struct Lay {
+    static constexpr int NT4 = (NT + 3) & ~3;
+    static constexpr int NH = (((NT + 1) / 2) + 1) & ~1;  // transitions prepared by the first lane of a record's pair (even)
+    static constexpr int TP = 32;                    // byte offset of tp[] in a record
+    static constexpr int UO = TP + 16 * NT;          // byte offset of U[]
+    static constexpr int SC = UO + 4 * NT4;          // byte offset of sc[]
+    static constexpr int RECB = SC + 4 * NT4;        // record bytes (multiple of 16)
+    // group stride: LOC_CHUNK records, padded so that the four groups start 8 banks apart (32-bit reads of the four
+    // groups in one instruction do not collide)
+    static constexpr int GW0 = LOC_CHUNK * RECB / 4;
+    static constexpr int GSB = 4 * (GW0 + ((8 + 32 - GW0 % 32) % 32));
+    // per-lane partial sums (a_t, b_t) of the round: [group][t][lane], rows of 10 float2 (8 used) = 80 bytes: the
+    // reducing lanes of a group read 8 different rows with LDS.128 conflict free; then one row of 8 floats: the lanes'
+    // sums of phi.  Groups 16 banks apart.
+    static constexpr int ROWB = 80;
+    static constexpr int PHI = NT * ROWB;
+    static constexpr int PW0 = (NT * ROWB + 32) / 4;
+    static constexpr int PGB = 4 * (PW0 + ((16 + 32 - PW0 % 32) % 32));
+    static constexpr int OFF_REC = 0;                                  // relative to the table base
+    static constexpr int OFF_CLS = OFF_REC + LOC_GROUPS * GSB;
+    static constexpr int OFF_PART = OFF_CLS + 4 * LOC_CHUNK;
+    static constexpr int BYTES = OFF_PART + LOC_GROUPS * PGB;
 };
 
-// Prepare phase: lane (g, j) decodes record j of the chunk of group g, loads the cell's kinematics and line coefficients
-// and fills the tables, including the class word of round j (the same for the four groups).
-template <int NT>
-__device__ __forceinline__ void prepare_record(const Sim3D &P, uint2 rec, float d0, float d1, float d2, float sf, WarpTables<NT> &T, int g,
-                                               int j)
+// ---- shared memory through 32-bit addresses with immediate offsets ------------------------------------------------
+__device__ __forceinline__ float rcpf(float x)
 {
-    RecS r;
-    r.A = 0.f;
-    r.ky = 0.f;
-    r.lamp = -INFINITY;  // phi = 2^(-inf) = 0 for records that are not steps: the round leaves their spectra untouched
-    r.wbop = 0u;
-    T.cell[g][j] = rec.x;
-    T.opdz[g][j] = rec.y;
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+template <int OFF = 0>
+__device__ __forceinline__ float4 lds128(unsigned a)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+%5];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a), "n"(OFF));
+    return v;
+}
+template <int OFF = 0>
+__device__ __forceinline__ uint4 lds128u(unsigned a)
+{
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4+%5];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a), "n"(OFF));
+    return v;
+}
+template <int OFF = 0>
+__device__ __forceinline__ float lds32(unsigned a)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v) : "r"(a), "n"(OFF));
+    return v;
+}
+template <int OFF = 0>
+__device__ __forceinline__ unsigned lds32u(unsigned a)
+{
+    unsigned v;
+    asm volatile("ld.shared.u32 %0, [%1+%2];" : "=r"(v) : "r"(a), "n"(OFF));
+    return v;
+}
+template <int OFF = 0>
+__device__ __forceinline__ float2 lds64(unsigned a)
+{
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2+%3];" : "=f"(v.x), "=f"(v.y) : "r"(a), "n"(OFF));
+    return v;
+}
+template <int OFF = 0>
+__device__ __forceinline__ void sts128(unsigned a, float4 v)
+{
+    asm volatile("st.shared.v4.f32 [%0+%1], {%2, %3, %4, %5};" ::"r"(a), "n"(OFF), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+template <int OFF = 0>
+__device__ __forceinline__ void sts128u(unsigned a, uint4 v)
+{
+    asm volatile("st.shared.v4.u32 [%0+%1], {%2, %3, %4, %5};" ::"r"(a), "n"(OFF), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+template <int OFF = 0>
+__device__ __forceinline__ void sts64(unsigned a, float2 v)
+{
+    asm volatile("st.shared.v2.f32 [%0+%1], {%2, %3};" ::"r"(a), "n"(OFF), "f"(v.x), "f"(v.y) : "memory");
+}
+template <int OFF = 0>
+__device__ __forceinline__ void sts32(unsigned a, float v)
+{
+    asm volatile("st.shared.f32 [%0+%1], %2;" ::"r"(a), "n"(OFF), "f"(v) : "memory");
+}
+template <int OFF = 0>
+__device__ __forceinline__ void sts32u(unsigned a, unsigned v)
+{
+    asm volatile("st.shared.u32 [%0+%1], %2;" ::"r"(a), "n"(OFF), "r"(v) : "memory");
+}
+
+
+// Cell data of one stream record as the prepare phase needs it: lane `half` (0 / 1) of the record's lane pair holds the
+// kinematics and the (kappa, eps) pairs of its transitions  half * NH .. half * NH + NH - 1.
+template <int NT>
+struct CellRegs {
+    float4 kin;
+    float4 cf[Lay<NT>::NH / 2];
+};
+
+template <int NT>
+__device__ __forceinline__ void load_cell(const Sim3D &P, uint2 rec, int half, CellRegs<NT> &C)
+{
+    typedef Lay<NT> L;
+    if ((rec.y >> 24) != LOC_OP_STEP) return;
+    C.kin = __ldg(P.kin + rec.x);
+    // records are 16-byte aligned: nsp, slot0 and NH are even (the pad element after an odd NT is read but not used)
+    const float4 *cf = reinterpret_cast<const float4 *>(P.coef + (long long)rec.x * P.nsp + P.slot0 + half * L::NH);
+#pragma unroll
+    for (int i = 0; i < L::NH / 2; i++)
+        if (half * L::NH + 2 * i < NT) C.cf[i] = __ldg(cf + i);
+}
+
+// Prepare phase: lanes (g, 2 j) and (g, 2 j + 1) decode record j of the chunk of group g and fill its shared-memory
+// record at `rb`; returns the record's flag bits (LOC_RS_*).  `nact` = number of channels within 5 sigma of the line
+// centre (the counting rule of the metric) for STEP records when the geometry counters are on.
+template <int NT>
+__device__ __forceinline__ unsigned prepare_record(const Sim3D &P, uint2 rec, const CellRegs<NT> &C, float d0, float d1, float d2, float sf,
+                                                   unsigned rb, int half, int &nact)
+{
+    typedef Lay<NT> L;
     const unsigned op = rec.y >> 24;
     const bool step = op == LOC_OP_STEP;
-    unsigned cls = (op == LOC_OP_BG || op == LOC_OP_SAVE || op == LOC_OP_LOAD) ? LOC_CLS_CTRL : 0u;
-    float2 ke[NT];
+    unsigned flags = (op == LOC_OP_BG || op == LOC_OP_SAVE || op == LOC_OP_LOAD) ? LOC_RS_CTRL : 0u;
+    const int t0 = half * L::NH;
+    float2 ke[L::NH];
+#pragma unroll
+    for (int i = 0; i < L::NH; i++) ke[i] = make_float2(0.f, 0.f);
     float s = 0.f, w = 0.f, amp = 0.f, tau0m = 0.f;
     float4 k = make_float4(0.f, 0.f, 0.f, 1.f);
-    unsigned mexp = 0u, mser = 0u;
     if (step) {
-        k = __ldg(P.kin + rec.x);
+        k = C.kin;
         const unsigned dz = rec.y & 0x1fffffu;
         const int lev = (rec.y >> 21) & 7;
         s = (float)dz * sf;
         w = (float)dz * P.inv_ndir * __int_as_float((127 - LOC_LB + lev) << 23);
-        amp = P.dv * 0.3989422804f * __fdividef(1.0f, k.w);
-        const float2 *cf = P.coef + (long long)rec.x * P.nsp + P.slot0;
+        amp = P.dv * 0.3989422804f * rcpf(k.w);
 #pragma unroll
-        for (int t = 0; t < NT; t++) {
-            ke[t] = __ldg(cf + t);
-            const float tau0 = fabsf(ke[t].x * s) * amp;
-            tau0m = fmaxf(tau0m, tau0);
-            if (tau0 > LOC_SER_TAU) mexp |= 1u << t;
-            if (tau0 < LOC_EXP_TAU) mser |= 1u << t;
+        for (int i = 0; i < L::NH; i += 2) {
+            ke[i] = make_float2(C.cf[i / 2].x, C.cf[i / 2].y);
+            ke[i + 1] = make_float2(C.cf[i / 2].z, C.cf[i / 2].w);
         }
-        cls |= LOC_CLS_STEP | mexp | (mser << LOC_CLS_THIN_SHIFT);
-    } else {
 #pragma unroll
-        for (int t = 0; t < NT; t++) ke[t] = make_float2(0.f, 0.f);
+        for (int i = 0; i < L::NH; i++)
+            if (t0 + i < NT) tau0m = fmaxf(tau0m, fabsf(ke[i].x * s) * amp);
+        flags |= LOC_RS_STEP;
     }
-    unsigned thick = 0u;
+    tau0m = fmaxf(tau0m, __shfl_xor_sync(0xffffffffu, tau0m, 1));
+    float q0 = -INFINITY, q1 = 0.f, q2 = 0.f;  // phi = 2^(-inf) = 0 for records that are not steps: the round leaves their spectra untouched
+    unsigned wb = 0u, win = 1u;                // clo = 1 > chi = 0: empty window
+    nact = 0;
     if (step) {
         // window half-width in sigma: the profile mass left outside stays a fixed fraction (that of xmin at tau0 <= 1) of
         // the escape sum  sum_c phi_c f(tau_c) ~ 1/tau0  of an optically thick step (DESIGN 5.3)
         const float v0 = -(k.x * d0 + k.y * d1 + k.z * d2);  // DESIGN R6
         float X = P.xmin;
         if (tau0m > 1.0f) X = sqrtf(fmaf(2.0f, __logf(tau0m), X * X));
-        const float inv_dv = __fdividef(1.0f, P.dv);
-        const float cc = fmaf(v0, inv_dv, 0.5f * (float)(P.nch - 1));
+        const float inv_dv = rcpf(P.dv);
+        const float cc = fmaf(v0, inv_dv, 0.5f * (float)(P.nch - 1));  // line centre in channel units
         const float sigch = k.w * inv_dv;
         const float hw = X * sigch;
         const int clo = max(0, (int)ceilf(cc - hw)), chi = min(P.nch - 1, (int)floorf(cc + hw));
         // the span: 32 channels from a multiple of 4, centred on the line, inside the band
         const int wbmax = (P.nch - LOC_SPAN) & ~3;
-        int wb = 4 * (int)rintf((cc - 15.5f) * 0.25f);
-        wb = max(0, min(wb, wbmax));
+        int iwb = 4 * (int)rintf((cc - 15.5f) * 0.25f);
+        iwb = max(0, min(iwb, wbmax));
         const float lim = LOC_XCLIP * sigch;
-        const bool fast = P.nch >= LOC_SPAN && (clo >= wb || cc - (float)wb >= lim) && (chi <= wb + LOC_SPAN - 1 || (float)(wb + LOC_SPAN - 1) - cc >= lim);
-        if (P.nch < LOC_SPAN) wb = 0;
-        if (!fast) {
-            cls |= LOC_CLS_SLOW;
-            T.win[g][j] = make_int2(clo, chi);
-        }
-        r.ky = 0.8493218f * __fdividef(1.0f, sigch);  // sqrt(log2(e) / 2) in channel units
-        r.A = ((float)wb - cc) * r.ky;
-        r.lamp = __log2f(amp);
-        r.wbop = (unsigned)wb | LOC_RS_STEP;
-    } else {
-        T.win[g][j] = make_int2(0, -1);
+        const bool fast = P.nch >= LOC_SPAN && (clo >= iwb || cc - (float)iwb >= lim) && (chi <= iwb + LOC_SPAN - 1 || (float)(iwb + LOC_SPAN - 1) - cc >= lim);
+        if (P.nch < LOC_SPAN) iwb = 0;
+        if (!fast) flags |= LOC_RS_SLOW;
+        if (chi >= clo) win = (unsigned)clo | ((unsigned)chi << 16);
+        // log2 phi(channel wb + 16 + j) = lamp - (A + j ky)^2 with A = (wb + 16 - cc) ky: the quadratic in j is expanded
+        // around the middle of the span, where |A| is a few channels only (no cancellation between large terms)
+        const float ky = 0.8493218f * rcpf(sigch);  // sqrt(log2(e) / 2) in channel units
+        const float A = ((float)(iwb + 16) - cc) * ky;
+        q0 = fmaf(-A, A, __log2f(amp));
+        q1 = -2.0f * A * ky;
+        q2 = -ky * ky;
+        wb = (unsigned)iwb;
+        if (P.geom) nact = max(0, min(P.nch - 1, (int)floorf(cc + 5.0f * sigch)) - max(0, (int)ceilf(cc - 5.0f * sigch)) + 1);
     }
-    T.w[g][j] = w;
-    // class of the round: OR over the four groups (lanes j, 8 + j, 16 + j, 24 + j)
-    cls |= __shfl_xor_sync(0xffffffffu, cls, 8);
-    cls |= __shfl_xor_sync(0xffffffffu, cls, 16);
-    if (g == 0) T.cls[j] = cls;
-    const unsigned any_exp = cls & 0xfffu, any_ser = (cls >> LOC_CLS_THIN_SHIFT) & 0xfffu;
-    // form per transition: the series unless some ray of the round must use the exponential; in a round that holds both
-    // extremes every ray takes the form its own tau0 prefers
-    thick = (any_exp & ~any_ser) | (any_exp & any_ser & ~mser);
+    if (half == 0) {
+        sts128u(rb, make_uint4(__float_as_uint(q0), __float_as_uint(q1), __float_as_uint(q2), wb | flags));
+        const unsigned coff = step ? rec.x * (unsigned)P.nsp + (unsigned)P.slot0 : rec.x;
+        sts128u(rb + 16, make_uint4(coff, __float_as_uint(w), rec.y, win));
+    }
+    // per transition, branch free: the exponential form from tau0 >= LOC_EXP_TAU (header comment); records that are not
+    // steps have kappa = eps = s = w = 0 and get all-zero coefficients
+    const float wos = w * rcpf(s);  // not used when s = 0
 #pragma unroll
-    for (int t = 0; t < NT; t++) {
-        const float ks = ke[t].x * s;
-        float2 q;
-        if ((thick >> t) & 1u) {
-            q.x = -ks * LOC_LOG2E;
-            q.y = __fdividef(ke[t].y, ke[t].x);  // source function in occupation-number units
-        } else {
-            q.x = ks;
-            q.y = ke[t].y * s;
+    for (int i = 0; i < L::NH; i++) {
+        const int t = t0 + i;
+        if (t < NT) {
+            const float ks = ke[i].x * s;
+            const bool thick = fabsf(ks) * amp >= LOC_EXP_TAU;
+            const float rk = rcpf(ke[i].x);
+            float4 tp;
+            tp.x = thick ? 0.0f : ks;
+            tp.y = thick ? -ks * LOC_LOG2E : 0.0f;
+            tp.z = thick ? ke[i].y * rk : ke[i].y * s;   // source function in occupation-number units | eps s
+            tp.w = thick ? -1.0f : -ks;
+            sts128(rb + L::TP + 16 * t, tp);
+            sts32(rb + L::UO + 4 * t, thick ? 0.0f : 1.0f);
+            sts32(rb + L::SC + 4 * t, thick ? wos * rk : w);  // the sums of the exponential form carry a factor kappa s
         }
-        T.tp[g][j][t] = step ? q : make_float2(0.f, 0.f);
     }
-    r.wbop |= (step ? thick : 0u) << LOC_THICK_SHIFT;
-    T.rs[g][j] = r;
+    return flags;
 }
 
-// One pass over a span of 32 channels for the four ray steps of a round: lane l8 of a group updates the quad at `sq`
-// (its channels have the offsets jf[0..3] from the span start of RecS) for all NT transitions.
-//   MASK = false: the common path -- no masks, the quad is known to lie inside the spectrum
-//   MASK = true : channel k takes part iff m[k]; the quad is loaded / stored iff `inq`
-// Accumulates the lane's partial sums a[t] += sum_k n_k X_k, b[t] += sum_k X_k, sphi += sum_k phi_k.
-#define LOC_SERIES(C0, P, B2, B3, B4, B5) fma2(C0, fma2(C0, fma2(C0, fma2(C0, B5, B4), B3), B2), P)
-template <int NT, bool MASK>
-__device__ __forceinline__ void span_pass(float *sq, int nchp, const float2 *tpr, const RecS &rs, const float (&jf)[4], unsigned thick,
-                                          unsigned any_thick, unsigned any_thin, bool inq, const bool (&m)[4], float (&a)[NT], float (&b)[NT],
-                                          float &sphi)
+// Masked multi-pass round for one lane's ray step (rare: DESIGN 6.4): passes of 32 channels over the nominal window
+// [clo, chi].  Adds the lane's partial sums to its slots of the `part` rows (zeroed here) and returns the lane's sum of
+// phi.  Scalar arithmetic, rolled over the transitions; same expressions as the common round.
+template <int NT>
+__device__ __forceinline__ float slow_round(unsigned rb, unsigned sqg, unsigned pl, int l8, int nchp)
 {
-    float e[4];
-#pragma unroll
-    for (int k = 0; k < 4; k++) {
-        const float y = fmaf(jf[k], rs.ky, rs.A);
-        e[k] = ex2f(fmaf(-y, y, rs.lamp));
-        if (MASK) e[k] = m[k] ? e[k] : 0.0f;
+    typedef Lay<NT> L;
+    const float4 h0 = lds128(rb);
+    const uint4 h1 = lds128u(rb + 16);
+    const unsigned wbop = __float_as_uint(h0.w);
+    const int wb = (int)(wbop & LOC_WB_MASK);
+    int clo = (int)(h1.w & 0xffffu), chi = (int)(h1.w >> 16);
+    if (!(wbop & LOC_RS_STEP)) {
+        clo = 1;
+        chi = 0;
     }
-    sphi += (e[0] + e[1]) + (e[2] + e[3]);
-    const f32x2 P01 = pk2(e[0], e[1]), P23 = pk2(e[2], e[3]);
-    const f32x2 ONE2 = pk2(1.0f, 1.0f), MONE2 = pk2(-1.0f, -1.0f);
-    f32x2 B2a = 0ull, B2b = 0ull, B3a = 0ull, B3b = 0ull, B4a = 0ull, B4b = 0ull, B5a = 0ull, B5b = 0ull;
-    // powers of phi for the series, shared by the transitions of the round that use it (all rays thin, or mixed)
-    if ((~any_thick | any_thin) & ((1u << NT) - 1u)) {
-        const f32x2 K2 = pk2(-0.5f, -0.5f), K3 = pk2(1.0f / 6.0f, 1.0f / 6.0f), K4 = pk2(-1.0f / 24.0f, -1.0f / 24.0f);
-        const f32x2 s01 = mul2(P01, P01), s23 = mul2(P23, P23);
-        B2a = mul2(s01, K2);
-        B2b = mul2(s23, K2);
-        B3a = mul2(mul2(s01, P01), K3);
-        B3b = mul2(mul2(s23, P23), K3);
-        B4a = mul2(mul2(s01, s01), K4);
-        B4b = mul2(mul2(s23, s23), K4);
-        const f32x2 K5 = pk2(-0.2f, -0.2f);
-        B5a = mul2(mul2(B4a, P01), K5);
-        B5b = mul2(mul2(B4b, P23), K5);
-    }
-    // Three phases, so that the loads and the common tail of all transitions are straight-line code the scheduler can
-    // interleave (the form of X is chosen by warp-uniform branches per transition).
-    float2 q[NT];
-    float4 n4[NT];
+#pragma unroll 1
+    for (int t = 0; t < NT; t++) sts64(pl + t * L::ROWB, make_float2(0.f, 0.f));
+    float sphi = 0.f;
+    int base = clo & ~3;
+    while (__any_sync(0xffffffffu, base <= chi)) {
+        const int cb = base + 4 * l8;
+        float e[4];
+        bool inq = false;
 #pragma unroll
-    for (int t = 0; t < NT; t++) {
-        q[t] = tpr[t];
-        n4[t] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (!MASK || inq) n4[t] = *reinterpret_cast<const float4 *>(sq + t * nchp);
-    }
-    f32x2 X01[NT], X23[NT];
-    float al[NT];
+        for (int k = 0; k < 4; k++) {
+            const int c = cb + k;
+            const bool m = c >= clo && c <= chi;
+            const float j = (float)(c - (wb + 16));
+            e[k] = m ? ex2f(fmaf(j, fmaf(j, h0.z, h0.y), h0.x)) : 0.0f;
+            inq |= m;
+        }
+        sphi += (e[0] + e[1]) + (e[2] + e[3]);
+        if (inq) {
+#pragma unroll 1
+            for (int t = 0; t < NT; t++) {
+                const float4 tp = lds128(rb + L::TP + 16 * t);
+                const float U = lds32(rb + L::UO + 4 * t);
+                const unsigned sa = sqg + 4 * base + 4 * t * nchp;
+                const float4 n4 = lds128(sa);
+                float n[4] = {n4.x, n4.y, n4.z, n4.w};
+                float a = 0.f, b = 0.f;
 #pragma unroll
-    for (int t = 0; t < NT; t++) {
-        const f32x2 C0 = pk2(q[t].x, q[t].x);
-        if (!((any_thick >> t) & 1u)) {  // every stepping ray of the warp uses the series in this transition
-            X01[t] = LOC_SERIES(C0, P01, B2a, B3a, B4a, B5a);
-            X23[t] = LOC_SERIES(C0, P23, B2b, B3b, B4b, B5b);
-            al[t] = -q[t].x;
-        } else {
-            float z0, z1, z2, z3;
-            upk2(mul2(C0, P01), z0, z1);
-            upk2(mul2(C0, P23), z2, z3);
-            const f32x2 E01 = pk2(ex2f(z0), ex2f(z1)), E23 = pk2(ex2f(z2), ex2f(z3));
-            X01[t] = fma2(E01, MONE2, ONE2);
-            X23[t] = fma2(E23, MONE2, ONE2);
-            al[t] = -1.0f;
-            if ((any_thin >> t) & 1u) {  // mixed: both forms, selected per ray
-                const bool tk = (thick >> t) & 1u;
-                float x0, x1, x2, x3, s0, s1, s2, s3;
-                upk2(X01[t], x0, x1);
-                upk2(X23[t], x2, x3);
-                upk2(LOC_SERIES(C0, P01, B2a, B3a, B4a, B5a), s0, s1);
-                upk2(LOC_SERIES(C0, P23, B2b, B3b, B4b, B5b), s2, s3);
-                X01[t] = pk2(tk ? x0 : s0, tk ? x1 : s1);
-                X23[t] = pk2(tk ? x2 : s2, tk ? x3 : s3);
-                al[t] = tk ? -1.0f : -q[t].x;
+                for (int k = 0; k < 4; k++) {
+                    const float p = e[k];
+                    const float X = fmaf(tp.x, fmaf(tp.x, p * p * p * (1.0f / 6.0f), -0.5f * p * p), fmaf(U, p, 1.0f - ex2f(tp.y * p)));
+                    a = fmaf(n[k], X, a);
+                    b += X;
+                    n[k] = fmaf(X, fmaf(tp.w, n[k], tp.z), n[k]);
+                }
+                sts128(sa, make_float4(n[0], n[1], n[2], n[3]));
+                const float2 pv = lds64(pl + t * L::ROWB);
+                sts64(pl + t * L::ROWB, make_float2(pv.x + a, pv.y + b));
             }
         }
+        base += LOC_SPAN;
+    }
+    return sphi;
+}
+
+// The common round: one pass over the span for all NT transitions, straight-line code.  `sq` = shared address of the
+// lane's quad in transition 0, `rowb` = bytes between the spectra of consecutive transitions, `pl` = the lane's slot in
+// row 0 of the group's partial sums.  Returns the lane's sum of phi.
+template <int NT>
+__device__ __forceinline__ float fast_round(unsigned rb, unsigned sq, int rowb, unsigned pl, const float4 h0, const f32x2 J01, const f32x2 J23)
+{
+    typedef Lay<NT> L;
+    // profile: log2 phi = q0 + j (q1 + j q2)
+    const f32x2 Q0 = pk2(h0.x, h0.x), Q1 = pk2(h0.y, h0.y), Q2 = pk2(h0.z, h0.z);
+    float y0, y1, y2, y3;
+    upk2(fma2(J01, fma2(J01, Q2, Q1), Q0), y0, y1);
+    upk2(fma2(J23, fma2(J23, Q2, Q1), Q0), y2, y3);
+    const f32x2 P01 = pk2(ex2f(y0), ex2f(y1)), P23 = pk2(ex2f(y2), ex2f(y3));
+    float sa, sb;
+    upk2(add2(P01, P23), sa, sb);
+    const float sphi = sa + sb;
+    const f32x2 ONE2 = pk2(1.0f, 1.0f), MONE2 = pk2(-1.0f, -1.0f);
+    const f32x2 K2 = pk2(-0.5f, -0.5f), K3 = pk2(1.0f / 6.0f, 1.0f / 6.0f);
+    const f32x2 s01 = mul2(P01, P01), s23 = mul2(P23, P23);
+    const f32x2 B2a = mul2(s01, K2), B2b = mul2(s23, K2);
+    const f32x2 B3a = mul2(mul2(s01, P01), K3), B3b = mul2(mul2(s23, P23), K3);
+    float Uv[L::NT4];
+#pragma unroll
+    for (int t = 0; t < L::NT4; t += 4) {
+        const float4 u = lds128(rb + L::UO + 4 * t);
+        Uv[t] = u.x;
+        Uv[t + 1] = u.y;
+        Uv[t + 2] = u.z;
+        Uv[t + 3] = u.w;
+    }
+    // three phases (all loads, arithmetic, all stores): the shared-memory accesses are ordered among themselves, the
+    // arithmetic of the NT transitions in between is free to interleave
+    float4 tp[NT], n4[NT];  // tp = C0, Ce, c1, alpha
+#pragma unroll
+    for (int t = 0; t < NT; t++) {
+        tp[t] = lds128(rb + L::TP + 16 * t);
+        n4[t] = lds128(sq + t * rowb);
+    }
+    float2 ab[NT];
+#pragma unroll
+    for (int t = 0; t < NT; t++) {
+        const f32x2 C0 = pk2(tp[t].x, tp[t].x), CE = pk2(tp[t].y, tp[t].y), C1 = pk2(tp[t].z, tp[t].z), AL = pk2(tp[t].w, tp[t].w),
+                    UU = pk2(Uv[t], Uv[t]);
+        float z0, z1, z2, z3;
+        upk2(mul2(CE, P01), z0, z1);
+        upk2(mul2(CE, P23), z2, z3);
+        const f32x2 E01 = pk2(ex2f(z0), ex2f(z1)), E23 = pk2(ex2f(z2), ex2f(z3));
+        const f32x2 X01 = fma2(C0, fma2(C0, B3a, B2a), fma2(UU, P01, fma2(E01, MONE2, ONE2)));
+        const f32x2 X23 = fma2(C0, fma2(C0, B3b, B2b), fma2(UU, P23, fma2(E23, MONE2, ONE2)));
+        const f32x2 N01 = pk2(n4[t].x, n4[t].y), N23 = pk2(n4[t].z, n4[t].w);
+        float a0, a1, b0, b1;
+        upk2(fma2(N01, X01, mul2(N23, X23)), a0, a1);
+        upk2(add2(X01, X23), b0, b1);
+        ab[t] = make_float2(a0 + a1, b0 + b1);
+        upk2(fma2(X01, fma2(AL, N01, C1), N01), n4[t].x, n4[t].y);
+        upk2(fma2(X23, fma2(AL, N23, C1), N23), n4[t].z, n4[t].w);
     }
 #pragma unroll
     for (int t = 0; t < NT; t++) {
-        const f32x2 N01 = pk2(n4[t].x, n4[t].y), N23 = pk2(n4[t].z, n4[t].w);
-        const f32x2 C1 = pk2(q[t].y, q[t].y), AL = pk2(al[t], al[t]);
-        float a0, a1, b0, b1;
-        upk2(fma2(N01, X01[t], mul2(N23, X23[t])), a0, a1);
-        upk2(add2(X01[t], X23[t]), b0, b1);
-        if (MASK) {  // several passes may follow one another
-            a[t] += a0 + a1;
-            b[t] += b0 + b1;
-        } else {
-            a[t] = a0 + a1;
-            b[t] = b0 + b1;
-        }
-        float r0, r1, r2, r3;
-        upk2(fma2(X01[t], fma2(AL, N01, C1), N01), r0, r1);
-        upk2(fma2(X23[t], fma2(AL, N23, C1), N23), r2, r3);
-        if (!MASK || inq) *reinterpret_cast<float4 *>(sq + t * nchp) = make_float4(r0, r1, r2, r3);
+        sts128(sq + t * rowb, n4[t]);
+        sts64(pl + t * L::ROWB, ab[t]);
     }
+    return sphi;
 }
 
-template <int NT, bool GEOM>
-__global__ void __launch_bounds__(32) k_sim3d(Sim3D P)
+// NCHP_T: spectrum row length in floats when known at compile time (immediate offsets), 0 = P.nchp
+template <int NT, int NCHP_T>
+__global__ void __maxnreg__(192) k_sim3d(Sim3D P)
 {
-    extern __shared__ __align__(16) float smem[];
-    __shared__ WarpTables<NT> T;               // separate object: no aliasing with the spectra
-    const int lane = threadIdx.x, grp = lane >> 3, l8 = lane & 7;
-    const int nchp = P.nchp;
+    typedef Lay<NT> L;
+    extern __shared__ __align__(16) float smem[];  // [4][NT][nchp] spectra, then the tables of Lay<NT>
+    const int lane = threadIdx.x, grp = lane >> 3, l8 = lane & 7, rj = l8 >> 1, half = l8 & 1;
+    const int nchp = NCHP_T ? NCHP_T : P.nchp;
     const int spec = NT * nchp;                // floats per ray spectrum
-    float *sn_all = smem;                      // [4][NT][nchp]
-    float *sn = sn_all + grp * spec;
+    const int rowb = 4 * nchp;
+    float *sn_all = smem;
+    const unsigned sm0 = (unsigned)__cvta_generic_to_shared(smem);
+    const unsigned tb = sm0 + 4u * LOC_GROUPS * spec;
+    const unsigned rec_g = tb + L::OFF_REC + grp * L::GSB;
+    const unsigned part_g = tb + L::OFF_PART + grp * L::PGB;
+    const unsigned pl = part_g + 8 * l8;             // my slot in row 0
+    const unsigned prow = part_g + L::ROWB * l8;     // row l8 (reducing lane)
+    const unsigned sq_g = sm0 + 4u * grp * spec + 16 * l8;
     float *slots_warp = P.pool + (long long)blockIdx.x * LOC_GROUPS * P.nslot * spec;
-    const float jf[4] = {(float)(4 * l8), (float)(4 * l8 + 1), (float)(4 * l8 + 2), (float)(4 * l8 + 3)};
+    const float jb = (float)(4 * l8 - 16);
+    const f32x2 J01 = pk2(jb, jb + 1.0f), J23 = pk2(jb + 2.0f, jb + 3.0f);
+    float2 *const cnt_l = P.cnt + l8;
+    const uint2 NOPREC = make_uint2(0u, LOC_OP_NOP << 24);
 
-    long long off = 0, end = 0;  // this group's position in the stream
-    bool done = false;
+    long long off = 0, end = 0;  // this group's position in the stream (first record of the current chunk)
+    bool done = false, fresh = false;
     float d0 = 0.f, d1 = 0.f, d2 = 0.f, sf = 0.f;
-    unsigned long long mysteps = 0, myactive = 0;
-    uint2 nrec = make_uint2(0u, LOC_OP_NOP << 24);  // record of the next chunk, fetched one chunk ahead
-    bool have_next = false;
+    unsigned mysteps = 0;
+    unsigned long long myactive = 0;
+    // software pipeline over chunks: r0 = records of this chunk, r1 / r2 = of the next two (r2 in flight), `cell` = cell
+    // data of r0's record, loaded during the previous chunk's rounds
+    uint2 r0 = NOPREC, r1 = NOPREC, r2 = NOPREC;
+    CellRegs<NT> cell;
+    cell.kin = make_float4(0.f, 0.f, 0.f, 1.f);
+#pragma unroll
+    for (int i = 0; i < L::NH / 2; i++) cell.cf[i] = make_float4(0.f, 0.f, 0.f, 0.f);
 
     for (;;) {
         // ---- refill: groups whose task is exhausted take the next root ray from the queue ----
         {
             const bool need = !done && off >= end;
-            long long task = 0;
-            if (need && l8 == 0) task = atomicAdd(P.queue, 1u);
-            task = __shfl_sync(0xffffffffu, task, grp * 8);
-            if (need) {
-                have_next = false;
-                if (task >= P.ntask) {
-                    done = true;
-                } else {
-                    const Dir3 *Dp = P.dirs + P.task_dir[task];
-                    d0 = __ldg(&Dp->d[0]);
-                    d1 = __ldg(&Dp->d[1]);
-                    d2 = __ldg(&Dp->d[2]);
-                    sf = __ldg(&Dp->sf);
-                    off = __ldg(P.task_off + task);
-                    end = __ldg(P.task_off + task + 1);
+            if (__any_sync(0xffffffffu, need)) {
+                long long task = 0;
+                if (need && l8 == 0) task = atomicAdd(P.queue, 1u);
+                task = __shfl_sync(0xffffffffu, task, grp * 8);
+                if (need) {
+                    if (task >= P.ntask) {
+                        done = true;
+                        r0 = r1 = r2 = NOPREC;
+                    } else {
+                        const Dir3 *Dp = P.dirs + P.task_dir[task];
+                        d0 = __ldg(&Dp->d[0]);
+                        d1 = __ldg(&Dp->d[1]);
+                        d2 = __ldg(&Dp->d[2]);
+                        sf = __ldg(&Dp->sf);
+                        off = __ldg(P.task_off + task);
+                        end = __ldg(P.task_off + task + 1);
+                        fresh = true;
+                    }
                 }
+                if (__all_sync(0xffffffffu, done)) break;
             }
         }
-        if (__all_sync(0xffffffffu, done)) break;
-        // ---- prepare: lane l8 of each group decodes record off + l8 of its ray ----
-        uint2 rec = make_uint2(0u, LOC_OP_NOP << 24);
-        if (have_next)
-            rec = nrec;
-        else if (!done && off + l8 < end)
-            rec = __ldg(P.stream + off + l8);
-        off += LOC_CHUNK;
-        have_next = !done && off < end;
-        nrec = make_uint2(0u, LOC_OP_NOP << 24);
-        if (have_next && off + l8 < end) nrec = __ldg(P.stream + off + l8);
-        prepare_record<NT>(P, rec, d0, d1, d2, sf, T, grp, l8);
+        if (fresh) {  // first chunk of a ray: nothing was prefetched
+            r0 = __ldg(P.stream + off + rj);
+            r1 = (off + LOC_CHUNK < end) ? __ldg(P.stream + off + LOC_CHUNK + rj) : NOPREC;
+            load_cell<NT>(P, r0, half, cell);
+            fresh = false;
+        }
+        r2 = (!done && off + 2 * LOC_CHUNK < end) ? __ldg(P.stream + off + 2 * LOC_CHUNK + rj) : NOPREC;
+        // ---- prepare: lane pair rj of each group decodes record off + rj of its ray ----
+        int nact;
+        unsigned flags = prepare_record<NT>(P, r0, cell, d0, d1, d2, sf, rec_g + rj * L::RECB, half, nact);
+        if (half == 0) {
+            mysteps += flags >> 31;
+            myactive += nact;
+        }
+        // class of round rj: OR of the record flags over the four groups
+        flags |= __shfl_xor_sync(0xffffffffu, flags, 8);
+        flags |= __shfl_xor_sync(0xffffffffu, flags, 16);
+        load_cell<NT>(P, r1, half, cell);  // for the next chunk (NOP records load nothing)
         __syncwarp();
 
-        // ---- 8 rounds: every group consumes one record per round ----
+        // ---- LOC_CHUNK rounds: every group consumes one record per round ----
+#pragma unroll 1
         for (int r = 0; r < LOC_CHUNK; r++) {
-            const unsigned cls = T.cls[r];
-            if (cls & LOC_CLS_CTRL) {
+            const unsigned cls = __shfl_sync(0xffffffffu, flags, 2 * r);
+            const unsigned rb = rec_g + r * L::RECB;
+            if (cls & LOC_RS_CTRL) {
                 // spectrum operations, executed by the whole warp for one group at a time
                 for (int g = 0; g < LOC_GROUPS; g++) {
-                    const unsigned gop = T.opdz[g][r] >> 24, gx = T.cell[g][r];
+                    const uint4 gh = lds128u(tb + L::OFF_REC + g * L::GSB + r * L::RECB + 16);
+                    const unsigned gop = gh.z >> 24, gx = gh.x;
                     float *gs = sn_all + g * spec;
                     float *slot = slots_warp + ((long long)g * P.nslot + gx) * spec;
                     if (gop == LOC_OP_BG) {
-#pragma unroll
                         for (int t = 0; t < NT; t++) {
                             const float bg = P.S.bgocc[P.slot0 + t];
                             for (int c = lane; c < nchp; c += 32) gs[t * nchp + c] = bg;
@@ -369,93 +527,64 @@ __global__ void __launch_bounds__(32) k_sim3d(Sim3D P)
                 }
                 __syncwarp();
             }
-            if (!(cls & LOC_CLS_STEP)) continue;
-            const unsigned any_thick = cls & 0xfffu, any_thin = (cls >> LOC_CLS_THIN_SHIFT) & 0xfffu;
-            const RecS rs = T.rs[grp][r];
-            const unsigned thick = (rs.wbop >> LOC_THICK_SHIFT) & 0xfffu;
-            const int wb = (int)(rs.wbop & LOC_WB_MASK);
-            const float2 *tpr = T.tp[grp][r];
-
-            float a[NT], b[NT];
-#pragma unroll
-            for (int t = 0; t < NT; t++) a[t] = b[t] = 0.f;
-            float sphi = 0.f;
-            if (!(cls & LOC_CLS_SLOW)) {
-                const bool nomask[4] = {true, true, true, true};
-                span_pass<NT, false>(sn + wb + 4 * l8, nchp, tpr, rs, jf, thick, any_thick, any_thin, true, nomask, a, b, sphi);
-            } else {
-                // masked passes of 32 channels over the nominal window (several when the line is very thick)
-                const int2 win = T.win[grp][r];
-                int base = win.x & ~3;
-                while (__any_sync(0xffffffffu, base <= win.y)) {
-                    const int cb = base + 4 * l8;  // the lane's quad in this pass (win.y < nch <= nchp: in range if cb <= win.y)
-                    const float ob = (float)(base - wb);
-                    const float jo[4] = {jf[0] + ob, jf[1] + ob, jf[2] + ob, jf[3] + ob};
-                    const bool m[4] = {cb >= win.x && cb <= win.y, cb + 1 >= win.x && cb + 1 <= win.y, cb + 2 >= win.x && cb + 2 <= win.y,
-                                       cb + 3 >= win.x && cb + 3 <= win.y};
-                    span_pass<NT, true>(sn + cb, nchp, tpr, rs, jo, thick, any_thick, any_thin, cb <= win.y, m, a, b, sphi);
-                    base += LOC_SPAN;
-                }
-            }
-            // ---- reduction over the 8 lanes of each group, through shared memory (no selects, DESIGN 6.4) ----
-            sphi += __shfl_xor_sync(0xffffffffu, sphi, 4);
-            sphi += __shfl_xor_sync(0xffffffffu, sphi, 2);
-            sphi += __shfl_xor_sync(0xffffffffu, sphi, 1);
-            float2 *pg = T.part[grp];
-#pragma unroll
-            for (int t = 0; t < NT; t++) pg[t * WarpTables<NT>::ROW + l8] = make_float2(a[t], b[t]);
+            if (!(cls & LOC_RS_STEP)) continue;
+            const float4 h0 = lds128(rb);
+            const unsigned wbop = __float_as_uint(h0.w);
+            float sphi;
+            if (!(cls & LOC_RS_SLOW))
+                sphi = fast_round<NT>(rb, sq_g + 4u * (wbop & LOC_WB_MASK), rowb, pl, h0, J01, J23);
+            else
+                sphi = slow_round<NT>(rb, sq_g, pl, l8, nchp);
+            sts32(part_g + L::PHI + 4 * l8, sphi);
             __syncwarp();
-            // lane t of a group adds up row t and issues the two float atomics of (cell, transition t) as one 64-bit RED
-            const bool step = rs.wbop & LOC_RS_STEP;
-            const unsigned cell = T.cell[grp][r];
-            const float w = T.w[grp][r];
-            const float wesc = w - w * sphi;  // photons emitted outside the updated channels escape (DESIGN 5.3)
+            // ---- reduction over the 8 lanes of each group: lane t adds up row t and issues the two float atomics of
+            //      (cell, transition t) as one 64-bit RED ----
+            const bool step = wbop & LOC_RS_STEP;
+            const uint4 h1 = lds128u(rb + 16);  // coff, w, opdz, win
+            const float4 f0 = lds128(part_g + L::PHI), f1 = lds128(part_g + L::PHI + 16);
+            float fa, fb;
+            upk2(add2(add2(pk2(f0.x, f0.y), pk2(f0.z, f0.w)), add2(pk2(f1.x, f1.y), pk2(f1.z, f1.w))), fa, fb);
+            const float w = __uint_as_float(h1.y);
+            const float wesc = fmaf(-w, fa + fb, w);  // photons emitted outside the updated channels escape (DESIGN 5.3)
 #pragma unroll
             for (int t0 = 0; t0 < NT; t0 += 8) {
-                const int t = t0 + l8;
-                if (step && t < NT) {
-                    const float4 *row = reinterpret_cast<const float4 *>(pg + t * WarpTables<NT>::ROW);
-                    const float4 r0 = row[0], r1 = row[1], r2 = row[2], r3 = row[3];
-                    const f32x2 s01 = add2(add2(pk2(r0.x, r0.y), pk2(r0.z, r0.w)), add2(pk2(r1.x, r1.y), pk2(r1.z, r1.w)));
-                    const f32x2 s23 = add2(add2(pk2(r2.x, r2.y), pk2(r2.z, r2.w)), add2(pk2(r3.x, r3.y), pk2(r3.z, r3.w)));
+                if (step && t0 + l8 < NT) {
+                    const float4 a0 = lds128(prow + t0 * L::ROWB), a1 = lds128(prow + t0 * L::ROWB + 16), a2 = lds128(prow + t0 * L::ROWB + 32),
+                                 a3 = lds128(prow + t0 * L::ROWB + 48);
+                    const float sc = lds32(rb + L::SC + 4 * t0 + 4 * l8);
+                    const f32x2 s01 = add2(add2(pk2(a0.x, a0.y), pk2(a0.z, a0.w)), add2(pk2(a1.x, a1.y), pk2(a1.z, a1.w)));
+                    const f32x2 s23 = add2(add2(pk2(a2.x, a2.y), pk2(a2.z, a2.w)), add2(pk2(a3.x, a3.y), pk2(a3.z, a3.w)));
                     float A, B;
                     upk2(add2(s01, s23), A, B);
-                    // scale of the sums: w for the series form, w / (kappa s) for the exponential form (c0 = -kappa s log2 e)
-                    const float sc = ((thick >> t) & 1u) ? __fdividef(-LOC_LOG2E * w, tpr[t].x) : w;
-                    float2 *cn = P.cnt + (long long)cell * P.nsp + P.slot0 + t;
+                    float2 *cn = cnt_l + (h1.x + (unsigned)t0);
                     asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(cn), "f"(A * sc), "f"(fmaf(B, sc, wesc)) : "memory");
                 }
             }
-            if (step && l8 == 0) {
-                mysteps++;
-                if (GEOM) {
-                    atomicAdd(&P.visits[cell], 1u);
-                    atomicAdd(&P.pathz[cell], T.opdz[grp][r] & 0x1fffffu);
-                    const float h5 = 5.0f * 0.8493218f / rs.ky, cc = (float)wb - rs.A / rs.ky;  // 5 sigma in channels, line centre
-                    myactive += max(0, min(P.nch - 1, (int)floorf(cc + h5)) - max(0, (int)ceilf(cc - h5)) + 1);
-                }
+            if (P.geom && step && l8 == 0) {
+                const unsigned cellidx = (h1.x - (unsigned)P.slot0) / (unsigned)P.nsp;
+                atomicAdd(&P.visits[cellidx], 1u);
+                atomicAdd(&P.pathz[cellidx], h1.z & 0x1fffffu);
             }
             __syncwarp();  // the next round's quads were written by other lanes
         }
+        off += LOC_CHUNK;
+        r0 = r1;
+        r1 = r2;
     }
     // per-warp totals
+    unsigned long long ms = mysteps;
     for (int o = 16; o >= 1; o >>= 1) {
-        mysteps += __shfl_xor_sync(0xffffffffu, mysteps, o);
+        ms += __shfl_xor_sync(0xffffffffu, ms, o);
         myactive += __shfl_xor_sync(0xffffffffu, myactive, o);
     }
-    if (lane == 0 && mysteps) atomicAdd(P.nsteps, mysteps);
-    if (GEOM && lane == 0 && myactive) atomicAdd(P.nsteps + 1, myactive);
+    if (lane == 0 && ms) atomicAdd(P.nsteps, ms);
+    if (P.geom && lane == 0 && myactive) atomicAdd(P.nsteps + 1, myactive);
 }
 
-template <int NT>
-static int launch3d(loc_model *m, Sim3D &P, int geom)
+template <int NT, int NCHP_T>
+static int launch3d_t(loc_model *m, Sim3D &P, size_t smem)
 {
-    const size_t smem = sizeof(float) * LOC_GROUPS * NT * P.nchp;  // + static: the prepare tables
-    if (smem > 200 * 1024 || P.nch > (int)LOC_WB_MASK) {
-        snprintf(m->err, sizeof(m->err), "nchannel * ntrans too large for the shared-memory spectra (%zu bytes per warp)", smem);
-        return LOC_EINVAL;
-    }
-    auto kern = geom ? k_sim3d<NT, true> : k_sim3d<NT, false>;
+    auto kern = k_sim3d<NT, NCHP_T>;
     LOC_CUDA_CHECK(m, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int bps = 0;
     LOC_CUDA_CHECK(m, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kern, 32, smem));
@@ -471,6 +600,21 @@ static int launch3d(loc_model *m, Sim3D &P, int geom)
     m->launches++;
     LOC_CUDA_CHECK(m, cudaGetLastError());
     return LOC_OK;
+}
+
+static size_t spectra_bytes(int nt, int nchp) { return sizeof(float) * LOC_GROUPS * (size_t)nt * nchp; }
+
+template <int NT>
+static int launch3d(loc_model *m, Sim3D &P)
+{
+    const size_t smem = spectra_bytes(NT, P.nchp) + Lay<NT>::BYTES;
+    if (smem > 200 * 1024 || P.nch > (int)LOC_WB_MASK || P.nch > 0xffff) {
+        snprintf(m->err, sizeof(m->err), "nchannel * ntrans too large for the shared-memory spectra (%zu bytes per warp)", smem);
+        return LOC_EINVAL;
+    }
+    if (P.nchp == 128) return launch3d_t<NT, 128>(m, P, smem);
+    if (P.nchp == 256) return launch3d_t<NT, 256>(m, P, smem);
+    return launch3d_t<NT, 0>(m, P, smem);
 }
 
 int loc_launch_sim3d(loc_model *m, int geom)
@@ -498,25 +642,31 @@ int loc_launch_sim3d(loc_model *m, int geom)
     P.queue = m->d_queue;
     P.pool = m->spec_pool;
     P.S = m->selh;
-    // Transitions are traced in `npart` launches of nearly equal size: the per-ray spectra of one launch then need less
-    // shared memory, so more rays are in flight per SM (latency hiding), at the price of repeating the per-step scalar
-    // work once per launch.  Default: parts of at most 5 transitions.
+    if ((long long)m->ncell * P.nsp >= (1ll << 32)) {
+        snprintf(m->err, sizeof(m->err), "ncell * ntrans exceeds the 32-bit counter offsets of the 3D kernel");
+        return LOC_EINVAL;
+    }
+    // All traced transitions go through one launch while the spectra of a warp's four rays fit 24 KB of shared memory
+    // (9 transitions x 128 channels = 18 KB); otherwise they are split into `npart` launches of nearly equal size, at the
+    // price of repeating the per-step work (profiles/r1_v5_sim3d_C3.md: ~10 ms per extra launch on C3).
     int nsel = m->selh.nsel;
-    int npart = (nsel + 4) / 5;
+    int npart = 1;
+    while (npart < nsel && spectra_bytes((nsel + npart - 1) / npart, P.nchp) > 24 * 1024) npart++;
     if (getenv("LOC_SIM3D_PARTS")) npart = std::max(1, std::min(nsel, atoi(getenv("LOC_SIM3D_PARTS"))));
     int slot = 0;
     for (int part = 0; part < npart; part++) {
         int n = (nsel - slot + (npart - part) - 1) / (npart - part);
+        if (part + 1 < npart) n = std::min(nsel - slot, (n + 1) & ~1);  // even parts: 16-byte aligned coefficient records
         P.slot0 = slot;
         int rc = LOC_EINVAL;
         // the step / active-channel statistics are taken by the first part only
-        int g = geom && part == 0;
+        P.geom = geom && part == 0;
         unsigned long long *keep = P.nsteps;
         if (part > 0) P.nsteps = m->d_steps + 2;  // scratch slot
         switch (n) {
-#define C3(N)                        \
-    case N:                          \
-        rc = launch3d<N>(m, P, g);   \
+#define C3(N)                     \
+    case N:                       \
+        rc = launch3d<N>(m, P);   \
         break;
             C3(1) C3(2) C3(3) C3(4) C3(5) C3(6) C3(7) C3(8) C3(9) C3(10) C3(11) C3(12)
 #undef C3
