@@ -174,6 +174,22 @@ def run_reference(args):
     print(json.dumps(out))
 
 
+# ---- multi-process plumbing (replicas only: DESIGN.md section 9) -----------------------------------------------------
+def max_over_ranks(values, device="cpu"):
+    """max over the ranks of a list of floats (device-timed seconds); identity when torch.distributed is not initialised"""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
+def whole_job_value(updates_per_rank_step: float, steps: int, world: int, seconds: float) -> float:
+    """`value` of the JSON line: units all ranks processed / max-over-ranks time (weak scaling: every rank runs a replica)"""
+    return world * updates_per_rank_step * steps / seconds
+
+
 # ---- own arm ------------------------------------------------------------------------------------------------------------
 def roofline(stats_geom, nt, t_sim_s, hbm_gbs, sm_mhz, peak_kind):
     """T_roof = max(bytes / HBM, MUFU ops / MUFU rate, FP32 instructions / issue rate) for the simulation
@@ -259,11 +275,8 @@ def run_own(args):
     launches = g.stats()["kernel_launches"] - l0
     t_sim = sum(e[0].elapsed_time(e[1]) for e in ev) * 1e-3
     t_all = sum(e[0].elapsed_time(e[2]) for e in ev) * 1e-3
-    tt = torch.tensor([t_all, t_sim], dtype=torch.float64, device=f"cuda:{local}")
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    t_all, t_sim = float(tt[0]), float(tt[1])
-    value = world * u_nom * args.steps / t_all
+    t_all, t_sim = max_over_ranks([t_all, t_sim], device=f"cuda:{local}")
+    value = whole_job_value(u_nom, args.steps, world, t_all)
 
     # ---- end to end: host buffers -> device -> one ALI iteration -> populations back to the host ----
     names = ["density", "tkin", "sigma", "abundance"] + (["vx", "vy", "vz"] if is3d else ["vx"])
@@ -296,10 +309,8 @@ def run_own(args):
         e2e_step()
     e1.record()
     barrier()
-    te = torch.tensor([e0.elapsed_time(e1) * 1e-3], dtype=torch.float64, device=f"cuda:{local}")
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_val = world * u_nom * n_e2e / float(te[0])
+    (t_e2e,) = max_over_ranks([e0.elapsed_time(e1) * 1e-3], device=f"cuda:{local}")
+    e2e_val = whole_job_value(u_nom, n_e2e, world, t_e2e)
 
     if rank == 0:
         hbm, sm_max, kind = load_peaks()

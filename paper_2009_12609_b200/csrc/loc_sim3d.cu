@@ -115,6 +115,16 @@ __device__ __forceinline__ float rcpf(float x)
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
+__device__ __forceinline__ float4 ldg_keep(const float *p, unsigned long long pol)
+{
+    float4 v;
+    asm volatile("ld.global.L2::cache_hint.v4.f32 {%0, %1, %2, %3}, [%4], %5;" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ void stg_keep(float *p, float4 v, unsigned long long pol)
+{
+    asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w), "l"(pol) : "memory");
+}
 template <int OFF = 0>
 __device__ __forceinline__ float4 lds128(unsigned a)
 {
@@ -441,6 +451,10 @@ __global__ void __maxnreg__(192) k_sim3d(Sim3D P)
     const float jb = (float)(4 * l8 - 16);
     const f32x2 J01 = pk2(jb, jb + 1.0f), J23 = pk2(jb + 2.0f, jb + 3.0f);
     float2 *const cnt_l = P.cnt + l8;
+    // the spectrum slots of the resident warps (donor spectra, DESIGN 6.3) are re-read by every ray born from them: keep
+    // them in L2 against the streaming traffic of the step records, coefficients and counters
+    unsigned long long pol_keep;
+    asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_keep));
     const uint2 NOPREC = make_uint2(0u, LOC_OP_NOP << 24);
 
     long long off = 0, end = 0;  // this group's position in the stream (first record of the current chunk)
@@ -520,9 +534,19 @@ __global__ void __maxnreg__(192) k_sim3d(Sim3D P)
                             for (int c = lane; c < nchp; c += 32) gs[t * nchp + c] = bg;
                         }
                     } else if (gop == LOC_OP_SAVE) {
-                        for (int i = lane * 4; i < spec; i += 128) *reinterpret_cast<float4 *>(slot + i) = *reinterpret_cast<const float4 *>(gs + i);
+                        for (int i = lane * 4; i < spec; i += 128) stg_keep(slot + i, *reinterpret_cast<const float4 *>(gs + i), pol_keep);
                     } else if (gop == LOC_OP_LOAD) {
-                        for (int i = lane * 4; i < spec; i += 128) *reinterpret_cast<float4 *>(gs + i) = *reinterpret_cast<const float4 *>(slot + i);
+                        // all loads of a batch in flight before the first store: one L2 latency per batch, not per quad
+                        constexpr int NB = 9;
+                        for (int i0 = lane * 4; i0 < spec; i0 += 128 * NB) {
+                            float4 v[NB];
+#pragma unroll
+                            for (int k = 0; k < NB; k++)
+                                if (i0 + 128 * k < spec) v[k] = ldg_keep(slot + i0 + 128 * k, pol_keep);
+#pragma unroll
+                            for (int k = 0; k < NB; k++)
+                                if (i0 + 128 * k < spec) *reinterpret_cast<float4 *>(gs + i0 + 128 * k) = v[k];
+                        }
                     }
                 }
                 __syncwarp();

@@ -117,3 +117,33 @@ def test_blackbody_enclosure_gpu():
     p0 = p0.cpu().numpy()[:, leaf]
     g.close()
     assert np.max(np.abs(p1 - p0) / p0) < 2e-5 and change < 2e-5
+
+
+def test_full_size_path_invariant_and_enclosure():
+    """BASELINE size, the launch configuration bench.py times (C3: 128^3, 48 directions, 128 channels, 9 transitions).
+    The oracle cannot run this size inside a test, so properties that hold at any size are checked instead:
+      * pin P7: every leaf's summed main-axis path is h_l * NDIR exactly (integer), total visits = steps of the stream;
+      * pin P4: with T_bg = T_kin one ALI iteration from LTE leaves the populations unchanged (all normalisations);
+      * the escape fractions of an iteration lie in (0, 1] and the counters are finite."""
+    m = W.cloud_config(3)
+    m.t_bg = 10.0  # = T_kin of C3: blackbody enclosure
+    g = _model(m)
+    g.init_lte()
+    g.simulate(geometry_counters=True)
+    vis, pz = g.geometry_counters()
+    st = g.stats()
+    vis, pz = vis.cpu().numpy().astype(np.int64), pz.cpu().numpy().astype(np.int64)
+    leaf = m.child < 0
+    expect = (len(m.dirs) << 20) >> m.level.astype(np.int64)
+    assert np.array_equal(pz[leaf], expect[leaf]) and np.all(pz[~leaf] == 0)
+    assert vis.sum() == st["steps"] == st["setup_steps"] and vis[leaf].min() >= len(m.dirs)
+    sj, esc = g.counters()
+    sj, esc = sj.cpu().numpy(), esc.cpu().numpy()
+    assert np.isfinite(sj).all() and np.isfinite(esc).all()
+    assert esc[leaf].min() > 0 and esc[leaf].max() <= 1.0 + 1e-5
+    p0 = g.pops.clone()
+    change = g.iterate(1)
+    p1, p0 = g.pops.cpu().numpy()[:, leaf], p0.cpu().numpy()[:, leaf]
+    g.close()
+    big = p0 > 1e-10 * p0.sum(axis=0, keepdims=True)
+    assert np.max(np.abs(p1 - p0)[big] / p0[big]) < 5e-5 and change < 5e-5
