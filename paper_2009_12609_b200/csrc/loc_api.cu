@@ -261,7 +261,9 @@ static int build_selection(loc_model *m, int nsel, const int *idx)
 {
     Selection &S = m->selh;
     if (nsel == 0) {
-        nsel = std::min(m->ntrans, LOC_MAX_TRANS);
+        // default selection: the first transitions, as many as the model was created for (the per-cell records of the
+        // workspace hold max_trans entries)
+        nsel = std::min(std::min(m->ntrans, LOC_MAX_TRANS), m->max_trans);
         for (int k = 0; k < nsel; k++) S.sel[k] = k;
     } else {
         if (nsel < 0 || nsel > LOC_MAX_TRANS || nsel > m->max_trans) return fail(m, LOC_EINVAL, "loc_simulate: nsel out of range");

@@ -61,7 +61,9 @@ def test_geometry_per_direction():
 
 
 RAD_CASES = [dict(nroot=6, nlev=1, nside=1, nch=48), dict(nroot=4, nlev=3, nside=1, nch=40, frac=0.4),
-             dict(nroot=4, nlev=3, nside=2, nch=32, frac=0.5, seed=9), dict(which=5, nroot=4, nlev=2, nside=1, nch=64, frac=0.4, nls=10)]
+             dict(nroot=4, nlev=3, nside=2, nch=32, frac=0.5, seed=9), dict(which=5, nroot=4, nlev=2, nside=1, nch=64, frac=0.4, nls=10),
+             # 3 of 9 transitions traced on a grid large enough that a record stride of 9 would leave the 3-transition workspace
+             dict(which=5, nroot=10, nlev=2, nside=1, nch=64, frac=0.3, nls=10)]
 
 
 @pytest.mark.parametrize("cfg", RAD_CASES)
