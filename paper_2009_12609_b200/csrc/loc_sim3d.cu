@@ -3,20 +3,24 @@
 // transfer of Eq. 3 and the two per-cell sums (Eq. 2 first term; escape fraction of PAPER.md:81) for all traced
 // transitions at once (the "all transitions in one pass" option the paper leaves open).
 //
-// Work decomposition (DESIGN 6.4).  A warp carries FOUR rays at a time, one per quarter-warp ("group" of 8 lanes).  Every
+// Work decomposition (DESIGN 6.4).  A CTA of TWO warps carries FOUR rays at a time; both warps walk the same four rays in
+// lock step and split the traced TRANSITIONS between them (warp 0 the first half, warp 1 the rest): the rays' spectra and
+// per-step records in shared memory are shared, so twice as many warps are resident for the same shared memory, and
+// each warp prepares and reduces only its own transitions.  Within a warp each ray has a quarter-warp ("group" of 8
+// lanes).  Every
 // step touches a SPAN of 32 consecutive channels that starts at a multiple of 4 and is centred on the Doppler-shifted
 // line; lane l8 of the group owns the aligned quad  span + 4 l8 .. + 3, so that
 //   * the photon spectrum of a ray lives in shared memory and is read / written with one 128-bit access per lane and
 //     transition, conflict free for any span position (a quarter-warp is one shared-memory phase);
 //   * the per-channel arithmetic is done on packed pairs (fma.rn.f32x2) and is ONE straight-line expression for both
-//     regimes of the optical depth (below): no masks, no selects, no branches per transition, so that the 2 NT
-//     independent chains of a round give the instruction-level parallelism that ~2 warps per scheduler need;
+//     regimes of the optical depth (below): no masks, no selects, no branches per transition;
 //   * the sums over a lane's 4 channels are free, and the cross-lane reduction goes through shared memory: lane t of
 //     the group adds up the 8 partial sums of transition t and issues ONE 64-bit RED for the cell's (SJ, ESC) pair;
 //   * all per-step scalar work (record decode, Doppler shift, window, per-transition coefficients, scale of the sums,
-//     counter offset) is done in a "prepare" phase, two lanes per record for 4 records x 4 rays at once, from cell data
-//     prefetched into registers one chunk ahead, and left in one shared-memory record per (ray, round): the round
-//     addresses everything with immediate offsets from one register.
+//     counter offset) is done in a "prepare" phase, two lanes of each warp per record for 4 records x 4 rays at once,
+//     from cell data prefetched into registers one chunk ahead, and left in one shared-memory record per (ray, round):
+//     the round addresses everything with immediate offsets from one register.  Two CTA barriers per chunk of 4 rounds
+//     (records complete / records free) are the only synchronisation between the two warps.
 // All traced transitions (up to the shared-memory limit) go through ONE launch: the per-step overhead is paid once
 // (profiles/r1_v5_sim3d_C3.md: splitting 9 transitions over 2 launches cost ~10 ms per launch on C3).
 //
@@ -71,7 +75,7 @@ struct Sim3D {
 //   +16  uint  coff           cell * nsp + slot0 : element offset of the cell's counter record (STEP); slot (SAVE / LOAD)
 //   +20  float w              a s / V_eff = dzeta / (h NDIR)
 //   +24  uint  opdz           opcode | level | dzeta (stream word)
-//   +28  uint  win            nominal channel window clo | chi << 16 (masked path; chi < clo = empty)
+//   +28  float cc             line centre in channel units (masked path)
 //   +32  float4 tp[NT]        (C0, Ce, c1, alpha) per transition (header comment)
 //   +32 + 16 NT   float U[NT4]    1 = series, 0 = exponential; NT4 = NT rounded up to 4
 //   then          float sc[NT4]   scale of the channel sums: w (series) or w / (kappa s) (exponential)
@@ -80,13 +84,13 @@ struct Sim3D {
 #define LOC_RS_CTRL 0x40000000u
 #define LOC_RS_STEP 0x80000000u
 
-#define LOC_XCLIP 3.9f     // a span may cut the nominal window, but never closer than this many sigma to the line centre
+#define LOC_XCLIP 3.9f     // the span reaches at least this many sigma to both sides of the line centre, or the step is masked
 #define LOC_EXP_TAU 0.03f  // line-centre optical depth of a step from which the exponential form is used
 
 template <int NT>
 struct Lay {
     static constexpr int NT4 = (NT + 3) & ~3;
-    static constexpr int NH = (((NT + 1) / 2) + 1) & ~1;  // transitions prepared by the first lane of a record's pair (even)
+    static constexpr int NT0 = (NT + 1) / 2;         // transitions of warp 0; warp 1 has the other NT - NT0
     static constexpr int TP = 32;                    // byte offset of tp[] in a record
     static constexpr int UO = TP + 16 * NT;          // byte offset of U[]
     static constexpr int SC = UO + 4 * NT4;          // byte offset of sc[]
@@ -96,15 +100,16 @@ struct Lay {
     static constexpr int GW0 = LOC_CHUNK * RECB / 4;
     static constexpr int GSB = 4 * (GW0 + ((8 + 32 - GW0 % 32) % 32));
     // per-lane partial sums (a_t, b_t) of the round: [group][t][lane], rows of 10 float2 (8 used) = 80 bytes: the
-    // reducing lanes of a group read 8 different rows with LDS.128 conflict free; then one row of 8 floats: the lanes'
-    // sums of phi.  Groups 16 banks apart.
+    // reducing lanes of a group read 8 different rows with LDS.128 conflict free; then per warp one row of 8 floats:
+    // the lanes' sums of phi.  Groups 16 banks apart.
     static constexpr int ROWB = 80;
-    static constexpr int PHI = NT * ROWB;
-    static constexpr int PW0 = (NT * ROWB + 32) / 4;
+    static constexpr int PHI = NT * ROWB;            // + 32 * warp
+    static constexpr int PW0 = (NT * ROWB + 64) / 4;
     static constexpr int PGB = 4 * (PW0 + ((16 + 32 - PW0 % 32) % 32));
     static constexpr int OFF_REC = 0;                                  // relative to the table base
-    static constexpr int OFF_CLS = OFF_REC + LOC_GROUPS * GSB;
-    static constexpr int OFF_PART = OFF_CLS + 4 * LOC_CHUNK;
+    static constexpr int OFF_CLS = OFF_REC + LOC_GROUPS * GSB;         // class word of each round of the chunk
+    static constexpr int OFF_TASK = OFF_CLS + 4 * LOC_CHUNK;           // task taken from the queue, per group
+    static constexpr int OFF_PART = OFF_TASK + 4 * LOC_GROUPS;
     static constexpr int BYTES = OFF_PART + LOC_GROUPS * PGB;
 };
 
@@ -187,114 +192,112 @@ __device__ __forceinline__ void sts32u(unsigned a, unsigned v)
 }
 
 
-// Cell data of one stream record as the prepare phase needs it: lane `half` (0 / 1) of the record's lane pair holds the
-// kinematics and the (kappa, eps) pairs of its transitions  half * NH .. half * NH + NH - 1.
-template <int NT>
-struct CellRegs {
-    float4 kin;
-    float4 cf[Lay<NT>::NH / 2];
+
+// Split of the transitions: warp W of the CTA owns transitions TB .. TB + NW - 1; lane `half` (0 / 1) of a record's lane
+// pair prepares NHW of them, from T0(half).
+template <int NT, int W>
+struct Own {
+    static constexpr int TB = W ? Lay<NT>::NT0 : 0;
+    static constexpr int NW = W ? NT - Lay<NT>::NT0 : Lay<NT>::NT0;
+    static constexpr int NHW = (NW + 1) / 2;
+    static constexpr int NHR = NHW > 0 ? NHW : 1;  // array sizes
+    // the warp with fewer transitions also prepares the record headers, keeps the statistics and the geometry counters
+    static constexpr int HW = (NT - Lay<NT>::NT0 > 0 && NT - Lay<NT>::NT0 < Lay<NT>::NT0) ? 1 : 0;
+    static constexpr bool HEAD = W == HW;
 };
 
-template <int NT>
-__device__ __forceinline__ void load_cell(const Sim3D &P, uint2 rec, int half, CellRegs<NT> &C)
+// Cell data of one stream record as the prepare phase needs it: the kinematics and the (kappa, eps) pairs of the lane's
+// transitions.
+template <int NT, int W>
+struct CellRegs {
+    float4 kin;
+    float2 cf[Own<NT, W>::NHR];
+};
+
+template <int NT, int W>
+__device__ __forceinline__ void load_cell(const Sim3D &P, uint2 rec, int half, CellRegs<NT, W> &C)
 {
-    typedef Lay<NT> L;
+    typedef Own<NT, W> O;
     if ((rec.y >> 24) != LOC_OP_STEP) return;
     C.kin = __ldg(P.kin + rec.x);
-    // records are 16-byte aligned: nsp, slot0 and NH are even (the pad element after an odd NT is read but not used)
-    const float4 *cf = reinterpret_cast<const float4 *>(P.coef + (long long)rec.x * P.nsp + P.slot0 + half * L::NH);
+    const float2 *cf = P.coef + (long long)rec.x * P.nsp + P.slot0 + O::TB + half * O::NHW;
 #pragma unroll
-    for (int i = 0; i < L::NH / 2; i++)
-        if (half * L::NH + 2 * i < NT) C.cf[i] = __ldg(cf + i);
+    for (int i = 0; i < O::NHW; i++)
+        if (half * O::NHW + i < O::NW) C.cf[i] = __ldg(cf + i);
 }
 
-// Prepare phase: lanes (g, 2 j) and (g, 2 j + 1) decode record j of the chunk of group g and fill its shared-memory
-// record at `rb`; returns the record's flag bits (LOC_RS_*).  `nact` = number of channels within 5 sigma of the line
-// centre (the counting rule of the metric) for STEP records when the geometry counters are on.
-template <int NT>
-__device__ __forceinline__ unsigned prepare_record(const Sim3D &P, uint2 rec, const CellRegs<NT> &C, float d0, float d1, float d2, float sf,
-                                                   unsigned rb, int half, int &nact)
+// Prepare phase: lanes (g, 2 j) and (g, 2 j + 1) of each warp decode record j of the chunk of group g; every lane fills
+// the coefficients of its own transitions in the record at `rb`, lane half 0 of the header warp (Own::HEAD) also the header.  Returns the
+// record's flag bits (LOC_RS_*).  `nact` = number of channels within 5 sigma of the line centre (the counting rule of
+// the metric) for STEP records when the geometry counters are on.
+template <int NT, int W>
+__device__ __forceinline__ unsigned prepare_record(const Sim3D &P, uint2 rec, const CellRegs<NT, W> &C, float4 dir, unsigned rb, int half,
+                                                   int &nact)
 {
     typedef Lay<NT> L;
+    typedef Own<NT, W> O;
     const unsigned op = rec.y >> 24;
     const bool step = op == LOC_OP_STEP;
     unsigned flags = (op == LOC_OP_BG || op == LOC_OP_SAVE || op == LOC_OP_LOAD) ? LOC_RS_CTRL : 0u;
-    const int t0 = half * L::NH;
-    float2 ke[L::NH];
-#pragma unroll
-    for (int i = 0; i < L::NH; i++) ke[i] = make_float2(0.f, 0.f);
-    float s = 0.f, w = 0.f, amp = 0.f, tau0m = 0.f;
+    float s = 0.f, w = 0.f, amp = 0.f;
     float4 k = make_float4(0.f, 0.f, 0.f, 1.f);
     if (step) {
         k = C.kin;
         const unsigned dz = rec.y & 0x1fffffu;
         const int lev = (rec.y >> 21) & 7;
-        s = (float)dz * sf;
+        s = (float)dz * dir.w;
         w = (float)dz * P.inv_ndir * __int_as_float((127 - LOC_LB + lev) << 23);
         amp = P.dv * 0.3989422804f * rcpf(k.w);
-#pragma unroll
-        for (int i = 0; i < L::NH; i += 2) {
-            ke[i] = make_float2(C.cf[i / 2].x, C.cf[i / 2].y);
-            ke[i + 1] = make_float2(C.cf[i / 2].z, C.cf[i / 2].w);
-        }
-#pragma unroll
-        for (int i = 0; i < L::NH; i++)
-            if (t0 + i < NT) tau0m = fmaxf(tau0m, fabsf(ke[i].x * s) * amp);
         flags |= LOC_RS_STEP;
     }
-    tau0m = fmaxf(tau0m, __shfl_xor_sync(0xffffffffu, tau0m, 1));
-    float q0 = -INFINITY, q1 = 0.f, q2 = 0.f;  // phi = 2^(-inf) = 0 for records that are not steps: the round leaves their spectra untouched
-    unsigned wb = 0u, win = 1u;                // clo = 1 > chi = 0: empty window
     nact = 0;
-    if (step) {
-        // window half-width in sigma: the profile mass left outside stays a fixed fraction (that of xmin at tau0 <= 1) of
-        // the escape sum  sum_c phi_c f(tau_c) ~ 1/tau0  of an optically thick step (DESIGN 5.3)
-        const float v0 = -(k.x * d0 + k.y * d1 + k.z * d2);  // DESIGN R6
-        float X = P.xmin;
-        if (tau0m > 1.0f) X = sqrtf(fmaf(2.0f, __logf(tau0m), X * X));
-        const float inv_dv = rcpf(P.dv);
-        const float cc = fmaf(v0, inv_dv, 0.5f * (float)(P.nch - 1));  // line centre in channel units
-        const float sigch = k.w * inv_dv;
-        const float hw = X * sigch;
-        const int clo = max(0, (int)ceilf(cc - hw)), chi = min(P.nch - 1, (int)floorf(cc + hw));
-        // the span: 32 channels from a multiple of 4, centred on the line, inside the band
-        const int wbmax = (P.nch - LOC_SPAN) & ~3;
-        int iwb = 4 * (int)rintf((cc - 15.5f) * 0.25f);
-        iwb = max(0, min(iwb, wbmax));
-        const float lim = LOC_XCLIP * sigch;
-        const bool fast = P.nch >= LOC_SPAN && (clo >= iwb || cc - (float)iwb >= lim) && (chi <= iwb + LOC_SPAN - 1 || (float)(iwb + LOC_SPAN - 1) - cc >= lim);
-        if (P.nch < LOC_SPAN) iwb = 0;
-        if (!fast) flags |= LOC_RS_SLOW;
-        if (chi >= clo) win = (unsigned)clo | ((unsigned)chi << 16);
-        // log2 phi(channel wb + 16 + j) = lamp - (A + j ky)^2 with A = (wb + 16 - cc) ky: the quadratic in j is expanded
-        // around the middle of the span, where |A| is a few channels only (no cancellation between large terms)
-        const float ky = 0.8493218f * rcpf(sigch);  // sqrt(log2(e) / 2) in channel units
-        const float A = ((float)(iwb + 16) - cc) * ky;
-        q0 = fmaf(-A, A, __log2f(amp));
-        q1 = -2.0f * A * ky;
-        q2 = -ky * ky;
-        wb = (unsigned)iwb;
-        if (P.geom) nact = max(0, min(P.nch - 1, (int)floorf(cc + 5.0f * sigch)) - max(0, (int)ceilf(cc - 5.0f * sigch)) + 1);
-    }
-    if (half == 0) {
+    if (O::HEAD && half == 0) {
+        float q0 = -INFINITY, q1 = 0.f, q2 = 0.f, cc = 0.f;  // phi = 2^(-inf) = 0 for records that are not steps
+        unsigned wb = 0u;
+        if (step) {
+            const float v0 = -(k.x * dir.x + k.y * dir.y + k.z * dir.z);  // DESIGN R6
+            const float inv_dv = rcpf(P.dv);
+            cc = fmaf(v0, inv_dv, 0.5f * (float)(P.nch - 1));  // line centre in channel units
+            const float sigch = k.w * inv_dv;
+            // the span: 32 channels from a multiple of 4, centred on the line, inside the band; it serves the step if it
+            // reaches LOC_XCLIP sigma to both sides of the line centre (the nominal window of DESIGN 5.3 may be wider for
+            // a thick line and is then cut there); otherwise the step takes the masked path with its exact window
+            const int wbmax = (P.nch - LOC_SPAN) & ~3;
+            int iwb = 4 * (int)rintf((cc - 15.5f) * 0.25f);
+            iwb = max(0, min(iwb, wbmax));
+            const float lim = LOC_XCLIP * sigch;
+            const bool fast = P.nch >= LOC_SPAN && cc - (float)iwb >= lim && (float)(iwb + LOC_SPAN - 1) - cc >= lim;
+            if (P.nch < LOC_SPAN) iwb = 0;
+            if (!fast) flags |= LOC_RS_SLOW;
+            // log2 phi(channel wb + 16 + j) = lamp - (A + j ky)^2 with A = (wb + 16 - cc) ky: the quadratic in j is
+            // expanded around the middle of the span, where |A| is a few channels only
+            const float ky = 0.8493218f * rcpf(sigch);  // sqrt(log2(e) / 2) in channel units
+            const float A = ((float)(iwb + 16) - cc) * ky;
+            q0 = fmaf(-A, A, __log2f(amp));
+            q1 = -2.0f * A * ky;
+            q2 = -ky * ky;
+            wb = (unsigned)iwb;
+            if (P.geom) nact = max(0, min(P.nch - 1, (int)floorf(cc + 5.0f * sigch)) - max(0, (int)ceilf(cc - 5.0f * sigch)) + 1);
+        }
         sts128u(rb, make_uint4(__float_as_uint(q0), __float_as_uint(q1), __float_as_uint(q2), wb | flags));
         const unsigned coff = step ? rec.x * (unsigned)P.nsp + (unsigned)P.slot0 : rec.x;
-        sts128u(rb + 16, make_uint4(coff, __float_as_uint(w), rec.y, win));
+        sts128u(rb + 16, make_uint4(coff, __float_as_uint(w), rec.y, __float_as_uint(cc)));
     }
     // per transition, branch free: the exponential form from tau0 >= LOC_EXP_TAU (header comment); records that are not
     // steps have kappa = eps = s = w = 0 and get all-zero coefficients
     const float wos = w * rcpf(s);  // not used when s = 0
 #pragma unroll
-    for (int i = 0; i < L::NH; i++) {
-        const int t = t0 + i;
-        if (t < NT) {
-            const float ks = ke[i].x * s;
+    for (int i = 0; i < O::NHW; i++) {
+        if (half * O::NHW + i < O::NW) {
+            const int t = O::TB + half * O::NHW + i;
+            const float2 ke = step ? C.cf[i] : make_float2(0.f, 0.f);
+            const float ks = ke.x * s;
             const bool thick = fabsf(ks) * amp >= LOC_EXP_TAU;
-            const float rk = rcpf(ke[i].x);
+            const float rk = rcpf(ke.x);
             float4 tp;
             tp.x = thick ? 0.0f : ks;
             tp.y = thick ? -ks * LOC_LOG2E : 0.0f;
-            tp.z = thick ? ke[i].y * rk : ke[i].y * s;   // source function in occupation-number units | eps s
+            tp.z = thick ? ke.y * rk : ke.y * s;   // source function in occupation-number units | eps s
             tp.w = thick ? -1.0f : -ks;
             sts128(rb + L::TP + 16 * t, tp);
             sts32(rb + L::UO + 4 * t, thick ? 0.0f : 1.0f);
@@ -304,24 +307,41 @@ __device__ __forceinline__ unsigned prepare_record(const Sim3D &P, uint2 rec, co
     return flags;
 }
 
-// Masked multi-pass round for one lane's ray step (rare: DESIGN 6.4): passes of 32 channels over the nominal window
-// [clo, chi].  Adds the lane's partial sums to its slots of the `part` rows (zeroed here) and returns the lane's sum of
-// phi.  Scalar arithmetic, rolled over the transitions; same expressions as the common round.
-template <int NT>
-__device__ __forceinline__ float slow_round(unsigned rb, unsigned sqg, unsigned pl, int l8, int nchp)
+// Masked multi-pass round for one lane's ray step (rare: DESIGN 6.4): passes of 32 channels over the step's nominal
+// window [clo, chi], which is formed here from the record (the largest line-centre optical depth of ALL transitions sets
+// its width, DESIGN 5.3), for the warp's own transitions.  Adds the lane's partial sums to its slots of the `part` rows
+// (zeroed here) and returns the lane's sum of phi.  Scalar arithmetic, rolled over the transitions; same expressions as
+// the common round.
+template <int NT, int W>
+__device__ __forceinline__ float slow_round(const Sim3D &P, unsigned rb, unsigned sqg, unsigned pl, int l8, int nchp)
 {
     typedef Lay<NT> L;
+    typedef Own<NT, W> O;
     const float4 h0 = lds128(rb);
     const uint4 h1 = lds128u(rb + 16);
     const unsigned wbop = __float_as_uint(h0.w);
     const int wb = (int)(wbop & LOC_WB_MASK);
-    int clo = (int)(h1.w & 0xffffu), chi = (int)(h1.w >> 16);
-    if (!(wbop & LOC_RS_STEP)) {
-        clo = 1;
-        chi = 0;
+    int clo = 1, chi = 0;
+    if (wbop & LOC_RS_STEP) {
+        const float ky = sqrtf(-h0.z);
+        const float sigch = 0.8493218f * rcpf(ky);
+        const float A = -0.5f * h0.y * rcpf(ky);
+        const float amp = ex2f(fmaf(A, A, h0.x));
+        float km = 0.f;  // largest |kappa s| of the step
+#pragma unroll 1
+        for (int t = 0; t < NT; t++) {
+            const float4 tp = lds128(rb + L::TP + 16 * t);
+            km = fmaxf(km, fmaxf(fabsf(tp.x), fabsf(tp.y) * 0.6931472f));
+        }
+        const float tau0m = km * amp;
+        float X = P.xmin;
+        if (tau0m > 1.0f) X = sqrtf(fmaf(2.0f, __logf(tau0m), X * X));
+        const float cc = __uint_as_float(h1.w), hw = X * sigch;
+        clo = max(0, (int)ceilf(cc - hw));
+        chi = min(P.nch - 1, (int)floorf(cc + hw));
     }
 #pragma unroll 1
-    for (int t = 0; t < NT; t++) sts64(pl + t * L::ROWB, make_float2(0.f, 0.f));
+    for (int t = O::TB; t < O::TB + O::NW; t++) sts64(pl + t * L::ROWB, make_float2(0.f, 0.f));
     float sphi = 0.f;
     int base = clo & ~3;
     while (__any_sync(0xffffffffu, base <= chi)) {
@@ -339,7 +359,7 @@ __device__ __forceinline__ float slow_round(unsigned rb, unsigned sqg, unsigned 
         sphi += (e[0] + e[1]) + (e[2] + e[3]);
         if (inq) {
 #pragma unroll 1
-            for (int t = 0; t < NT; t++) {
+            for (int t = O::TB; t < O::TB + O::NW; t++) {
                 const float4 tp = lds128(rb + L::TP + 16 * t);
                 const float U = lds32(rb + L::UO + 4 * t);
                 const unsigned sa = sqg + 4 * base + 4 * t * nchp;
@@ -364,13 +384,14 @@ __device__ __forceinline__ float slow_round(unsigned rb, unsigned sqg, unsigned 
     return sphi;
 }
 
-// The common round: one pass over the span for all NT transitions, straight-line code.  `sq` = shared address of the
-// lane's quad in transition 0, `rowb` = bytes between the spectra of consecutive transitions, `pl` = the lane's slot in
-// row 0 of the group's partial sums.  Returns the lane's sum of phi.
-template <int NT>
+// The common round: one pass over the span for the warp's NW transitions, straight-line code.  `sq` = shared address of
+// the lane's quad in transition 0, `rowb` = bytes between the spectra of consecutive transitions, `pl` = the lane's slot
+// in row 0 of the group's partial sums.  Returns the lane's sum of phi.
+template <int NT, int W>
 __device__ __forceinline__ float fast_round(unsigned rb, unsigned sq, int rowb, unsigned pl, const float4 h0, const f32x2 J01, const f32x2 J23)
 {
     typedef Lay<NT> L;
+    typedef Own<NT, W> O;
     // profile: log2 phi = q0 + j (q1 + j q2)
     const f32x2 Q0 = pk2(h0.x, h0.x), Q1 = pk2(h0.y, h0.y), Q2 = pk2(h0.z, h0.z);
     float y0, y1, y2, y3;
@@ -385,57 +406,55 @@ __device__ __forceinline__ float fast_round(unsigned rb, unsigned sq, int rowb, 
     const f32x2 s01 = mul2(P01, P01), s23 = mul2(P23, P23);
     const f32x2 B2a = mul2(s01, K2), B2b = mul2(s23, K2);
     const f32x2 B3a = mul2(mul2(s01, P01), K3), B3b = mul2(mul2(s23, P23), K3);
-    float Uv[L::NT4];
-#pragma unroll
-    for (int t = 0; t < L::NT4; t += 4) {
-        const float4 u = lds128(rb + L::UO + 4 * t);
-        Uv[t] = u.x;
-        Uv[t + 1] = u.y;
-        Uv[t + 2] = u.z;
-        Uv[t + 3] = u.w;
-    }
     // three phases (all loads, arithmetic, all stores): the shared-memory accesses are ordered among themselves, the
-    // arithmetic of the NT transitions in between is free to interleave
-    float4 tp[NT], n4[NT];  // tp = C0, Ce, c1, alpha
+    // arithmetic of the transitions in between is free to interleave
+    float4 tp[O::NHR * 2], n4[O::NHR * 2];  // tp = C0, Ce, c1, alpha
+    float Uv[O::NHR * 2];
 #pragma unroll
-    for (int t = 0; t < NT; t++) {
-        tp[t] = lds128(rb + L::TP + 16 * t);
-        n4[t] = lds128(sq + t * rowb);
+    for (int i = 0; i < O::NW; i++) {
+        tp[i] = lds128(rb + L::TP + 16 * (O::TB + i));
+        Uv[i] = lds32(rb + L::UO + 4 * (O::TB + i));
+        n4[i] = lds128(sq + (O::TB + i) * rowb);
     }
-    float2 ab[NT];
+    float2 ab[O::NHR * 2];
 #pragma unroll
-    for (int t = 0; t < NT; t++) {
-        const f32x2 C0 = pk2(tp[t].x, tp[t].x), CE = pk2(tp[t].y, tp[t].y), C1 = pk2(tp[t].z, tp[t].z), AL = pk2(tp[t].w, tp[t].w),
-                    UU = pk2(Uv[t], Uv[t]);
+    for (int i = 0; i < O::NW; i++) {
+        const f32x2 C0 = pk2(tp[i].x, tp[i].x), CE = pk2(tp[i].y, tp[i].y), C1 = pk2(tp[i].z, tp[i].z), AL = pk2(tp[i].w, tp[i].w),
+                    UU = pk2(Uv[i], Uv[i]);
         float z0, z1, z2, z3;
         upk2(mul2(CE, P01), z0, z1);
         upk2(mul2(CE, P23), z2, z3);
         const f32x2 E01 = pk2(ex2f(z0), ex2f(z1)), E23 = pk2(ex2f(z2), ex2f(z3));
         const f32x2 X01 = fma2(C0, fma2(C0, B3a, B2a), fma2(UU, P01, fma2(E01, MONE2, ONE2)));
         const f32x2 X23 = fma2(C0, fma2(C0, B3b, B2b), fma2(UU, P23, fma2(E23, MONE2, ONE2)));
-        const f32x2 N01 = pk2(n4[t].x, n4[t].y), N23 = pk2(n4[t].z, n4[t].w);
+        const f32x2 N01 = pk2(n4[i].x, n4[i].y), N23 = pk2(n4[i].z, n4[i].w);
         float a0, a1, b0, b1;
         upk2(fma2(N01, X01, mul2(N23, X23)), a0, a1);
         upk2(add2(X01, X23), b0, b1);
-        ab[t] = make_float2(a0 + a1, b0 + b1);
-        upk2(fma2(X01, fma2(AL, N01, C1), N01), n4[t].x, n4[t].y);
-        upk2(fma2(X23, fma2(AL, N23, C1), N23), n4[t].z, n4[t].w);
+        ab[i] = make_float2(a0 + a1, b0 + b1);
+        upk2(fma2(X01, fma2(AL, N01, C1), N01), n4[i].x, n4[i].y);
+        upk2(fma2(X23, fma2(AL, N23, C1), N23), n4[i].z, n4[i].w);
     }
 #pragma unroll
-    for (int t = 0; t < NT; t++) {
-        sts128(sq + t * rowb, n4[t]);
-        sts64(pl + t * L::ROWB, ab[t]);
+    for (int i = 0; i < O::NW; i++) {
+        sts128(sq + (O::TB + i) * rowb, n4[i]);
+        sts64(pl + (O::TB + i) * L::ROWB, ab[i]);
     }
     return sphi;
 }
 
-// NCHP_T: spectrum row length in floats when known at compile time (immediate offsets), 0 = P.nchp
-template <int NT, int NCHP_T>
-__global__ void __maxnreg__(192) k_sim3d(Sim3D P)
+__device__ __forceinline__ void cta_sync()  // both warps of the CTA
+{
+    asm volatile("bar.sync 0, 64;" ::: "memory");
+}
+
+// One warp of the CTA.  NCHP_T: spectrum row length in floats when known at compile time (immediate offsets), 0 = P.nchp
+template <int NT, int NCHP_T, int W>
+__device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
 {
     typedef Lay<NT> L;
-    extern __shared__ __align__(16) float smem[];  // [4][NT][nchp] spectra, then the tables of Lay<NT>
-    const int lane = threadIdx.x, grp = lane >> 3, l8 = lane & 7, rj = l8 >> 1, half = l8 & 1;
+    typedef Own<NT, W> O;
+    const int lane = threadIdx.x & 31, grp = lane >> 3, l8 = lane & 7, rj = l8 >> 1, half = l8 & 1;
     const int nchp = NCHP_T ? NCHP_T : P.nchp;
     const int spec = NT * nchp;                // floats per ray spectrum
     const int rowb = 4 * nchp;
@@ -444,108 +463,106 @@ __global__ void __maxnreg__(192) k_sim3d(Sim3D P)
     const unsigned tb = sm0 + 4u * LOC_GROUPS * spec;
     const unsigned rec_g = tb + L::OFF_REC + grp * L::GSB;
     const unsigned part_g = tb + L::OFF_PART + grp * L::PGB;
-    const unsigned pl = part_g + 8 * l8;             // my slot in row 0
-    const unsigned prow = part_g + L::ROWB * l8;     // row l8 (reducing lane)
+    const unsigned pl = part_g + 8 * l8;                        // my slot in row 0
+    const unsigned prow = part_g + L::ROWB * (O::TB + l8);      // row of my transition (reducing lane)
+    const unsigned phi_g = part_g + L::PHI + 32 * W;
     const unsigned sq_g = sm0 + 4u * grp * spec + 16 * l8;
     float *slots_warp = P.pool + (long long)blockIdx.x * LOC_GROUPS * P.nslot * spec;
     const float jb = (float)(4 * l8 - 16);
     const f32x2 J01 = pk2(jb, jb + 1.0f), J23 = pk2(jb + 2.0f, jb + 3.0f);
-    float2 *const cnt_l = P.cnt + l8;
-    // the spectrum slots of the resident warps (donor spectra, DESIGN 6.3) are re-read by every ray born from them: keep
+    float2 *const cnt_l = P.cnt + O::TB + l8;
+    // the spectrum slots of the resident CTAs (donor spectra, DESIGN 6.3) are re-read by every ray born from them: keep
     // them in L2 against the streaming traffic of the step records, coefficients and counters
     unsigned long long pol_keep;
     asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_keep));
     const uint2 NOPREC = make_uint2(0u, LOC_OP_NOP << 24);
+    const int row0 = O::TB * nchp, rown = O::NW * nchp;  // my rows of a spectrum, in floats
 
     long long off = 0, end = 0;  // this group's position in the stream (first record of the current chunk)
     bool done = false, fresh = false;
-    float d0 = 0.f, d1 = 0.f, d2 = 0.f, sf = 0.f;
+    float4 dir = make_float4(0.f, 0.f, 0.f, 0.f);  // (d0, d1, d2, sf) of the group's ray
     unsigned mysteps = 0;
     unsigned long long myactive = 0;
     // software pipeline over chunks: r0 = records of this chunk, r1 / r2 = of the next two (r2 in flight), `cell` = cell
     // data of r0's record, loaded during the previous chunk's rounds
     uint2 r0 = NOPREC, r1 = NOPREC, r2 = NOPREC;
-    CellRegs<NT> cell;
+    CellRegs<NT, W> cell;
     cell.kin = make_float4(0.f, 0.f, 0.f, 1.f);
 #pragma unroll
-    for (int i = 0; i < L::NH / 2; i++) cell.cf[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int i = 0; i < O::NHR; i++) cell.cf[i] = make_float2(0.f, 0.f);
 
     for (;;) {
-        // ---- refill: groups whose task is exhausted take the next root ray from the queue ----
-        {
-            const bool need = !done && off >= end;
-            if (__any_sync(0xffffffffu, need)) {
-                long long task = 0;
-                if (need && l8 == 0) task = atomicAdd(P.queue, 1u);
-                task = __shfl_sync(0xffffffffu, task, grp * 8);
-                if (need) {
-                    if (task >= P.ntask) {
-                        done = true;
-                        r0 = r1 = r2 = NOPREC;
-                    } else {
-                        const Dir3 *Dp = P.dirs + P.task_dir[task];
-                        d0 = __ldg(&Dp->d[0]);
-                        d1 = __ldg(&Dp->d[1]);
-                        d2 = __ldg(&Dp->d[2]);
-                        sf = __ldg(&Dp->sf);
-                        off = __ldg(P.task_off + task);
-                        end = __ldg(P.task_off + task + 1);
-                        fresh = true;
-                    }
-                }
-                if (__all_sync(0xffffffffu, done)) break;
+        // ---- refill: groups whose task is exhausted take the next root ray from the queue (warp 0 asks, both read) ----
+        const bool need = !done && off >= end;
+        if (W == 0 && need && l8 == 0) sts32u(tb + L::OFF_TASK + 4 * grp, atomicAdd(P.queue, 1u));
+        cta_sync();  // the previous chunk's records are free; the tasks are posted
+        if (need) {
+            const long long task = lds32u(tb + L::OFF_TASK + 4 * grp);
+            if (task >= P.ntask) {
+                done = true;
+                r0 = r1 = r2 = NOPREC;
+            } else {
+                const Dir3 *Dp = P.dirs + P.task_dir[task];
+                dir = make_float4(__ldg(&Dp->d[0]), __ldg(&Dp->d[1]), __ldg(&Dp->d[2]), __ldg(&Dp->sf));
+                off = __ldg(P.task_off + task);
+                end = __ldg(P.task_off + task + 1);
+                fresh = true;
             }
         }
+        if (__all_sync(0xffffffffu, done)) break;  // the same in both warps
         if (fresh) {  // first chunk of a ray: nothing was prefetched
             r0 = __ldg(P.stream + off + rj);
             r1 = (off + LOC_CHUNK < end) ? __ldg(P.stream + off + LOC_CHUNK + rj) : NOPREC;
-            load_cell<NT>(P, r0, half, cell);
+            load_cell<NT, W>(P, r0, half, cell);
             fresh = false;
         }
         r2 = (!done && off + 2 * LOC_CHUNK < end) ? __ldg(P.stream + off + 2 * LOC_CHUNK + rj) : NOPREC;
         // ---- prepare: lane pair rj of each group decodes record off + rj of its ray ----
         int nact;
-        unsigned flags = prepare_record<NT>(P, r0, cell, d0, d1, d2, sf, rec_g + rj * L::RECB, half, nact);
-        if (half == 0) {
-            mysteps += flags >> 31;
-            myactive += nact;
+        unsigned flags = prepare_record<NT, W>(P, r0, cell, dir, rec_g + rj * L::RECB, half, nact);
+        if (O::HEAD) {
+            if (half == 0) {
+                mysteps += flags >> 31;
+                myactive += nact;
+            }
+            // class of round rj: OR of the record flags over the four groups
+            flags |= __shfl_xor_sync(0xffffffffu, flags, 8);
+            flags |= __shfl_xor_sync(0xffffffffu, flags, 16);
+            if (lane == 2 * rj) sts32u(tb + L::OFF_CLS + 4 * rj, flags);
         }
-        // class of round rj: OR of the record flags over the four groups
-        flags |= __shfl_xor_sync(0xffffffffu, flags, 8);
-        flags |= __shfl_xor_sync(0xffffffffu, flags, 16);
-        load_cell<NT>(P, r1, half, cell);  // for the next chunk (NOP records load nothing)
-        __syncwarp();
+        load_cell<NT, W>(P, r1, half, cell);  // for the next chunk (NOP records load nothing)
+        cta_sync();  // the records of the chunk are complete
 
         // ---- LOC_CHUNK rounds: every group consumes one record per round ----
 #pragma unroll 1
         for (int r = 0; r < LOC_CHUNK; r++) {
-            const unsigned cls = __shfl_sync(0xffffffffu, flags, 2 * r);
+            const unsigned cls = lds32u(tb + L::OFF_CLS + 4 * r);
             const unsigned rb = rec_g + r * L::RECB;
             if (cls & LOC_RS_CTRL) {
-                // spectrum operations, executed by the whole warp for one group at a time
+                // spectrum operations on the warp's own rows, executed by the whole warp for one group at a time
                 for (int g = 0; g < LOC_GROUPS; g++) {
                     const uint4 gh = lds128u(tb + L::OFF_REC + g * L::GSB + r * L::RECB + 16);
                     const unsigned gop = gh.z >> 24, gx = gh.x;
-                    float *gs = sn_all + g * spec;
-                    float *slot = slots_warp + ((long long)g * P.nslot + gx) * spec;
+                    float *gs = sn_all + g * spec + row0;
+                    float *slot = slots_warp + ((long long)g * P.nslot + gx) * spec + row0;
                     if (gop == LOC_OP_BG) {
-                        for (int t = 0; t < NT; t++) {
-                            const float bg = P.S.bgocc[P.slot0 + t];
+                        for (int t = 0; t < O::NW; t++) {
+                            const float bg = P.S.bgocc[P.slot0 + O::TB + t];
                             for (int c = lane; c < nchp; c += 32) gs[t * nchp + c] = bg;
                         }
                     } else if (gop == LOC_OP_SAVE) {
-                        for (int i = lane * 4; i < spec; i += 128) stg_keep(slot + i, *reinterpret_cast<const float4 *>(gs + i), pol_keep);
+                        for (int i = lane * 4; i < rown; i += 128) stg_keep(slot + i, *reinterpret_cast<const float4 *>(gs + i), pol_keep);
                     } else if (gop == LOC_OP_LOAD) {
                         // all loads of a batch in flight before the first store: one L2 latency per batch, not per quad
-                        constexpr int NB = 9;
-                        for (int i0 = lane * 4; i0 < spec; i0 += 128 * NB) {
+                        constexpr int NB = 6;
+                        for (int i0 = lane * 4; i0 < rown; i0 += 128 * NB) {
                             float4 v[NB];
 #pragma unroll
                             for (int k = 0; k < NB; k++)
-                                if (i0 + 128 * k < spec) v[k] = ldg_keep(slot + i0 + 128 * k, pol_keep);
+                                if (i0 + 128 * k < rown) v[k] = ldg_keep(slot + i0 + 128 * k, pol_keep);
 #pragma unroll
                             for (int k = 0; k < NB; k++)
-                                if (i0 + 128 * k < spec) *reinterpret_cast<float4 *>(gs + i0 + 128 * k) = v[k];
+                                if (i0 + 128 * k < rown) *reinterpret_cast<float4 *>(gs + i0 + 128 * k) = v[k];
                         }
                     }
                 }
@@ -556,35 +573,31 @@ __global__ void __maxnreg__(192) k_sim3d(Sim3D P)
             const unsigned wbop = __float_as_uint(h0.w);
             float sphi;
             if (!(cls & LOC_RS_SLOW))
-                sphi = fast_round<NT>(rb, sq_g + 4u * (wbop & LOC_WB_MASK), rowb, pl, h0, J01, J23);
+                sphi = fast_round<NT, W>(rb, sq_g + 4u * (wbop & LOC_WB_MASK), rowb, pl, h0, J01, J23);
             else
-                sphi = slow_round<NT>(rb, sq_g, pl, l8, nchp);
-            sts32(part_g + L::PHI + 4 * l8, sphi);
+                sphi = slow_round<NT, W>(P, rb, sq_g, pl, l8, nchp);
+            sts32(phi_g + 4 * l8, sphi);
             __syncwarp();
-            // ---- reduction over the 8 lanes of each group: lane t adds up row t and issues the two float atomics of
-            //      (cell, transition t) as one 64-bit RED ----
+            // ---- reduction over the 8 lanes of each group: lane i adds up the row of the warp's i-th transition and
+            //      issues the two float atomics of (cell, transition) as one 64-bit RED ----
             const bool step = wbop & LOC_RS_STEP;
-            const uint4 h1 = lds128u(rb + 16);  // coff, w, opdz, win
-            const float4 f0 = lds128(part_g + L::PHI), f1 = lds128(part_g + L::PHI + 16);
-            float fa, fb;
-            upk2(add2(add2(pk2(f0.x, f0.y), pk2(f0.z, f0.w)), add2(pk2(f1.x, f1.y), pk2(f1.z, f1.w))), fa, fb);
-            const float w = __uint_as_float(h1.y);
-            const float wesc = fmaf(-w, fa + fb, w);  // photons emitted outside the updated channels escape (DESIGN 5.3)
-#pragma unroll
-            for (int t0 = 0; t0 < NT; t0 += 8) {
-                if (step && t0 + l8 < NT) {
-                    const float4 a0 = lds128(prow + t0 * L::ROWB), a1 = lds128(prow + t0 * L::ROWB + 16), a2 = lds128(prow + t0 * L::ROWB + 32),
-                                 a3 = lds128(prow + t0 * L::ROWB + 48);
-                    const float sc = lds32(rb + L::SC + 4 * t0 + 4 * l8);
-                    const f32x2 s01 = add2(add2(pk2(a0.x, a0.y), pk2(a0.z, a0.w)), add2(pk2(a1.x, a1.y), pk2(a1.z, a1.w)));
-                    const f32x2 s23 = add2(add2(pk2(a2.x, a2.y), pk2(a2.z, a2.w)), add2(pk2(a3.x, a3.y), pk2(a3.z, a3.w)));
-                    float A, B;
-                    upk2(add2(s01, s23), A, B);
-                    float2 *cn = cnt_l + (h1.x + (unsigned)t0);
-                    asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(cn), "f"(A * sc), "f"(fmaf(B, sc, wesc)) : "memory");
-                }
+            const uint4 h1 = lds128u(rb + 16);  // coff, w, opdz, cc
+            if (step && l8 < O::NW) {
+                const float4 f0 = lds128(phi_g), f1 = lds128(phi_g + 16);
+                const float4 a0 = lds128(prow), a1 = lds128(prow + 16), a2 = lds128(prow + 32), a3 = lds128(prow + 48);
+                const float sc = lds32(rb + L::SC + 4 * (O::TB + l8));
+                float fa, fb;
+                upk2(add2(add2(pk2(f0.x, f0.y), pk2(f0.z, f0.w)), add2(pk2(f1.x, f1.y), pk2(f1.z, f1.w))), fa, fb);
+                const float w = __uint_as_float(h1.y);
+                const float wesc = fmaf(-w, fa + fb, w);  // photons emitted outside the updated channels escape (DESIGN 5.3)
+                const f32x2 s01 = add2(add2(pk2(a0.x, a0.y), pk2(a0.z, a0.w)), add2(pk2(a1.x, a1.y), pk2(a1.z, a1.w)));
+                const f32x2 s23 = add2(add2(pk2(a2.x, a2.y), pk2(a2.z, a2.w)), add2(pk2(a3.x, a3.y), pk2(a3.z, a3.w)));
+                float A, B;
+                upk2(add2(s01, s23), A, B);
+                float2 *cn = cnt_l + h1.x;
+                asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(cn), "f"(A * sc), "f"(fmaf(B, sc, wesc)) : "memory");
             }
-            if (P.geom && step && l8 == 0) {
+            if (O::HEAD && P.geom && step && l8 == 0) {
                 const unsigned cellidx = (h1.x - (unsigned)P.slot0) / (unsigned)P.nsp;
                 atomicAdd(&P.visits[cellidx], 1u);
                 atomicAdd(&P.pathz[cellidx], h1.z & 0x1fffffu);
@@ -595,14 +608,25 @@ __global__ void __maxnreg__(192) k_sim3d(Sim3D P)
         r0 = r1;
         r1 = r2;
     }
-    // per-warp totals
-    unsigned long long ms = mysteps;
-    for (int o = 16; o >= 1; o >>= 1) {
-        ms += __shfl_xor_sync(0xffffffffu, ms, o);
-        myactive += __shfl_xor_sync(0xffffffffu, myactive, o);
+    if (O::HEAD) {  // per-warp totals
+        unsigned long long ms = mysteps;
+        for (int o = 16; o >= 1; o >>= 1) {
+            ms += __shfl_xor_sync(0xffffffffu, ms, o);
+            myactive += __shfl_xor_sync(0xffffffffu, myactive, o);
+        }
+        if (lane == 0 && ms) atomicAdd(P.nsteps, ms);
+        if (P.geom && lane == 0 && myactive) atomicAdd(P.nsteps + 1, myactive);
     }
-    if (lane == 0 && ms) atomicAdd(P.nsteps, ms);
-    if (P.geom && lane == 0 && myactive) atomicAdd(P.nsteps + 1, myactive);
+}
+
+template <int NT, int NCHP_T>
+__global__ void __maxnreg__(128) k_sim3d(Sim3D P)
+{
+    extern __shared__ __align__(16) float smem[];  // [4][NT][nchp] spectra, then the tables of Lay<NT>
+    if (threadIdx.x < 32)
+        run_warp<NT, NCHP_T, 0>(P, smem);
+    else
+        run_warp<NT, NCHP_T, 1>(P, smem);
 }
 
 template <int NT, int NCHP_T>
@@ -611,7 +635,7 @@ static int launch3d_t(loc_model *m, Sim3D &P, size_t smem)
     auto kern = k_sim3d<NT, NCHP_T>;
     LOC_CUDA_CHECK(m, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int bps = 0;
-    LOC_CUDA_CHECK(m, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kern, 32, smem));
+    LOC_CUDA_CHECK(m, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kern, 64, smem));
     if (bps < 1) bps = 1;
     int nsm = 148;
     cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, 0);
@@ -620,7 +644,7 @@ static int launch3d_t(loc_model *m, Sim3D &P, size_t smem)
     blocks = std::min<long long>(blocks, m->max_warps);
     if (blocks < 1) blocks = 1;
     LOC_CUDA_CHECK(m, cudaMemsetAsync(m->d_queue, 0, sizeof(unsigned int), m->stream));
-    kern<<<(unsigned)blocks, 32, smem, m->stream>>>(P);
+    kern<<<(unsigned)blocks, 64, smem, m->stream>>>(P);
     m->launches++;
     LOC_CUDA_CHECK(m, cudaGetLastError());
     return LOC_OK;
