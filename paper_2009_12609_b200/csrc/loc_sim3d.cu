@@ -32,8 +32,12 @@
 // (Ce = 0, U = 1, C0 = kappa s, c1 = eps s, alpha = -C0: X = phi f(tau), f = 1 - tau/2 + tau^2/6, truncation
 // tau^3/24 < 1.2e-6; ex2(0) = 1 exactly, so the first bracket vanishes).  1 - e^-tau by ex2.approx and a subtraction
 // has an absolute error of ~1e-7 per channel, i.e. < 1e-5 of the channel sums for tau0 >= 0.03.
-// Steps whose window does not fit one span (bands narrower than 32 channels, lines cut by the band edge, very wide
-// lines) take a masked multi-pass path written as a rolled loop.  The four groups stay in lock step: every round each
+// Reach of the span (DESIGN 5.3).  The profile is carried out to X sigma, X^2 = LOC_XCLIP^2 + 2 ln max(1, tau0m) with tau0m
+// the largest line-centre optical depth of the step over ALL transitions.  The profile mass beyond the span is known
+// analytically (wing_mass): it enters the escape fraction as it stands, and the photons of the span's edge channels
+// stand for those of the thin wings beyond them in the absorbed-photon sum ("wing correction").  A step whose centred
+// span does not reach X sigma takes two adjacent spans (WIDE round: two passes of the same code); bands narrower than
+// the spans take a masked multi-pass path written as a rolled loop.  The four groups stay in lock step: every round each
 // group consumes exactly one stream record (tasks are padded to whole chunks by the path builder); the rare spectrum
 // operations (background, save, load) are executed by the whole warp for the group that needs them.
 #include <math.h>
@@ -52,7 +56,7 @@ struct Sim3D {
     int nch, nchp, nsp, nslot;
     int slot0;  // first counter / coefficient slot handled by this launch (transitions may be split over launches)
     int geom;   // also accumulate the geometry counters (visits, path sums, active channels)
-    float dv, xmin, eps_tau, inv_ndir;
+    float dv, xmin, xclip, inv_ndir;
     const Dir3 *dirs;
     const unsigned char *task_dir;
     const long long *task_off;
@@ -70,28 +74,33 @@ struct Sim3D {
 
 // ---- shared-memory record of one (ray, round), written by the prepare phase --------------------------------------
 //   +0   float q0, q1, q2     log2 phi(channel wb + 16 + j) = q0 + j (q1 + j q2)      (j = -16 .. 15 inside the span)
-//   +12  uint  wbop           bits 0..9 first channel of the span, bit 29 = needs the masked path,
+//   +12  uint  wbop           bits 0..9 first channel of the span,
 //                             bit 30 = spectrum operation (BG / SAVE / LOAD), bit 31 = the record is a STEP
 //   +16  uint  coff           cell * nsp + slot0 : element offset of the cell's counter record (STEP); slot (SAVE / LOAD)
 //   +20  float w              a s / V_eff = dzeta / (h NDIR)
 //   +24  uint  opdz           opcode | level | dzeta (stream word)
-//   +28  float cc             line centre in channel units (masked path)
-//   +32  float4 tp[NT]        (C0, Ce, c1, alpha) per transition (header comment)
-//   +32 + 16 NT   float U[NT4]    1 = series, 0 = exponential; NT4 = NT rounded up to 4
+//   +28  float cc             line centre in channel units
+//   +32  float tm[4]          largest line-centre optical depth among the transitions of preparing lane 2 W + half
+//   +48  float ql, qh, qe     profile mass below / above the span (wing correction), and outside it (or -1), 1 pad word
+//   +64  float4 tp[NT]        (C0, Ce, c1, alpha) per transition (header comment)
+//   +64 + 16 NT   float U[NT4]    1 = series, 0 = exponential; NT4 = NT rounded up to 4
 //   then          float sc[NT4]   scale of the channel sums: w (series) or w / (kappa s) (exponential)
 #define LOC_WB_MASK 0x3ffu
-#define LOC_RS_SLOW 0x20000000u
+#define LOC_RS_WIDE 0x10000000u  // mode bits of a step, formed after the prepare phase (step_mode): two spans
+#define LOC_RS_SLOW 0x20000000u  //   masked multi-pass path
 #define LOC_RS_CTRL 0x40000000u
 #define LOC_RS_STEP 0x80000000u
 
-#define LOC_XCLIP 3.9f     // the span reaches at least this many sigma to both sides of the line centre, or the step is masked
-#define LOC_EXP_TAU 0.03f  // line-centre optical depth of a step from which the exponential form is used
+#define LOC_XCLIP 3.4f     // the span reaches at least this many sigma to both sides of the line centre, or the step is masked
+#define LOC_EXP_TAU 0.05f  // line-centre optical depth of a step from which the exponential form is used
 
 template <int NT>
 struct Lay {
     static constexpr int NT4 = (NT + 3) & ~3;
     static constexpr int NT0 = (NT + 1) / 2;         // transitions of warp 0; warp 1 has the other NT - NT0
-    static constexpr int TP = 32;                    // byte offset of tp[] in a record
+    static constexpr int TM = 32;                    // byte offset of tm[]
+    static constexpr int QW = 48;                    // byte offset of (ql, qh)
+    static constexpr int TP = 64;                    // byte offset of tp[] in a record
     static constexpr int UO = TP + 16 * NT;          // byte offset of U[]
     static constexpr int SC = UO + 4 * NT4;          // byte offset of sc[]
     static constexpr int RECB = SC + 4 * NT4;        // record bytes (multiple of 16)
@@ -193,6 +202,18 @@ __device__ __forceinline__ void sts32u(unsigned a, unsigned v)
 
 
 
+// Profile mass below channel s0 and above channel s0 + len - 1 for a line centred at channel cc with 1 / sigma = rs (per
+// channel): Q(x) = phi(x) / (x + 1/(x + 2/(x + 3/(x + 4/x)))), good to ~1e-5 of Q for the distances x >= 3 sigma that
+// occur; `far` = both distances are.  Their sum is 1 - sum phi over the channels s0 .. s0 + len - 1, far more accurate
+// than that difference in float32 (the escape fraction of a thick cell is ~1e-3).
+__device__ __forceinline__ void wing_mass(float cc, float rs, float s0, float len, float &Ql, float &Qh, bool &far)
+{
+    const float xl = (cc - (s0 - 0.5f)) * rs, xh = ((s0 + len - 0.5f) - cc) * rs;
+    Ql = 0.3989422804f * ex2f(-0.7213475f * xl * xl) * rcpf(xl + rcpf(xl + 2.0f * rcpf(xl + 3.0f * rcpf(xl + 4.0f * rcpf(xl)))));
+    Qh = 0.3989422804f * ex2f(-0.7213475f * xh * xh) * rcpf(xh + rcpf(xh + 2.0f * rcpf(xh + 3.0f * rcpf(xh + 4.0f * rcpf(xh)))));
+    far = xl >= 3.0f && xh >= 3.0f;
+}
+
 // Split of the transitions: warp W of the CTA owns transitions TB .. TB + NW - 1; lane `half` (0 / 1) of a record's lane
 // pair prepares NHW of them, from T0(half).
 template <int NT, int W>
@@ -252,23 +273,19 @@ __device__ __forceinline__ unsigned prepare_record(const Sim3D &P, uint2 rec, co
     }
     nact = 0;
     if (O::HEAD && half == 0) {
-        float q0 = -INFINITY, q1 = 0.f, q2 = 0.f, cc = 0.f;  // phi = 2^(-inf) = 0 for records that are not steps
+        float q0 = -INFINITY, q1 = 0.f, q2 = 0.f, cc = 0.f, ql = 0.f, qh = 0.f, qe = -1.f;  // phi = 2^(-inf) = 0 for records that are not steps
         unsigned wb = 0u;
         if (step) {
             const float v0 = -(k.x * dir.x + k.y * dir.y + k.z * dir.z);  // DESIGN R6
             const float inv_dv = rcpf(P.dv);
             cc = fmaf(v0, inv_dv, 0.5f * (float)(P.nch - 1));  // line centre in channel units
             const float sigch = k.w * inv_dv;
-            // the span: 32 channels from a multiple of 4, centred on the line, inside the band; it serves the step if it
-            // reaches LOC_XCLIP sigma to both sides of the line centre (the nominal window of DESIGN 5.3 may be wider for
-            // a thick line and is then cut there); otherwise the step takes the masked path with its exact window
+            // the span: 32 channels from a multiple of 4, centred on the line, inside the band (whether it serves the
+            // step is decided by step_mode, once the optical depths of all transitions are known)
             const int wbmax = (P.nch - LOC_SPAN) & ~3;
             int iwb = 4 * (int)rintf((cc - 15.5f) * 0.25f);
             iwb = max(0, min(iwb, wbmax));
-            const float lim = LOC_XCLIP * sigch;
-            const bool fast = P.nch >= LOC_SPAN && cc - (float)iwb >= lim && (float)(iwb + LOC_SPAN - 1) - cc >= lim;
             if (P.nch < LOC_SPAN) iwb = 0;
-            if (!fast) flags |= LOC_RS_SLOW;
             // log2 phi(channel wb + 16 + j) = lamp - (A + j ky)^2 with A = (wb + 16 - cc) ky: the quadratic in j is
             // expanded around the middle of the span, where |A| is a few channels only
             const float ky = 0.8493218f * rcpf(sigch);  // sqrt(log2(e) / 2) in channel units
@@ -277,22 +294,36 @@ __device__ __forceinline__ unsigned prepare_record(const Sim3D &P, uint2 rec, co
             q1 = -2.0f * A * ky;
             q2 = -ky * ky;
             wb = (unsigned)iwb;
+            // qe = profile mass outside the span (-1: the round takes 1 - sum phi); ql, qh feed the wing correction
+            // (header comment) and vanish at the edges of the band, where no channels follow
+            {
+                float Ql, Qh;
+                bool far;
+                wing_mass(cc, rcpf(sigch), (float)iwb, (float)LOC_SPAN, Ql, Qh, far);
+                qe = far ? Ql + Qh : -1.0f;
+                ql = (iwb == 0 || !far) ? 0.0f : Ql;
+                qh = (iwb + LOC_SPAN >= P.nch || !far) ? 0.0f : Qh;
+            }
             if (P.geom) nact = max(0, min(P.nch - 1, (int)floorf(cc + 5.0f * sigch)) - max(0, (int)ceilf(cc - 5.0f * sigch)) + 1);
         }
         sts128u(rb, make_uint4(__float_as_uint(q0), __float_as_uint(q1), __float_as_uint(q2), wb | flags));
         const unsigned coff = step ? rec.x * (unsigned)P.nsp + (unsigned)P.slot0 : rec.x;
         sts128u(rb + 16, make_uint4(coff, __float_as_uint(w), rec.y, __float_as_uint(cc)));
+        sts128(rb + L::QW, make_float4(ql, qh, qe, 0.f));
     }
     // per transition, branch free: the exponential form from tau0 >= LOC_EXP_TAU (header comment); records that are not
     // steps have kappa = eps = s = w = 0 and get all-zero coefficients
     const float wos = w * rcpf(s);  // not used when s = 0
+    float tm = 0.f;
 #pragma unroll
     for (int i = 0; i < O::NHW; i++) {
         if (half * O::NHW + i < O::NW) {
             const int t = O::TB + half * O::NHW + i;
             const float2 ke = step ? C.cf[i] : make_float2(0.f, 0.f);
             const float ks = ke.x * s;
-            const bool thick = fabsf(ks) * amp >= LOC_EXP_TAU;
+            const float tau0 = fabsf(ks) * amp;
+            tm = fmaxf(tm, tau0);
+            const bool thick = tau0 >= LOC_EXP_TAU;
             const float rk = rcpf(ke.x);
             float4 tp;
             tp.x = thick ? 0.0f : ks;
@@ -302,6 +333,53 @@ __device__ __forceinline__ unsigned prepare_record(const Sim3D &P, uint2 rec, co
             sts128(rb + L::TP + 16 * t, tp);
             sts32(rb + L::UO + 4 * t, thick ? 0.0f : 1.0f);
             sts32(rb + L::SC + 4 * t, thick ? wos * rk : w);  // the sums of the exponential form carry a factor kappa s
+        }
+    }
+    sts32(rb + L::TM + 4 * (2 * W + half), tm);
+    return flags;
+}
+
+// first channel of the pair of spans (64 channels from a multiple of 4, centred on the line, inside the band) of a WIDE step
+__device__ __forceinline__ int wide_start(int nch, float cc)
+{
+    const int wmax = (nch - 2 * LOC_SPAN) & ~3;
+    return max(0, min(4 * (int)rintf((cc - 31.5f) * 0.25f), wmax));
+}
+
+// Mode of a ray step, formed by one lane per record after the prepare phase of both warps (the largest line-centre
+// optical depth tau0m of ALL transitions is needed): the profile must be carried out to X sigma with
+// X^2 = LOC_XCLIP^2 + 2 ln max(1, tau0m), so that the mass left outside stays the same fraction of the step's escape
+// sum  sum phi f(tau) ~ 1 / tau0  as LOC_XCLIP sigma for a thin line (DESIGN 5.3).  If the centred 32-channel span reaches
+// that far on both sides (or to the edge of the band) the step is a common round; else, if two adjacent spans do, a WIDE
+// round (two passes); else a masked round over its exact window.  Returns the record's flags with the mode bits.
+template <int NT>
+__device__ __forceinline__ unsigned step_mode(const Sim3D &P, unsigned rb, float &qe_wide)
+{
+    qe_wide = -1.0f;  // profile mass outside the pair of spans of a WIDE step (-1: the round takes 1 - sum phi)
+    typedef Lay<NT> L;
+    const float4 h0 = lds128(rb);
+    const unsigned wbop = __float_as_uint(h0.w);
+    unsigned flags = wbop & (LOC_RS_STEP | LOC_RS_CTRL);
+    if (wbop & LOC_RS_STEP) {
+        const float4 tm = lds128(rb + L::TM);
+        const float cc = lds32(rb + 28);
+        const float tau0m = fmaxf(fmaxf(tm.x, tm.y), fmaxf(tm.z, tm.w));
+        float X2 = P.xclip * P.xclip;
+        if (tau0m > 1.0f) X2 = fmaf(1.3862944f, __log2f(tau0m), X2);  // 2 ln tau0m
+        float need;  // X sigma in channels = sqrt(X2) * 0.8493218 / sqrt(-q2)
+        asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(need) : "f"(X2 * 0.7213475f * rcpf(-h0.z)));
+        const int wb = (int)(wbop & LOC_WB_MASK);
+        const bool ok1 = P.nch >= LOC_SPAN && (wb == 0 || cc - (float)wb >= need) && (wb + LOC_SPAN >= P.nch || (float)(wb + LOC_SPAN - 1) - cc >= need);
+        if (!ok1) {
+            const int ww = wide_start(P.nch, cc);
+            const bool ok2 = P.nch >= 2 * LOC_SPAN && (ww == 0 || cc - (float)ww >= need) && (ww + 2 * LOC_SPAN >= P.nch || (float)(ww + 2 * LOC_SPAN - 1) - cc >= need);
+            flags |= ok2 ? LOC_RS_WIDE : LOC_RS_SLOW;
+            if (ok2) {
+                float Ql, Qh;
+                bool far;
+                wing_mass(cc, 1.1774100f * sqrtf(-h0.z), (float)ww, (float)(2 * LOC_SPAN), Ql, Qh, far);
+                if (far) qe_wide = Ql + Qh;
+            }
         }
     }
     return flags;
@@ -325,15 +403,8 @@ __device__ __forceinline__ float slow_round(const Sim3D &P, unsigned rb, unsigne
     if (wbop & LOC_RS_STEP) {
         const float ky = sqrtf(-h0.z);
         const float sigch = 0.8493218f * rcpf(ky);
-        const float A = -0.5f * h0.y * rcpf(ky);
-        const float amp = ex2f(fmaf(A, A, h0.x));
-        float km = 0.f;  // largest |kappa s| of the step
-#pragma unroll 1
-        for (int t = 0; t < NT; t++) {
-            const float4 tp = lds128(rb + L::TP + 16 * t);
-            km = fmaxf(km, fmaxf(fabsf(tp.x), fabsf(tp.y) * 0.6931472f));
-        }
-        const float tau0m = km * amp;
+        const float4 tm = lds128(rb + L::TM);
+        const float tau0m = fmaxf(fmaxf(tm.x, tm.y), fmaxf(tm.z, tm.w));
         float X = P.xmin;
         if (tau0m > 1.0f) X = sqrtf(fmaf(2.0f, __logf(tau0m), X * X));
         const float cc = __uint_as_float(h1.w), hw = X * sigch;
@@ -387,8 +458,12 @@ __device__ __forceinline__ float slow_round(const Sim3D &P, unsigned rb, unsigne
 // The common round: one pass over the span for the warp's NW transitions, straight-line code.  `sq` = shared address of
 // the lane's quad in transition 0, `rowb` = bytes between the spectra of consecutive transitions, `pl` = the lane's slot
 // in row 0 of the group's partial sums.  Returns the lane's sum of phi.
-template <int NT, int W>
-__device__ __forceinline__ float fast_round(unsigned rb, unsigned sq, int rowb, unsigned pl, const float4 h0, const f32x2 J01, const f32x2 J23)
+// ACC: second pass of a WIDE round, the partial sums are added to those of the first pass.
+// el, eh: wing correction of the lane (profile mass below / above the span for the lanes that own its first / last
+// channel, else 0): the incoming photons of the edge channel stand for those of the wing beyond it.
+template <int NT, int W, bool ACC>
+__device__ __forceinline__ float fast_round(unsigned rb, unsigned sq, int rowb, unsigned pl, const float4 h0, const f32x2 J01, const f32x2 J23, float el,
+                                            float eh)
 {
     typedef Lay<NT> L;
     typedef Own<NT, W> O;
@@ -431,7 +506,13 @@ __device__ __forceinline__ float fast_round(unsigned rb, unsigned sq, int rowb, 
         float a0, a1, b0, b1;
         upk2(fma2(N01, X01, mul2(N23, X23)), a0, a1);
         upk2(add2(X01, X23), b0, b1);
-        ab[i] = make_float2(a0 + a1, b0 + b1);
+        // wing term in the units of the sum: phi n for the series, kappa s phi n for the exponential form (Ce = -kappa s log2 e)
+        ab[i] = make_float2(fmaf(fmaf(-0.6931472f, tp[i].y, Uv[i]), fmaf(el, n4[i].x, eh * n4[i].w), a0 + a1), b0 + b1);
+        if (ACC) {
+            const float2 pv = lds64(pl + (O::TB + i) * L::ROWB);
+            ab[i].x += pv.x;
+            ab[i].y += pv.y;
+        }
         upk2(fma2(X01, fma2(AL, N01, C1), N01), n4[i].x, n4[i].y);
         upk2(fma2(X23, fma2(AL, N23, C1), N23), n4[i].z, n4[i].w);
     }
@@ -520,23 +601,24 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
         // ---- prepare: lane pair rj of each group decodes record off + rj of its ray ----
         int nact;
         unsigned flags = prepare_record<NT, W>(P, r0, cell, dir, rec_g + rj * L::RECB, half, nact);
-        if (O::HEAD) {
-            if (half == 0) {
-                mysteps += flags >> 31;
-                myactive += nact;
-            }
-            // class of round rj: OR of the record flags over the four groups
-            flags |= __shfl_xor_sync(0xffffffffu, flags, 8);
-            flags |= __shfl_xor_sync(0xffffffffu, flags, 16);
-            if (lane == 2 * rj) sts32u(tb + L::OFF_CLS + 4 * rj, flags);
+        if (O::HEAD && half == 0) {
+            mysteps += flags >> 31;
+            myactive += nact;
         }
         load_cell<NT, W>(P, r1, half, cell);  // for the next chunk (NOP records load nothing)
         cta_sync();  // the records of the chunk are complete
+        // mode of record rj (the lanes of a pair agree), then the class of round rj: OR over the four groups
+        float myqew;
+        const unsigned myflags = step_mode<NT>(P, rec_g + rj * L::RECB, myqew);
+        unsigned orflags = myflags | __shfl_xor_sync(0xffffffffu, myflags, 8);
+        orflags |= __shfl_xor_sync(0xffffffffu, orflags, 16);
 
         // ---- LOC_CHUNK rounds: every group consumes one record per round ----
 #pragma unroll 1
         for (int r = 0; r < LOC_CHUNK; r++) {
-            const unsigned cls = lds32u(tb + L::OFF_CLS + 4 * r);
+            const unsigned cls = __shfl_sync(0xffffffffu, orflags, 2 * r);
+            const unsigned mode = __shfl_sync(0xffffffffu, myflags, 8 * grp + 2 * r);
+            const float qew = __shfl_sync(0xffffffffu, myqew, 8 * grp + 2 * r);
             const unsigned rb = rec_g + r * L::RECB;
             if (cls & LOC_RS_CTRL) {
                 // spectrum operations on the warp's own rows, executed by the whole warp for one group at a time
@@ -571,11 +653,27 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
             if (!(cls & LOC_RS_STEP)) continue;
             const float4 h0 = lds128(rb);
             const unsigned wbop = __float_as_uint(h0.w);
+            const float4 qw = lds128(rb + L::QW);
+            const float el = l8 == 0 ? qw.x : 0.0f, eh = l8 == 7 ? qw.y : 0.0f;
             float sphi;
-            if (!(cls & LOC_RS_SLOW))
-                sphi = fast_round<NT, W>(rb, sq_g + 4u * (wbop & LOC_WB_MASK), rowb, pl, h0, J01, J23);
-            else
+            if (cls & LOC_RS_SLOW) {
                 sphi = slow_round<NT, W>(P, rb, sq_g, pl, l8, nchp);
+            } else if (!(cls & LOC_RS_WIDE)) {
+                sphi = fast_round<NT, W, false>(rb, sq_g + 4u * (wbop & LOC_WB_MASK), rowb, pl, h0, J01, J23, el, eh);
+            } else {
+                // two passes: a WIDE ray over its pair of spans, the other rays over their span and then over nothing
+                const bool wide = mode & LOC_RS_WIDE;
+                const int wb = (int)(wbop & LOC_WB_MASK);
+                const int w1 = wide ? wide_start(P.nch, lds32(rb + 28)) : wb;
+                const float d1 = (float)(w1 - wb), d2 = d1 + (float)LOC_SPAN;
+                float4 ha = h0, hb = h0;  // the profile's quadratic, re-centred on the spans that start at w1 and w1 + 32
+                ha.x = fmaf(d1, fmaf(d1, h0.z, h0.y), h0.x);
+                ha.y = fmaf(2.0f * d1, h0.z, h0.y);
+                hb.x = wide ? fmaf(d2, fmaf(d2, h0.z, h0.y), h0.x) : -INFINITY;
+                hb.y = fmaf(2.0f * d2, h0.z, h0.y);
+                sphi = fast_round<NT, W, false>(rb, sq_g + 4u * w1, rowb, pl, ha, J01, J23, wide ? 0.0f : el, wide ? 0.0f : eh);
+                sphi += fast_round<NT, W, true>(rb, sq_g + 4u * (wide ? w1 + LOC_SPAN : w1), rowb, pl, hb, J01, J23, 0.0f, 0.0f);
+            }
             sts32(phi_g + 4 * l8, sphi);
             __syncwarp();
             // ---- reduction over the 8 lanes of each group: lane i adds up the row of the warp's i-th transition and
@@ -589,7 +687,12 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
                 float fa, fb;
                 upk2(add2(add2(pk2(f0.x, f0.y), pk2(f0.z, f0.w)), add2(pk2(f1.x, f1.y), pk2(f1.z, f1.w))), fa, fb);
                 const float w = __uint_as_float(h1.y);
-                const float wesc = fmaf(-w, fa + fb, w);  // photons emitted outside the updated channels escape (DESIGN 5.3)
+                // photons emitted outside the updated channels escape (DESIGN 5.3): analytic mass of the wings for a common
+                // round, 1 - sum phi otherwise
+                float qe = qw.z;
+                if (cls & LOC_RS_SLOW) qe = -1.0f;
+                else if (mode & LOC_RS_WIDE) qe = qew;
+                const float wesc = qe < 0.0f ? fmaf(-w, fa + fb, w) : w * qe;
                 const f32x2 s01 = add2(add2(pk2(a0.x, a0.y), pk2(a0.z, a0.w)), add2(pk2(a1.x, a1.y), pk2(a1.z, a1.w)));
                 const f32x2 s23 = add2(add2(pk2(a2.x, a2.y), pk2(a2.z, a2.w)), add2(pk2(a3.x, a3.y), pk2(a3.z, a3.w)));
                 float A, B;
@@ -674,7 +777,7 @@ int loc_launch_sim3d(loc_model *m, int geom)
     P.nslot = std::max(m->nlev - 1, 1);
     P.dv = (float)m->dv;
     P.xmin = m->xmin;
-    P.eps_tau = m->eps_tau;
+    P.xclip = getenv("LOC_XCLIP") ? (float)atof(getenv("LOC_XCLIP")) : LOC_XCLIP;
     P.inv_ndir = 1.0f / (float)m->ndir;
     P.dirs = m->d_dirs;
     P.task_dir = m->d_task_dir;

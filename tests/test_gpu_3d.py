@@ -17,9 +17,11 @@ def _model(m, **kw):
     return LocModel(m, **kw)
 
 
-def small(which=4, nroot=4, nlev=3, nch=32, nside=1, frac=0.35, nls=4, seed=None):
-    return W.cloud_config(which, nroot=nroot, nlev=nlev, nchannel=nch, nside=nside, refine_frac=frac,
-                          nlevel_species=nls, seed_config=seed)
+def small(which=4, nroot=4, nlev=3, nch=32, nside=1, frac=0.35, nls=4, seed=None, dens=1.0):
+    m = W.cloud_config(which, nroot=nroot, nlev=nlev, nchannel=nch, nside=nside, refine_frac=frac,
+                       nlevel_species=nls, seed_config=seed)
+    m.density *= np.float32(dens)  # dens > 1: optically thick cells (line-centre optical depths of a step up to ~1e3)
+    return m
 
 
 GEOM_CASES = [dict(nroot=4, nlev=1, nside=2), dict(nroot=4, nlev=2, nside=2, frac=0.4), dict(nroot=4, nlev=3, nside=2),
@@ -63,7 +65,12 @@ def test_geometry_per_direction():
 RAD_CASES = [dict(nroot=6, nlev=1, nside=1, nch=48), dict(nroot=4, nlev=3, nside=1, nch=40, frac=0.4),
              dict(nroot=4, nlev=3, nside=2, nch=32, frac=0.5, seed=9), dict(which=5, nroot=4, nlev=2, nside=1, nch=64, frac=0.4, nls=10),
              # 3 of 9 transitions traced on a grid large enough that a record stride of 9 would leave the 3-transition workspace
-             dict(which=5, nroot=10, nlev=2, nside=1, nch=64, frac=0.3, nls=10)]
+             dict(which=5, nroot=10, nlev=2, nside=1, nch=64, frac=0.3, nls=10),
+             # the channel width of C3 / C4 (sigma = 3.3 channels: the 32-channel span is tight) with thin and with very
+             # thick cells: common, two-span and masked rounds, series and exponential forms in one warp
+             dict(which=3, nroot=12, nlev=1, nside=1, nch=128, frac=0.0, nls=10),
+             dict(which=3, nroot=12, nlev=1, nside=1, nch=128, frac=0.0, nls=10, dens=30.0),
+             dict(which=4, nroot=6, nlev=3, nside=1, nch=128, frac=0.5, nls=6, dens=100.0)]
 
 
 @pytest.mark.parametrize("cfg", RAD_CASES)
