@@ -148,7 +148,7 @@ __device__ __forceinline__ float ex2f(float x)
 }
 
 // Packed float32 pairs (sm_100a `*.f32x2`): one instruction updates two channels.  On B200 an FFMA2 holds the FMA pipe
-// for two cycles like two FFMA, but takes ONE issue slot (measured, profiles/r1_pipe_microbench.md) -- the 3D kernel is
+// for two cycles like two FFMA, but takes ONE issue slot (measured: profiles/r1_pipe_microbench.md) -- the 3D kernel is
 // issue bound, so the bulk per-channel arithmetic is written in pairs.
 typedef unsigned long long f32x2;
 __device__ __forceinline__ f32x2 pk2(float lo, float hi)
