@@ -196,11 +196,14 @@ __global__ void __launch_bounds__(128) k_solve(int64_t n, SpeciesDev sp, Selecti
                 f = (T - sp.temps[j]) / (sp.temps[j + 1] - sp.temps[j]);
             }
         }
+        // Boltzmann factors g_k exp(-(E_k - E_0) / T) once per level (one exp per level instead of one per collisional pair)
+        double bz[NLMAX];
+        for (int k = 0; k < NL; k++) bz[k] = sp.g[k] * exp(-(sp.energy_K[k] - sp.energy_K[0]) / T);
         for (int k = 0; k < sp.ncoll; k++) {
             int u = sp.cu[k], l = sp.cl[k];
             double gd = sp.rates[(int64_t)j * sp.ncoll + k];
             if (sp.ntemp > 1) gd = (1.0 - f) * gd + f * sp.rates[(int64_t)(j + 1) * sp.ncoll + k];
-            double gu = gd * sp.g[u] / sp.g[l] * exp(-(sp.energy_K[u] - sp.energy_K[l]) / T);
+            double gu = gd * bz[u] / bz[l];
             R[u * NL + l] += dens * gd;
             R[l * NL + u] += dens * gu;
         }
