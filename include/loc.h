@@ -161,6 +161,20 @@ int loc_solve(loc_model *m, double *max_rel_change);
 /* niter x (loc_simulate with the remembered selection; loc_solve); no early exit.          */
 int loc_iterate(loc_model *m, int niter, double *max_rel_change);
 
+/* ali = 1 (default): accelerated lambda iteration -- loc_solve scales A_ul by the escape probability ESC and uses the
+ * radiation field of the other cells only.  ali = 0: plain lambda iteration ("it is also possible to run
+ * LOC without ALI"): A_ul unscaled, and the self term of Eq. 2 is kept, i.e. the photons a
+ * cell absorbs from its own emission, (1 - ESC) times the source function of the populations the rays were traced
+ * with, are added to SJ.  Both modes share loc_simulate and its counters and have the same fixed point; only
+ * loc_solve differs.  Returns LOC_EINVAL for any other value.                                                */
+int loc_set_ali(loc_model *m, int ali);
+
+/* Convergence-controlled iteration ("repeated until the level populations converge"):
+ * (loc_simulate; loc_solve) until max_rel_change <= tol or max_iter iterations were done.  niter_done (host, may be
+ * NULL) receives the number of iterations run, max_rel_change (host, may be NULL) the change of the last one.
+ * Synchronises the stream once per iteration.  max_iter = 0 runs nothing and reports a change of 0.          */
+int loc_iterate_until(loc_model *m, int max_iter, double tol, int *niter_done, double *max_rel_change);
+
 /* Spectral map: for each pixel one line of sight through the model with the current
  * populations, T_A(c) = (c^2 / 2 k nu^2)(I_c - B_nu(T_bg)), written to dev_out float [ny][nx][nchannel] (K).
  * Octree: lines of sight run along `dir` (host double[3]); pixel (ix,iy) starts on the upstream face at the

@@ -18,7 +18,8 @@ LOC_OK, LOC_EINVAL, LOC_ESTATE, LOC_ENOMEM, LOC_ECUDA = 0, -1, -2, -3, -4
 LOC_GRID_SHELL, LOC_GRID_OCTREE = 1, 2
 
 SYMBOLS = ("loc_workspace_bytes", "loc_create_model", "loc_set_species", "loc_refresh_cells", "loc_set_directions", "loc_set_populations",
-           "loc_init_lte", "loc_simulate", "loc_get_counters", "loc_solve", "loc_iterate", "loc_spectra",
+           "loc_init_lte", "loc_simulate", "loc_get_counters", "loc_solve", "loc_iterate", "loc_set_ali",
+           "loc_iterate_until", "loc_spectra",
            "loc_get_stats", "loc_destroy_model", "loc_last_error")
 
 
@@ -77,6 +78,8 @@ def lib():
                                        C.POINTER(C.c_void_p)]
         L.loc_solve.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.loc_iterate.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double)]
+        L.loc_set_ali.argtypes = [C.c_void_p, C.c_int]
+        L.loc_iterate_until.argtypes = [C.c_void_p, C.c_int, C.c_double, C.POINTER(C.c_int), C.POINTER(C.c_double)]
         L.loc_spectra.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
         L.loc_get_stats.argtypes = [C.c_void_p, C.POINTER(loc_stats)]
         L.loc_destroy_model.argtypes = [C.c_void_p]
@@ -193,6 +196,17 @@ def loc_iterate(h, niter: int) -> float:
     r = C.c_double(0.0)
     _check(lib().loc_iterate(h, int(niter), C.byref(r)), h)
     return r.value
+
+
+def loc_set_ali(h, ali: bool) -> None:
+    _check(lib().loc_set_ali(h, int(bool(ali))), h)
+
+
+def loc_iterate_until(h, max_iter: int, tol: float):
+    """returns (iterations run, max relative change of the last one)"""
+    r, n = C.c_double(0.0), C.c_int(0)
+    _check(lib().loc_iterate_until(h, int(max_iter), float(tol), C.byref(n), C.byref(r)), h)
+    return n.value, r.value
 
 
 def loc_spectra(h, trans, dev_out, nx, ny=1, dir=None, aff=None, offsets_cm=None):

@@ -154,7 +154,7 @@ __global__ void k_coef(int64_t n, Selection S, const float *pops, float2 *coef)
 template <int NLMAX>
 __global__ void __launch_bounds__(128) k_solve(int64_t n, SpeciesDev sp, Selection S, const float *density, const float *tkin,
                                                const float *abundance, const float2 *cnt, float *pops, float2 *coef,
-                                               unsigned int *maxrel_bits, const int32_t *child)
+                                               unsigned int *maxrel_bits, const int32_t *child, int ali)
 {
     int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     bool act = i < n;
@@ -176,6 +176,15 @@ __global__ void __launch_bounds__(128) k_solve(int64_t n, SpeciesDev sp, Selecti
                     float2 c = cnt[i * S.nsp + k];
                     sj = c.x;
                     esc = c.y;
+                    if (!ali) {
+                        // plain lambda iteration ("possible to run LOC without ALI"): the self term of
+                        // Eq. 2 goes back into the radiation field and A_ul stays unscaled.  Step by step it equals
+                        // (1 - ESC) times the source function of the populations the rays were traced with, whose
+                        // occupation number is em / kap of the cell's coefficient record (DESIGN 5.2, 6.2)
+                        float2 ke = coef[i * S.nsp + k];
+                        if (ke.x != 0.0f) sj += (1.0 - esc) * ((double)ke.y / (double)ke.x);
+                        esc = 1.0;
+                    }
                 }
             double Slu = gr * sp.A[t] * sj;  // = B_lu * Jbar
             R[u * NL + l] += sp.A[t] * esc + Slu / gr;
@@ -352,6 +361,7 @@ extern "C" int loc_create_model(const loc_grid *g, const loc_cells *cells, int n
     m->tbg = tbg;
     m->cells = *cells;
     m->xmin = 4.5f;
+    m->ali = 1;
     m->eps_tau = 1e-6f;
     if (getenv("LOC_XMIN")) m->xmin = (float)atof(getenv("LOC_XMIN"));
     if (getenv("LOC_EPS_TAU")) m->eps_tau = (float)atof(getenv("LOC_EPS_TAU"));
@@ -628,7 +638,7 @@ static int solve_async(loc_model *m)
     unsigned nb = (unsigned)((n + 127) / 128);
 #define LOC_SOLVE(NLMAX)                                                                                                     \
     k_solve<NLMAX><<<nb, 128, 0, m->stream>>>(n, m->sp, m->selh, m->cells.density, m->cells.tkin, m->cells.abundance, m->cnt, \
-                                              m->pops, m->coef, m->d_maxrel, ch)
+                                              m->pops, m->coef, m->d_maxrel, ch, m->ali)
     if (m->nlevel <= 6) LOC_SOLVE(6);
     else if (m->nlevel <= 10) LOC_SOLVE(10);
     else if (m->nlevel <= 16) LOC_SOLVE(16);
@@ -674,6 +684,34 @@ extern "C" int loc_iterate(loc_model *m, int niter, double *max_rel_change)
         if (rc) return rc;
     }
     return fetch_maxrel(m, max_rel_change);
+}
+
+extern "C" int loc_set_ali(loc_model *m, int ali)
+{
+    if (!m || (ali != 0 && ali != 1)) return LOC_EINVAL;
+    m->ali = ali;
+    return LOC_OK;
+}
+
+extern "C" int loc_iterate_until(loc_model *m, int max_iter, double tol, int *niter_done, double *max_rel_change)
+{
+    if (!m || max_iter < 0 || !(tol >= 0.0)) return LOC_EINVAL;
+    double ch = 0.0;
+    int it = 0;
+    while (it < max_iter) {
+        int rc = loc_simulate(m, 0, nullptr, 0);
+        if (rc) return rc;
+        LOC_CUDA_CHECK(m, cudaMemsetAsync(m->d_maxrel, 0, sizeof(unsigned int), m->stream));
+        rc = solve_async(m);
+        if (rc) return rc;
+        rc = fetch_maxrel(m, &ch);  // one host synchronisation per iteration: the stopping rule needs the scalar
+        if (rc) return rc;
+        it++;
+        if (ch <= tol) break;
+    }
+    if (niter_done) *niter_done = it;
+    if (max_rel_change) *max_rel_change = ch;
+    return LOC_OK;
 }
 
 extern "C" int loc_spectra(loc_model *m, int trans, const double *dir, int nx, int ny, const int64_t *aff, const double *offsets_cm,

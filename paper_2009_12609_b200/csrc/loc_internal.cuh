@@ -100,6 +100,7 @@ struct loc_model {
     double *h_A, *h_freq;
     Selection selh;
     bool coef_valid;
+    int ali;  // 1: accelerated lambda iteration (default), 0: plain lambda iteration (loc_set_ali)
     float *pops;  // registered [nlevel][ncell]
     // accuracy knobs (DESIGN 5.3)
     float xmin, eps_tau;

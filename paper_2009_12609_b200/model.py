@@ -95,6 +95,13 @@ class LocModel:
     def iterate(self, niter) -> float:
         return B.loc_iterate(self.h, niter)
 
+    def set_ali(self, ali: bool) -> None:
+        B.loc_set_ali(self.h, ali)
+
+    def iterate_until(self, max_iter, tol):
+        """(iterations run, last max relative change)"""
+        return B.loc_iterate_until(self.h, max_iter, tol)
+
     def stats(self) -> dict:
         return B.loc_get_stats(self.h)
 
