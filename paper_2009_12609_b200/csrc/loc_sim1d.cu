@@ -9,6 +9,7 @@
 // step, and one float atomic per (cell, transition, counter).  The paper's kernel used one work item per ray
 // and one transition at a time.
 #include <stdio.h>
+#include <stdlib.h>
 
 #include "loc_internal.cuh"
 
@@ -150,9 +151,150 @@ __global__ void __launch_bounds__(1024) k_sim1d(Sim1D P)
     }
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// k_sim1d_w: one WARP per ray (profiles/r1_sim1d_C2.md: the block-per-ray kernel above is issue bound at 2600 warp
+// instructions per ray step, most of them per-step scalar work repeated by every warp of the block and the two-stage
+// reduction).  The ray's spectra [NT][nchp] live in shared memory; per step the lanes cover the profile window in
+// aligned quads of channels (one 128-bit shared-memory access per lane and transition, conflict free), sum their
+// channels in registers, and ONE halving-butterfly reduction per step leaves each of the 2 NT + 1 totals in one lane,
+// which issues the counter's atomic itself: no block barrier, no second reduction stage.  The step's table entries, cell
+// kinematics and line coefficients are loaded one step ahead.  Same per-channel arithmetic (channel_update), same
+// window rule and wing term as k_sim1d.
+// ------------------------------------------------------------------------------------------------------------------
+#define LOC_1D_WARPS 2  // rays per block
+
+struct Step1D {
+    int k;
+    float s, mu, w;
+    float4 kin;
+    float2 ke;  // lanes < NT: (kap, em) of transition `lane`
+};
+
+template <int NT>
+__device__ __forceinline__ void load_step1d(const Sim1D &P, int j, int nin, int k0, long long off, int lane, Step1D &S)
+{
+    seg1d(P, j, nin, k0, off, S.k, S.s, S.mu, S.w);
+    S.kin = __ldg(P.kin + S.k);
+    if (lane < NT) S.ke = __ldg(P.coef + (long long)S.k * P.nsp + lane);
+}
+
+template <int NT, bool GEOM>
+__global__ void __launch_bounds__(LOC_1D_WARPS * 32) k_sim1d_w(Sim1D P, int nray)
+{
+    constexpr int NV = 2 * NT + 1;
+    extern __shared__ __align__(16) float s_w[];  // per warp: [NT][nchp] spectra, then NT TParam
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int slot = blockIdx.x * LOC_1D_WARPS + warp;
+    if (slot >= nray) return;  // the warps of a block never synchronise with each other
+    const int nchp = (P.nch + 3) & ~3;
+    float *sn = s_w + warp * (NT * nchp + 4 * NT);
+    TParam *stp = reinterpret_cast<TParam *>(sn + NT * nchp);
+    const int ray = P.order[slot];
+    const int k0 = P.k0[ray];
+    const long long off = P.off[ray];
+    const int nin = P.ns - 1 - k0, nseg = 2 * nin + 1;
+#pragma unroll
+    for (int t = 0; t < NT; t++) {
+        const float bg = P.S.bgocc[t];  // Eq. 1: background photons, as occupation number
+        for (int c = lane; c < nchp; c += 32) sn[t * nchp + c] = bg;
+    }
+    const float inv_dv = 1.0f / P.dv, chalf = 0.5f * (float)(P.nch - 1);
+    unsigned long long nact = 0;
+    Step1D cur, nxt;
+    cur.ke = nxt.ke = make_float2(0.f, 0.f);
+    load_step1d<NT>(P, 0, nin, k0, off, lane, cur);
+
+    for (int j = 0; j < nseg; j++) {
+        nxt = cur;
+        if (j + 1 < nseg) load_step1d<NT>(P, j + 1, nin, k0, off, lane, nxt);  // used one iteration later
+        const float s = cur.s, w = cur.w, sig = cur.kin.w;
+        const float v0 = -cur.kin.x * cur.mu;  // DESIGN R6, mu at the entry of the step
+        const float amp = P.dv * 0.3989422804f / sig;
+        __syncwarp();  // the previous step's reads of stp and writes of the spectra are done
+        float tau0 = 0.f;
+        if (lane < NT) {
+            stp[lane] = make_tparam(cur.ke, s, w, amp);
+            tau0 = fabsf(cur.ke.x * s) * amp;
+        }
+        const float tau0m = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(tau0)));
+        __syncwarp();
+        // ---- profile window of this step (DESIGN 5.3) ----
+        float X = P.xmin;
+        if (tau0m > P.eps_tau) X = fmaxf(X, sqrtf(2.0f * __logf(tau0m / P.eps_tau)));
+        const float cc = v0 * inv_dv + chalf;
+        const float hw = X * sig * inv_dv;
+        const int c_lo = max(0, (int)ceilf(cc - hw)), c_hi = min(P.nch - 1, (int)floorf(cc + hw));
+        if (GEOM) {
+            const float h5 = 5.0f * sig * inv_dv;
+            nact += (unsigned long long)max(0, min(P.nch - 1, (int)floorf(cc + h5)) - max(0, (int)ceilf(cc - h5)) + 1);
+        }
+        const float ky = 0.8493218f / sig;  // sqrt(log2(e)/2) / sigma
+        const float lamp = __log2f(amp);
+        float v[NV];
+#pragma unroll
+        for (int i = 0; i < NV; i++) v[i] = 0.f;
+        for (int cb = (c_lo & ~3) + 4 * lane; cb <= c_hi; cb += 128) {
+            float phi[4];
+#pragma unroll
+            for (int i = 0; i < 4; i++) {
+                const int c = cb + i;
+                const float y = (((float)c - chalf) * P.dv - v0) * ky;
+                phi[i] = (c >= c_lo && c <= c_hi) ? ex2f(fmaf(-y, y, lamp)) : 0.0f;
+            }
+            v[2 * NT] += (phi[0] + phi[1]) + (phi[2] + phi[3]);
+#pragma unroll
+            for (int t = 0; t < NT; t++) {
+                const TParam tp = stp[t];
+                float4 n4 = *reinterpret_cast<float4 *>(sn + t * nchp + cb);
+                float a = 0.f, b = 0.f;
+                channel_update(n4.x, phi[0], tp, a, b);
+                channel_update(n4.y, phi[1], tp, a, b);
+                channel_update(n4.z, phi[2], tp, a, b);
+                channel_update(n4.w, phi[3], tp, a, b);
+                *reinterpret_cast<float4 *>(sn + t * nchp + cb) = n4;
+                v[t] += a;
+                v[NT + t] += b;
+            }
+        }
+        int owner;
+        const float tot = warp_multi_reduce<NV>(v, lane, owner);
+        const unsigned mphi = __ballot_sync(0xffffffffu, owner == 2 * NT);
+        const float sphi = __shfl_sync(0xffffffffu, tot, __ffs(mphi) - 1);
+        if (owner >= 0 && owner < 2 * NT) {
+            const int t = owner < NT ? owner : owner - NT;
+            float2 *cn = P.cnt + (long long)cur.k * P.nsp + t;
+            float val = tot * stp[t].scale;
+            // photons emitted outside the window escape (DESIGN 5.3): w (1 - sum phi)
+            if (owner >= NT) val += fmaf(-w, sphi, w);
+            atomicAdd(owner < NT ? &cn->x : &cn->y, val);
+        }
+        if (GEOM && lane == 0) atomicAdd(&P.visits[cur.k], 1u);
+        cur = nxt;
+    }
+    if (GEOM && lane == 0 && nact) atomicAdd(P.nactive, nact);
+}
+
 template <int NT>
 static int launch1d(loc_model *m, const Sim1D &P, int geom)
 {
+    // warp-per-ray kernel while the spectra of a block's rays fit shared memory; LOC_SIM1D_BLOCK=1 forces the
+    // block-per-ray kernel (A/B measurements, very wide bands)
+    const int nchp = (m->nch + 3) & ~3;
+    const size_t smem_w = sizeof(float) * LOC_1D_WARPS * ((size_t)NT * nchp + 4 * NT);
+    const char *force = getenv("LOC_SIM1D_BLOCK");
+    if (smem_w <= 96 * 1024 && !(force && atoi(force))) {
+        const int blocks = (m->nray + LOC_1D_WARPS - 1) / LOC_1D_WARPS;
+        if (geom) {
+            LOC_CUDA_CHECK(m, cudaFuncSetAttribute(k_sim1d_w<NT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_w));
+            k_sim1d_w<NT, true><<<blocks, LOC_1D_WARPS * 32, smem_w, m->stream>>>(P, m->nray);
+        } else {
+            LOC_CUDA_CHECK(m, cudaFuncSetAttribute(k_sim1d_w<NT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_w));
+            k_sim1d_w<NT, false><<<blocks, LOC_1D_WARPS * 32, smem_w, m->stream>>>(P, m->nray);
+        }
+        m->launches++;
+        LOC_CUDA_CHECK(m, cudaGetLastError());
+        return LOC_OK;
+    }
     int threads = (m->nch + 31) / 32 * 32;
     int nwarp = threads / 32;
     size_t smem = sizeof(float) * 2 * (nwarp * (2 * NT + 1) + 4);
