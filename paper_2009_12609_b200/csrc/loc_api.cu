@@ -260,6 +260,166 @@ __global__ void __launch_bounds__(128) k_solve(int64_t n, SpeciesDev sp, Selecti
     if ((threadIdx.x & 31) == 0 && rel > 0.0f) atomicMax(maxrel_bits, __float_as_uint(rel));
 }
 
+// k_solve_s: the same equations and the same GTH elimination as k_solve, laid out for the SM instead of for the
+// compiler's local-memory stack (profiles/r1_solve.md: k_solve<10> keeps R in 960 B of local memory per thread, 1.1 MB per
+// SM at its occupancy -- the L1 hit rate is 60 % and 34 of 35 issue slots wait on the long scoreboard).  Here the rate
+// matrix of a thread is a column of a shared-memory array R[NL*NL][threads] of doubles (conflict free, never leaves the
+// SM), the species tables are staged in shared memory once per block, and NL is a compile-time constant for the common
+// level counts (NLX > 0), so that the elimination is fully unrolled with static addresses and x[], bz[] are registers.
+#define LOC_SOLVE_THREADS 64
+struct SolveTabs {   // byte offsets into the block's shared memory, after R
+    int g, energy, A, bg, upper, lower, cu, cl, temps, rates, bytes;
+};
+
+template <int NLX>
+__global__ void __launch_bounds__(LOC_SOLVE_THREADS) k_solve_s(int64_t n, SpeciesDev sp, Selection S, const float *density, const float *tkin,
+                                                               const float *abundance, const float2 *cnt, float *pops, float2 *coef,
+                                                               unsigned int *maxrel_bits, const int32_t *child, int ali, SolveTabs TB)
+{
+    constexpr int NLM = NLX > 0 ? NLX : 16;
+    extern __shared__ __align__(16) unsigned char s_raw[];
+    const int NL = NLX > 0 ? NLX : sp.nlevel;
+    const int tid = threadIdx.x;
+    double *Rs = reinterpret_cast<double *>(s_raw);
+    unsigned char *tb = s_raw + sizeof(double) * (NL * NL + NL) * LOC_SOLVE_THREADS;
+    double *t_g = reinterpret_cast<double *>(tb + TB.g), *t_e = reinterpret_cast<double *>(tb + TB.energy);
+    double *t_A = reinterpret_cast<double *>(tb + TB.A), *t_bg = reinterpret_cast<double *>(tb + TB.bg);
+    double *t_temps = reinterpret_cast<double *>(tb + TB.temps), *t_rates = reinterpret_cast<double *>(tb + TB.rates);
+    int *t_up = reinterpret_cast<int *>(tb + TB.upper), *t_lo = reinterpret_cast<int *>(tb + TB.lower);
+    int *t_cu = reinterpret_cast<int *>(tb + TB.cu), *t_cl = reinterpret_cast<int *>(tb + TB.cl);
+    for (int k = tid; k < NL; k += LOC_SOLVE_THREADS) {
+        t_g[k] = sp.g[k];
+        t_e[k] = sp.energy_K[k];
+    }
+    for (int k = tid; k < sp.ntrans; k += LOC_SOLVE_THREADS) {
+        t_A[k] = sp.A[k];
+        t_bg[k] = sp.bgocc[k];
+        t_up[k] = sp.upper[k];
+        t_lo[k] = sp.lower[k];
+    }
+    for (int k = tid; k < sp.ncoll; k += LOC_SOLVE_THREADS) {
+        t_cu[k] = sp.cu[k];
+        t_cl[k] = sp.cl[k];
+    }
+    for (int k = tid; k < sp.ntemp; k += LOC_SOLVE_THREADS) t_temps[k] = sp.temps[k];
+    for (int k = tid; k < sp.ntemp * sp.ncoll; k += LOC_SOLVE_THREADS) t_rates[k] = sp.rates[k];
+    __syncthreads();
+#define RM(a) Rs[(a) * LOC_SOLVE_THREADS + tid]
+#define VX(a) Rs[(NL * NL + (a)) * LOC_SOLVE_THREADS + tid]  // NL more doubles per thread: Boltzmann factors, then the solution
+    int64_t i = blockIdx.x * (int64_t)LOC_SOLVE_THREADS + tid;
+    bool act = i < n;
+    if (act && child && child[i] >= 0) act = false;  // refined cell: no gas of its own
+    float rel = 0.0f;
+    if (act) {
+#pragma unroll
+        for (int k = 0; k < NLM * NLM; k++)
+            if (k < NL * NL) RM(k) = 0.0;
+        const double dens = density[i], T = tkin[i];
+        const double ntot = dens * (double)abundance[i];
+        // radiative rates: traced transitions from their counters, the others see the background only (DESIGN R23)
+        for (int t = 0; t < sp.ntrans; t++) {
+            const int u = t_up[t], l = t_lo[t];
+            const double gr = t_g[u] / t_g[l];
+            double sj = t_bg[t], esc = 1.0;
+            for (int k = 0; k < S.nsel; k++)
+                if (S.sel[k] == t) {
+                    const float2 c = cnt[i * S.nsp + k];
+                    sj = c.x;
+                    esc = c.y;
+                    if (!ali) {  // plain lambda iteration: see k_solve
+                        const float2 ke = coef[i * S.nsp + k];
+                        if (ke.x != 0.0f) sj += (1.0 - esc) * ((double)ke.y / (double)ke.x);
+                        esc = 1.0;
+                    }
+                }
+            const double Slu = gr * t_A[t] * sj;  // = B_lu * Jbar
+            RM(u * NL + l) += t_A[t] * esc + Slu / gr;
+            RM(l * NL + u) += Slu;
+        }
+        // collisions: linear interpolation in T, clamped; upward by detailed balance
+        int j = 0;
+        double f = 0.0;
+        if (sp.ntemp > 1) {
+            if (T <= t_temps[0]) {
+                j = 0;
+                f = 0.0;
+            } else if (T >= t_temps[sp.ntemp - 1]) {
+                j = sp.ntemp - 2;
+                f = 1.0;
+            } else {
+                while (T > t_temps[j + 1]) j++;
+                f = (T - t_temps[j]) / (t_temps[j + 1] - t_temps[j]);
+            }
+        }
+        // g_k exp(-(E_k - E_0) / T), once per level
+        for (int k = 0; k < NL; k++) VX(k) = t_g[k] * exp(-(t_e[k] - t_e[0]) / T);
+        for (int k = 0; k < sp.ncoll; k++) {
+            const int u = t_cu[k], l = t_cl[k];
+            double gd = t_rates[j * sp.ncoll + k];
+            if (sp.ntemp > 1) gd = (1.0 - f) * gd + f * t_rates[(j + 1) * sp.ncoll + k];
+            RM(u * NL + l) += dens * gd;
+            RM(l * NL + u) += dens * (gd * VX(u) / VX(l));
+        }
+        // GTH elimination
+#pragma unroll
+        for (int q = NLM - 1; q >= 1; q--) {
+            if (q < NL) {
+                double sm = 0.0;
+#pragma unroll
+                for (int c = 0; c < q; c++) sm += RM(q * NL + c);
+                const double inv = sm > 0.0 ? 1.0 / sm : 0.0;
+#pragma unroll
+                for (int r = 0; r < q; r++) {
+                    const double rq = RM(r * NL + q) * inv;
+                    RM(r * NL + q) = rq;
+#pragma unroll
+                    for (int c = 0; c < q; c++)
+                        if (c != r) RM(r * NL + c) += rq * RM(q * NL + c);
+                }
+            }
+        }
+        double x[NLM];
+        x[0] = 1.0;
+        double tot = 1.0;
+#pragma unroll
+        for (int q = 1; q < NLM; q++) {
+            if (q < NL) {
+                double sm = 0.0;
+#pragma unroll
+                for (int r = 0; r < q; r++) sm += x[r] * RM(r * NL + q);
+                x[q] = sm;
+                tot += sm;
+            }
+        }
+        const double sc = ntot / tot;
+#pragma unroll
+        for (int l = 0; l < NLM; l++) {
+            if (l < NL) {
+                const double nw = x[l] * sc;
+                const double old = pops[(int64_t)l * n + i];
+                if (ntot > 0.0 && (nw >= 1e-10 * ntot || old >= 1e-10 * ntot))
+                    rel = fmaxf(rel, (float)(fabs(nw - old) / fmax(nw, 1e-300)));
+                VX(l) = nw;
+                pops[(int64_t)l * n + i] = (float)nw;
+            }
+        }
+        // refresh the line coefficients of the traced transitions from the unrounded solution
+        for (int k = 0; k < S.nsp; k++) {
+            float2 v = make_float2(0.f, 0.f);
+            if (k < S.nsel) {
+                const double xu = VX(S.upper[k]), xl = VX(S.lower[k]);
+                v.x = (float)(S.ck[k] * (xl * (double)S.gratio[k] - xu));
+                v.y = (float)(S.ck[k] * xu);
+            }
+            coef[i * S.nsp + k] = v;
+        }
+    }
+#undef RM
+#undef VX
+    for (int o = 16; o >= 1; o >>= 1) rel = fmaxf(rel, __shfl_xor_sync(0xffffffffu, rel, o));
+    if ((threadIdx.x & 31) == 0 && rel > 0.0f) atomicMax(maxrel_bits, __float_as_uint(rel));
+}
+
 // ------------------------------------------------------------------------------------------------
 // helpers
 // ------------------------------------------------------------------------------------------------
@@ -639,6 +799,50 @@ static int solve_async(loc_model *m)
 #define LOC_SOLVE(NLMAX)                                                                                                     \
     k_solve<NLMAX><<<nb, 128, 0, m->stream>>>(n, m->sp, m->selh, m->cells.density, m->cells.tkin, m->cells.abundance, m->cnt, \
                                               m->pops, m->coef, m->d_maxrel, ch, m->ali)
+    // shared-memory solver (k_solve_s) while a block's matrices and the species tables fit; LOC_SOLVE_LOCAL=1 forces the
+    // local-memory kernel (A/B measurements)
+    {
+        const int NL = m->nlevel;
+        SolveTabs T;
+        int o = 0;
+        auto take = [&](int bytes) {
+            int at = o;
+            o += (bytes + 7) & ~7;
+            return at;
+        };
+        T.g = take(8 * NL);
+        T.energy = take(8 * NL);
+        T.A = take(8 * m->ntrans);
+        T.bg = take(8 * m->ntrans);
+        T.temps = take(8 * m->ntemp);
+        T.rates = take(8 * m->ntemp * m->ncoll);
+        T.upper = take(4 * m->ntrans);
+        T.lower = take(4 * m->ntrans);
+        T.cu = take(4 * m->ncoll);
+        T.cl = take(4 * m->ncoll);
+        T.bytes = o;
+        const size_t smem = sizeof(double) * (size_t)(NL * NL + NL) * LOC_SOLVE_THREADS + (size_t)o;
+        const char *force = getenv("LOC_SOLVE_LOCAL");
+        if (NL <= 16 && smem <= 200 * 1024 && !(force && atoi(force))) {
+            const unsigned nbs = (unsigned)((n + LOC_SOLVE_THREADS - 1) / LOC_SOLVE_THREADS);
+#define LOC_SOLVE_S(NLX)                                                                                                          \
+    do {                                                                                                                          \
+        LOC_CUDA_CHECK(m, cudaFuncSetAttribute(k_solve_s<NLX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));          \
+        k_solve_s<NLX><<<nbs, LOC_SOLVE_THREADS, smem, m->stream>>>(n, m->sp, m->selh, m->cells.density, m->cells.tkin,          \
+                                                                    m->cells.abundance, m->cnt, m->pops, m->coef, m->d_maxrel, ch, \
+                                                                    m->ali, T);                                                   \
+    } while (0)
+            if (NL == 10) LOC_SOLVE_S(10);
+            else if (NL == 5) LOC_SOLVE_S(5);
+            else if (NL == 4) LOC_SOLVE_S(4);
+            else LOC_SOLVE_S(0);
+#undef LOC_SOLVE_S
+            m->launches++;
+            LOC_CUDA_CHECK(m, cudaGetLastError());
+            m->coef_valid = true;
+            return LOC_OK;
+        }
+    }
     if (m->nlevel <= 6) LOC_SOLVE(6);
     else if (m->nlevel <= 10) LOC_SOLVE(10);
     else if (m->nlevel <= 16) LOC_SOLVE(16);
