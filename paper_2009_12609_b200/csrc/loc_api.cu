@@ -268,7 +268,7 @@ __global__ void __launch_bounds__(128) k_solve(int64_t n, SpeciesDev sp, Selecti
 // level counts (NLX > 0), so that the elimination is fully unrolled with static addresses and x[], bz[] are registers.
 #define LOC_SOLVE_THREADS 64
 struct SolveTabs {   // byte offsets into the block's shared memory, after R
-    int g, energy, A, bg, upper, lower, cu, cl, temps, rates, bytes;
+    int g, energy, A, bg, gr, upper, lower, cu, cl, temps, rates, bytes;
 };
 
 template <int NLX>
@@ -281,9 +281,9 @@ __global__ void __launch_bounds__(LOC_SOLVE_THREADS) k_solve_s(int64_t n, Specie
     const int NL = NLX > 0 ? NLX : sp.nlevel;
     const int tid = threadIdx.x;
     double *Rs = reinterpret_cast<double *>(s_raw);
-    unsigned char *tb = s_raw + sizeof(double) * (NL * NL + NL) * LOC_SOLVE_THREADS;
+    unsigned char *tb = s_raw + sizeof(double) * (NL * NL + 2 * NL) * LOC_SOLVE_THREADS;
     double *t_g = reinterpret_cast<double *>(tb + TB.g), *t_e = reinterpret_cast<double *>(tb + TB.energy);
-    double *t_A = reinterpret_cast<double *>(tb + TB.A), *t_bg = reinterpret_cast<double *>(tb + TB.bg);
+    double *t_A = reinterpret_cast<double *>(tb + TB.A), *t_bg = reinterpret_cast<double *>(tb + TB.bg), *t_gr = reinterpret_cast<double *>(tb + TB.gr);
     double *t_temps = reinterpret_cast<double *>(tb + TB.temps), *t_rates = reinterpret_cast<double *>(tb + TB.rates);
     int *t_up = reinterpret_cast<int *>(tb + TB.upper), *t_lo = reinterpret_cast<int *>(tb + TB.lower);
     int *t_cu = reinterpret_cast<int *>(tb + TB.cu), *t_cl = reinterpret_cast<int *>(tb + TB.cl);
@@ -293,6 +293,7 @@ __global__ void __launch_bounds__(LOC_SOLVE_THREADS) k_solve_s(int64_t n, Specie
     }
     for (int k = tid; k < sp.ntrans; k += LOC_SOLVE_THREADS) {
         t_A[k] = sp.A[k];
+        t_gr[k] = sp.g[sp.upper[k]] / sp.g[sp.lower[k]];
         t_bg[k] = sp.bgocc[k];
         t_up[k] = sp.upper[k];
         t_lo[k] = sp.lower[k];
@@ -305,7 +306,8 @@ __global__ void __launch_bounds__(LOC_SOLVE_THREADS) k_solve_s(int64_t n, Specie
     for (int k = tid; k < sp.ntemp * sp.ncoll; k += LOC_SOLVE_THREADS) t_rates[k] = sp.rates[k];
     __syncthreads();
 #define RM(a) Rs[(a) * LOC_SOLVE_THREADS + tid]
-#define VX(a) Rs[(NL * NL + (a)) * LOC_SOLVE_THREADS + tid]  // NL more doubles per thread: Boltzmann factors, then the solution
+#define VX(a) Rs[(NL * NL + (a)) * LOC_SOLVE_THREADS + tid]  // 2 NL more doubles per thread: Boltzmann factors (then the solution)
+#define VI(a) Rs[(NL * NL + NL + (a)) * LOC_SOLVE_THREADS + tid]  //   and their inverses
     int64_t i = blockIdx.x * (int64_t)LOC_SOLVE_THREADS + tid;
     bool act = i < n;
     if (act && child && child[i] >= 0) act = false;  // refined cell: no gas of its own
@@ -319,7 +321,7 @@ __global__ void __launch_bounds__(LOC_SOLVE_THREADS) k_solve_s(int64_t n, Specie
         // radiative rates: traced transitions from their counters, the others see the background only (DESIGN R23)
         for (int t = 0; t < sp.ntrans; t++) {
             const int u = t_up[t], l = t_lo[t];
-            const double gr = t_g[u] / t_g[l];
+            const double gr = t_gr[t];
             double sj = t_bg[t], esc = 1.0;
             for (int k = 0; k < S.nsel; k++)
                 if (S.sel[k] == t) {
@@ -332,9 +334,9 @@ __global__ void __launch_bounds__(LOC_SOLVE_THREADS) k_solve_s(int64_t n, Specie
                         esc = 1.0;
                     }
                 }
-            const double Slu = gr * t_A[t] * sj;  // = B_lu * Jbar
-            RM(u * NL + l) += t_A[t] * esc + Slu / gr;
-            RM(l * NL + u) += Slu;
+            const double Aul = t_A[t];
+            RM(u * NL + l) += Aul * esc + Aul * sj;  // spontaneous (scaled by the escape probability) + induced
+            RM(l * NL + u) += gr * Aul * sj;          // S_lu = B_lu * Jbar
         }
         // collisions: linear interpolation in T, clamped; upward by detailed balance
         int j = 0;
@@ -352,13 +354,18 @@ __global__ void __launch_bounds__(LOC_SOLVE_THREADS) k_solve_s(int64_t n, Specie
             }
         }
         // g_k exp(-(E_k - E_0) / T), once per level
-        for (int k = 0; k < NL; k++) VX(k) = t_g[k] * exp(-(t_e[k] - t_e[0]) / T);
+        const double invT = 1.0 / T;
+        for (int k = 0; k < NL; k++) {
+            const double b = t_g[k] * exp(-(t_e[k] - t_e[0]) * invT);
+            VX(k) = b;
+            VI(k) = 1.0 / b;  // one division per level instead of one per collisional pair
+        }
         for (int k = 0; k < sp.ncoll; k++) {
             const int u = t_cu[k], l = t_cl[k];
             double gd = t_rates[j * sp.ncoll + k];
             if (sp.ntemp > 1) gd = (1.0 - f) * gd + f * t_rates[(j + 1) * sp.ncoll + k];
             RM(u * NL + l) += dens * gd;
-            RM(l * NL + u) += dens * (gd * VX(u) / VX(l));
+            RM(l * NL + u) += dens * (gd * VX(u) * VI(l));
         }
         // GTH elimination
 #pragma unroll
@@ -416,6 +423,7 @@ __global__ void __launch_bounds__(LOC_SOLVE_THREADS) k_solve_s(int64_t n, Specie
     }
 #undef RM
 #undef VX
+#undef VI
     for (int o = 16; o >= 1; o >>= 1) rel = fmaxf(rel, __shfl_xor_sync(0xffffffffu, rel, o));
     if ((threadIdx.x & 31) == 0 && rel > 0.0f) atomicMax(maxrel_bits, __float_as_uint(rel));
 }
@@ -814,6 +822,7 @@ static int solve_async(loc_model *m)
         T.energy = take(8 * NL);
         T.A = take(8 * m->ntrans);
         T.bg = take(8 * m->ntrans);
+        T.gr = take(8 * m->ntrans);
         T.temps = take(8 * m->ntemp);
         T.rates = take(8 * m->ntemp * m->ncoll);
         T.upper = take(4 * m->ntrans);
@@ -821,7 +830,7 @@ static int solve_async(loc_model *m)
         T.cu = take(4 * m->ncoll);
         T.cl = take(4 * m->ncoll);
         T.bytes = o;
-        const size_t smem = sizeof(double) * (size_t)(NL * NL + NL) * LOC_SOLVE_THREADS + (size_t)o;
+        const size_t smem = sizeof(double) * (size_t)(NL * NL + 2 * NL) * LOC_SOLVE_THREADS + (size_t)o;
         const char *force = getenv("LOC_SOLVE_LOCAL");
         if (NL <= 16 && smem <= 200 * 1024 && !(force && atoi(force))) {
             const unsigned nbs = (unsigned)((n + LOC_SOLVE_THREADS - 1) / LOC_SOLVE_THREADS);
