@@ -229,6 +229,37 @@ __device__ __forceinline__ void channel_update(float &n, float phi, const TParam
     }
 }
 
+// channel_update for a quad of channels in packed pairs (same operations per element as channel_update, so the same
+// results; half the issue slots).  n01 / n23 and phi01 / phi23 hold channels (0, 1) / (2, 3); acc += the quad's sums.
+__device__ __forceinline__ void channel_update4(f32x2 &n01, f32x2 &n23, f32x2 phi01, f32x2 phi23, const TParam &p, float &accA, float &accB)
+{
+    const f32x2 C0 = pk2(p.c0, p.c0), C1 = pk2(p.c1, p.c1);
+    const f32x2 ONE = pk2(1.0f, 1.0f), MONE = pk2(-1.0f, -1.0f);
+    float a0, a1, b0, b1;
+    if (p.thick) {
+        float z0, z1, z2, z3;
+        upk2(mul2(phi01, C0), z0, z1);
+        upk2(mul2(phi23, C0), z2, z3);
+        const f32x2 om01 = fma2(pk2(ex2f(z0), ex2f(z1)), MONE, ONE), om23 = fma2(pk2(ex2f(z2), ex2f(z3)), MONE, ONE);
+        upk2(fma2(n01, om01, mul2(n23, om23)), a0, a1);
+        upk2(add2(om01, om23), b0, b1);
+        n01 = fma2(om01, fma2(n01, MONE, C1), n01);
+        n23 = fma2(om23, fma2(n23, MONE, C1), n23);
+    } else {
+        const f32x2 K4 = pk2(-1.0f / 24.0f, -1.0f / 24.0f), K3 = pk2(1.0f / 6.0f, 1.0f / 6.0f), K2 = pk2(-0.5f, -0.5f);
+        const f32x2 t01 = mul2(phi01, C0), t23 = mul2(phi23, C0);
+        const f32x2 P01 = fma2(t01, fma2(t01, fma2(t01, K4, K3), K2), ONE), P23 = fma2(t23, fma2(t23, fma2(t23, K4, K3), K2), ONE);
+        const f32x2 q01 = mul2(phi01, P01), q23 = mul2(phi23, P23);
+        const f32x2 om01 = mul2(t01, P01), om23 = mul2(t23, P23);
+        upk2(fma2(n01, q01, mul2(n23, q23)), a0, a1);
+        upk2(add2(q01, q23), b0, b1);
+        n01 = fma2(C1, q01, fma2(mul2(n01, MONE), om01, n01));
+        n23 = fma2(C1, q23, fma2(mul2(n23, MONE), om23, n23));
+    }
+    accA += a0 + a1;
+    accB += b0 + b1;
+}
+
 // Reduce NV per-lane values across the warp with a halving butterfly (about NV shuffles in total instead of
 // 5 NV).  On return v[0] of lane L holds the warp total of value index *owner (or *owner = -1); every value index has
 // exactly one owner lane.

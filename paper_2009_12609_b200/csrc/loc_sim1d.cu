@@ -242,18 +242,16 @@ __global__ void __launch_bounds__(LOC_1D_WARPS * 32) k_sim1d_w(Sim1D P, int nray
                 phi[i] = (c >= c_lo && c <= c_hi) ? ex2f(fmaf(-y, y, lamp)) : 0.0f;
             }
             v[2 * NT] += (phi[0] + phi[1]) + (phi[2] + phi[3]);
+            const f32x2 phi01 = pk2(phi[0], phi[1]), phi23 = pk2(phi[2], phi[3]);
 #pragma unroll
             for (int t = 0; t < NT; t++) {
                 const TParam tp = stp[t];
                 float4 n4 = *reinterpret_cast<float4 *>(sn + t * nchp + cb);
-                float a = 0.f, b = 0.f;
-                channel_update(n4.x, phi[0], tp, a, b);
-                channel_update(n4.y, phi[1], tp, a, b);
-                channel_update(n4.z, phi[2], tp, a, b);
-                channel_update(n4.w, phi[3], tp, a, b);
+                f32x2 n01 = pk2(n4.x, n4.y), n23 = pk2(n4.z, n4.w);
+                channel_update4(n01, n23, phi01, phi23, tp, v[t], v[NT + t]);
+                upk2(n01, n4.x, n4.y);
+                upk2(n23, n4.z, n4.w);
                 *reinterpret_cast<float4 *>(sn + t * nchp + cb) = n4;
-                v[t] += a;
-                v[NT + t] += b;
             }
         }
         int owner;
