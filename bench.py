@@ -316,8 +316,40 @@ def run_own(args):
     (t_e2e,) = max_over_ranks([e0.elapsed_time(e1) * 1e-3], device=f"cuda:{local}")
     e2e_val = whole_job_value(u_nom, n_e2e, world, t_e2e)
 
+    # ---- S10: spectral cube of the first traced line along +z, one pixel per finest cell (C5: 1024 x 1024 x
+    #      256 channels), and its line-area map; after the iterations above, timed apart from `value` ----
+    map_info = None
+    if is3d and not args.no_map:
+        nfine = int(m.nx) << (int(m.nlev) - 1)
+        pix = (1 << 20) >> (int(m.nlev) - 1)
+        aff = np.array([pix // 2, pix // 2, pix, 0, 0, pix], np.int64)
+        zdir = np.array([0.0, 0.0, 1.0])
+        t0 = int(sel[0]) if sel is not None else 0
+        cube = g.spectra(t0, nfine, nfine, dir=zdir, aff=aff)
+        wmap = g.line_area(cube)
+        me = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        nrep = 3
+        barrier()
+        me[0].record()
+        for _ in range(nrep):
+            B.loc_spectra(g.h, t0, cube, nfine, nfine, zdir, aff, None)
+        me[1].record()
+        for _ in range(nrep):
+            B.loc_line_area(g.h, cube, nfine * nfine, wmap)
+        me[2].record()
+        barrier()
+        t_map, t_area = max_over_ranks([me[0].elapsed_time(me[1]) * 1e-3 / nrep, me[1].elapsed_time(me[2]) * 1e-3 / nrep],
+                                       device=f"cuda:{local}")
+        area_bytes = float(nfine) * nfine * (4 * m.nchannel + 4)
+        map_info = {"pixels": [nfine, nfine], "channels": int(m.nchannel), "transition": t0, "ms_spectra": 1e3 * t_map,
+                    "ms_line_area": 1e3 * t_area, "line_area_gbs": area_bytes / t_area / 1e9,
+                    "cube_bytes": int(cube.numel() * 4), "w_mean_K_kms": float(wmap.mean())}
+        del cube, wmap
+
     if rank == 0:
         hbm, sm_max, kind = load_peaks()
+        if map_info is not None:
+            map_info["line_area_hbm_frac"] = map_info["line_area_gbs"] / hbm
         roof = roofline(sg, nt, t_sim / args.steps, hbm, sm_max, kind)
         cpu = None
         if world == 1 and not args.no_cpu:
@@ -340,6 +372,8 @@ def run_own(args):
                "gpu_launches": int(launches)}
         if cpu is not None:
             out["cpu_baseline"] = cpu
+        if map_info is not None:
+            out["map"] = map_info
         print(json.dumps(out))
     g.close()
     if world > 1:
@@ -355,6 +389,7 @@ def main():
     ap.add_argument("--workload", default=os.environ.get("LOC_BENCH_WORKLOAD", DEFAULT_WORKLOAD))
     ap.add_argument("--ref-budget", type=float, default=6e9, help="nominal updates per oracle sample (about 10-30 s of CPU)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-map", action="store_true", help="skip the spectral-cube / line-area leg of the 3D workloads")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -184,6 +184,11 @@ int loc_iterate_until(loc_model *m, int max_iter, double tol, int *niter_done, d
 int loc_spectra(loc_model *m, int trans, const double *dir, int nx, int ny, const int64_t *aff,
                 const double *offsets_cm, float *dev_out);
 
+/* Line-area map (Fig. 5c "line area"): W[p] = sum_c T_A[p][c] * dv, in K km/s, for npix spectra of the
+ * model's nchannel channels as loc_spectra writes them.  dev_cube: DEVICE float [npix][nchannel] (K); dev_w: DEVICE
+ * float [npix].  Enqueued on the model's stream; npix = 0 is a no-op.                                          */
+int loc_line_area(loc_model *m, const float *dev_cube, int64_t npix, float *dev_w);
+
 int loc_get_stats(loc_model *m, loc_stats *out);
 void loc_destroy_model(loc_model *m);
 const char *loc_last_error(const loc_model *m); /* m may be NULL: error of the last failed loc_create_model */

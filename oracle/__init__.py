@@ -196,6 +196,12 @@ def spectra_1d(sp: OSpecies, m, pops, t, b):
     return TA
 
 
+def line_area(TA, dv_cm_s):
+    """Line-area map (Fig. 5c): W = sum over channels of T_A dv, K km/s; the definition written out in
+    float64.  TA [..., nchannel] in K, dv in cm/s."""
+    return np.asarray(TA, np.float64).sum(axis=-1) * (float(dv_cm_s) * 1e-5)
+
+
 def sim_3d(sp: OSpecies, m, pops, sel=None, ali=True, geom_only=False, dirs=None, off64=(25, 41)):
     """m: loc_workloads.OctreeModel.  pops [ncell][NL] float64.  Returns dict of counters."""
     G = OGrid(m)

@@ -936,6 +936,12 @@ extern "C" int loc_spectra(loc_model *m, int trans, const double *dir, int nx, i
     return loc_launch_spectra(m, trans, dir, nx, ny, aff, offsets_cm, dev_out);
 }
 
+extern "C" int loc_line_area(loc_model *m, const float *dev_cube, int64_t npix, float *dev_w)
+{
+    if (!m || npix < 0 || (npix > 0 && (!dev_cube || !dev_w))) return LOC_EINVAL;
+    return loc_launch_line_area(m, dev_cube, (long long)npix, dev_w);
+}
+
 extern "C" int loc_get_stats(loc_model *m, loc_stats *out)
 {
     if (!m || !out) return LOC_EINVAL;

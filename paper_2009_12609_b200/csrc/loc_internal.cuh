@@ -55,6 +55,7 @@ struct Dir3 {
     int ax[3];              // model axis (0=x,1=y,2=z) of the working axes
     int flip[3];            // per working axis: mirrored?
     unsigned long long T[2];  // fixed-point inverse slopes of p, q: shift(zeta) = floor(zeta 2^32 / T); 0 = zero slope
+    unsigned long long M[2];  // floor(2^64 / T): reciprocal for the exact division by multiplication (shift_of)
     int W[3];               // model extent along the working axes in grid units (2^20 per root cell)
     int np, nq;             // root lines along p, q
     float d[3];             // snapped unit propagation direction, model frame
@@ -321,9 +322,42 @@ struct Tree {
 
 #define LOC_ZINF (1ll << 40)
 
-__device__ __forceinline__ long long shift_of(unsigned long long T, long long z)
+// floor(z 2^32 / T), exactly, without a 64-bit division (about 100 instructions, several per ray step in the path
+// builder): q' = mulhi(n, M) with M = floor(2^64 / T) satisfies q - 1 <= q' <= q for n = z 2^32 < 2^63 and T >= 2^32
+// (n (2^64/T - M) / 2^64 < 1), so one remainder test makes it exact; the loop form costs nothing and needs no such bound.
+__device__ __forceinline__ long long shift_of(const Dir3 &D, int k, long long z)
 {
-    return T ? (long long)(((unsigned long long)z << 32) / T) : 0ll;
+    const unsigned long long T = D.T[k];
+    if (T == 0) return 0ll;
+    const unsigned long long n = (unsigned long long)z << 32;
+    unsigned long long q = __umul64hi(n, D.M[k]);
+    unsigned long long r = n - q * T;
+    while (r >= T) {
+        r -= T;
+        q++;
+    }
+    return (long long)q;
+}
+
+// a / W and a - (a / W) W (floor division) for a that lies within a few W of [0, W): the transverse wrap-around count
+__device__ __forceinline__ long long wrap_of(long long a, long long W, long long &rem)
+{
+    if (a >= 8 * W || a < -8 * W) {
+        const long long w = (a >= 0) ? a / W : -((-a + W - 1) / W);
+        rem = a - w * W;
+        return w;
+    }
+    long long w = 0;
+    while (a >= W) {
+        a -= W;
+        w++;
+    }
+    while (a < 0) {
+        a += W;
+        w--;
+    }
+    rem = a;
+    return w;
 }
 
 // smallest zeta with shift_of(T, zeta) >= D
@@ -337,7 +371,6 @@ __device__ __forceinline__ long long cross_of(unsigned long long T, long long D)
     return (long long)((hi << 32) | (lo2 >> 32));
 }
 
-__device__ __forceinline__ long long floordiv(long long a, long long b) { return (a >= 0) ? a / b : -((-a + b - 1) / b); }
 
 struct LeafPos {
     int cell[LOC_MAXL];  // global cell index of the ancestor at each level (last = the leaf)
@@ -391,6 +424,7 @@ int loc_launch_sim3d(loc_model *m, int geom);
 int loc_setup3d(loc_model *m);
 int loc_launch_spectra(loc_model *m, int trans, const double *dir, int nx, int ny, const int64_t *aff,
                        const double *offsets_cm, float *dev_out);
+int loc_launch_line_area(loc_model *m, const float *dev_cube, long long npix, float *dev_w);
 int loc_build_streams(loc_model *m);
 void loc_fill_dir(loc_model *m, const double *din, Dir3 *D);
 

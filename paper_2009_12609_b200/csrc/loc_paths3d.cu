@@ -37,9 +37,11 @@ void loc_fill_dir(loc_model *m, const double *din, Dir3 *D)
         unsigned long long S = (unsigned long long)nearbyint(s * (double)LOC_H0);  // round half even (DESIGN R7)
         if (S == 0) {
             D->T[k] = 0;
+            D->M[k] = 0;
             sl[k] = 0.0;
         } else {
             D->T[k] = ((1ull << 52) + S / 2) / S;
+            D->M[k] = (unsigned long long)((((unsigned __int128)1) << 64) / D->T[k]);
             sl[k] = 4294967296.0 / (double)D->T[k];
         }
     }
@@ -121,10 +123,11 @@ __global__ void __launch_bounds__(128) k_build_paths(BuildArgs A)
         bool first = true;
         long long wrp = 0, wrq = 0;
         while (zeta < Wz) {
-            const long long Sp = shift_of(D.T[0], zeta), Sq = shift_of(D.T[1], zeta);
+            const long long Sp = shift_of(D, 0, zeta), Sq = shift_of(D, 1, zeta);
             const long long up = cur.bp + Sp, uq = cur.bq + Sq;
-            const long long wp_ = up / Wp, wq_ = uq / Wq;
-            const int fp = (int)(up - wp_ * Wp), fq = (int)(uq - wq_ * Wq);
+            long long rp, rq;
+            const long long wp_ = wrap_of(up, Wp, rp), wq_ = wrap_of(uq, Wq, rq);
+            const int fp = (int)rp, fq = (int)rq;
             const bool wrapped = !first && (wp_ != wrp || wq_ != wrq);
             wrp = wp_;
             wrq = wq_;
@@ -154,11 +157,12 @@ __global__ void __launch_bounds__(128) k_build_paths(BuildArgs A)
                                 src = LOC_SRC_BG;
                             } else {
                                 const long long zb = zin - 1;
-                                const long long pb = ap + shift_of(D.T[0], zb) - Sp, qb = aq + shift_of(D.T[1], zb) - Sq;
-                                const long long pi = ap + shift_of(D.T[0], zin) - Sp, qi = aq + shift_of(D.T[1], zin) - Sq;
-                                const long long wpb = floordiv(pb, Wp), wqb = floordiv(qb, Wq);
-                                if (level_at(G, D, (int)zb, (int)(pb - wpb * Wp), (int)(qb - wqb * Wq)) >= j + 1) continue;  // alive already
-                                if (wpb != floordiv(pi, Wp) || wqb != floordiv(qi, Wq)) src = LOC_SRC_BG;
+                                const long long pb = ap + shift_of(D, 0, zb) - Sp, qb = aq + shift_of(D, 1, zb) - Sq;
+                                const long long pi = ap + shift_of(D, 0, zin) - Sp, qi = aq + shift_of(D, 1, zin) - Sq;
+                                long long rpb, rqb, rdummy;
+                                const long long wpb = wrap_of(pb, Wp, rpb), wqb = wrap_of(qb, Wq, rqb);
+                                if (level_at(G, D, (int)zb, (int)rpb, (int)rqb) >= j + 1) continue;  // alive already
+                                if (wpb != wrap_of(pi, Wp, rdummy) || wqb != wrap_of(qi, Wq, rdummy)) src = LOC_SRC_BG;
                             }
                             if (saved < 0) {
                                 saved = j;
@@ -175,9 +179,11 @@ __global__ void __launch_bounds__(128) k_build_paths(BuildArgs A)
                             }
                             if (sp < LOC_BUILD_STACK) {
                                 Pending c;
-                                long long bb = (ap - Sp) % Wp, bc = (aq - Sq) % Wq;
-                                c.bp = (int)(bb < 0 ? bb + Wp : bb);
-                                c.bq = (int)(bc < 0 ? bc + Wq : bc);
+                                long long bb, bc;
+                                wrap_of(ap - Sp, Wp, bb);
+                                wrap_of(aq - Sq, Wq, bc);
+                                c.bp = (int)bb;
+                                c.bq = (int)bc;
                                 c.zeta = (int)zin;
                                 c.tag = (unsigned char)(j + 1);
                                 c.src = (unsigned char)(src == LOC_SRC_BG ? LOC_SRC_BG : saved);

@@ -92,7 +92,7 @@ __global__ void __launch_bounds__(32 * LOC_SPEC_WARPS) k_spectra3d(Spec3D P)
     if (bp < 0) zeta = max(zeta, cross_of(D.T[0], -bp));
     if (bq < 0) zeta = max(zeta, cross_of(D.T[1], -bq));
     while (zeta < Wz) {
-        const long long up = bp + shift_of(D.T[0], zeta), uq = bq + shift_of(D.T[1], zeta);
+        const long long up = bp + shift_of(D, 0, zeta), uq = bq + shift_of(D, 1, zeta);
         if (up < 0 || uq < 0 || up >= Wp || uq >= Wq) break;  // left through a side face
         LeafPos L;
         find_leaf(P.G, D, (int)zeta, (int)up, (int)uq, L);
@@ -218,5 +218,30 @@ int loc_launch_spectra(loc_model *m, int trans, const double *dir, int nx, int n
         m->launches++;
         LOC_CUDA_CHECK(m, cudaGetLastError());
     }
+    return LOC_OK;
+}
+
+// ---- line-area map (Fig. 5c: W = integral of T_A over velocity) -------------------------------------------
+// One warp per pixel: coalesced reads of the pixel's spectrum, butterfly sum, W = dv[km/s] * sum_c T_A(c).  HBM bound:
+// 4 nch bytes read per pixel, 4 written.
+__global__ void __launch_bounds__(256) k_line_area(const float *__restrict__ cube, long long npix, int nch, float dv_kms, float *__restrict__ w)
+{
+    const int lane = threadIdx.x & 31;
+    const long long pix = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5;
+    if (pix >= npix) return;
+    const float *sp = cube + pix * nch;
+    float a = 0.f;
+    for (int c = lane; c < nch; c += 32) a += __ldg(sp + c);
+    for (int o = 16; o >= 1; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+    if (lane == 0) w[pix] = a * dv_kms;
+}
+
+int loc_launch_line_area(loc_model *m, const float *dev_cube, long long npix, float *dev_w)
+{
+    if (npix == 0) return LOC_OK;
+    const long long threads = npix * 32;
+    k_line_area<<<(unsigned)((threads + 255) / 256), 256, 0, m->stream>>>(dev_cube, npix, m->nch, (float)(m->dv * 1e-5), dev_w);
+    m->launches++;
+    LOC_CUDA_CHECK(m, cudaGetLastError());
     return LOC_OK;
 }

@@ -123,6 +123,14 @@ class LocModel:
         B.loc_spectra(self.h, trans, out, nx, ny, dir, aff, offsets_cm)
         return out
 
+    def line_area(self, cube):
+        """W = sum_c T_A dv in K km/s for a cube [..., nchannel] of loc_spectra (float32 CUDA tensor)"""
+        cube = cube.contiguous()
+        npix = cube.numel() // self.nch
+        out = torch.empty(cube.shape[:-1], dtype=torch.float32, device=self.dev)
+        B.loc_line_area(self.h, cube, npix, out)
+        return out
+
     def close(self):
         if getattr(self, "h", None) is not None:
             B.loc_destroy_model(self.h)

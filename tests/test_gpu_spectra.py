@@ -104,3 +104,30 @@ def test_spectra_error_paths():
     with pytest.raises(LocError):
         g.spectra(0, 4, 4, dir=np.array([0.0, 0.5, 1.0]), aff=np.zeros(6, np.int64))  # not a unit vector
     g.close()
+
+
+@pytest.mark.parametrize("nch,npix", [(64, 300), (67, 33), (256, 1025), (5, 7)])
+def test_line_area(nch, npix):
+    """loc_line_area against the oracle's definition on the same float32 cube: spectra of the 1D model plus seeded noise
+    of both signs (ragged channel counts, more pixels than one block, a band narrower than a warp)."""
+    import torch
+    from paper_2009_12609_b200 import LocModel
+    m = W.shell_config(1, ns=12, nchannel=nch)
+    sp = O.OSpecies(m.species)
+    _, pops32 = f32_pops_from_oracle_lte(sp, m)
+    g = LocModel(m)
+    g.set_populations(pops32)
+    b = np.linspace(0.0, 1.02, npix) * m.r_out[-1]
+    cube = g.spectra(0, npix, offsets_cm=b)[0]
+    rng = np.random.default_rng(1234 + nch)
+    cube = (cube + torch.from_numpy(rng.normal(0.0, 0.05, (npix, nch)).astype(np.float32)).to(cube.device)).contiguous()
+    w = g.line_area(cube).cpu().numpy()
+    c64 = cube.cpu().numpy().astype(np.float64)
+    dv = 2.0 * m.band_half / nch
+    ref = O.line_area(c64, dv)
+    scale = np.abs(c64).sum(axis=-1) * dv * 1e-5
+    assert w.shape == ref.shape
+    assert np.max(np.abs(w - ref) / scale) < 2e-6  # float32 summation of nch terms
+    # empty input
+    g.line_area(cube[:0])
+    g.close()

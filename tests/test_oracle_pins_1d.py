@@ -242,3 +242,20 @@ def test_P12_velocity_mirror(sp5):
     # infall: near side (outbound half) is red-shifted -> self-absorption asymmetry: blue peak stronger (R6)
     TA = O.spectra_1d(os_, m if False else W.shell_config(1, ns=12, nchannel=64), pops, 0, np.array([0.0]))[0]
     assert TA[:32].sum() != TA[32:].sum()
+
+
+def test_P9_line_area_closed_forms():
+    """oracle line_area: (i) a Gaussian line T0 exp(-v^2 / 2 s^2) sampled at the channel centres of a band
+    much wider than s with dv << s integrates to T0 s sqrt(2 pi) (the rectangle rule is exponentially accurate for a
+    Gaussian); (ii) a flat spectrum T0 gives T0 times the full band width; (iii) linear in T_A.  Catches a wrong channel
+    width, a cm/s vs km/s slip, a sum over the wrong axis."""
+    nch, band = 400, 6.0e5  # +-6 km/s
+    dv = 2.0 * band / nch
+    v = (np.arange(nch) - 0.5 * (nch - 1)) * dv
+    s_kms, T0 = 0.35, 7.5
+    g = T0 * np.exp(-0.5 * (v / (s_kms * 1e5)) ** 2)
+    W = O.line_area(np.stack([g, 2.0 * g, np.full(nch, T0)]), dv)
+    assert abs(W[0] - T0 * s_kms * np.sqrt(2.0 * np.pi)) < 1e-12 * W[0]
+    assert abs(W[1] - 2.0 * W[0]) < 1e-14 * W[1]
+    assert abs(W[2] - T0 * 12.0) < 1e-12 * W[2]
+    assert O.line_area(np.zeros((3, 2, nch)), dv).shape == (3, 2)
