@@ -30,8 +30,8 @@ DEFAULT_WORKLOAD = "C4"
 # ---- roofline constants -----------------------------------------------------------------------------
 N_SM = 148
 # DRAM bytes read + written by one launch of the dominant kernel, from the committed `ncu --set full` captures
-# (profiles/r1_v7_sim3d.md); workloads without a capture report null
-NCU_TRAFFIC_BYTES = {"C3": 19.07e9 + 7.87e9, "C4": 903.7e9 + 301.0e9}
+# (profiles/r1_v8_sim3d.md, profiles/r1_sim1d_C2.md); workloads without a capture report null
+NCU_TRAFFIC_BYTES = {"C2": 24.3e6, "C3": 19.08e9 + 7.88e9, "C4": 904.4e9 + 299.9e9}
 FP32_LANES_PER_SM_CLK = 128  # 4 sub-partitions x 1 warp instruction / clk
 MUFU_PER_SM_CLK = 16
 
@@ -216,7 +216,7 @@ def roofline(stats_geom, nt, t_sim_s, hbm_gbs, sm_mhz, peak_kind):
              "unit": "Tinstr/s (FP32-pipe lane instructions)"}
     r["frac"] = t_roof / t_sim_s
     r["traffic"] = NCU_TRAFFIC_BYTES.get(stats_geom.get("workload"))
-    r.update({"kernel": "k_sim3d" if stats_geom.get("is3d") else "k_sim1d", "peak_source": peak_kind + " HBM copy; ALU peaks derived at sm_max clock",
+    r.update({"kernel": "k_sim3d" if stats_geom.get("is3d") else "k_sim1d_w", "peak_source": peak_kind + " HBM copy; ALU peaks derived at sm_max clock",
               "algorithmic_bytes_per_launch": byt, "active_updates_per_launch": u_active, "hbm_gbs_achieved": byt / t_sim_s / 1e9,
               "hbm_frac": t_hbm / t_sim_s, "mufu_frac": t_mufu / t_sim_s, "fp32_frac": t_fp32 / t_sim_s,
               "t_kernel_ms": 1e3 * t_sim_s})

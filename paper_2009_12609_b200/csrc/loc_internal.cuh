@@ -9,7 +9,7 @@
 #define LOC_LB 20              // log2(grid units per root cell)
 #define LOC_H0 (1 << LOC_LB)   // grid units per root cell
 #define LOC_MAXL LOC_MAX_TREE_LEVELS
-#define LOC_BUILD_BATCH 65536  // root lines traced per launch of the path builder
+#define LOC_BUILD_BATCH 262144  // root lines traced per launch of the path builder (16 B x LOC_BUILD_STACK of stack each)
 #define LOC_BUILD_STACK 256    // pending rays per root line (PAPER.md:119 estimates ~7*3^(NL-1) stored rays)
 
 // physical constants (CGS, CODATA 2018) -- DESIGN R1

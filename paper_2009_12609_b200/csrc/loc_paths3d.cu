@@ -79,18 +79,24 @@ struct BuildArgs {
 };
 
 // Path builder: traces root line `task` and all its descendants depth first (DESIGN 6.3).
+// SIMT shape.  A thread's sequence of operations is the plain depth-first walk; what the warp executes is arranged in two
+// phases per round so that the long, rare part does not serialise the short, common one: phase 1 -- every lane steps its
+// ray from leaf to leaf until the ray ends or stands on the upstream face of a refined ancestor (a possible donor event);
+// phase 2 -- after the warp has reconverged, the lanes that stopped for a donor event evaluate it together (the same 21
+// candidate positions each), then step.  Taken lane by lane inside one loop, the donor evaluation (~1300 instructions even
+// when it finds nothing) was paid by the whole warp in 9 of 10 iterations (C4: 6.9 s of set-up).
 __global__ void __launch_bounds__(128) k_build_paths(BuildArgs A)
 {
-    long long task = A.task_begin + blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (task >= A.task_end) return;
+    const long long task = A.task_begin + blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    bool finished = task >= A.task_end;  // such lanes stay for the warp-wide votes
     const Tree &G = A.G;
-    const Dir3 D = A.dirs[A.task_dir[task]];
+    const Dir3 D = A.dirs[finished ? 0 : A.task_dir[task]];
     Pending *stack = A.stacks + (blockIdx.x * (long long)blockDim.x + threadIdx.x) * LOC_BUILD_STACK;
     int sp = 0;
     long long nrec = 0, nstep = 0;
-    uint2 *out = A.emit ? A.stream + A.task_off[task] : nullptr;
+    uint2 *out = (A.emit && !finished) ? A.stream + A.task_off[task] : nullptr;
     const int Wz = D.W[0], Wp = D.W[1], Wq = D.W[2];
-    {
+    if (!finished) {
         long long lt = task - D.task0;
         const int O_p = 25 * (LOC_H0 / 64), O_q = 41 * (LOC_H0 / 64);  // DESIGN R8
         Pending r;
@@ -108,111 +114,154 @@ __global__ void __launch_bounds__(128) k_build_paths(BuildArgs A)
         if (out) out[nrec] = make_uint2(x_, y_); \
         nrec++;                                  \
     } while (0)
+    // step through the leaf L from zeta
+#define STEP_LEAF()                                                                                              \
+    do {                                                                                                         \
+        const int h = LOC_H0 >> L.level;                                                                         \
+        long long znext = (zeta & ~(long long)(h - 1)) + h, z;                                                   \
+        z = cross_of(D.T[0], Sp + (fp & ~(h - 1)) + h - fp); if (z < znext) znext = z;                           \
+        z = cross_of(D.T[1], Sq + (fq & ~(h - 1)) + h - fq); if (z < znext) znext = z;                           \
+        EMIT((unsigned)L.cell[L.level], LOC_REC(LOC_OP_STEP, L.level, (unsigned)(znext - zeta)));                \
+        nstep++;                                                                                                 \
+        zeta = znext;                                                                                            \
+        first = false;                                                                                           \
+    } while (0)
     int just_saved = -1;  // slot of the SAVE that was the last record emitted (-1: the last record was something else)
-    while (sp > 0) {
-        const Pending cur = stack[--sp];
-        const int tag = cur.tag;
-        // the ray starts from the background or from a saved spectrum; the first ray served after a SAVE finds that very
-        // spectrum still in place, so its LOAD is left out (a quarter of all LOADs of a refined model)
-        if (cur.src == LOC_SRC_BG)
-            EMIT(0u, LOC_REC(LOC_OP_BG, 0, 0));
-        else if ((int)cur.src != just_saved)
-            EMIT((unsigned)cur.src, LOC_REC(LOC_OP_LOAD, 0, 0));
-        just_saved = -1;
-        long long zeta = cur.zeta;
-        bool first = true;
-        long long wrp = 0, wrq = 0;
-        while (zeta < Wz) {
-            const long long Sp = shift_of(D, 0, zeta), Sq = shift_of(D, 1, zeta);
-            const long long up = cur.bp + Sp, uq = cur.bq + Sq;
-            long long rp, rq;
-            const long long wp_ = wrap_of(up, Wp, rp), wq_ = wrap_of(uq, Wq, rq);
-            const int fp = (int)rp, fq = (int)rq;
-            const bool wrapped = !first && (wp_ != wrp || wq_ != wrq);
-            wrp = wp_;
-            wrq = wq_;
-            LeafPos L;
-            find_leaf(G, D, (int)zeta, fp, fq, L);
-            if (L.level < tag) break;  // entering a region refined to less than the tag: terminated
-            if (wrapped) EMIT(0u, LOC_REC(LOC_OP_BG, 0, 0));  // left through a side, re-enters opposite
-            // ---- donor duty: upstream face of refined ancestors entered now ----
-            if (!(first && cur.resumed)) {
-                int saved = -1;
-                for (int j = tag; j < L.level; j++) {
-                    const int hj = LOC_H0 >> j, hk = hj >> 1;
-                    if (zeta & (hj - 1)) continue;
-                    const int op = fp & ~(hj - 1), oq = fq & ~(hj - 1);
-                    for (int dj = -3; dj <= 1; dj++)
-                        for (int di = -3; di <= 1; di++) {
-                            if (!((di | dj) & 1)) continue;  // member of the coarser lattice P_j
-                            const long long ap = (long long)fp + di * hk, aq = (long long)fq + dj * hk;
-                            long long zin = zeta, zout = zeta + hj, z;
-                            z = cross_of(D.T[0], Sp + op - ap); if (z > zin) zin = z;
-                            z = cross_of(D.T[1], Sq + oq - aq); if (z > zin) zin = z;
-                            z = cross_of(D.T[0], Sp + op + hj - ap); if (z < zout) zout = z;
-                            z = cross_of(D.T[1], Sq + oq + hj - aq); if (z < zout) zout = z;
-                            if (zout <= zin) continue;  // does not cross this cell
-                            int src = -1;               // -1: slot of this event
-                            if (zin == 0) {
-                                src = LOC_SRC_BG;
-                            } else {
-                                const long long zb = zin - 1;
-                                const long long pb = ap + shift_of(D, 0, zb) - Sp, qb = aq + shift_of(D, 1, zb) - Sq;
-                                const long long pi = ap + shift_of(D, 0, zin) - Sp, qi = aq + shift_of(D, 1, zin) - Sq;
-                                long long rpb, rqb, rdummy;
-                                const long long wpb = wrap_of(pb, Wp, rpb), wqb = wrap_of(qb, Wq, rqb);
-                                if (level_at(G, D, (int)zb, (int)rpb, (int)rqb) >= j + 1) continue;  // alive already
-                                if (wpb != wrap_of(pi, Wp, rdummy) || wqb != wrap_of(qi, Wq, rdummy)) src = LOC_SRC_BG;
-                            }
-                            if (saved < 0) {
-                                saved = j;
-                                just_saved = j;
-                                EMIT((unsigned)j, LOC_REC(LOC_OP_SAVE, 0, 0));
-                                if (sp < LOC_BUILD_STACK) {
-                                    Pending c = cur;
-                                    c.zeta = (int)zeta;
-                                    c.src = (unsigned char)j;
-                                    c.resumed = 1;
-                                    stack[sp++] = c;
-                                } else
-                                    *A.errflag = 1;
-                            }
+    // state of the ray being walked
+    Pending cur;
+    cur.bp = cur.bq = cur.zeta = 0;
+    cur.tag = cur.src = cur.resumed = cur.pad = 0;
+    int tag = 0, fp = 0, fq = 0;
+    long long zeta = 0, wrp = 0, wrq = 0, Sp = 0, Sq = 0;
+    bool first = true, walking = false;
+    LeafPos L;
+    L.level = 0;
+    for (;;) {
+        if (__all_sync(0xffffffffu, finished)) break;
+        // ---- next ray of this root line ----
+        if (!finished && !walking) {
+            if (sp == 0) {
+                while (nrec & (LOC_TASK_ALIGN - 1)) EMIT(0u, LOC_REC(LOC_OP_NOP, 0, 0));  // tasks are whole chunks of records
+                if (!A.emit) {
+                    A.task_off[task] = nrec;
+                    atomicAdd(A.nsteps, (unsigned long long)nstep);
+                }
+                finished = true;
+            } else {
+                cur = stack[--sp];
+                tag = cur.tag;
+                // the ray starts from the background or from a saved spectrum; the first ray served after a SAVE finds that
+                // very spectrum still in place, so its LOAD is left out (a quarter of all LOADs of a refined model)
+                if (cur.src == LOC_SRC_BG)
+                    EMIT(0u, LOC_REC(LOC_OP_BG, 0, 0));
+                else if ((int)cur.src != just_saved)
+                    EMIT((unsigned)cur.src, LOC_REC(LOC_OP_LOAD, 0, 0));
+                just_saved = -1;
+                zeta = cur.zeta;
+                first = true;
+                wrp = wrq = 0;
+                walking = true;
+            }
+        }
+        // ---- phase 1: leaf to leaf until the ray ends or may have donor duty ----
+        bool donor = false;
+        if (!finished) {
+            while (walking) {
+                if (zeta >= Wz) {
+                    walking = false;
+                    break;
+                }
+                Sp = shift_of(D, 0, zeta);
+                Sq = shift_of(D, 1, zeta);
+                const long long up = cur.bp + Sp, uq = cur.bq + Sq;
+                long long rp, rq;
+                const long long wp_ = wrap_of(up, Wp, rp), wq_ = wrap_of(uq, Wq, rq);
+                fp = (int)rp;
+                fq = (int)rq;
+                const bool wrapped = !first && (wp_ != wrp || wq_ != wrq);
+                wrp = wp_;
+                wrq = wq_;
+                find_leaf(G, D, (int)zeta, fp, fq, L);
+                if (L.level < tag) {  // entering a region refined to less than the tag: terminated
+                    walking = false;
+                    break;
+                }
+                if (wrapped) EMIT(0u, LOC_REC(LOC_OP_BG, 0, 0));  // left through a side, re-enters opposite
+                // donor duty is possible where the ray stands on the upstream face of a refined ancestor
+                if (!(first && cur.resumed))
+                    for (int j = tag; j < L.level; j++) donor |= !(zeta & ((LOC_H0 >> j) - 1));
+                if (donor) break;
+                STEP_LEAF();
+            }
+        }
+        __syncwarp();
+        // ---- phase 2: donor duty: upstream face of refined ancestors entered now ----
+        if (donor) {
+            int saved = -1;
+            for (int j = tag; j < L.level; j++) {
+                const int hj = LOC_H0 >> j, hk = hj >> 1;
+                if (zeta & (hj - 1)) continue;
+                const int op = fp & ~(hj - 1), oq = fq & ~(hj - 1);
+                for (int dj = -3; dj <= 1; dj++)
+                    for (int di = -3; di <= 1; di++) {
+                        if (!((di | dj) & 1)) continue;  // member of the coarser lattice P_j
+                        const long long ap = (long long)fp + di * hk, aq = (long long)fq + dj * hk;
+                        long long zin = zeta, zout = zeta + hj, z;
+                        z = cross_of(D.T[0], Sp + op - ap); if (z > zin) zin = z;
+                        z = cross_of(D.T[1], Sq + oq - aq); if (z > zin) zin = z;
+                        z = cross_of(D.T[0], Sp + op + hj - ap); if (z < zout) zout = z;
+                        z = cross_of(D.T[1], Sq + oq + hj - aq); if (z < zout) zout = z;
+                        if (zout <= zin) continue;  // does not cross this cell
+                        int src = -1;               // -1: slot of this event
+                        if (zin == 0) {
+                            src = LOC_SRC_BG;
+                        } else {
+                            const long long zb = zin - 1;
+                            const long long pb = ap + shift_of(D, 0, zb) - Sp, qb = aq + shift_of(D, 1, zb) - Sq;
+                            const long long pi = ap + shift_of(D, 0, zin) - Sp, qi = aq + shift_of(D, 1, zin) - Sq;
+                            long long rpb, rqb, rdummy;
+                            const long long wpb = wrap_of(pb, Wp, rpb), wqb = wrap_of(qb, Wq, rqb);
+                            if (level_at(G, D, (int)zb, (int)rpb, (int)rqb) >= j + 1) continue;  // alive already
+                            if (wpb != wrap_of(pi, Wp, rdummy) || wqb != wrap_of(qi, Wq, rdummy)) src = LOC_SRC_BG;
+                        }
+                        if (saved < 0) {
+                            saved = j;
+                            just_saved = j;
+                            EMIT((unsigned)j, LOC_REC(LOC_OP_SAVE, 0, 0));
                             if (sp < LOC_BUILD_STACK) {
-                                Pending c;
-                                long long bb, bc;
-                                wrap_of(ap - Sp, Wp, bb);
-                                wrap_of(aq - Sq, Wq, bc);
-                                c.bp = (int)bb;
-                                c.bq = (int)bc;
-                                c.zeta = (int)zin;
-                                c.tag = (unsigned char)(j + 1);
-                                c.src = (unsigned char)(src == LOC_SRC_BG ? LOC_SRC_BG : saved);
-                                c.resumed = 0;
-                                c.pad = 0;
+                                Pending c = cur;
+                                c.zeta = (int)zeta;
+                                c.src = (unsigned char)j;
+                                c.resumed = 1;
                                 stack[sp++] = c;
                             } else
                                 *A.errflag = 1;
                         }
-                }
-                if (saved >= 0) break;  // children first; this ray resumes from the saved spectrum afterwards
+                        if (sp < LOC_BUILD_STACK) {
+                            Pending c;
+                            long long bb, bc;
+                            wrap_of(ap - Sp, Wp, bb);
+                            wrap_of(aq - Sq, Wq, bc);
+                            c.bp = (int)bb;
+                            c.bq = (int)bc;
+                            c.zeta = (int)zin;
+                            c.tag = (unsigned char)(j + 1);
+                            c.src = (unsigned char)(src == LOC_SRC_BG ? LOC_SRC_BG : saved);
+                            c.resumed = 0;
+                            c.pad = 0;
+                            stack[sp++] = c;
+                        } else
+                            *A.errflag = 1;
+                    }
             }
-            // ---- step through the leaf ----
-            const int h = LOC_H0 >> L.level;
-            long long znext = (zeta & ~(long long)(h - 1)) + h, z;
-            z = cross_of(D.T[0], Sp + (fp & ~(h - 1)) + h - fp); if (z < znext) znext = z;
-            z = cross_of(D.T[1], Sq + (fq & ~(h - 1)) + h - fq); if (z < znext) znext = z;
-            EMIT((unsigned)L.cell[L.level], LOC_REC(LOC_OP_STEP, L.level, (unsigned)(znext - zeta)));
-            nstep++;
-            zeta = znext;
-            first = false;
+            if (saved >= 0)
+                walking = false;  // children first; this ray resumes from the saved spectrum afterwards
+            else
+                STEP_LEAF();
         }
     }
-    while (nrec & (LOC_TASK_ALIGN - 1)) EMIT(0u, LOC_REC(LOC_OP_NOP, 0, 0));  // tasks are whole chunks of records
+#undef STEP_LEAF
 #undef EMIT
-    if (!A.emit) {
-        A.task_off[task] = nrec;
-        atomicAdd(A.nsteps, (unsigned long long)nstep);
-    }
 }
 
 // exclusive scan of counts[0..n) in place (one block), total written to counts[n]
