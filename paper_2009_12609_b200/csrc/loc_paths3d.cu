@@ -85,6 +85,9 @@ struct BuildArgs {
 // phase 2 -- after the warp has reconverged, the lanes that stopped for a donor event evaluate it together (the same 21
 // candidate positions each), then step.  Taken lane by lane inside one loop, the donor evaluation (~1300 instructions even
 // when it finds nothing) was paid by the whole warp in 9 of 10 iterations (C4: 6.9 s of set-up).
+// steps a lane may take in phase 1 before the warp looks at the donor events collected so far (C4 set-up: unlimited 2.74 s,
+// 24 -> 2.48 s, 8 -> 2.28 s: lanes that stopped early do not wait for the longest event-free run of the warp)
+#define LOC_BUILD_K 8
 __global__ void __launch_bounds__(128) k_build_paths(BuildArgs A)
 {
     const long long task = A.task_begin + blockIdx.x * (long long)blockDim.x + threadIdx.x;
@@ -166,7 +169,8 @@ __global__ void __launch_bounds__(128) k_build_paths(BuildArgs A)
         // ---- phase 1: leaf to leaf until the ray ends or may have donor duty ----
         bool donor = false;
         if (!finished) {
-            while (walking) {
+            int budget = LOC_BUILD_K;
+            while (walking && budget-- > 0) {
                 if (zeta >= Wz) {
                     walking = false;
                     break;
