@@ -1,0 +1,137 @@
+"""GPU parity on the edges of the method and of the library's limits, against the float64 oracle (same tolerances as
+the main parity tests): degenerate grids (two shells, a root grid of 2^3 cells, one root cell refined three times), bands narrower than a warp / than the 3D kernel's span,
+cells without gas, the largest transition count of one ray pass (LOC_MAX_TRANS = 12), level counts that take the
+generic shared-memory solver (7) and the local-memory solver (20 > 16), a single transition."""
+import numpy as np
+import pytest
+
+import loc_workloads as W
+import oracle as O
+from parity import check_pops, f32_pops_from_oracle_lte, oracle_SJ_ESC, rel_err
+from test_gpu_3d import small
+
+pytestmark = pytest.mark.gpu
+
+TOL_SJ = 1e-4
+TOL_POP = 1e-3
+
+
+def _model(m, **kw):
+    from paper_2009_12609_b200 import LocModel
+    return LocModel(m, **kw)
+
+
+def _leaf(m):
+    return (m.child < 0) if hasattr(m, "child") else np.ones(len(m.density), bool)
+
+
+def _resolve(m):
+    """narrow the band of a model with very few channels so that the line profile stays resolved (dv = sigma_turb / 2;
+    DESIGN 5.3: the window rule assumes dv <= sigma, as in every model of the paper): the lines then also run over the
+    edges of the band"""
+    m.band_half = 0.5 * m.nchannel * 0.5 * float(np.min(m.sigma))
+    return m
+
+
+def _counters_case(m, sel=None):
+    """first simulate from LTE: visits bit-exact, SJ / ESC within tolerance; returns nothing"""
+    sp = O.OSpecies(m.species)
+    is3d = hasattr(m, "child")
+    sel = np.arange(sp.ntrans, dtype=np.int32) if sel is None else np.asarray(sel, np.int32)
+    pops64, pops32 = f32_pops_from_oracle_lte(sp, m)
+    ref = O.sim_3d(sp, m, pops64, sel) if is3d else O.sim_1d(sp, m, pops64, sel)
+    sj_o, esc_o = oracle_SJ_ESC(sp, m, ref, sel)
+    g = _model(m, ntrans_sim=len(sel))
+    g.set_populations(pops32)
+    g.simulate(sel if len(sel) != sp.ntrans else None, geometry_counters=True)
+    sj, esc = g.counters()
+    vis, _ = g.geometry_counters()
+    sj, esc, vis = sj.cpu().numpy(), esc.cpu().numpy(), vis.cpu().numpy()
+    g.close()
+    leaf = _leaf(m)
+    assert np.array_equal(vis.astype(np.int64), ref["visits"])
+    gas = leaf & (np.asarray(m.density) * np.asarray(m.abundance) > 0)
+    assert rel_err(sj[leaf], sj_o[leaf]).max() < TOL_SJ
+    assert np.max(np.abs(esc[gas] - esc_o[gas]) / (np.abs(esc_o[gas]) + 3e-3)) < TOL_SJ
+
+
+def _iterate_case(m, niter, sel=None):
+    sp = O.OSpecies(m.species)
+    pops_o, _ = O.iterate(sp, m, niter, sel=sel)
+    g = _model(m, ntrans_sim=(len(sel) if sel is not None else None))
+    g.init_lte()
+    if sel is not None:
+        g.simulate(np.asarray(sel, np.int32))  # remember the selection
+        g.init_lte()
+    g.iterate(niter)
+    pg = g.pops.cpu().numpy()
+    g.close()
+    leaf = _leaf(m)
+    worst, small_abs = check_pops(pg[:, leaf], pops_o[leaf])
+    assert worst < TOL_POP and small_abs < 1e-10
+    return pg
+
+
+@pytest.mark.parametrize("cfg", [dict(which=1, ns=2, nchannel=16), dict(which=1, ns=2, nchannel=5), dict(which=1, ns=9, nchannel=4, nsub=2),
+                                 dict(which=2, ns=30, nchannel=33, nsub=1, nlevel=2)])
+def test_1d_degenerate_grids_and_bands(cfg):
+    m = W.shell_config(**cfg)
+    if m.nchannel < 16:
+        _resolve(m)
+    _counters_case(m)
+    _iterate_case(m, 3)
+
+
+@pytest.mark.parametrize("cfg", [dict(nroot=2, nlev=1, nside=1, nch=8), dict(nroot=2, nlev=1, nside=1, nch=4, nls=2),
+                                 dict(nroot=1, nlev=3, nside=1, nch=20, frac=1.0), dict(nroot=3, nlev=2, nside=2, nch=31, frac=0.5, nls=2)])
+def test_3d_degenerate_grids_and_bands(cfg):
+    m = small(**cfg)
+    if m.nchannel < 32:
+        _resolve(m)
+    _counters_case(m)
+    _iterate_case(m, 2)
+
+
+def test_cells_without_gas():
+    """density = 0 in a third of the cells: no opacity, no emission, populations stay 0; the other cells follow the oracle"""
+    m = W.shell_config(1, ns=24, nchannel=32)
+    m.density[::3] = 0.0
+    _counters_case(m)
+    pg = _iterate_case(m, 3)
+    assert np.all(pg[:, ::3] == 0.0)
+    m3 = small(nroot=4, nlev=2, nside=1, nch=32, frac=0.4)
+    leaf = np.flatnonzero(m3.child < 0)
+    m3.density[leaf[::3]] = 0.0
+    _counters_case(m3)
+    pg = _iterate_case(m3, 2)
+    assert np.all(pg[:, leaf[::3]] == 0.0)
+
+
+def test_max_transitions_and_local_memory_solver():
+    """20 levels (k_solve, the local-memory solver: more than 16 levels) with the first 12 of 19 transitions traced
+    (LOC_MAX_TRANS); the other 7 see the background only (DESIGN R23) on both sides"""
+    m = W.shell_config(2, ns=40, nchannel=64, nsub=2, nlevel=20)
+    sel = np.arange(12, dtype=np.int32)
+    _counters_case(m, sel)
+    _iterate_case(m, 3, sel)
+    m3 = small(which=4, nroot=4, nlev=2, nside=1, nch=32, frac=0.4, nls=13)  # 12 transitions, all traced in 3D
+    _counters_case(m3)
+    _iterate_case(m3, 2)
+
+
+@pytest.mark.parametrize("nlevel", [3, 7, 16])
+def test_generic_shared_memory_solver(nlevel):
+    """level counts without a compile-time instance of k_solve_s"""
+    m = W.shell_config(2, ns=30, nchannel=64, nsub=1, nlevel=nlevel)
+    sel = None if nlevel - 1 <= 12 else np.arange(12, dtype=np.int32)
+    _iterate_case(m, 3, sel)
+
+
+def test_default_selection_is_capped_by_the_model():
+    """a model created for 12 traced transitions of a 20-level species traces the first 12 by default"""
+    m = W.shell_config(2, ns=10, nchannel=32, nsub=1, nlevel=20)
+    g = _model(m, ntrans_sim=12)
+    g.init_lte()
+    g.simulate()
+    assert g.stats()["ntrans_sim"] == 12
+    g.close()
