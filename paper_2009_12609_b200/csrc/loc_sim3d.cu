@@ -621,8 +621,12 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
             const float qew = __shfl_sync(0xffffffffu, myqew, 8 * grp + 2 * r);
             const unsigned rb = rec_g + r * L::RECB;
             if (cls & LOC_RS_CTRL) {
-                // spectrum operations on the warp's own rows, executed by the whole warp for one group at a time
-                for (int g = 0; g < LOC_GROUPS; g++) {
+                // spectrum operations on the warp's own rows, executed by the whole warp for one group at a time; only the
+                // groups that have one are visited (their lanes hold the record's CTRL bit in `mode`)
+                unsigned cm = __ballot_sync(0xffffffffu, mode & LOC_RS_CTRL);
+                while (cm) {
+                    const int g = (__ffs(cm) - 1) >> 3;
+                    cm &= ~(0xffu << (8 * g));
                     const uint4 gh = lds128u(tb + L::OFF_REC + g * L::GSB + r * L::RECB + 16);
                     const unsigned gop = gh.z >> 24, gx = gh.x;
                     float *gs = sn_all + g * spec + row0;
@@ -630,7 +634,7 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
                     if (gop == LOC_OP_BG) {
                         for (int t = 0; t < O::NW; t++) {
                             const float bg = P.S.bgocc[P.slot0 + O::TB + t];
-                            for (int c = lane; c < nchp; c += 32) gs[t * nchp + c] = bg;
+                            for (int c = 4 * lane; c < nchp; c += 128) *reinterpret_cast<float4 *>(gs + t * nchp + c) = make_float4(bg, bg, bg, bg);
                         }
                     } else if (gop == LOC_OP_SAVE) {
                         for (int i = lane * 4; i < rown; i += 128) stg_keep(slot + i, *reinterpret_cast<const float4 *>(gs + i), pol_keep);
