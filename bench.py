@@ -30,8 +30,8 @@ DEFAULT_WORKLOAD = "C4"
 # ---- roofline constants -----------------------------------------------------------------------------
 N_SM = 148
 # DRAM bytes read + written by one launch of the dominant kernel, from the committed `ncu --set full` captures
-# (profiles/r1_v8_sim3d.md, profiles/r1_sim1d_C2.md); workloads without a capture report null
-NCU_TRAFFIC_BYTES = {"C2": 24.3e6, "C3": 19.08e9 + 7.88e9, "C4": 904.4e9 + 299.9e9}
+# (profiles/r1_v9_summary.md, profiles/r1_sim1d_C2.md); workloads without a capture report null
+NCU_TRAFFIC_BYTES = {"C2": 24.3e6, "C3": 19.09e9 + 7.88e9, "C4": 904.4e9 + 299.2e9}
 FP32_LANES_PER_SM_CLK = 128  # 4 sub-partitions x 1 warp instruction / clk
 MUFU_PER_SM_CLK = 16
 
