@@ -266,7 +266,7 @@ __global__ void __launch_bounds__(128) k_solve(int64_t n, SpeciesDev sp, Selecti
 // matrix of a thread is a column of a shared-memory array R[NL*NL][threads] of doubles (conflict free, never leaves the
 // SM), the species tables are staged in shared memory once per block, and NL is a compile-time constant for the common
 // level counts (NLX > 0), so that the elimination is fully unrolled with static addresses and x[], bz[] are registers.
-#define LOC_SOLVE_THREADS 64
+#define LOC_SOLVE_THREADS 32  // cells per block: 31 KB of matrices at 10 levels, 7 blocks per SM (64: 62 KB, 3 blocks = 6 warps; C3 1.50 -> 1.35 ms)
 struct SolveTabs {   // byte offsets into the block's shared memory, after R
     int g, energy, A, bg, gr, upper, lower, cu, cl, temps, rates, bytes;
 };
