@@ -184,6 +184,12 @@ int loc_iterate_until(loc_model *m, int max_iter, double tol, int *niter_done, d
 int loc_spectra(loc_model *m, int trans, const double *dir, int nx, int ny, const int64_t *aff,
                 const double *offsets_cm, float *dev_out);
 
+/* Excitation temperature of transition `trans` in every cell from the current populations (Fig. 4: the
+ * quantity whose change per iteration and per density bin the paper uses to judge convergence; the binning is left to
+ * the caller):  T_ex = -(h nu / k) / ln(n_u g_l / (n_l g_u)), K.  dev_tex: DEVICE float [ncell]; 0 in refined (non-leaf)
+ * cells and in cells without molecules.  Enqueued on the model's stream.                                        */
+int loc_tex(loc_model *m, int trans, float *dev_tex);
+
 /* Line-area map (Fig. 5c "line area"): W[p] = sum_c T_A[p][c] * dv, in K km/s, for npix spectra of the
  * model's nchannel channels as loc_spectra writes them.  dev_cube: DEVICE float [npix][nchannel] (K); dev_w: DEVICE
  * float [npix].  Enqueued on the model's stream; npix = 0 is a no-op.                                          */

@@ -19,7 +19,7 @@ LOC_GRID_SHELL, LOC_GRID_OCTREE = 1, 2
 
 SYMBOLS = ("loc_workspace_bytes", "loc_create_model", "loc_set_species", "loc_refresh_cells", "loc_set_directions", "loc_set_populations",
            "loc_init_lte", "loc_simulate", "loc_get_counters", "loc_solve", "loc_iterate", "loc_set_ali",
-           "loc_iterate_until", "loc_spectra", "loc_line_area",
+           "loc_iterate_until", "loc_spectra", "loc_line_area", "loc_tex",
            "loc_get_stats", "loc_destroy_model", "loc_last_error")
 
 
@@ -81,6 +81,7 @@ def lib():
         L.loc_set_ali.argtypes = [C.c_void_p, C.c_int]
         L.loc_iterate_until.argtypes = [C.c_void_p, C.c_int, C.c_double, C.POINTER(C.c_int), C.POINTER(C.c_double)]
         L.loc_spectra.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.loc_tex.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
         L.loc_line_area.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]
         L.loc_get_stats.argtypes = [C.c_void_p, C.POINTER(loc_stats)]
         L.loc_destroy_model.argtypes = [C.c_void_p]
@@ -197,6 +198,10 @@ def loc_iterate(h, niter: int) -> float:
     r = C.c_double(0.0)
     _check(lib().loc_iterate(h, int(niter), C.byref(r)), h)
     return r.value
+
+
+def loc_tex(h, trans: int, dev_tex) -> None:
+    _check(lib().loc_tex(h, int(trans), _dp(dev_tex)), h)
 
 
 def loc_line_area(h, dev_cube, npix: int, dev_w) -> None:

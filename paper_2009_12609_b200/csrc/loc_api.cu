@@ -936,6 +936,32 @@ extern "C" int loc_spectra(loc_model *m, int trans, const double *dir, int nx, i
     return loc_launch_spectra(m, trans, dir, nx, ny, aff, offsets_cm, dev_out);
 }
 
+// T_ex = -(h nu / k) / ln(n_u g_l / (n_l g_u)) per cell (Fig. 4); 0 where the cell holds no molecules
+__global__ void k_tex(int64_t n, const float *pop_u, const float *pop_l, double gl_over_gu, double hnu_over_k, const int32_t *child, float *out)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float t = 0.0f;
+    const double nu_ = pop_u[i], nl_ = pop_l[i];
+    if (!(child && child[i] >= 0) && nu_ > 0.0 && nl_ > 0.0) t = (float)(-hnu_over_k / log(nu_ * gl_over_gu / nl_));
+    out[i] = t;
+}
+
+extern "C" int loc_tex(loc_model *m, int trans, float *dev_tex)
+{
+    if (!m || !dev_tex) return LOC_EINVAL;
+    if (!m->have_species || !m->pops) return fail(m, LOC_ESTATE, "species and populations must be set before loc_tex");
+    if (trans < 0 || trans >= m->ntrans) return fail(m, LOC_EINVAL, "loc_tex: bad transition");
+    const int u = m->h_upper[trans], l = m->h_lower[trans];
+    const int64_t n = m->ncell;
+    k_tex<<<(unsigned)((n + 255) / 256), 256, 0, m->stream>>>(n, m->pops + (int64_t)u * n, m->pops + (int64_t)l * n, m->h_g[l] / m->h_g[u],
+                                                              LOC_HP * m->h_freq[trans] / LOC_KB,
+                                                              m->kind == LOC_GRID_OCTREE ? m->child : nullptr, dev_tex);
+    m->launches++;
+    LOC_CUDA_CHECK(m, cudaGetLastError());
+    return LOC_OK;
+}
+
 extern "C" int loc_line_area(loc_model *m, const float *dev_cube, int64_t npix, float *dev_w)
 {
     if (!m || npix < 0 || (npix > 0 && (!dev_cube || !dev_w))) return LOC_EINVAL;

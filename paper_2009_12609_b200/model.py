@@ -123,6 +123,12 @@ class LocModel:
         B.loc_spectra(self.h, trans, out, nx, ny, dir, aff, offsets_cm)
         return out
 
+    def tex(self, trans):
+        """T_ex [ncell] (K) of a transition from the current populations; 0 in non-leaf cells / cells without molecules"""
+        out = torch.empty(self.ncell, dtype=torch.float32, device=self.dev)
+        B.loc_tex(self.h, trans, out)
+        return out
+
     def line_area(self, cube):
         """W = sum_c T_A dv in K km/s for a cube [..., nchannel] of loc_spectra (float32 CUDA tensor)"""
         cube = cube.contiguous()

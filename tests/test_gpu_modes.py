@@ -110,3 +110,31 @@ def test_mode_calls_reject_bad_arguments():
     assert lib.loc_iterate_until(g.h, -1, C.c_double(1e-3), None, None) == B.LOC_EINVAL
     assert lib.loc_iterate_until(g.h, 1, C.c_double(-1.0), None, None) == B.LOC_EINVAL
     g.close()
+
+
+def test_tex_per_cell():
+    """loc_tex against the oracle's T_ex (O.tex, pinned by the LTE limit P3): from LTE populations it returns T_kin, after
+    iterations it follows the oracle's populations; refined cells and cells without gas give 0"""
+    m = small(nroot=4, nlev=2, nside=1, nch=32, frac=0.4)
+    leaf = m.child < 0
+    empty = np.flatnonzero(leaf)[::5]
+    m.density[empty] = 0.0
+    gas = leaf & (m.density > 0)
+    sp = O.OSpecies(m.species)
+    g = _model(m)
+    g.init_lte()
+    for t in range(sp.ntrans):
+        te = g.tex(t).cpu().numpy()
+        assert np.max(np.abs(te[gas] - m.tkin[gas]) / m.tkin[gas]) < 2e-5  # float32 populations
+        assert np.all(te[~gas] == 0.0)
+    g.iterate(3)
+    pops_o, _ = O.iterate(sp, m, 3)
+    for t in range(sp.ntrans):
+        u, l = m.species.upper[t], m.species.lower[t]
+        ref = np.array([O.tex(sp, t, pops_o[c, u], pops_o[c, l]) for c in np.flatnonzero(gas)])
+        te = g.tex(t).cpu().numpy()[gas]
+        assert rel_err(te, ref).max() < TOL_POP
+    from paper_2009_12609_b200 import binding as B
+    with pytest.raises(B.LocError):
+        g.tex(99)
+    g.close()
