@@ -161,7 +161,7 @@ __global__ void __launch_bounds__(1024) k_sim1d(Sim1D P)
 // kinematics and line coefficients are loaded one step ahead.  Same per-channel arithmetic (channel_update), same
 // window rule and wing term as k_sim1d.
 // ------------------------------------------------------------------------------------------------------------------
-#define LOC_1D_WARPS 2  // rays per block
+#define LOC_1D_WARPS 1  // rays per block (C2: 1 -> 3.80 ms, 2 -> 4.15 ms, 4 -> 4.13 ms: 24 instead of 22 resident rays per SM, finer scheduling)
 
 struct Step1D {
     int k;
