@@ -109,3 +109,41 @@ def test_error_paths():
     bad.r_out = bad.r_out[::-1].copy()
     with pytest.raises(B.LocError):
         _model(bad)
+
+
+def test_full_size_C2_invariants_and_enclosure():
+    """BASELINE size, the launch configuration bench.py times (C2: 1000 shells, 4000 rays, 256 channels, 9 transitions,
+    k_sim1d_w).  The oracle needs minutes per iteration at this size, so properties that hold at any size are checked:
+      * every ray visits the shells of its path once in and once out: total visits = sum over rays of 2 (NS - 1 - k0) + 1
+        = the library's step count, and shell k is visited by every ray whose tangent shell lies at or inside it;
+      * pin P4 (blackbody enclosure): with T_bg = T_kin everywhere, one ALI iteration from LTE leaves the populations
+        unchanged -- every normalisation of the ray weights, path lengths and counters enters;
+      * escape fractions lie in (0, 1], counters are finite."""
+    m = W.shell_config(2)
+    m.tkin[:] = 10.0
+    m.t_bg = 10.0
+    g = _model(m)
+    g.init_lte()
+    g.simulate(geometry_counters=True)
+    vis, _ = g.geometry_counters()
+    vis = vis.cpu().numpy().astype(np.int64)
+    st = g.stats()
+    k0 = np.searchsorted(m.r_out, m.ray_p, side="right")  # tangent shell of each ray: first shell whose outer radius exceeds p
+    ns = len(m.r_out)
+    inside = k0 < ns
+    expect = np.zeros(ns, np.int64)
+    for k in k0[inside]:
+        expect[k] += 1
+        expect[k + 1:] += 2
+    assert np.array_equal(vis, expect)
+    assert vis.sum() == st["steps"] == int(np.sum(2 * (ns - 1 - k0[inside]) + 1))
+    sj, esc = g.counters()
+    sj, esc = sj.cpu().numpy(), esc.cpu().numpy()
+    assert np.isfinite(sj).all() and np.isfinite(esc).all()
+    assert esc.min() > 0 and esc.max() <= 1.0 + 1e-5
+    p0 = g.pops.clone()
+    change = g.iterate(1)
+    p1, p0 = g.pops.cpu().numpy(), p0.cpu().numpy()
+    g.close()
+    big = p0 > 1e-10 * p0.sum(axis=0, keepdims=True)
+    assert np.max(np.abs(p1 - p0)[big] / p0[big]) < 5e-5 and change < 5e-5
