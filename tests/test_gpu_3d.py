@@ -128,14 +128,17 @@ def test_blackbody_enclosure_gpu():
     assert np.max(np.abs(p1 - p0) / p0) < 2e-5 and change < 2e-5
 
 
-def test_full_size_path_invariant_and_enclosure():
-    """BASELINE size, the launch configuration bench.py times (C3: 128^3, 48 directions, 128 channels, 9 transitions).
+@pytest.mark.parametrize("which", [3, 4])
+def test_full_size_path_invariant_and_enclosure(which):
+    """BASELINE size, the launch configuration bench.py times (C3: 128^3, 48 directions, 128 channels, 9 transitions; C4, the
+    default workload of the bench: octree root 64^3 + 3 levels, 36.6 M cells, ray births and donor spectra included).
     The oracle cannot run this size inside a test, so properties that hold at any size are checked instead:
       * pin P7: every leaf's summed main-axis path is h_l * NDIR exactly (integer), total visits = steps of the stream;
       * pin P4: with T_bg = T_kin one ALI iteration from LTE leaves the populations unchanged (all normalisations);
       * the escape fractions of an iteration lie in (0, 1] and the counters are finite."""
-    m = W.cloud_config(3)
-    m.t_bg = 10.0  # = T_kin of C3: blackbody enclosure
+    m = W.cloud_config(which)
+    m.tkin[:] = 10.0
+    m.t_bg = 10.0  # = T_kin: blackbody enclosure
     g = _model(m)
     g.init_lte()
     g.simulate(geometry_counters=True)
