@@ -18,9 +18,21 @@
  * Pins (tests/test_oracle_*.py): slab closed form, optically thin limit, LTE
  * limit, blackbody enclosure, two-level closed form, photon ledger, path
  * invariants, ALI == Lambda fixed point, brute-force ray/box geometry, full
- * refinement == finer grid, mirror symmetry, GTH cross-check of the solver.
- * Parity unpinned: none of the functions below (absolute T_ex profiles of the
- * paper's figures are not reproducible: their inputs are not available).
+ * refinement == finer grid, mirror symmetry, GTH cross-check of the solver;
+ * since round 2 also: collision-rate interpolation against numpy.interp
+ * (nodes, midpoints, clamps), the untraced-transition branch of orc_solve
+ * (two-level closed form with nsel = 0; thin limit), the entry cosine of the
+ * 1D path (mu r_entry = ray abscissa), the donor spectrum at ray births on a
+ * layered model with partial refinement (every level's leaves == the uniform
+ * Cartesian grid of that resolution), the thick closed form of orc_spectra_1d,
+ * 90-degree rotation / z-mirror of the direction set in 3D.
+ * Parity unpinned: none of the functions below.  One READING stays constrained
+ * by invariants only (blackbody enclosure P4, ledger P6): at a SIDE-face birth
+ * the donor is the line that entered the level-(tag-1) ancestor through its
+ * upstream face (R9/R10) -- the paper's text fixes no
+ * more than that, and no closed form distinguishes the transverse choice.
+ * (Absolute T_ex profiles of the paper's figures are not reproducible: their
+ * inputs are not available.)
  */
 #include <math.h>
 #include <stdint.h>

@@ -259,3 +259,178 @@ def test_P9_line_area_closed_forms():
     assert abs(W[1] - 2.0 * W[0]) < 1e-14 * W[1]
     assert abs(W[2] - T0 * 12.0) < 1e-12 * W[2]
     assert O.line_area(np.zeros((3, 2, nch)), dv).shape == (3, 2)
+
+
+# ----------------------------------------------------------------------------------------------------------------------
+# round 2: the parts of the oracle that no test reached (VERDICT r1 "parity unpinned" list)
+# ----------------------------------------------------------------------------------------------------------------------
+def _species_ntemp(nlevel, temps, config=1, spread=3.0):
+    """rotor with a temperature-dependent collision table: row j = base rates times a per-pair factor that differs
+    from row to row (so that a swapped weight or an off-by-one row cannot cancel)"""
+    s = W.rotor_species(nlevel, config)
+    rs = np.random.default_rng([77, nlevel, len(temps)])
+    base = s.rate_down[0]
+    rows = [base * rs.uniform(1.0 / spread, spread, size=base.shape) for _ in temps]
+    s.temps_K = np.asarray(temps, float)
+    s.rate_down = np.stack(rows)
+    return s
+
+
+def test_coll_gamma_interpolation_nodes_midpoints_clamps():
+    """R18 / PAPER.md:161 (LAMDA tables): downward rate coefficients are tabulated at a few temperatures; the oracle
+    interpolates linearly in T and clamps outside.  With S = 0 and beta = 0 the rate matrix holds n*gamma_ul(T) alone in
+    its u->l entries, so gamma(T) is read off orc_rate_matrix and compared with numpy.interp (clamped linear
+    interpolation, a library routine) on an UNEVENLY spaced 4-node table: node -> that row exactly, midpoint -> the
+    arithmetic mean, quarter point -> 3:1 weights, outside -> the end rows.  A swapped weight f / 1-f, an off-by-one in
+    the row index, or a missing clamp fails here."""
+    temps = [10.0, 20.0, 50.0, 55.0]
+    s = _species_ntemp(4, temps)
+    os_ = O.OSpecies(s)
+    n = 1e5
+    nt = s.ntrans
+    for T in (10.0, 20.0, 50.0, 55.0, 15.0, 35.0, 27.5, 52.5, 51.25, 3.0, 9.999, 55.001, 300.0):
+        R = O.rate_matrix(os_, n, T, np.zeros(nt), np.zeros(nt))
+        got = np.array([R[u, l] for u, l in zip(s.cu, s.cl)]) / n
+        expect = np.array([np.interp(T, temps, s.rate_down[:, k]) for k in range(len(s.cu))])
+        assert np.max(np.abs(got / expect - 1)) < 1e-14, T
+        # upward by detailed balance from the SAME interpolated coefficient
+        up = np.array([R[l, u] for u, l in zip(s.cu, s.cl)]) / n
+        db = expect * s.g[s.cu] / s.g[s.cl] * np.exp(-(s.energy_K[s.cu] - s.energy_K[s.cl]) / T)
+        assert np.max(np.abs(up / db - 1)) < 1e-13, T
+    # the rows really differ (the test has teeth): midpoint differs from both neighbours by > 5 % for some pair
+    assert np.max(np.abs(s.rate_down[1] / s.rate_down[2] - 1)) > 0.05
+    # exact statements, not through interp: node returns the node row bit for bit, midpoint the arithmetic mean
+    R = O.rate_matrix(os_, 1.0, 20.0, np.zeros(nt), np.zeros(nt))
+    assert all(R[u, l] == s.rate_down[1, k] for k, (u, l) in enumerate(zip(s.cu, s.cl)))
+    R = O.rate_matrix(os_, 1.0, 35.0, np.zeros(nt), np.zeros(nt))
+    assert all(abs(R[u, l] - 0.5 * (s.rate_down[1, k] + s.rate_down[2, k])) < 1e-26 for k, (u, l) in enumerate(zip(s.cu, s.cl)))
+
+
+def test_two_level_closed_form_at_interpolated_temperature():
+    """P5 with a 3-node collision table: shells at T between the nodes, at a node and outside the table; the closed
+    form n_u/n_l = (S + C_lu)/(A + S g_l/g_u + C_ul) uses numpy.interp for gamma(T).  Goes through orc_solve."""
+    temps = [8.0, 12.0, 30.0]
+    s = _species_ntemp(2, temps)
+    os_ = O.OSpecies(s)
+    m = W.shell_config(2, ns=12, nchannel=64, nsub=1)
+    m.species = s
+    m.tkin[:] = np.array([5, 8, 9, 10, 11, 12, 14, 21, 29, 30, 33, 60], np.float32)
+    m.abundance[:] = 1e-14  # thin
+    m.density[:] = np.float32(3e3)  # collisions comparable with A (n gamma ~ A): the ratio depends on gamma(T)
+    pops, _ = O.iterate(os_, m, 3)
+    nu = os_.freq(0)
+    A = s.einstein_A[0]
+    gr = s.g[1] / s.g[0]
+    S = gr * A / math.expm1(H * nu / (K * m.t_bg))
+    seen = []
+    for k in range(12):
+        n, T = float(m.density[k]), float(m.tkin[k])
+        Cul = n * np.interp(T, temps, s.rate_down[:, 0])
+        Clu = Cul * gr * math.exp(-(s.energy_K[1] - s.energy_K[0]) / T)
+        ratio = (S + Clu) / (A + S / gr + Cul)
+        assert abs(pops[k, 1] / pops[k, 0] / ratio - 1) < 2e-5
+        seen.append(Cul / A)
+    assert 0.05 < min(seen) and max(seen) < 20  # neither radiatively nor collisionally dominated
+
+
+def test_R23_untraced_transitions_see_the_background_only(sp5):
+    """R23 ("the number of transitions for which RT computations are actually performed"):
+    a transition that is not ray traced enters the solve with S = (g_u/g_l) A / (e^{h nu/k T_bg} - 1) and beta = 1.
+    (i) two levels, NO transition traced (nsel = 0): the solve alone must give P5's closed form, to rounding;
+    (ii) five levels in the optically thin limit: tracing only 1-0, tracing nothing and tracing everything agree to
+         O(tau), because every traced transition then also sees the background only;
+    (iii) T_bg = 0: the untraced S vanishes and an untraced two-level system relaxes to the collisional/radiative
+          ratio C_lu / (A + C_ul)."""
+    s2 = W.rotor_species(2, 1)
+    o2 = O.OSpecies(s2)
+    nu = o2.freq(0)
+    A, gr = s2.einstein_A[0], s2.g[1] / s2.g[0]
+    dens, tk, ab = np.array([2e3, 5e4, 1e6]), np.array([9.0, 14.0, 30.0]), np.full(3, 1e-6)
+    for tbg in (2.73, 15.0, 0.0):
+        pops = O.lte(o2, dens, tk, ab)
+        none = np.zeros(0, np.int32)
+        O.solve(o2, dens, tk, ab, np.ones(3), none, np.zeros((0, 3)), np.zeros((0, 3)), 1e3, tbg, pops)
+        S = gr * A / math.expm1(H * nu / (K * tbg)) if tbg > 0 else 0.0
+        for k in range(3):
+            Cul = dens[k] * s2.rate_down[0, 0]
+            Clu = Cul * gr * math.exp(-(s2.energy_K[1] - s2.energy_K[0]) / tk[k])
+            assert abs(pops[k, 1] / pops[k, 0] / ((S + Clu) / (A + S / gr + Cul)) - 1) < 1e-12
+            assert abs(pops[k].sum() / (dens[k] * ab[k]) - 1) < 1e-14
+    # (ii)
+    s, os_ = sp5
+    m = W.shell_config(1, ns=10, nchannel=64)
+    m.abundance[:] = 1e-13
+    p_all, _ = O.iterate(os_, m, 2)
+    p_one, _ = O.iterate(os_, m, 2, sel=[0])
+    p_two, _ = O.iterate(os_, m, 2, sel=[1, 3])
+    p_none, _ = O.iterate(os_, m, 2, sel=np.zeros(0, np.int32))
+    for p in (p_one, p_two, p_none):
+        assert np.max(np.abs(p / p_all - 1)) < 3e-5  # O(tau) + the band tails of the traced lines
+    assert np.max(np.abs(p_none / O.lte(os_, m.density, m.tkin, m.abundance) - 1)) > 0.1  # far from LTE: the test has teeth
+    # a thick model separates them: the untraced transition keeps beta = 1 while the traced one is trapped
+    m.abundance[:] = 1e-4
+    m.density *= 10
+    q_all, _ = O.iterate(os_, m, 2)
+    q_one, _ = O.iterate(os_, m, 2, sel=[0])
+    assert np.max(np.abs(q_one / q_all - 1)) > 1e-2
+
+
+def test_P7_entry_cosine_times_radius_is_the_ray_abscissa():
+    """O7 / PAPER.md:137 ("Doppler shifts are evaluated only at the beginning of each step"): along a ray with impact
+    parameter p the abscissa is x = -sqrt(R^2 - p^2) + (path so far); at the entry point of step j, at radius r_entry,
+    the cosine between the ray and the outward radial direction is mu = x / r_entry.  r_entry is the OUTER radius r_k of
+    an inbound shell (and of the tangent shell) and the INNER radius r_{k-1} of an outbound shell.  Pins the magnitude of
+    mu (the sign alone is P7): taking r_{k-1} inbound, r_k outbound, or the exit point fails."""
+    for which, ns, nsub in ((1, 24, 3), (2, 40, 2)):
+        m = W.shell_config(which, ns=ns, nsub=nsub)
+        r = m.r_out
+        R = r[-1]
+        for p in m.ray_p:
+            sh, s, mu = O.path_1d(r, p)
+            k0 = int(sh.min())
+            nin = ns - 1 - k0
+            x = -math.sqrt(R * R - p * p) + np.concatenate([[0.0], np.cumsum(s)[:-1]])
+            r_entry = np.array([r[k] for k in sh[:nin + 1]] + [r[k - 1] for k in sh[nin + 1:]])
+            assert np.max(np.abs(mu * r_entry - x)) < 1e-12 * R
+            assert np.all(np.abs(mu) <= 1.0)
+        # the magnitudes matter: cosines of one ray span (0, 1)
+        sh, s, mu = O.path_1d(r, m.ray_p[len(m.ray_p) // 3])
+        assert np.abs(mu).min() < 0.6 and np.abs(mu).max() > 0.99
+
+
+def test_spectra_1d_thick_uniform_sphere_closed_form():
+    """P1 for orc_spectra_1d in the optically THICK regime (the thin limit is P2): a uniform sphere at rest is a
+    homogeneous slab of length 2 sqrt(R^2 - b^2) along the line of sight at impact parameter b:
+    T_A(c) = (h nu / k)(S - n_bg)(1 - e^{-tau_c}), tau_c = kappa phi_c 2 sqrt(R^2 - b^2), written with the textbook
+    Einstein-B absorption coefficient.  Catches a wrong source function, a missing 1 - e^-tau, a wrong path."""
+    s = W.rotor_species(4, 1)
+    os_ = O.OSpecies(s)
+    m = W.shell_config(1, ns=9, nchannel=72)
+    m.species = s
+    m.density[:] = 4e4
+    m.tkin[:] = 13.0
+    m.sigma[:] = 0.18e5
+    m.vrad[:] = 0.0
+    m.abundance[:] = 3e-5
+    pops = O.lte(os_, m.density, m.tkin, m.abundance)
+    pops[:, 1] *= 0.8  # sub-thermal upper level: S differs from B(T_kin)
+    dv = 2 * m.band_half / m.nchannel
+    R = m.r_out[-1]
+    b = np.array([0.0, 0.31, 0.77, 0.999]) * R
+    for t in (0, 1):
+        TA = O.spectra_1d(os_, m, pops, t, b)
+        u, l = s.upper[t], s.lower[t]
+        sigma = math.sqrt(0.18e5 ** 2 + K * 13.0 / (s.mass_amu * 1.66053906660e-24))
+        phi = O.profile(m.nchannel, dv, sigma, 0.0)
+        kap, nu = _einstein_kappa(s, t, pops[0, u], pops[0, l], phi, dv)
+        S_occ = 1.0 / (pops[0, l] * s.g[u] / (pops[0, u] * s.g[l]) - 1.0)
+        bg_occ = 1.0 / math.expm1(H * nu / (K * m.t_bg))
+        for i, bi in enumerate(b):
+            tau = kap * 2.0 * math.sqrt(R * R - bi * bi)
+            expect = H * nu / K * (S_occ - bg_occ) * -np.expm1(-tau)
+            assert np.max(np.abs(TA[i] - expect)) < 1e-11 * np.max(np.abs(expect))
+        tau0 = (kap * 2.0 * R).max()
+        assert tau0 > 20.0, tau0  # thick: the line is saturated at the centre ...
+    assert abs(TA[0, 36] / (H * nu / K * (S_occ - bg_occ)) - 1) < 1e-6  # ... T_A = (h nu/k)(S - n_bg) there
+    # outside the cloud: no line
+    assert np.all(O.spectra_1d(os_, m, pops, 0, np.array([1.5 * R])) == 0.0)
