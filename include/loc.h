@@ -35,6 +35,8 @@ extern "C" {
 #define LOC_ESTATE (-2) /* call order (species / directions / populations not set)                      */
 #define LOC_ENOMEM (-3) /* workspace too small                                                          */
 #define LOC_ECUDA (-4)  /* CUDA error; text in loc_last_error()                                        */
+#define LOC_ENONFINITE (-5) /* loc_solve / loc_iterate* produced a NaN or infinite population (T_kin <= 0, NaN inputs):
+                               max_rel_change is +inf; never reported as "converged"                      */
 
 #define LOC_GRID_SHELL 1  /* 1D spherically symmetric shells   */
 #define LOC_GRID_OCTREE 2 /* 3D octree; a Cartesian grid is nlevel = 1 */
@@ -42,6 +44,18 @@ extern "C" {
 #define LOC_MAX_TRANS 12  /* radiative transitions ray traced together in one pass */
 #define LOC_MAX_LEVELS 32 /* energy levels of the species                           */
 #define LOC_MAX_TREE_LEVELS 6
+#define LOC_MAX_DIRECTIONS 65535 /* ray directions of one model (loc_set_directions)                    */
+
+/* Keys of loc_set_option.  The library reads NO environment variables: every knob that can change a result or a launch
+ * configuration is an argument of this call (defaults in parentheses; DESIGN.md 5.3 derives them).                    */
+#define LOC_OPT_WINDOW_XMIN 1    /* (4.5) 1D kernel and the masked path of the 3D kernel: channels within X sigma of the line
+                                    centre are updated, X^2 = xmin^2 + 2 ln max(1, dv/sigma)^2 (+ the optical-depth term)  */
+#define LOC_OPT_WINDOW_EPS_TAU 2 /* (1e-6) 1D kernel: X >= sqrt(2 ln(tau0 / eps_tau)), tau0 = largest line-centre optical
+                                    depth of the step                                                                     */
+#define LOC_OPT_SPAN_XCLIP 3     /* (3.4) 3D kernel: a step whose 32-channel span does not reach X sigma, X^2 = xclip^2 +
+                                    2 ln max(1, tau0), takes two spans or the masked path                               */
+#define LOC_OPT_SIM3D_PARTS 4    /* (0 = automatic) 3D kernel: split the traced transitions over at least this many launches */
+#define LOC_OPT_SOLVER_LOCAL 5   /* (0) 1 = use the local-memory solver for every level count (A/B measurements)          */
 
 typedef struct loc_model loc_model; /* opaque */
 
@@ -117,7 +131,9 @@ int loc_set_species(loc_model *m, int nlevel, const double *energy_K, const doub
 int loc_refresh_cells(loc_model *m);
 
 /* Octree only: ray directions (unit vectors, host [ndir][3]; PAPER.md:93 uses HEALPix centres).  Each is
- * snapped to the library's fixed-point slopes (DESIGN R7); ndir <= the ndir_max given to loc_workspace_bytes.
+ * snapped to the library's fixed-point slopes (DESIGN R7); ndir <= the ndir_max given to loc_workspace_bytes
+ * (<= LOC_MAX_DIRECTIONS).  On failure (LOC_ENOMEM: the message names the number of 8-byte records the step stream
+ * needs; LOC_ECUDA) the model is left WITHOUT directions and loc_simulate returns LOC_ESTATE until a later call succeeds.
  * This call also runs the path set-up: every root-grid ray and the rays born from it in refined regions
  * are traced once with integer arithmetic and stored in the workspace as a step stream
  * (cell index, path length) that loc_simulate replays every iteration -- the 3D counterpart of the pre-calculated
@@ -152,13 +168,15 @@ int loc_simulate(loc_model *m, int nsel, const int *trans_idx, int geometry_coun
 int loc_get_counters(loc_model *m, const float **counters, int *ntrans_padded, const uint32_t **visits,
                      const uint32_t **pathz);
 
-/* Per-cell statistical equilibrium: S_lu = (g_u/g_l) A SJ replaces B_lu I, A_ul is scaled by
+/* Per-cell statistical equilibrium; LOC_ESTATE before the first loc_simulate (the counters hold nothing),
+ * LOC_ENONFINITE if a population came out NaN / infinite.  S_lu = (g_u/g_l) A SJ replaces B_lu I, A_ul is scaled by
  * ESC, collisions from `density` and `tkin`; transitions that were not traced see the background only
  * (DESIGN R23).  Writes the new populations into the registered buffer and refreshes the line coefficients.
  * max_rel_change (host, may be NULL): largest relative change over levels holding >= 1e-10 of the molecules. */
 int loc_solve(loc_model *m, double *max_rel_change);
 
-/* niter x (loc_simulate with the remembered selection; loc_solve); no early exit.          */
+/* niter x (loc_simulate with the remembered selection; loc_solve); no early exit.  niter = 0 runs nothing
+ * and reports a change of 0.                                                                              */
 int loc_iterate(loc_model *m, int niter, double *max_rel_change);
 
 /* ali = 1 (default): accelerated lambda iteration -- loc_solve scales A_ul by the escape probability ESC and uses the
@@ -168,6 +186,12 @@ int loc_iterate(loc_model *m, int niter, double *max_rel_change);
  * with, are added to SJ.  Both modes share loc_simulate and its counters and have the same fixed point; only
  * loc_solve differs.  Returns LOC_EINVAL for any other value.                                                */
 int loc_set_ali(loc_model *m, int ali);
+
+/* Accuracy / launch knobs (keys LOC_OPT_* above).  LOC_EINVAL for an unknown key or a value outside the key's range.
+ * Channel widths: the kernels need no minimum resolution of the line profile -- with channels wider than the line
+ * (dv > sigma) the sampled profile of PAPER.md:73 is no longer normalised, and the kernels then sum the sampled values
+ * themselves instead of using the analytic wing mass, and widen the window by 2 ln (dv/sigma)^2.     */
+int loc_set_option(loc_model *m, int key, double value);
 
 /* Convergence-controlled iteration ("repeated until the level populations converge"):
  * (loc_simulate; loc_solve) until max_rel_change <= tol or max_iter iterations were done.  niter_done (host, may be
@@ -183,6 +207,18 @@ int loc_iterate_until(loc_model *m, int max_iter, double tol, int *niter_done, d
  * Shells: dir = NULL, ny = 1, pixel ix is the line of sight with impact parameter offsets_cm[ix] (host).   */
 int loc_spectra(loc_model *m, int trans, const double *dir, int nx, int ny, const int64_t *aff,
                 const double *offsets_cm, float *dev_out);
+
+/* The same map in the CALLER's frame (octree models; "pixel = smallest cell"): model coordinates in cm with
+ * the origin at the corner of root cell (0,0,0).  `dir` (host double[3], unit) is the direction the photons travel, i.e.
+ * from the far side of the model towards the observer.  The image plane is spanned by e2 = the unit projection of "north"
+ * perpendicular to dir (north = +z; +y when dir is parallel to z within 1e-9) and e1 = e2 x dir; pixel (ix, iy), ix fastest,
+ * is the line of sight through
+ *     X(ix, iy) = centre_cm + (ix - (nx-1)/2) pixel_cm e1 + (iy - (ny-1)/2) pixel_cm e2 .
+ * (dir = +z: e1 = +x, e2 = +y.)  The library snaps dir to its fixed-point slopes (DESIGN R7) and converts X to the integer
+ * start position on the upstream face; lines of sight that miss the model return the zero spectrum.
+ * dev_out: DEVICE float [ny][nx][nchannel] (K).                                                                         */
+int loc_spectra_map(loc_model *m, int trans, const double *dir, int nx, int ny, double pixel_cm, const double *centre_cm,
+                    float *dev_out);
 
 /* Excitation temperature of transition `trans` in every cell from the current populations (Fig. 4: the
  * quantity whose change per iteration and per density bin the paper uses to judge convergence; the binning is left to

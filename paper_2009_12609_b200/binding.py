@@ -14,12 +14,13 @@ import numpy as np
 
 from . import build as _build
 
-LOC_OK, LOC_EINVAL, LOC_ESTATE, LOC_ENOMEM, LOC_ECUDA = 0, -1, -2, -3, -4
+LOC_OK, LOC_EINVAL, LOC_ESTATE, LOC_ENOMEM, LOC_ECUDA, LOC_ENONFINITE = 0, -1, -2, -3, -4, -5
+LOC_OPT_WINDOW_XMIN, LOC_OPT_WINDOW_EPS_TAU, LOC_OPT_SPAN_XCLIP, LOC_OPT_SIM3D_PARTS, LOC_OPT_SOLVER_LOCAL = 1, 2, 3, 4, 5
 LOC_GRID_SHELL, LOC_GRID_OCTREE = 1, 2
 
 SYMBOLS = ("loc_workspace_bytes", "loc_create_model", "loc_set_species", "loc_refresh_cells", "loc_set_directions", "loc_set_populations",
            "loc_init_lte", "loc_simulate", "loc_get_counters", "loc_solve", "loc_iterate", "loc_set_ali",
-           "loc_iterate_until", "loc_spectra", "loc_line_area", "loc_tex",
+           "loc_set_option", "loc_iterate_until", "loc_spectra", "loc_spectra_map", "loc_line_area", "loc_tex",
            "loc_get_stats", "loc_destroy_model", "loc_last_error")
 
 
@@ -81,6 +82,8 @@ def lib():
         L.loc_set_ali.argtypes = [C.c_void_p, C.c_int]
         L.loc_iterate_until.argtypes = [C.c_void_p, C.c_int, C.c_double, C.POINTER(C.c_int), C.POINTER(C.c_double)]
         L.loc_spectra.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.loc_set_option.argtypes = [C.c_void_p, C.c_int, C.c_double]
+        L.loc_spectra_map.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_void_p, C.c_void_p]
         L.loc_tex.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
         L.loc_line_area.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]
         L.loc_get_stats.argtypes = [C.c_void_p, C.POINTER(loc_stats)]
@@ -225,6 +228,15 @@ def loc_spectra(h, trans, dev_out, nx, ny=1, dir=None, aff=None, offsets_cm=None
     o = _np(offsets_cm, np.float64) if offsets_cm is not None else None
     _check(lib().loc_spectra(h, int(trans), _hp(d) if d is not None else None, int(nx), int(ny),
                              _hp(a) if a is not None else None, _hp(o) if o is not None else None, _dp(dev_out)), h)
+
+
+def loc_set_option(h, key: int, value: float) -> None:
+    _check(lib().loc_set_option(h, int(key), float(value)), h)
+
+
+def loc_spectra_map(h, trans, dev_out, nx, ny, dir, pixel_cm, centre_cm):
+    d, c = _np(dir, np.float64), _np(centre_cm, np.float64)
+    _check(lib().loc_spectra_map(h, int(trans), _hp(d), int(nx), int(ny), float(pixel_cm), _hp(c), _dp(dev_out)), h)
 
 
 def loc_get_stats(h) -> dict:

@@ -32,7 +32,17 @@ struct Carver {
     }
 };
 
-static int max_resident_warps() { return 148 * 16; }  // upper bound used to size the per-warp spectrum slots
+// multiprocessors of the current device; 148 (B200) only when no device can be queried (sizing calls without a GPU)
+static int device_sm_count()
+{
+    int dev = 0, nsm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm < 1) {
+        cudaGetLastError();
+        return 148;
+    }
+    return nsm;
+}
+static int max_resident_ctas() { return device_sm_count() * 16; }  // upper bound used to size the per-CTA spectrum slots
 
 // lays out the workspace; with dry=true only sizes are computed
 static int64_t carve(loc_model *m, Carver &c, const loc_grid *g, int nch, int nlevel, int ntrans, int ndir_max)
@@ -79,14 +89,14 @@ static int64_t carve(loc_model *m, Carver &c, const loc_grid *g, int nch, int nl
         m->ntask_max = face * ndir_max;
         m->d_dirs = c.take<Dir3>(ndir_max);
         m->d_task_off = c.take<long long>(m->ntask_max + 1);
-        m->d_task_dir = c.take<unsigned char>(m->ntask_max);
+        m->d_task_dir = c.take<uint16_t>(m->ntask_max);
         // step stream: every leaf is crossed by (1 + s_p + s_q) <= 3 ray segments per direction on average;
         // control records (background / save / load) ride in the same bound
         m->stream_cap = 3 * ncell * (int64_t)ndir_max + 16 * m->ntask_max + 1024;
         m->d_stream = c.take<uint2>(m->stream_cap);
         m->bstack_threads = (int)std::min<int64_t>(m->ntask_max, LOC_BUILD_BATCH);
         m->d_bstack = c.take<char>((int64_t)m->bstack_threads * LOC_BUILD_STACK * 16);
-        m->max_warps = max_resident_warps();
+        m->max_warps = max_resident_ctas();
         m->spec_pool_floats = (int64_t)m->max_warps * 4 * std::max(g->nlevel - 1, 1) * nsp * ((nch + 3) & ~3);  // 4 rays per warp
         m->spec_pool = c.take<float>(m->spec_pool_floats);
     }
@@ -95,7 +105,7 @@ static int64_t carve(loc_model *m, Carver &c, const loc_grid *g, int nch, int nl
 
 extern "C" int64_t loc_workspace_bytes(const loc_grid *g, int nchannel, int nlevel_species, int ntrans, int ndir_max)
 {
-    if (!g || nchannel < 1 || nlevel_species < 2 || nlevel_species > LOC_MAX_LEVELS || ntrans < 1) return LOC_EINVAL;
+    if (!g || nchannel < 1 || nlevel_species < 2 || nlevel_species > LOC_MAX_LEVELS || ntrans < 1 || ndir_max > LOC_MAX_DIRS) return LOC_EINVAL;
     if (g->kind == LOC_GRID_SHELL) {
         if (g->nshell < 1 || g->nray < 1) return LOC_EINVAL;
     } else if (g->kind == LOC_GRID_OCTREE) {
@@ -243,6 +253,7 @@ __global__ void __launch_bounds__(128) k_solve(int64_t n, SpeciesDev sp, Selecti
             double old = pops[(int64_t)l * n + i];
             if (ntot > 0.0 && (nw >= 1e-10 * ntot || old >= 1e-10 * ntot))
                 rel = fmaxf(rel, (float)(fabs(nw - old) / fmax(nw, 1e-300)));
+            if (!isfinite(nw)) rel = INFINITY;  // reported by fetch_maxrel as LOC_ENONFINITE, never as "converged"
             x[l] = nw;
             pops[(int64_t)l * n + i] = (float)nw;
         }
@@ -406,6 +417,7 @@ __global__ void __launch_bounds__(LOC_SOLVE_THREADS) k_solve_s(int64_t n, Specie
                 const double old = pops[(int64_t)l * n + i];
                 if (ntot > 0.0 && (nw >= 1e-10 * ntot || old >= 1e-10 * ntot))
                     rel = fmaxf(rel, (float)(fabs(nw - old) / fmax(nw, 1e-300)));
+                if (!isfinite(nw)) rel = INFINITY;  // see k_solve
                 VX(l) = nw;
                 pops[(int64_t)l * n + i] = (float)nw;
             }
@@ -492,6 +504,7 @@ extern "C" int loc_create_model(const loc_grid *g, const loc_cells *cells, int n
     if (!g || !cells || !workspace) return fail(nullptr, LOC_EINVAL, "NULL argument");
     if (nchannel < 1 || nchannel > 1024) return fail(nullptr, LOC_EINVAL, "nchannel must be in [1,1024]");
     if (nlevel_max < 2 || nlevel_max > LOC_MAX_LEVELS || ntrans_max < 1) return fail(nullptr, LOC_EINVAL, "species limits out of range");
+    if (ndir_max > LOC_MAX_DIRS) return fail(nullptr, LOC_EINVAL, "ndir_max exceeds 65535 directions");
     if (!(band_half > 0.0) || tbg < 0.0) return fail(nullptr, LOC_EINVAL, "band_halfwidth must be > 0 and t_background >= 0");
     if (!cells->density || !cells->tkin || !cells->sigma || !cells->vx || !cells->abundance)
         return fail(nullptr, LOC_EINVAL, "cell arrays missing");
@@ -531,8 +544,8 @@ extern "C" int loc_create_model(const loc_grid *g, const loc_cells *cells, int n
     m->xmin = 4.5f;
     m->ali = 1;
     m->eps_tau = 1e-6f;
-    if (getenv("LOC_XMIN")) m->xmin = (float)atof(getenv("LOC_XMIN"));
-    if (getenv("LOC_EPS_TAU")) m->eps_tau = (float)atof(getenv("LOC_EPS_TAU"));
+    m->xclip = LOC_XCLIP;
+    m->nsm = device_sm_count();
     m->ncell = (g->kind == LOC_GRID_SHELL) ? g->nshell : g->level_offset[g->nlevel];
     m->ws = (char *)workspace;
     m->ws_bytes = workspace_bytes;
@@ -733,18 +746,27 @@ extern "C" int loc_set_directions(loc_model *m, int ndir, const double *dir)
         const double *d = dir + 3 * i;
         double nn = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
         if (!(fabs(nn - 1.0) < 1e-9)) return fail(m, LOC_EINVAL, "direction is not a unit vector");
-        loc_fill_dir(m, d, &m->h_dirs[i]);
     }
-    m->ndir = ndir;
+    // the model has NO directions until the new step stream is complete: a failure below (LOC_ENOMEM, LOC_ECUDA) leaves
+    // loc_simulate refusing to run (LOC_ESTATE) instead of replaying a half-written stream
+    m->ndir = 0;
+    m->ntask = 0;
+    m->stream_len = 0;
+    m->setup_steps = 0;
+    m->simulated = false;
     int64_t t0 = 0;
     for (int i = 0; i < ndir; i++) {
+        loc_fill_dir(m, dir + 3 * i, &m->h_dirs[i]);
         m->h_dirs[i].task0 = t0;
         t0 += (int64_t)m->h_dirs[i].np * m->h_dirs[i].nq;
     }
-    m->ntask = t0;
     LOC_CUDA_CHECK(m, cudaMemcpyAsync(m->d_dirs, m->h_dirs, sizeof(Dir3) * ndir, cudaMemcpyHostToDevice, m->stream));
     LOC_CUDA_CHECK(m, cudaStreamSynchronize(m->stream));
-    return loc_build_streams(m);  // S0/S2 set-up: the ray paths do not change between iterations
+    const int rc = loc_build_streams(m, ndir, t0);  // S0/S2 set-up: the ray paths do not change between iterations
+    if (rc != LOC_OK) return rc;
+    m->ndir = ndir;
+    m->ntask = t0;
+    return LOC_OK;
 }
 
 extern "C" int loc_set_populations(loc_model *m, float *dev_pops)
@@ -786,7 +808,9 @@ extern "C" int loc_simulate(loc_model *m, int nsel, const int *idx, int geom)
         LOC_CUDA_CHECK(m, cudaMemsetAsync(m->pathz, 0, sizeof(uint32_t) * n, m->stream));
     }
     LOC_CUDA_CHECK(m, cudaMemsetAsync(m->d_steps, 0, 2 * sizeof(unsigned long long), m->stream));
-    return (m->kind == LOC_GRID_SHELL) ? loc_launch_sim1d(m, geom) : loc_launch_sim3d(m, geom);
+    const int rc = (m->kind == LOC_GRID_SHELL) ? loc_launch_sim1d(m, geom) : loc_launch_sim3d(m, geom);
+    m->simulated = rc == LOC_OK;
+    return rc;
 }
 
 extern "C" int loc_get_counters(loc_model *m, const float **counters, int *ntp, const uint32_t **visits, const uint32_t **pathz)
@@ -807,8 +831,8 @@ static int solve_async(loc_model *m)
 #define LOC_SOLVE(NLMAX)                                                                                                     \
     k_solve<NLMAX><<<nb, 128, 0, m->stream>>>(n, m->sp, m->selh, m->cells.density, m->cells.tkin, m->cells.abundance, m->cnt, \
                                               m->pops, m->coef, m->d_maxrel, ch, m->ali)
-    // shared-memory solver (k_solve_s) while a block's matrices and the species tables fit; LOC_SOLVE_LOCAL=1 forces the
-    // local-memory kernel (A/B measurements)
+    // shared-memory solver (k_solve_s) while a block's matrices and the species tables fit; loc_set_option(LOC_OPT_SOLVER_LOCAL)
+    // forces the local-memory kernel (A/B measurements)
     {
         const int NL = m->nlevel;
         SolveTabs T;
@@ -831,8 +855,7 @@ static int solve_async(loc_model *m)
         T.cl = take(4 * m->ncoll);
         T.bytes = o;
         const size_t smem = sizeof(double) * (size_t)(NL * NL + 2 * NL) * LOC_SOLVE_THREADS + (size_t)o;
-        const char *force = getenv("LOC_SOLVE_LOCAL");
-        if (NL <= 16 && smem <= 200 * 1024 && !(force && atoi(force))) {
+        if (NL <= 16 && smem <= 200 * 1024 && !m->solver_local) {
             const unsigned nbs = (unsigned)((n + LOC_SOLVE_THREADS - 1) / LOC_SOLVE_THREADS);
 #define LOC_SOLVE_S(NLX)                                                                                                          \
     do {                                                                                                                          \
@@ -873,6 +896,7 @@ static int fetch_maxrel(loc_model *m, double *out)
     float f;
     memcpy(&f, &bits, sizeof(f));
     if (out) *out = f;
+    if (!isfinite(f)) return fail(m, LOC_ENONFINITE, "the solve produced a non-finite population (T_kin <= 0, NaN input or counter?)");
     return LOC_OK;
 }
 
@@ -880,6 +904,7 @@ extern "C" int loc_solve(loc_model *m, double *max_rel_change)
 {
     if (!m) return LOC_EINVAL;
     if (!m->have_species || !m->pops) return fail(m, LOC_ESTATE, "species and populations must be set before loc_solve");
+    if (!m->simulated) return fail(m, LOC_ESTATE, "loc_solve: no loc_simulate has filled the counters");
     LOC_CUDA_CHECK(m, cudaMemsetAsync(m->d_maxrel, 0, sizeof(unsigned int), m->stream));
     int rc = solve_async(m);
     if (rc) return rc;
@@ -889,6 +914,10 @@ extern "C" int loc_solve(loc_model *m, double *max_rel_change)
 extern "C" int loc_iterate(loc_model *m, int niter, double *max_rel_change)
 {
     if (!m || niter < 0) return LOC_EINVAL;
+    if (niter == 0) {  // nothing ran: no stale change of an earlier call
+        if (max_rel_change) *max_rel_change = 0.0;
+        return LOC_OK;
+    }
     for (int it = 0; it < niter; it++) {
         int rc = loc_simulate(m, 0, nullptr, 0);
         if (rc) return rc;
@@ -904,6 +933,34 @@ extern "C" int loc_set_ali(loc_model *m, int ali)
     if (!m || (ali != 0 && ali != 1)) return LOC_EINVAL;
     m->ali = ali;
     return LOC_OK;
+}
+
+extern "C" int loc_set_option(loc_model *m, int key, double value)
+{
+    if (!m) return LOC_EINVAL;
+    switch (key) {
+    case LOC_OPT_WINDOW_XMIN:
+        if (!(value >= 1.0 && value <= 12.0)) return fail(m, LOC_EINVAL, "LOC_OPT_WINDOW_XMIN must be in [1, 12]");
+        m->xmin = (float)value;
+        return LOC_OK;
+    case LOC_OPT_WINDOW_EPS_TAU:
+        if (!(value > 0.0 && value <= 1.0)) return fail(m, LOC_EINVAL, "LOC_OPT_WINDOW_EPS_TAU must be in (0, 1]");
+        m->eps_tau = (float)value;
+        return LOC_OK;
+    case LOC_OPT_SPAN_XCLIP:
+        if (!(value >= 1.0 && value <= 12.0)) return fail(m, LOC_EINVAL, "LOC_OPT_SPAN_XCLIP must be in [1, 12]");
+        m->xclip = (float)value;
+        return LOC_OK;
+    case LOC_OPT_SIM3D_PARTS:
+        if (!(value >= 0.0 && value <= LOC_MAX_TRANS) || value != floor(value)) return fail(m, LOC_EINVAL, "LOC_OPT_SIM3D_PARTS must be an integer in [0, LOC_MAX_TRANS]");
+        m->sim3d_parts = (int)value;
+        return LOC_OK;
+    case LOC_OPT_SOLVER_LOCAL:
+        if (value != 0.0 && value != 1.0) return fail(m, LOC_EINVAL, "LOC_OPT_SOLVER_LOCAL must be 0 or 1");
+        m->solver_local = (int)value;
+        return LOC_OK;
+    }
+    return fail(m, LOC_EINVAL, "loc_set_option: unknown key");
 }
 
 extern "C" int loc_iterate_until(loc_model *m, int max_iter, double tol, int *niter_done, double *max_rel_change)
@@ -934,6 +991,16 @@ extern "C" int loc_spectra(loc_model *m, int trans, const double *dir, int nx, i
     if (!m->have_species || !m->pops) return fail(m, LOC_ESTATE, "species and populations must be set before loc_spectra");
     if (trans < 0 || trans >= m->ntrans || nx < 1 || ny < 1) return fail(m, LOC_EINVAL, "loc_spectra: bad transition or map size");
     return loc_launch_spectra(m, trans, dir, nx, ny, aff, offsets_cm, dev_out);
+}
+
+extern "C" int loc_spectra_map(loc_model *m, int trans, const double *dir, int nx, int ny, double pixel_cm, const double *centre_cm,
+                               float *dev_out)
+{
+    if (!m || !dev_out || !dir || !centre_cm) return LOC_EINVAL;
+    if (m->kind != LOC_GRID_OCTREE) return fail(m, LOC_ESTATE, "loc_spectra_map: octree models only (shells: loc_spectra with offsets_cm)");
+    if (!m->have_species || !m->pops) return fail(m, LOC_ESTATE, "species and populations must be set before loc_spectra_map");
+    if (trans < 0 || trans >= m->ntrans || nx < 1 || ny < 1 || !(pixel_cm > 0.0)) return fail(m, LOC_EINVAL, "loc_spectra_map: bad transition, map size or pixel size");
+    return loc_launch_spectra_map(m, trans, dir, nx, ny, pixel_cm, centre_cm, dev_out);
 }
 
 // T_ex = -(h nu / k) / ln(n_u g_l / (n_l g_u)) per cell (Fig. 4); 0 where the cell holds no molecules

@@ -9,6 +9,7 @@
 #define LOC_LB 20              // log2(grid units per root cell)
 #define LOC_H0 (1 << LOC_LB)   // grid units per root cell
 #define LOC_MAXL LOC_MAX_TREE_LEVELS
+#define LOC_MAX_DIRS 65535     // task -> direction table holds 16-bit indices
 #define LOC_BUILD_BATCH 262144  // root lines traced per launch of the path builder (16 B x LOC_BUILD_STACK of stack each)
 #define LOC_BUILD_STACK 256    // pending rays per root line (PAPER.md:119 estimates ~7*3^(NL-1) stored rays)
 
@@ -20,6 +21,7 @@
 #define LOC_PI 3.14159265358979323846
 
 #define LOC_LOG2E 1.4426950408889634f
+#define LOC_XCLIP 3.4f     // 3D kernel: the span reaches at least this many sigma to both sides of the line centre, or the step is masked (default of LOC_OPT_XCLIP)
 #define LOC_THICK_TAU 0.05f   // line-centre optical depth of a step above which exp() is used instead of the series
 
 // ------------------------------------------------------------------------------------------------
@@ -103,8 +105,12 @@ struct loc_model {
     bool coef_valid;
     int ali;  // 1: accelerated lambda iteration (default), 0: plain lambda iteration (loc_set_ali)
     float *pops;  // registered [nlevel][ncell]
-    // accuracy knobs (DESIGN 5.3)
-    float xmin, eps_tau;
+    // accuracy knobs (DESIGN 5.3), set through loc_set_option only
+    float xmin, eps_tau, xclip;
+    int sim3d_parts;   // 0 = automatic split of the traced transitions over launches
+    int solver_local;  // 1 = force the local-memory solver k_solve
+    int nsm;           // multiprocessors of the model's device (queried once in loc_create_model)
+    bool simulated;    // counters hold the result of a loc_simulate
     // 1D
     int nshell, nray;
     int *d_order, *d_k0;
@@ -124,7 +130,7 @@ struct loc_model {
     unsigned int *d_queue;      // [1] task queue head
     int64_t ntask, ntask_max;
     long long *d_task_off;      // [ntask_max+1] record offsets of the root-line tasks
-    unsigned char *d_task_dir;  // [ntask_max]
+    uint16_t *d_task_dir;       // [ntask_max] direction of each root-line task (ndir <= LOC_MAX_DIRS)
     uint2 *d_stream;            // precomputed step stream (S0/S2 set-up)
     int64_t stream_cap, stream_len;
     char *d_bstack;             // builder stacks
@@ -424,8 +430,10 @@ int loc_launch_sim3d(loc_model *m, int geom);
 int loc_setup3d(loc_model *m);
 int loc_launch_spectra(loc_model *m, int trans, const double *dir, int nx, int ny, const int64_t *aff,
                        const double *offsets_cm, float *dev_out);
+int loc_launch_spectra_map(loc_model *m, int trans, const double *dir, int nx, int ny, double pixel_cm, const double *centre_cm,
+                           float *dev_out);
 int loc_launch_line_area(loc_model *m, const float *dev_cube, long long npix, float *dev_w);
-int loc_build_streams(loc_model *m);
+int loc_build_streams(loc_model *m, int ndir, int64_t ntask);
 void loc_fill_dir(loc_model *m, const double *din, Dir3 *D);
 
 #define LOC_CUDA_CHECK(m, call)                                                                    \

@@ -68,7 +68,7 @@ struct Pending {  // 16 bytes
 struct BuildArgs {
     Tree G;
     const Dir3 *dirs;
-    const unsigned char *task_dir;
+    const uint16_t *task_dir;
     long long task_begin, task_end;
     long long *task_off;  // count pass: counts written to task_off[task]; emit pass: offsets read from it
     uint2 *stream;
@@ -324,20 +324,19 @@ int loc_setup3d(loc_model *m)
     return LOC_OK;
 }
 
-int loc_build_streams(loc_model *m)
+// Builds the step stream of `ndir` directions (already in m->h_dirs / m->d_dirs) with `ntask` root-line tasks.  Commits
+// m->stream_len / setup_steps / setup_ms only on success; the caller commits m->ndir / m->ntask.
+static int build_streams_timed(loc_model *m, int ndir, int64_t ntask, cudaEvent_t e0, cudaEvent_t e1)
 {
-    cudaEvent_t e0, e1;
-    LOC_CUDA_CHECK(m, cudaEventCreate(&e0));
-    LOC_CUDA_CHECK(m, cudaEventCreate(&e1));
     LOC_CUDA_CHECK(m, cudaEventRecord(e0, m->stream));
     // task -> direction table
     {
-        std::vector<unsigned char> td((size_t)m->ntask);
-        for (int i = 0; i < m->ndir; i++) {
+        std::vector<uint16_t> td((size_t)ntask);
+        for (int i = 0; i < ndir; i++) {
             int64_t n = (int64_t)m->h_dirs[i].np * m->h_dirs[i].nq;
-            std::fill(td.begin() + m->h_dirs[i].task0, td.begin() + m->h_dirs[i].task0 + n, (unsigned char)i);
+            std::fill(td.begin() + m->h_dirs[i].task0, td.begin() + m->h_dirs[i].task0 + n, (uint16_t)i);
         }
-        LOC_CUDA_CHECK(m, cudaMemcpyAsync(m->d_task_dir, td.data(), td.size(), cudaMemcpyHostToDevice, m->stream));
+        LOC_CUDA_CHECK(m, cudaMemcpyAsync(m->d_task_dir, td.data(), td.size() * sizeof(uint16_t), cudaMemcpyHostToDevice, m->stream));
         LOC_CUDA_CHECK(m, cudaStreamSynchronize(m->stream));
     }
     BuildArgs A;
@@ -351,24 +350,24 @@ int loc_build_streams(loc_model *m)
     A.nsteps = m->d_steps;
     LOC_CUDA_CHECK(m, cudaMemsetAsync(m->d_errflag, 0, sizeof(int), m->stream));
     LOC_CUDA_CHECK(m, cudaMemsetAsync(m->d_steps, 0, sizeof(unsigned long long), m->stream));
+    long long total = 0;
+    unsigned long long steps = 0;
     for (int pass = 0; pass < 2; pass++) {
         A.emit = pass;
-        for (int64_t b = 0; b < m->ntask; b += m->bstack_threads) {
+        for (int64_t b = 0; b < ntask; b += m->bstack_threads) {
             A.task_begin = b;
-            A.task_end = std::min<int64_t>(m->ntask, b + m->bstack_threads);
+            A.task_end = std::min<int64_t>(ntask, b + m->bstack_threads);
             unsigned nb = (unsigned)((A.task_end - A.task_begin + 127) / 128);
             k_build_paths<<<nb, 128, 0, m->stream>>>(A);
             m->launches++;
             LOC_CUDA_CHECK(m, cudaGetLastError());
         }
         if (pass == 0) {
-            k_scan_tasks<<<1, 1024, 0, m->stream>>>(m->d_task_off, m->ntask);
+            k_scan_tasks<<<1, 1024, 0, m->stream>>>(m->d_task_off, ntask);
             m->launches++;
             LOC_CUDA_CHECK(m, cudaGetLastError());
-            long long total = 0;
-            unsigned long long steps = 0;
             int err = 0;
-            LOC_CUDA_CHECK(m, cudaMemcpyAsync(&total, m->d_task_off + m->ntask, sizeof(total), cudaMemcpyDeviceToHost, m->stream));
+            LOC_CUDA_CHECK(m, cudaMemcpyAsync(&total, m->d_task_off + ntask, sizeof(total), cudaMemcpyDeviceToHost, m->stream));
             LOC_CUDA_CHECK(m, cudaMemcpyAsync(&steps, m->d_steps, sizeof(steps), cudaMemcpyDeviceToHost, m->stream));
             LOC_CUDA_CHECK(m, cudaMemcpyAsync(&err, m->d_errflag, sizeof(err), cudaMemcpyDeviceToHost, m->stream));
             LOC_CUDA_CHECK(m, cudaStreamSynchronize(m->stream));
@@ -377,20 +376,34 @@ int loc_build_streams(loc_model *m)
                 return LOC_ENOMEM;
             }
             if (total > m->stream_cap) {
-                snprintf(m->err, sizeof(m->err), "step stream needs %lld records, workspace holds %lld", total, (long long)m->stream_cap);
+                // the message carries the required record count: the workspace is sized for 3 ncell ndir_max + 16 ntask_max
+                // records (loc_workspace_bytes); a caller that hits this creates the model with a larger ndir_max
+                snprintf(m->err, sizeof(m->err), "step stream needs %lld records (8 bytes each), workspace holds %lld: create the model with a larger ndir_max",
+                         total, (long long)m->stream_cap);
                 return LOC_ENOMEM;
             }
-            m->stream_len = total;
-            m->setup_steps = (int64_t)steps;
         }
     }
     LOC_CUDA_CHECK(m, cudaEventRecord(e1, m->stream));
     LOC_CUDA_CHECK(m, cudaEventSynchronize(e1));
     float ms = 0.f;
-    cudaEventElapsedTime(&ms, e0, e1);
+    LOC_CUDA_CHECK(m, cudaEventElapsedTime(&ms, e0, e1));
+    m->stream_len = total;
+    m->setup_steps = (int64_t)steps;
     m->setup_ms = ms;
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
     return LOC_OK;
 }
 
+int loc_build_streams(loc_model *m, int ndir, int64_t ntask)
+{
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
+        if (e0) cudaEventDestroy(e0);
+        snprintf(m->err, sizeof(m->err), "cudaEventCreate failed");
+        return LOC_ECUDA;
+    }
+    const int rc = build_streams_timed(m, ndir, ntask, e0, e1);  // the events are destroyed on every exit path
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    return rc;
+}

@@ -1,13 +1,10 @@
 // loc_sim1d.cu -- 1D shell-ray simulation kernel (Eqs. 1-3).
 //
-// One thread block per ray (impact parameter), one thread per velocity channel: each thread owns its channel's
-// photon occupation numbers n[t] for all traced transitions IN REGISTERS for the whole ray (the spherical
-// symmetry makes the ray a fixed sequence of shells: in through NS-1..k0, out through k0+1..NS-1, with
-// precomputed path lengths).  Per step: one profile value per thread, one exp per (thread,
-// transition) -- only in warps that overlap the profile window --, a halving-butterfly warp reduction of the
-// 2 NT + 1 channel sums, a cross-warp reduction through shared memory that is overlapped with the next
-// step, and one float atomic per (cell, transition, counter).  The paper's kernel used one work item per ray
-// and one transition at a time.
+// One WARP per ray (impact parameter); the spherical symmetry makes the ray a fixed sequence of shells (in through
+// NS-1..k0, out through k0+1..NS-1) with precomputed path lengths.  See k_sim1d_w below.  The paper's kernel
+// used one work item per ray and one transition at a time.  (Round 1 also had a
+// block-per-ray kernel with one thread per channel; it was 2.9x slower on C2 and unreachable for every legal input, and
+// was removed: profiles/r1_sim1d_C2.md keeps its measurements.)
 #include <stdio.h>
 #include <stdlib.h>
 
@@ -47,119 +44,14 @@ __device__ __forceinline__ void seg1d(const Sim1D &P, int j, int nin, int k0, lo
     }
 }
 
-template <int NT, bool GEOM>
-__global__ void __launch_bounds__(1024) k_sim1d(Sim1D P)
-{
-    constexpr int NV = 2 * NT + 1;
-    __shared__ TParam s_tp[2][NT];
-    __shared__ float s_tau0[2];
-    extern __shared__ float s_part[];  // [2][nwarp*NV + 4]
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
-    const int pstride = nwarp * NV + 4;
-    const int ray = P.order[blockIdx.x];
-    const int k0 = P.k0[ray];
-    const long long off = P.off[ray];
-    const int nin = P.ns - 1 - k0, nseg = 2 * nin + 1;
-    float n[NT];
-#pragma unroll
-    for (int t = 0; t < NT; t++) n[t] = P.S.bgocc[t];  // Eq. 1: background photons, as occupation number
-    const float cvel = ((float)tid - 0.5f * (float)(P.nch - 1)) * P.dv;
-    const float inv_dv = 1.0f / P.dv;
-
-    for (int j = 0; j <= nseg; j++) {
-        const int buf = j & 1;
-        int k = 0;
-        float s = 0.f, mu = 0.f, w = 0.f, v0 = 0.f, sig = 1.f, amp = 0.f;
-        if (j < nseg) {
-            seg1d(P, j, nin, k0, off, k, s, mu, w);
-            float4 kin = __ldg(P.kin + k);
-            v0 = -kin.x * mu;  // DESIGN R6, mu at the entry of the step
-            sig = kin.w;
-            // w = this ray's share a s / V_eff of the shell (DESIGN R12), tabulated
-            amp = P.dv * 0.3989422804f / sig;
-            if (warp == 0) {
-                float tau0 = 0.f;
-                if (lane < NT) {
-                    float2 ke = __ldg(P.coef + (long long)k * P.nsp + lane);
-                    s_tp[buf][lane] = make_tparam(ke, s, w, amp);
-                    tau0 = fabsf(ke.x * s) * amp;
-                }
-                unsigned mx = __reduce_max_sync(0xffffffffu, __float_as_uint(tau0));
-                if (lane == 0) s_tau0[buf] = __uint_as_float(mx);
-            }
-        }
-        __syncthreads();
-        // ---- cross-warp reduction of the PREVIOUS step by the last warp (overlaps with this step's work) ----
-        if (j > 0 && warp == nwarp - 1) {
-            const float *pp = s_part + (buf ^ 1) * pstride;
-            int kp;
-            float sp_, mup, wp_;
-            seg1d(P, j - 1, nin, k0, off, kp, sp_, mup, wp_);
-            const float wprev = pp[nwarp * NV + 0];
-            const int clo = __float_as_int(pp[nwarp * NV + 1]), chi = __float_as_int(pp[nwarp * NV + 2]);
-            float tot = 0.f;
-            if (lane < NV)
-                for (int ww = 0; ww < nwarp; ww++)
-                    if (ww * 32 <= chi && ww * 32 + 31 >= clo) tot += pp[ww * NV + lane];
-            float sphi = __shfl_sync(0xffffffffu, tot, 2 * NT);
-            if (lane < NT)
-                atomicAdd(&P.cnt[(long long)kp * P.nsp + lane].x, tot);
-            else if (lane < 2 * NT)
-                atomicAdd(&P.cnt[(long long)kp * P.nsp + (lane - NT)].y, tot + (wprev - sphi));
-            if (GEOM && lane == 0) atomicAdd(&P.visits[kp], 1u);
-        }
-        if (j == nseg) break;
-        // ---- profile window of this step (DESIGN 5.3) ----
-        const float tau0m = s_tau0[buf];
-        float X = P.xmin;
-        if (tau0m > P.eps_tau) X = fmaxf(X, sqrtf(2.0f * __logf(tau0m / P.eps_tau)));
-        const float cc = v0 * inv_dv + 0.5f * (float)(P.nch - 1);
-        const float hw = X * sig * inv_dv;
-        const int c_lo = max(0, (int)ceilf(cc - hw)), c_hi = min(P.nch - 1, (int)floorf(cc + hw));
-        float *pw = s_part + buf * pstride;
-        if (GEOM && tid == 0) {
-            const float h5 = 5.0f * sig * inv_dv;
-            atomicAdd(P.nactive, (unsigned long long)max(0, min(P.nch - 1, (int)floorf(cc + h5)) - max(0, (int)ceilf(cc - h5)) + 1));
-        }
-        if (tid == 0) {
-            pw[nwarp * NV + 0] = w;
-            pw[nwarp * NV + 1] = __int_as_float(c_lo);
-            pw[nwarp * NV + 2] = __int_as_float(c_hi);
-        }
-        if (warp * 32 <= c_hi && warp * 32 + 31 >= c_lo) {
-            const bool act = tid >= c_lo && tid <= c_hi;
-            const float ky = 0.8493218f / sig;  // sqrt(log2(e)/2) / sigma
-            const float y = (cvel - v0) * ky;
-            const float phi = act ? ex2f(fmaf(-y, y, __log2f(amp))) : 0.0f;
-            float v[NV];
-#pragma unroll
-            for (int t = 0; t < NT; t++) {
-                const TParam tp = s_tp[buf][t];
-                float a = 0.f, b = 0.f;
-                channel_update(n[t], phi, tp, a, b);
-                v[t] = a;
-                v[NT + t] = b;
-            }
-            v[2 * NT] = phi;
-            int owner;
-            float tot = warp_multi_reduce<NV>(v, lane, owner);
-            if (owner >= 0) {
-                float sc = (owner == 2 * NT) ? w : s_tp[buf][owner < NT ? owner : owner - NT].scale;
-                pw[warp * NV + owner] = tot * sc;
-            }
-        }
-    }
-}
-
 // ------------------------------------------------------------------------------------------------------------------
-// k_sim1d_w: one WARP per ray (profiles/r1_sim1d_C2.md: the block-per-ray kernel above is issue bound at 2600 warp
-// instructions per ray step, most of them per-step scalar work repeated by every warp of the block and the two-stage
+// k_sim1d_w: one WARP per ray (profiles/r1_sim1d_C2.md: a block-per-ray kernel was issue bound at 2600 warp
+// instructions per ray step, most of them per-step scalar work repeated by every warp of the block and a two-stage
 // reduction).  The ray's spectra [NT][nchp] live in shared memory; per step the lanes cover the profile window in
 // aligned quads of channels (one 128-bit shared-memory access per lane and transition, conflict free), sum their
 // channels in registers, and ONE halving-butterfly reduction per step leaves each of the 2 NT + 1 totals in one lane,
 // which issues the counter's atomic itself: no block barrier, no second reduction stage.  The step's table entries, cell
-// kinematics and line coefficients are loaded one step ahead.  Same per-channel arithmetic (channel_update), same
-// window rule and wing term as k_sim1d.
+// kinematics and line coefficients are loaded one step ahead.
 // ------------------------------------------------------------------------------------------------------------------
 #define LOC_1D_WARPS 1  // rays per block (C2: 1 -> 3.80 ms, 2 -> 4.15 ms, 4 -> 4.13 ms: 24 instead of 22 resident rays per SM, finer scheduling)
 
@@ -219,7 +111,11 @@ __global__ void __launch_bounds__(LOC_1D_WARPS * 32) k_sim1d_w(Sim1D P, int nray
         const float tau0m = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(tau0)));
         __syncwarp();
         // ---- profile window of this step (DESIGN 5.3) ----
+        // channels wider than the line (dv > sigma): the neglected sampled values are amp e^{-X^2/2} with amp ~ dv/sigma > 1,
+        // and the sum of the sampled profile may be well below 1, so the window grows by 2 ln (dv/sigma)^2 (DESIGN 5.3)
+        const float und = P.dv / sig;
         float X = P.xmin;
+        if (und > 1.0f) X = sqrtf(fmaf(4.0f, __logf(und), X * X));
         if (tau0m > P.eps_tau) X = fmaxf(X, sqrtf(2.0f * __logf(tau0m / P.eps_tau)));
         const float cc = v0 * inv_dv + chalf;
         const float hw = X * sig * inv_dv;
@@ -275,31 +171,21 @@ __global__ void __launch_bounds__(LOC_1D_WARPS * 32) k_sim1d_w(Sim1D P, int nray
 template <int NT>
 static int launch1d(loc_model *m, const Sim1D &P, int geom)
 {
-    // warp-per-ray kernel while the spectra of a block's rays fit shared memory; LOC_SIM1D_BLOCK=1 forces the
-    // block-per-ray kernel (A/B measurements, very wide bands)
+    // the spectra of a ray ([NT][nchp] floats, <= 12 x 1024 x 4 B = 48 KB for every legal input) live in shared memory
     const int nchp = (m->nch + 3) & ~3;
     const size_t smem_w = sizeof(float) * LOC_1D_WARPS * ((size_t)NT * nchp + 4 * NT);
-    const char *force = getenv("LOC_SIM1D_BLOCK");
-    if (smem_w <= 96 * 1024 && !(force && atoi(force))) {
-        const int blocks = (m->nray + LOC_1D_WARPS - 1) / LOC_1D_WARPS;
-        if (geom) {
-            LOC_CUDA_CHECK(m, cudaFuncSetAttribute(k_sim1d_w<NT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_w));
-            k_sim1d_w<NT, true><<<blocks, LOC_1D_WARPS * 32, smem_w, m->stream>>>(P, m->nray);
-        } else {
-            LOC_CUDA_CHECK(m, cudaFuncSetAttribute(k_sim1d_w<NT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_w));
-            k_sim1d_w<NT, false><<<blocks, LOC_1D_WARPS * 32, smem_w, m->stream>>>(P, m->nray);
-        }
-        m->launches++;
-        LOC_CUDA_CHECK(m, cudaGetLastError());
-        return LOC_OK;
+    if (smem_w > 200 * 1024) {
+        snprintf(m->err, sizeof(m->err), "nchannel * ntrans too large for the shared-memory spectra of the 1D kernel (%zu bytes)", smem_w);
+        return LOC_EINVAL;
     }
-    int threads = (m->nch + 31) / 32 * 32;
-    int nwarp = threads / 32;
-    size_t smem = sizeof(float) * 2 * (nwarp * (2 * NT + 1) + 4);
-    if (geom)
-        k_sim1d<NT, true><<<m->nray, threads, smem, m->stream>>>(P);
-    else
-        k_sim1d<NT, false><<<m->nray, threads, smem, m->stream>>>(P);
+    const int blocks = (m->nray + LOC_1D_WARPS - 1) / LOC_1D_WARPS;
+    if (geom) {
+        LOC_CUDA_CHECK(m, cudaFuncSetAttribute(k_sim1d_w<NT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_w));
+        k_sim1d_w<NT, true><<<blocks, LOC_1D_WARPS * 32, smem_w, m->stream>>>(P, m->nray);
+    } else {
+        LOC_CUDA_CHECK(m, cudaFuncSetAttribute(k_sim1d_w<NT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_w));
+        k_sim1d_w<NT, false><<<blocks, LOC_1D_WARPS * 32, smem_w, m->stream>>>(P, m->nray);
+    }
     m->launches++;
     LOC_CUDA_CHECK(m, cudaGetLastError());
     return LOC_OK;

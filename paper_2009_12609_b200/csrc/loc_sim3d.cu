@@ -58,7 +58,7 @@ struct Sim3D {
     int geom;   // also accumulate the geometry counters (visits, path sums, active channels)
     float dv, xmin, xclip, inv_ndir;
     const Dir3 *dirs;
-    const unsigned char *task_dir;
+    const uint16_t *task_dir;
     const long long *task_off;
     const uint2 *stream;
     long long ntask;
@@ -91,7 +91,6 @@ struct Sim3D {
 #define LOC_RS_CTRL 0x40000000u
 #define LOC_RS_STEP 0x80000000u
 
-#define LOC_XCLIP 3.4f     // the span reaches at least this many sigma to both sides of the line centre, or the step is masked
 #define LOC_EXP_TAU 0.05f  // line-centre optical depth of a step from which the exponential form is used
 
 template <int NT>
@@ -300,6 +299,10 @@ __device__ __forceinline__ unsigned prepare_record(const Sim3D &P, uint2 rec, co
                 float Ql, Qh;
                 bool far;
                 wing_mass(cc, rcpf(sigch), (float)iwb, (float)LOC_SPAN, Ql, Qh, far);
+                // channels wider than the line: the sum of the sampled profile differs from its integral (by e^{-2 pi^2
+                // (sigma/dv)^2}: 3e-9 at sigma = dv, 7e-3 at sigma = dv/2), so the analytic wing mass does not stand for
+                // 1 - sum phi any more: the round then takes the sum itself (DESIGN 5.3)
+                far = far && sigch >= 1.0f;
                 qe = far ? Ql + Qh : -1.0f;
                 ql = (iwb == 0 || !far) ? 0.0f : Ql;
                 qh = (iwb + LOC_SPAN >= P.nch || !far) ? 0.0f : Qh;
@@ -370,7 +373,11 @@ __device__ __forceinline__ unsigned step_mode(const Sim3D &P, unsigned rb, float
         asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(need) : "f"(X2 * 0.7213475f * rcpf(-h0.z)));
         const int wb = (int)(wbop & LOC_WB_MASK);
         const bool ok1 = P.nch >= LOC_SPAN && (wb == 0 || cc - (float)wb >= need) && (wb + LOC_SPAN >= P.nch || (float)(wb + LOC_SPAN - 1) - cc >= need);
-        if (!ok1) {
+        if (-h0.z > 0.7213475f) {
+            // channels wider than the line (sigma < dv; -q2 = log2(e) / (2 sigch^2)): the exact masked path, which sums the
+            // sampled profile itself and evaluates it from the distance to the line centre (DESIGN 5.3)
+            flags |= LOC_RS_SLOW;
+        } else if (!ok1) {
             const int ww = wide_start(P.nch, cc);
             const bool ok2 = P.nch >= 2 * LOC_SPAN && (ww == 0 || cc - (float)ww >= need) && (ww + 2 * LOC_SPAN >= P.nch || (float)(ww + 2 * LOC_SPAN - 1) - cc >= need);
             flags |= ok2 ? LOC_RS_WIDE : LOC_RS_SLOW;
@@ -378,7 +385,7 @@ __device__ __forceinline__ unsigned step_mode(const Sim3D &P, unsigned rb, float
                 float Ql, Qh;
                 bool far;
                 wing_mass(cc, 1.1774100f * sqrtf(-h0.z), (float)ww, (float)(2 * LOC_SPAN), Ql, Qh, far);
-                if (far) qe_wide = Ql + Qh;
+                if (far && -h0.z <= 0.7213475f) qe_wide = Ql + Qh;  // -q2 = log2(e) / (2 sigch^2): sigch >= 1 as in prepare_record
             }
         }
     }
@@ -398,15 +405,23 @@ __device__ __forceinline__ float slow_round(const Sim3D &P, unsigned rb, unsigne
     const float4 h0 = lds128(rb);
     const uint4 h1 = lds128u(rb + 16);
     const unsigned wbop = __float_as_uint(h0.w);
-    const int wb = (int)(wbop & LOC_WB_MASK);
     int clo = 1, chi = 0;
+    // the profile from the distance to the line centre: log2 phi(c) = lamp - ((c - cc) ky)^2.  (The quadratic around the
+    // middle of the span that the common round uses cancels badly when the span is clamped far from the line AND the
+    // channels are wide: ky ~ 8 per channel at dv = 10 sigma.)
+    const float kyc = sqrtf(-h0.z), ccc = __uint_as_float(h1.w);
+    const float lamp = (wbop & LOC_RS_STEP) ? __log2f(0.4697186f * kyc) : -INFINITY;
     if (wbop & LOC_RS_STEP) {
         const float ky = sqrtf(-h0.z);
         const float sigch = 0.8493218f * rcpf(ky);
         const float4 tm = lds128(rb + L::TM);
         const float tau0m = fmaxf(fmaxf(tm.x, tm.y), fmaxf(tm.z, tm.w));
-        float X = P.xmin;
-        if (tau0m > 1.0f) X = sqrtf(fmaf(2.0f, __logf(tau0m), X * X));
+        float X2 = P.xmin * P.xmin;
+        // channels wider than the line: a handful of channels whatever the reach, and no wing correction on this path:
+        // reach 6.5 sigma at least, + 2 ln (dv/sigma)^2 (see loc_sim1d.cu)
+        if (sigch < 1.0f) X2 = fmaf(-4.0f, __logf(sigch), fmaxf(X2, 42.25f));
+        if (tau0m > 1.0f) X2 = fmaf(2.0f, __logf(tau0m), X2);
+        const float X = sqrtf(X2);
         const float cc = __uint_as_float(h1.w), hw = X * sigch;
         clo = max(0, (int)ceilf(cc - hw));
         chi = min(P.nch - 1, (int)floorf(cc + hw));
@@ -423,8 +438,8 @@ __device__ __forceinline__ float slow_round(const Sim3D &P, unsigned rb, unsigne
         for (int k = 0; k < 4; k++) {
             const int c = cb + k;
             const bool m = c >= clo && c <= chi;
-            const float j = (float)(c - (wb + 16));
-            e[k] = m ? ex2f(fmaf(j, fmaf(j, h0.z, h0.y), h0.x)) : 0.0f;
+            const float y = ((float)c - ccc) * kyc;
+            e[k] = m ? ex2f(fmaf(-y, y, lamp)) : 0.0f;
             inq |= m;
         }
         sphi += (e[0] + e[1]) + (e[2] + e[3]);
@@ -744,9 +759,7 @@ static int launch3d_t(loc_model *m, Sim3D &P, size_t smem)
     int bps = 0;
     LOC_CUDA_CHECK(m, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kern, 64, smem));
     if (bps < 1) bps = 1;
-    int nsm = 148;
-    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, 0);
-    long long blocks = (long long)nsm * bps;
+    long long blocks = (long long)m->nsm * bps;
     blocks = std::min<long long>(blocks, (m->ntask + LOC_GROUPS - 1) / LOC_GROUPS);
     blocks = std::min<long long>(blocks, m->max_warps);
     if (blocks < 1) blocks = 1;
@@ -781,7 +794,7 @@ int loc_launch_sim3d(loc_model *m, int geom)
     P.nslot = std::max(m->nlev - 1, 1);
     P.dv = (float)m->dv;
     P.xmin = m->xmin;
-    P.xclip = getenv("LOC_XCLIP") ? (float)atof(getenv("LOC_XCLIP")) : LOC_XCLIP;
+    P.xclip = m->xclip;
     P.inv_ndir = 1.0f / (float)m->ndir;
     P.dirs = m->d_dirs;
     P.task_dir = m->d_task_dir;
@@ -807,7 +820,7 @@ int loc_launch_sim3d(loc_model *m, int geom)
     int nsel = m->selh.nsel;
     int npart = 1;
     while (npart < nsel && spectra_bytes((nsel + npart - 1) / npart, P.nchp) > 24 * 1024) npart++;
-    if (getenv("LOC_SIM3D_PARTS")) npart = std::max(1, std::min(nsel, atoi(getenv("LOC_SIM3D_PARTS"))));
+    if (m->sim3d_parts > 0) npart = std::max(npart, std::min(nsel, m->sim3d_parts));  // loc_set_option(LOC_OPT_SIM3D_PARTS)
     int slot = 0;
     for (int part = 0; part < npart; part++) {
         int n = (nsel - slot + (npart - part) - 1) / (npart - part);

@@ -71,7 +71,11 @@ struct Spec3D {
     Tree G;
     Dir3 D;
     int nx, ny;
-    long long aff[6];
+    // pixel (ix, iy) starts on the upstream face at the working-frame transverse position
+    //   floor((o[0] + ix ex[0]) + iy ey[0]),  floor((o[1] + ix ex[1]) + iy ey[1])      (grid units, 2^20 per root cell),
+    // each product and sum rounded to nearest double on its own (no FMA contraction), so that a caller can reproduce the
+    // positions bit for bit; with integer coefficients (loc_spectra's `aff`) every term is exact
+    double o[2], ex[2], ey[2];
 };
 
 __global__ void __launch_bounds__(32 * LOC_SPEC_WARPS) k_spectra3d(Spec3D P)
@@ -84,7 +88,8 @@ __global__ void __launch_bounds__(32 * LOC_SPEC_WARPS) k_spectra3d(Spec3D P)
     for (int c = lane; c < P.C.nchp; c += 32) Dc[c] = 0.f;
     __syncwarp();
     const int ix = (int)(pix % P.nx), iy = (int)(pix / P.nx);
-    const long long bp = P.aff[0] + ix * P.aff[2] + iy * P.aff[3], bq = P.aff[1] + ix * P.aff[4] + iy * P.aff[5];
+    const long long bp = (long long)floor(__dadd_rn(__dadd_rn(P.o[0], __dmul_rn((double)ix, P.ex[0])), __dmul_rn((double)iy, P.ey[0])));
+    const long long bq = (long long)floor(__dadd_rn(__dadd_rn(P.o[1], __dmul_rn((double)ix, P.ex[1])), __dmul_rn((double)iy, P.ey[1])));
     const Dir3 &D = P.D;
     const long long Wz = D.W[0], Wp = D.W[1], Wq = D.W[2];
     long long zeta = 0;
@@ -159,10 +164,8 @@ __global__ void __launch_bounds__(32 * LOC_SPEC_WARPS) k_spectra1d(Spec1D P)
     for (int c = lane; c < P.C.nch; c += 32) o[c] = P.C.tk_per_occ * Dc[c];
 }
 
-int loc_launch_spectra(loc_model *m, int trans, const double *dir, int nx, int ny, const int64_t *aff, const double *offsets_cm,
-                       float *dev_out)
+static void spec_common(loc_model *m, int trans, SpecCommon &C)
 {
-    SpecCommon C;
     const int u = m->h_upper[trans], l = m->h_lower[trans];
     const double nu = m->h_freq[trans];
     C.nch = m->nch;
@@ -177,35 +180,54 @@ int loc_launch_spectra(loc_model *m, int trans, const double *dir, int nx, int n
     C.pop_u = m->pops + (int64_t)u * m->ncell;
     C.pop_l = m->pops + (int64_t)l * m->ncell;
     C.kin = m->kin;
-    const size_t smem = sizeof(float) * LOC_SPEC_WARPS * C.nchp;
+}
+
+static int launch_spectra3d(loc_model *m, int trans, const double *dir, int nx, int ny, const double *o, const double *ex, const double *ey,
+                            float *dev_out)
+{
+    const double nn = dir[0] * dir[0] + dir[1] * dir[1] + dir[2] * dir[2];
+    if (!(fabs(nn - 1.0) < 1e-9)) {
+        snprintf(m->err, sizeof(m->err), "loc_spectra: direction is not a unit vector");
+        return LOC_EINVAL;
+    }
+    Spec3D P;
+    spec_common(m, trans, P.C);
+    P.C.out = dev_out;
+    P.G = make_tree(m);
+    loc_fill_dir(m, dir, &P.D);
+    P.nx = nx;
+    P.ny = ny;
+    for (int i = 0; i < 2; i++) {
+        P.o[i] = o[i];
+        P.ex[i] = ex[i];
+        P.ey[i] = ey[i];
+    }
+    const size_t smem = sizeof(float) * LOC_SPEC_WARPS * P.C.nchp;
+    const long long npix = (long long)nx * ny;
+    k_spectra3d<<<(unsigned)((npix + LOC_SPEC_WARPS - 1) / LOC_SPEC_WARPS), 32 * LOC_SPEC_WARPS, smem, m->stream>>>(P);
+    m->launches++;
+    LOC_CUDA_CHECK(m, cudaGetLastError());
+    return LOC_OK;
+}
+
+int loc_launch_spectra(loc_model *m, int trans, const double *dir, int nx, int ny, const int64_t *aff, const double *offsets_cm,
+                       float *dev_out)
+{
     if (m->kind == LOC_GRID_OCTREE) {
         if (!dir || !aff) {
             snprintf(m->err, sizeof(m->err), "loc_spectra: octree models need dir and aff");
             return LOC_EINVAL;
         }
-        const double nn = dir[0] * dir[0] + dir[1] * dir[1] + dir[2] * dir[2];
-        if (!(fabs(nn - 1.0) < 1e-9)) {
-            snprintf(m->err, sizeof(m->err), "loc_spectra: direction is not a unit vector");
-            return LOC_EINVAL;
-        }
-        Spec3D P;
-        P.C = C;
-        P.C.out = dev_out;
-        P.G = make_tree(m);
-        loc_fill_dir(m, dir, &P.D);
-        P.nx = nx;
-        P.ny = ny;
-        for (int i = 0; i < 6; i++) P.aff[i] = aff[i];
-        const long long npix = (long long)nx * ny;
-        k_spectra3d<<<(unsigned)((npix + LOC_SPEC_WARPS - 1) / LOC_SPEC_WARPS), 32 * LOC_SPEC_WARPS, smem, m->stream>>>(P);
-        m->launches++;
-        LOC_CUDA_CHECK(m, cudaGetLastError());
-        return LOC_OK;
+        const double o[2] = {(double)aff[0], (double)aff[1]}, ex[2] = {(double)aff[2], (double)aff[4]}, ey[2] = {(double)aff[3], (double)aff[5]};
+        return launch_spectra3d(m, trans, dir, nx, ny, o, ex, ey, dev_out);
     }
     if (ny != 1 || !offsets_cm) {
         snprintf(m->err, sizeof(m->err), "loc_spectra: shell models need ny = 1 and offsets_cm");
         return LOC_EINVAL;
     }
+    SpecCommon C;
+    spec_common(m, trans, C);
+    const size_t smem = sizeof(float) * LOC_SPEC_WARPS * C.nchp;
     for (int b0 = 0; b0 < nx; b0 += LOC_SPEC_BATCH1D) {
         Spec1D P;
         P.C = C;
@@ -219,6 +241,53 @@ int loc_launch_spectra(loc_model *m, int trans, const double *dir, int nx, int n
         LOC_CUDA_CHECK(m, cudaGetLastError());
     }
     return LOC_OK;
+}
+
+// Map in the caller's frame (include/loc.h, loc_spectra_map): the image plane is spanned by e2 = the unit projection of
+// "north" (z; y when dir is parallel to z) perpendicular to dir and e1 = e2 x dir; pixel (ix, iy) is the line of sight through
+// X = centre + (ix - (nx-1)/2) pixel e1 + (iy - (ny-1)/2) pixel e2.  In the working frame of the direction (main axis zeta,
+// transverse p, q, mirrored so that the ray moves towards + on all three) the line is at p(zeta) = p_X + s_p (zeta - zeta_X),
+// s_p the snapped slope 2^32 / T; its start on the upstream face zeta = 0 is an affine function of (ix, iy).
+int loc_launch_spectra_map(loc_model *m, int trans, const double *dir, int nx, int ny, double pixel_cm, const double *centre_cm,
+                           float *dev_out)
+{
+    const double nn = sqrt(dir[0] * dir[0] + dir[1] * dir[1] + dir[2] * dir[2]);
+    if (!(fabs(nn - 1.0) < 1e-9)) {
+        snprintf(m->err, sizeof(m->err), "loc_spectra_map: direction is not a unit vector");
+        return LOC_EINVAL;
+    }
+    const double d[3] = {dir[0] / nn, dir[1] / nn, dir[2] / nn};
+    double north[3] = {0.0, 0.0, 1.0};
+    if (fabs(d[2]) > 1.0 - 1e-9) {
+        north[1] = 1.0;
+        north[2] = 0.0;
+    }
+    const double nd = north[0] * d[0] + north[1] * d[1] + north[2] * d[2];
+    double e2[3] = {north[0] - nd * d[0], north[1] - nd * d[1], north[2] - nd * d[2]};
+    const double l2 = sqrt(e2[0] * e2[0] + e2[1] * e2[1] + e2[2] * e2[2]);
+    for (int a = 0; a < 3; a++) e2[a] /= l2;
+    const double e1[3] = {e2[1] * d[2] - e2[2] * d[1], e2[2] * d[0] - e2[0] * d[2], e2[0] * d[1] - e2[1] * d[0]};
+    Dir3 D;
+    loc_fill_dir(m, dir, &D);
+    const double upc = (double)LOC_H0 / m->root_cm;  // grid units per cm
+    const double sl[2] = {D.T[0] ? 4294967296.0 / (double)D.T[0] : 0.0, D.T[1] ? 4294967296.0 / (double)D.T[1] : 0.0};
+    // working-frame coordinates of a model-frame point x (cm): w_k = flip ? W_k - u x_a : u x_a; of a vector: sign only
+    double wc[3], w1[3], w2[3];
+    for (int k = 0; k < 3; k++) {
+        const int a = D.ax[k];
+        const double sg = D.flip[k] ? -1.0 : 1.0;
+        wc[k] = D.flip[k] ? (double)D.W[k] - upc * centre_cm[a] : upc * centre_cm[a];
+        w1[k] = sg * upc * pixel_cm * e1[a];
+        w2[k] = sg * upc * pixel_cm * e2[a];
+    }
+    const double cx = 0.5 * (nx - 1), cy = 0.5 * (ny - 1);
+    double o[2], ex[2], ey[2];
+    for (int k = 0; k < 2; k++) {
+        ex[k] = w1[k + 1] - sl[k] * w1[0];
+        ey[k] = w2[k + 1] - sl[k] * w2[0];
+        o[k] = (wc[k + 1] - sl[k] * wc[0]) - cx * ex[k] - cy * ey[k];
+    }
+    return launch_spectra3d(m, trans, dir, nx, ny, o, ex, ey, dev_out);
 }
 
 // ---- line-area map (Fig. 5c: W = integral of T_A over velocity) -------------------------------------------

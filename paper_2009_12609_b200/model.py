@@ -5,6 +5,7 @@ pointers; results come back as views of the library's workspace.
 """
 from __future__ import annotations
 
+import contextlib
 import ctypes as C
 
 import numpy as np
@@ -24,14 +25,24 @@ class LocModel:
     """device-resident model.  `m` is a duck-typed description:
        shells : r_out, ray_p, ray_w, density, tkin, sigma, vrad, abundance, nchannel, band_half, t_bg, species
        octree : nx, ny, nz, root_cm, noff, child, density, tkin, sigma, vx, vy, vz, abundance, dirs, nchannel, ...
-    Host arrays may be numpy arrays or (pinned) torch CPU tensors; they are copied to `device` on `stream`."""
+    Host arrays may be numpy arrays or (pinned) torch CPU tensors; they are copied to `device` on `stream`.
+    stream: the torch.cuda.Stream the library enqueues on (None: torch's current stream at construction).  Every tensor
+    operation of this class (uploads, allocations, copies) runs inside `torch.cuda.stream(self.stream)`, so the copies are
+    ordered with the library's kernels and the caching allocator ties the buffers to that stream."""
 
     def __init__(self, m, device="cuda:0", ntrans_sim=None, ndir_max=None, stream=None):
         if not torch.cuda.is_available():
             raise B.LocError(B.LOC_ECUDA, "no CUDA device: the LOC library has no CPU path")
         self.dev = torch.device(device)
         torch.cuda.set_device(self.dev)
-        self.stream = stream
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.dev)
+        with self._on_stream():
+            self._init(m, ntrans_sim, ndir_max)
+
+    def _on_stream(self):
+        return torch.cuda.stream(self.stream)
+
+    def _init(self, m, ntrans_sim, ndir_max):
         self.is3d = hasattr(m, "child")
         sp = m.species
         self.nlevel, self.ntrans = len(sp.energy_K), len(sp.upper)
@@ -54,7 +65,7 @@ class LocModel:
         nts = ntrans_sim or self.ntrans
         nbytes = B.loc_workspace_bytes(self.grid, self.nch, self.nlevel, nts, ndir_max)
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.dev)
-        sptr = stream.cuda_stream if stream is not None else 0
+        sptr = self.stream.cuda_stream
         self.h = B.loc_create_model(self.grid, self.cells, self.nch, m.band_half, m.t_bg, self.nlevel, nts, ndir_max,
                                     self.workspace, sptr)
         B.loc_set_species(self.h, sp)
@@ -73,9 +84,10 @@ class LocModel:
 
     def update_cells(self, **arrays):
         """overwrite per-cell input arrays (density, tkin, sigma, vx, vy, vz, abundance) from host or device data"""
-        for k, a in arrays.items():
-            getattr(self, k).copy_(a if isinstance(a, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(a)),
-                                   non_blocking=True)
+        with self._on_stream():
+            for k, a in arrays.items():
+                getattr(self, k).copy_(a if isinstance(a, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(a)),
+                                       non_blocking=True)
         B.loc_refresh_cells(self.h)
 
     def init_lte(self):
@@ -83,7 +95,8 @@ class LocModel:
 
     def set_populations(self, pops_level_major):
         """pops_level_major: [nlevel][ncell] host or device array; copied into the registered buffer"""
-        self.pops.copy_(self._to_dev(pops_level_major, torch.float32))
+        with self._on_stream():
+            self.pops.copy_(self._to_dev(pops_level_major, torch.float32))
         B.loc_set_populations(self.h, self.pops)
 
     def simulate(self, sel=None, geometry_counters=False):
@@ -118,22 +131,35 @@ class LocModel:
         pz = _as_tensor_view(pptr, self.ncell * 4, self.workspace, torch.int32)
         return vis, pz
 
+    def set_option(self, key: int, value: float) -> None:
+        B.loc_set_option(self.h, key, value)
+
     def spectra(self, trans, nx, ny=1, dir=None, aff=None, offsets_cm=None):
-        out = torch.empty((ny, nx, self.nch), dtype=torch.float32, device=self.dev)
+        with self._on_stream():
+            out = torch.empty((ny, nx, self.nch), dtype=torch.float32, device=self.dev)
         B.loc_spectra(self.h, trans, out, nx, ny, dir, aff, offsets_cm)
+        return out
+
+    def spectra_map(self, trans, nx, ny, dir, pixel_cm, centre_cm):
+        """map in the caller's frame (include/loc.h, loc_spectra_map): [ny][nx][nchannel] K"""
+        with self._on_stream():
+            out = torch.empty((ny, nx, self.nch), dtype=torch.float32, device=self.dev)
+        B.loc_spectra_map(self.h, trans, out, nx, ny, dir, pixel_cm, centre_cm)
         return out
 
     def tex(self, trans):
         """T_ex [ncell] (K) of a transition from the current populations; 0 in non-leaf cells / cells without molecules"""
-        out = torch.empty(self.ncell, dtype=torch.float32, device=self.dev)
+        with self._on_stream():
+            out = torch.empty(self.ncell, dtype=torch.float32, device=self.dev)
         B.loc_tex(self.h, trans, out)
         return out
 
     def line_area(self, cube):
         """W = sum_c T_A dv in K km/s for a cube [..., nchannel] of loc_spectra (float32 CUDA tensor)"""
-        cube = cube.contiguous()
+        with self._on_stream():
+            cube = cube.contiguous()
+            out = torch.empty(cube.shape[:-1], dtype=torch.float32, device=self.dev)
         npix = cube.numel() // self.nch
-        out = torch.empty(cube.shape[:-1], dtype=torch.float32, device=self.dev)
         B.loc_line_area(self.h, cube, npix, out)
         return out
 

@@ -1,5 +1,7 @@
 """GPU parity on the edges of the method and of the library's limits, against the float64 oracle (same tolerances as
-the main parity tests): degenerate grids (two shells, a root grid of 2^3 cells, one root cell refined three times), bands narrower than a warp / than the 3D kernel's span,
+the main parity tests): degenerate grids (two shells, a root grid of 2^3 cells, one root cell refined three times), bands narrower than a warp / than the 3D kernel's span
+-- with the configs' own band width, i.e. channels up to 5 sigma wide (under-resolved profiles: the sampled profile of
+PAPER.md:73 is then not normalised, and the kernels follow the oracle's sampled values; include/loc.h, loc_set_option) --,
 cells without gas, the largest transition count of one ray pass (LOC_MAX_TRANS = 12), level counts that take the
 generic shared-memory solver (7) and the local-memory solver (20 > 16), a single transition."""
 import numpy as np
@@ -25,11 +27,16 @@ def _leaf(m):
     return (m.child < 0) if hasattr(m, "child") else np.ones(len(m.density), bool)
 
 
-def _resolve(m):
-    """narrow the band of a model with very few channels so that the line profile stays resolved (dv = sigma_turb / 2;
-    DESIGN 5.3: the window rule assumes dv <= sigma, as in every model of the paper): the lines then also run over the
-    edges of the band"""
-    m.band_half = 0.5 * m.nchannel * 0.5 * float(np.min(m.sigma))
+def _physical_band(m):
+    """For the ITERATION cases only.  With channels wider than ~2.5 sigma a sampled profile value phi_c = dv / (sigma sqrt(2 pi))
+    exceeds 1, the self-absorbed fraction LAM of PAPER.md:81 exceeds 1 and the oracle's own ALI iteration leaves the physical
+    range (negative populations after two iterations of the 5-channel C1 model: nothing to compare).  The first-simulate
+    counters ARE compared at the configs' own band (dv up to 9.6 sigma); the iteration runs with dv = 2 sigma_turb, still
+    under-resolved (sum of the sampled profile 7e-3 off 1), where the method is defined."""
+    dv = 2.0 * m.band_half / m.nchannel
+    smin = float(np.min(m.sigma))
+    if dv > 2.0 * smin:
+        m.band_half = 0.5 * m.nchannel * 2.0 * smin
     return m
 
 
@@ -76,20 +83,16 @@ def _iterate_case(m, niter, sel=None):
                                  dict(which=2, ns=30, nchannel=33, nsub=1, nlevel=2)])
 def test_1d_degenerate_grids_and_bands(cfg):
     m = W.shell_config(**cfg)
-    if m.nchannel < 16:
-        _resolve(m)
     _counters_case(m)
-    _iterate_case(m, 3)
+    _iterate_case(_physical_band(m), 3)
 
 
 @pytest.mark.parametrize("cfg", [dict(nroot=2, nlev=1, nside=1, nch=8), dict(nroot=2, nlev=1, nside=1, nch=4, nls=2),
                                  dict(nroot=1, nlev=3, nside=1, nch=20, frac=1.0), dict(nroot=3, nlev=2, nside=2, nch=31, frac=0.5, nls=2)])
 def test_3d_degenerate_grids_and_bands(cfg):
     m = small(**cfg)
-    if m.nchannel < 32:
-        _resolve(m)
     _counters_case(m)
-    _iterate_case(m, 2)
+    _iterate_case(_physical_band(m), 2)
 
 
 def test_cells_without_gas():
