@@ -55,7 +55,11 @@ extern "C" {
 #define LOC_OPT_SPAN_XCLIP 3     /* (3.4) 3D kernel: a step whose 32-channel span does not reach X sigma, X^2 = xclip^2 +
                                     2 ln max(1, tau0), takes two spans or the masked path                               */
 #define LOC_OPT_SIM3D_PARTS 4    /* (0 = automatic) 3D kernel: split the traced transitions over at least this many launches */
-#define LOC_OPT_SOLVER_LOCAL 5   /* (0) 1 = use the local-memory solver for every level count (A/B measurements)          */
+#define LOC_OPT_SOLVER 5         /* (0 = automatic: float32 in registers for species of <= 12 levels whose transitions and
+                                    collisional pairs all run from the higher to the lower level index, else float64)
+                                    1 = float64 solver with the matrix in local memory, 2 = float64 solver with the matrix in
+                                    shared memory (<= 16 levels): A/B measurements and reference runs                    */
+#define LOC_OPT_SOLVER_LOCAL LOC_OPT_SOLVER /* earlier name of the key */
 
 typedef struct loc_model loc_model; /* opaque */
 

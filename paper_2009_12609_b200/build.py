@@ -14,7 +14,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libloc_b200.so")
-SOURCES = ["loc_api.cu", "loc_sim1d.cu", "loc_paths3d.cu", "loc_sim3d.cu", "loc_spectra.cu"]
+SOURCES = ["loc_api.cu", "loc_solve.cu", "loc_sim1d.cu", "loc_paths3d.cu", "loc_sim3d.cu", "loc_spectra.cu"]
 HEADERS = [os.path.join(CSRC, "loc_internal.cuh"), os.path.join(os.path.dirname(HERE), "include", "loc.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]

@@ -72,6 +72,7 @@ static int64_t carve(loc_model *m, Carver &c, const loc_grid *g, int nch, int nl
     m->sp.cl = c.take<int>(ncoll);
     m->sp.temps = c.take<double>(64);
     m->sp.rates = c.take<double>((int64_t)64 * ncoll);
+    m->d_rates_f = c.take<float>(64 * 66);
     if (g->kind == LOC_GRID_SHELL) {
         int64_t ntab = 0;
         // triangular tables: ray i with tangent shell k0 has nshell-k0 entries; bound by nray*nshell
@@ -156,288 +157,6 @@ __global__ void k_coef(int64_t n, Selection S, const float *pops, float2 *coef)
         }
         coef[i * S.nsp + k] = v;
     }
-}
-
-// Statistical equilibrium of one cell per thread (DESIGN 5.5).  The rate matrix is a
-// continuous-time Markov generator; its stationary vector is found with the subtraction-free GTH elimination
-// in double precision (the oracle uses pivoted Gaussian elimination on the same equations).
-template <int NLMAX>
-__global__ void __launch_bounds__(128) k_solve(int64_t n, SpeciesDev sp, Selection S, const float *density, const float *tkin,
-                                               const float *abundance, const float2 *cnt, float *pops, float2 *coef,
-                                               unsigned int *maxrel_bits, const int32_t *child, int ali)
-{
-    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    bool act = i < n;
-    if (act && child && child[i] >= 0) act = false;  // refined cell: no gas of its own
-    float rel = 0.0f;
-    if (act) {
-        const int NL = sp.nlevel;
-        double R[NLMAX * NLMAX];
-        for (int k = 0; k < NL * NL; k++) R[k] = 0.0;
-        double dens = density[i], T = tkin[i];
-        double ntot = dens * (double)abundance[i];
-        // radiative rates
-        for (int t = 0; t < sp.ntrans; t++) {
-            int u = sp.upper[t], l = sp.lower[t];
-            double gr = sp.g[u] / sp.g[l];
-            double sj = sp.bgocc[t], esc = 1.0;  // DESIGN R23: untraced transitions see the background only
-            for (int k = 0; k < S.nsel; k++)
-                if (S.sel[k] == t) {
-                    float2 c = cnt[i * S.nsp + k];
-                    sj = c.x;
-                    esc = c.y;
-                    if (!ali) {
-                        // plain lambda iteration ("possible to run LOC without ALI"): the self term of
-                        // Eq. 2 goes back into the radiation field and A_ul stays unscaled.  Step by step it equals
-                        // (1 - ESC) times the source function of the populations the rays were traced with, whose
-                        // occupation number is em / kap of the cell's coefficient record (DESIGN 5.2, 6.2)
-                        float2 ke = coef[i * S.nsp + k];
-                        if (ke.x != 0.0f) sj += (1.0 - esc) * ((double)ke.y / (double)ke.x);
-                        esc = 1.0;
-                    }
-                }
-            double Slu = gr * sp.A[t] * sj;  // = B_lu * Jbar
-            R[u * NL + l] += sp.A[t] * esc + Slu / gr;
-            R[l * NL + u] += Slu;
-        }
-        // collisions: linear interpolation in T, clamped; upward by detailed balance
-        int j = 0;
-        double f = 0.0;
-        if (sp.ntemp > 1) {
-            if (T <= sp.temps[0]) {
-                j = 0;
-                f = 0.0;
-            } else if (T >= sp.temps[sp.ntemp - 1]) {
-                j = sp.ntemp - 2;
-                f = 1.0;
-            } else {
-                while (T > sp.temps[j + 1]) j++;
-                f = (T - sp.temps[j]) / (sp.temps[j + 1] - sp.temps[j]);
-            }
-        }
-        // Boltzmann factors g_k exp(-(E_k - E_0) / T) once per level (one exp per level instead of one per collisional pair)
-        double bz[NLMAX];
-        for (int k = 0; k < NL; k++) bz[k] = sp.g[k] * exp(-(sp.energy_K[k] - sp.energy_K[0]) / T);
-        for (int k = 0; k < sp.ncoll; k++) {
-            int u = sp.cu[k], l = sp.cl[k];
-            double gd = sp.rates[(int64_t)j * sp.ncoll + k];
-            if (sp.ntemp > 1) gd = (1.0 - f) * gd + f * sp.rates[(int64_t)(j + 1) * sp.ncoll + k];
-            double gu = gd * bz[u] / bz[l];
-            R[u * NL + l] += dens * gd;
-            R[l * NL + u] += dens * gu;
-        }
-        // GTH elimination
-        for (int q = NL - 1; q >= 1; q--) {
-            double s = 0.0;
-            for (int c = 0; c < q; c++) s += R[q * NL + c];
-            double inv = s > 0.0 ? 1.0 / s : 0.0;
-            for (int r = 0; r < q; r++) R[r * NL + q] *= inv;
-            for (int r = 0; r < q; r++) {
-                double rq = R[r * NL + q];
-                for (int c = 0; c < q; c++)
-                    if (c != r) R[r * NL + c] += rq * R[q * NL + c];
-            }
-        }
-        double x[NLMAX];
-        x[0] = 1.0;
-        double tot = 1.0;
-        for (int q = 1; q < NL; q++) {
-            double s = 0.0;
-            for (int r = 0; r < q; r++) s += x[r] * R[r * NL + q];
-            x[q] = s;
-            tot += s;
-        }
-        double sc = ntot / tot;
-        for (int l = 0; l < NL; l++) {
-            double nw = x[l] * sc;
-            double old = pops[(int64_t)l * n + i];
-            if (ntot > 0.0 && (nw >= 1e-10 * ntot || old >= 1e-10 * ntot))
-                rel = fmaxf(rel, (float)(fabs(nw - old) / fmax(nw, 1e-300)));
-            if (!isfinite(nw)) rel = INFINITY;  // reported by fetch_maxrel as LOC_ENONFINITE, never as "converged"
-            x[l] = nw;
-            pops[(int64_t)l * n + i] = (float)nw;
-        }
-        // refresh the line coefficients of the traced transitions from the unrounded solution
-        for (int k = 0; k < S.nsp; k++) {
-            float2 v = make_float2(0.f, 0.f);
-            if (k < S.nsel) {
-                v.x = (float)(S.ck[k] * (x[S.lower[k]] * (double)S.gratio[k] - x[S.upper[k]]));
-                v.y = (float)(S.ck[k] * x[S.upper[k]]);
-            }
-            coef[i * S.nsp + k] = v;
-        }
-    }
-    for (int o = 16; o >= 1; o >>= 1) rel = fmaxf(rel, __shfl_xor_sync(0xffffffffu, rel, o));
-    if ((threadIdx.x & 31) == 0 && rel > 0.0f) atomicMax(maxrel_bits, __float_as_uint(rel));
-}
-
-// k_solve_s: the same equations and the same GTH elimination as k_solve, laid out for the SM instead of for the
-// compiler's local-memory stack (profiles/r1_solve.md: k_solve<10> keeps R in 960 B of local memory per thread, 1.1 MB per
-// SM at its occupancy -- the L1 hit rate is 60 % and 34 of 35 issue slots wait on the long scoreboard).  Here the rate
-// matrix of a thread is a column of a shared-memory array R[NL*NL][threads] of doubles (conflict free, never leaves the
-// SM), the species tables are staged in shared memory once per block, and NL is a compile-time constant for the common
-// level counts (NLX > 0), so that the elimination is fully unrolled with static addresses and x[], bz[] are registers.
-#define LOC_SOLVE_THREADS 32  // cells per block: 31 KB of matrices at 10 levels, 7 blocks per SM (64: 62 KB, 3 blocks = 6 warps; C3 1.50 -> 1.35 ms)
-struct SolveTabs {   // byte offsets into the block's shared memory, after R
-    int g, energy, A, bg, gr, upper, lower, cu, cl, temps, rates, bytes;
-};
-
-template <int NLX>
-__global__ void __launch_bounds__(LOC_SOLVE_THREADS) k_solve_s(int64_t n, SpeciesDev sp, Selection S, const float *density, const float *tkin,
-                                                               const float *abundance, const float2 *cnt, float *pops, float2 *coef,
-                                                               unsigned int *maxrel_bits, const int32_t *child, int ali, SolveTabs TB)
-{
-    constexpr int NLM = NLX > 0 ? NLX : 16;
-    extern __shared__ __align__(16) unsigned char s_raw[];
-    const int NL = NLX > 0 ? NLX : sp.nlevel;
-    const int tid = threadIdx.x;
-    double *Rs = reinterpret_cast<double *>(s_raw);
-    unsigned char *tb = s_raw + sizeof(double) * (NL * NL + 2 * NL) * LOC_SOLVE_THREADS;
-    double *t_g = reinterpret_cast<double *>(tb + TB.g), *t_e = reinterpret_cast<double *>(tb + TB.energy);
-    double *t_A = reinterpret_cast<double *>(tb + TB.A), *t_bg = reinterpret_cast<double *>(tb + TB.bg), *t_gr = reinterpret_cast<double *>(tb + TB.gr);
-    double *t_temps = reinterpret_cast<double *>(tb + TB.temps), *t_rates = reinterpret_cast<double *>(tb + TB.rates);
-    int *t_up = reinterpret_cast<int *>(tb + TB.upper), *t_lo = reinterpret_cast<int *>(tb + TB.lower);
-    int *t_cu = reinterpret_cast<int *>(tb + TB.cu), *t_cl = reinterpret_cast<int *>(tb + TB.cl);
-    for (int k = tid; k < NL; k += LOC_SOLVE_THREADS) {
-        t_g[k] = sp.g[k];
-        t_e[k] = sp.energy_K[k];
-    }
-    for (int k = tid; k < sp.ntrans; k += LOC_SOLVE_THREADS) {
-        t_A[k] = sp.A[k];
-        t_gr[k] = sp.g[sp.upper[k]] / sp.g[sp.lower[k]];
-        t_bg[k] = sp.bgocc[k];
-        t_up[k] = sp.upper[k];
-        t_lo[k] = sp.lower[k];
-    }
-    for (int k = tid; k < sp.ncoll; k += LOC_SOLVE_THREADS) {
-        t_cu[k] = sp.cu[k];
-        t_cl[k] = sp.cl[k];
-    }
-    for (int k = tid; k < sp.ntemp; k += LOC_SOLVE_THREADS) t_temps[k] = sp.temps[k];
-    for (int k = tid; k < sp.ntemp * sp.ncoll; k += LOC_SOLVE_THREADS) t_rates[k] = sp.rates[k];
-    __syncthreads();
-#define RM(a) Rs[(a) * LOC_SOLVE_THREADS + tid]
-#define VX(a) Rs[(NL * NL + (a)) * LOC_SOLVE_THREADS + tid]  // 2 NL more doubles per thread: Boltzmann factors (then the solution)
-#define VI(a) Rs[(NL * NL + NL + (a)) * LOC_SOLVE_THREADS + tid]  //   and their inverses
-    int64_t i = blockIdx.x * (int64_t)LOC_SOLVE_THREADS + tid;
-    bool act = i < n;
-    if (act && child && child[i] >= 0) act = false;  // refined cell: no gas of its own
-    float rel = 0.0f;
-    if (act) {
-#pragma unroll
-        for (int k = 0; k < NLM * NLM; k++)
-            if (k < NL * NL) RM(k) = 0.0;
-        const double dens = density[i], T = tkin[i];
-        const double ntot = dens * (double)abundance[i];
-        // radiative rates: traced transitions from their counters, the others see the background only (DESIGN R23)
-        for (int t = 0; t < sp.ntrans; t++) {
-            const int u = t_up[t], l = t_lo[t];
-            const double gr = t_gr[t];
-            double sj = t_bg[t], esc = 1.0;
-            for (int k = 0; k < S.nsel; k++)
-                if (S.sel[k] == t) {
-                    const float2 c = cnt[i * S.nsp + k];
-                    sj = c.x;
-                    esc = c.y;
-                    if (!ali) {  // plain lambda iteration: see k_solve
-                        const float2 ke = coef[i * S.nsp + k];
-                        if (ke.x != 0.0f) sj += (1.0 - esc) * ((double)ke.y / (double)ke.x);
-                        esc = 1.0;
-                    }
-                }
-            const double Aul = t_A[t];
-            RM(u * NL + l) += Aul * esc + Aul * sj;  // spontaneous (scaled by the escape probability) + induced
-            RM(l * NL + u) += gr * Aul * sj;          // S_lu = B_lu * Jbar
-        }
-        // collisions: linear interpolation in T, clamped; upward by detailed balance
-        int j = 0;
-        double f = 0.0;
-        if (sp.ntemp > 1) {
-            if (T <= t_temps[0]) {
-                j = 0;
-                f = 0.0;
-            } else if (T >= t_temps[sp.ntemp - 1]) {
-                j = sp.ntemp - 2;
-                f = 1.0;
-            } else {
-                while (T > t_temps[j + 1]) j++;
-                f = (T - t_temps[j]) / (t_temps[j + 1] - t_temps[j]);
-            }
-        }
-        // g_k exp(-(E_k - E_0) / T), once per level
-        const double invT = 1.0 / T;
-        for (int k = 0; k < NL; k++) {
-            const double b = t_g[k] * exp(-(t_e[k] - t_e[0]) * invT);
-            VX(k) = b;
-            VI(k) = 1.0 / b;  // one division per level instead of one per collisional pair
-        }
-        for (int k = 0; k < sp.ncoll; k++) {
-            const int u = t_cu[k], l = t_cl[k];
-            double gd = t_rates[j * sp.ncoll + k];
-            if (sp.ntemp > 1) gd = (1.0 - f) * gd + f * t_rates[(j + 1) * sp.ncoll + k];
-            RM(u * NL + l) += dens * gd;
-            RM(l * NL + u) += dens * (gd * VX(u) * VI(l));
-        }
-        // GTH elimination
-#pragma unroll
-        for (int q = NLM - 1; q >= 1; q--) {
-            if (q < NL) {
-                double sm = 0.0;
-#pragma unroll
-                for (int c = 0; c < q; c++) sm += RM(q * NL + c);
-                const double inv = sm > 0.0 ? 1.0 / sm : 0.0;
-#pragma unroll
-                for (int r = 0; r < q; r++) {
-                    const double rq = RM(r * NL + q) * inv;
-                    RM(r * NL + q) = rq;
-#pragma unroll
-                    for (int c = 0; c < q; c++)
-                        if (c != r) RM(r * NL + c) += rq * RM(q * NL + c);
-                }
-            }
-        }
-        double x[NLM];
-        x[0] = 1.0;
-        double tot = 1.0;
-#pragma unroll
-        for (int q = 1; q < NLM; q++) {
-            if (q < NL) {
-                double sm = 0.0;
-#pragma unroll
-                for (int r = 0; r < q; r++) sm += x[r] * RM(r * NL + q);
-                x[q] = sm;
-                tot += sm;
-            }
-        }
-        const double sc = ntot / tot;
-#pragma unroll
-        for (int l = 0; l < NLM; l++) {
-            if (l < NL) {
-                const double nw = x[l] * sc;
-                const double old = pops[(int64_t)l * n + i];
-                if (ntot > 0.0 && (nw >= 1e-10 * ntot || old >= 1e-10 * ntot))
-                    rel = fmaxf(rel, (float)(fabs(nw - old) / fmax(nw, 1e-300)));
-                if (!isfinite(nw)) rel = INFINITY;  // see k_solve
-                VX(l) = nw;
-                pops[(int64_t)l * n + i] = (float)nw;
-            }
-        }
-        // refresh the line coefficients of the traced transitions from the unrounded solution
-        for (int k = 0; k < S.nsp; k++) {
-            float2 v = make_float2(0.f, 0.f);
-            if (k < S.nsel) {
-                const double xu = VX(S.upper[k]), xl = VX(S.lower[k]);
-                v.x = (float)(S.ck[k] * (xl * (double)S.gratio[k] - xu));
-                v.y = (float)(S.ck[k] * xu);
-            }
-            coef[i * S.nsp + k] = v;
-        }
-    }
-#undef RM
-#undef VX
-#undef VI
-    for (int o = 16; o >= 1; o >>= 1) rel = fmaxf(rel, __shfl_xor_sync(0xffffffffu, rel, o));
-    if ((threadIdx.x & 31) == 0 && rel > 0.0f) atomicMax(maxrel_bits, __float_as_uint(rel));
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -693,6 +412,18 @@ extern "C" int loc_set_species(loc_model *m, int nlevel, const double *energy_K,
     memcpy(m->h_energy, energy_K, sizeof(double) * nlevel);
     memcpy(m->h_g, g, sizeof(double) * nlevel);
     free(m->h_upper); free(m->h_lower); free(m->h_A); free(m->h_freq);
+    free(m->h_cu); free(m->h_cl); free(m->h_temps); free(m->h_rates);
+    m->h_cu = (int *)malloc(sizeof(int) * std::max(ncoll, 1));
+    m->h_cl = (int *)malloc(sizeof(int) * std::max(ncoll, 1));
+    m->h_temps = (double *)malloc(sizeof(double) * ntemp);
+    m->h_rates = (double *)malloc(sizeof(double) * ntemp * std::max(ncoll, 1));
+    if (ncoll) {
+        memcpy(m->h_cu, cu, sizeof(int) * ncoll);
+        memcpy(m->h_cl, cl, sizeof(int) * ncoll);
+        memcpy(m->h_temps, temps_K, sizeof(double) * ntemp);
+        memcpy(m->h_rates, rate_down, sizeof(double) * ntemp * ncoll);
+    }
+    m->rates_f_valid = false;
     m->h_upper = (int *)malloc(sizeof(int) * ntrans);
     m->h_lower = (int *)malloc(sizeof(int) * ntrans);
     m->h_A = (double *)malloc(sizeof(double) * ntrans);
@@ -823,68 +554,6 @@ extern "C" int loc_get_counters(loc_model *m, const float **counters, int *ntp, 
     return LOC_OK;
 }
 
-static int solve_async(loc_model *m)
-{
-    int64_t n = m->ncell;
-    const int32_t *ch = m->kind == LOC_GRID_OCTREE ? m->child : nullptr;
-    unsigned nb = (unsigned)((n + 127) / 128);
-#define LOC_SOLVE(NLMAX)                                                                                                     \
-    k_solve<NLMAX><<<nb, 128, 0, m->stream>>>(n, m->sp, m->selh, m->cells.density, m->cells.tkin, m->cells.abundance, m->cnt, \
-                                              m->pops, m->coef, m->d_maxrel, ch, m->ali)
-    // shared-memory solver (k_solve_s) while a block's matrices and the species tables fit; loc_set_option(LOC_OPT_SOLVER_LOCAL)
-    // forces the local-memory kernel (A/B measurements)
-    {
-        const int NL = m->nlevel;
-        SolveTabs T;
-        int o = 0;
-        auto take = [&](int bytes) {
-            int at = o;
-            o += (bytes + 7) & ~7;
-            return at;
-        };
-        T.g = take(8 * NL);
-        T.energy = take(8 * NL);
-        T.A = take(8 * m->ntrans);
-        T.bg = take(8 * m->ntrans);
-        T.gr = take(8 * m->ntrans);
-        T.temps = take(8 * m->ntemp);
-        T.rates = take(8 * m->ntemp * m->ncoll);
-        T.upper = take(4 * m->ntrans);
-        T.lower = take(4 * m->ntrans);
-        T.cu = take(4 * m->ncoll);
-        T.cl = take(4 * m->ncoll);
-        T.bytes = o;
-        const size_t smem = sizeof(double) * (size_t)(NL * NL + 2 * NL) * LOC_SOLVE_THREADS + (size_t)o;
-        if (NL <= 16 && smem <= 200 * 1024 && !m->solver_local) {
-            const unsigned nbs = (unsigned)((n + LOC_SOLVE_THREADS - 1) / LOC_SOLVE_THREADS);
-#define LOC_SOLVE_S(NLX)                                                                                                          \
-    do {                                                                                                                          \
-        LOC_CUDA_CHECK(m, cudaFuncSetAttribute(k_solve_s<NLX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));          \
-        k_solve_s<NLX><<<nbs, LOC_SOLVE_THREADS, smem, m->stream>>>(n, m->sp, m->selh, m->cells.density, m->cells.tkin,          \
-                                                                    m->cells.abundance, m->cnt, m->pops, m->coef, m->d_maxrel, ch, \
-                                                                    m->ali, T);                                                   \
-    } while (0)
-            if (NL == 10) LOC_SOLVE_S(10);
-            else if (NL == 5) LOC_SOLVE_S(5);
-            else if (NL == 4) LOC_SOLVE_S(4);
-            else LOC_SOLVE_S(0);
-#undef LOC_SOLVE_S
-            m->launches++;
-            LOC_CUDA_CHECK(m, cudaGetLastError());
-            m->coef_valid = true;
-            return LOC_OK;
-        }
-    }
-    if (m->nlevel <= 6) LOC_SOLVE(6);
-    else if (m->nlevel <= 10) LOC_SOLVE(10);
-    else if (m->nlevel <= 16) LOC_SOLVE(16);
-    else LOC_SOLVE(32);
-    m->launches++;
-    LOC_CUDA_CHECK(m, cudaGetLastError());
-    m->coef_valid = true;
-    return LOC_OK;
-}
-
 static int fetch_maxrel(loc_model *m, double *out)
 {
     unsigned int bits = 0;
@@ -906,7 +575,7 @@ extern "C" int loc_solve(loc_model *m, double *max_rel_change)
     if (!m->have_species || !m->pops) return fail(m, LOC_ESTATE, "species and populations must be set before loc_solve");
     if (!m->simulated) return fail(m, LOC_ESTATE, "loc_solve: no loc_simulate has filled the counters");
     LOC_CUDA_CHECK(m, cudaMemsetAsync(m->d_maxrel, 0, sizeof(unsigned int), m->stream));
-    int rc = solve_async(m);
+    int rc = loc_launch_solve(m);
     if (rc) return rc;
     return fetch_maxrel(m, max_rel_change);
 }
@@ -922,7 +591,7 @@ extern "C" int loc_iterate(loc_model *m, int niter, double *max_rel_change)
         int rc = loc_simulate(m, 0, nullptr, 0);
         if (rc) return rc;
         LOC_CUDA_CHECK(m, cudaMemsetAsync(m->d_maxrel, 0, sizeof(unsigned int), m->stream));
-        rc = solve_async(m);
+        rc = loc_launch_solve(m);
         if (rc) return rc;
     }
     return fetch_maxrel(m, max_rel_change);
@@ -955,9 +624,9 @@ extern "C" int loc_set_option(loc_model *m, int key, double value)
         if (!(value >= 0.0 && value <= LOC_MAX_TRANS) || value != floor(value)) return fail(m, LOC_EINVAL, "LOC_OPT_SIM3D_PARTS must be an integer in [0, LOC_MAX_TRANS]");
         m->sim3d_parts = (int)value;
         return LOC_OK;
-    case LOC_OPT_SOLVER_LOCAL:
-        if (value != 0.0 && value != 1.0) return fail(m, LOC_EINVAL, "LOC_OPT_SOLVER_LOCAL must be 0 or 1");
-        m->solver_local = (int)value;
+    case LOC_OPT_SOLVER:
+        if (value != 0.0 && value != 1.0 && value != 2.0) return fail(m, LOC_EINVAL, "LOC_OPT_SOLVER must be 0, 1 or 2");
+        m->solver = (int)value;
         return LOC_OK;
     }
     return fail(m, LOC_EINVAL, "loc_set_option: unknown key");
@@ -972,7 +641,7 @@ extern "C" int loc_iterate_until(loc_model *m, int max_iter, double tol, int *ni
         int rc = loc_simulate(m, 0, nullptr, 0);
         if (rc) return rc;
         LOC_CUDA_CHECK(m, cudaMemsetAsync(m->d_maxrel, 0, sizeof(unsigned int), m->stream));
-        rc = solve_async(m);
+        rc = loc_launch_solve(m);
         if (rc) return rc;
         rc = fetch_maxrel(m, &ch);  // one host synchronisation per iteration: the stopping rule needs the scalar
         if (rc) return rc;
@@ -1060,6 +729,10 @@ extern "C" void loc_destroy_model(loc_model *m)
     free(m->h_lower);
     free(m->h_A);
     free(m->h_freq);
+    free(m->h_cu);
+    free(m->h_cl);
+    free(m->h_temps);
+    free(m->h_rates);
     free(m->h_rout);
     free(m->h_dirs);
     delete m;

@@ -101,6 +101,10 @@ struct loc_model {
     double h_energy[LOC_MAX_LEVELS], h_g[LOC_MAX_LEVELS];
     int *h_upper, *h_lower;
     double *h_A, *h_freq;
+    int *h_cu, *h_cl;           // host copies of the collisional pairs, temperatures and rates (dense tables of k_solve_f)
+    double *h_temps, *h_rates;
+    float *d_rates_f;           // [64][66] dense float32 rate table of k_solve_f (ntemp > 1)
+    bool rates_f_valid;
     Selection selh;
     bool coef_valid;
     int ali;  // 1: accelerated lambda iteration (default), 0: plain lambda iteration (loc_set_ali)
@@ -108,7 +112,7 @@ struct loc_model {
     // accuracy knobs (DESIGN 5.3), set through loc_set_option only
     float xmin, eps_tau, xclip;
     int sim3d_parts;   // 0 = automatic split of the traced transitions over launches
-    int solver_local;  // 1 = force the local-memory solver k_solve
+    int solver;        // loc_set_option(LOC_OPT_SOLVER): 0 = automatic, 1 = float64 local memory, 2 = float64 shared memory
     int nsm;           // multiprocessors of the model's device (queried once in loc_create_model)
     bool simulated;    // counters hold the result of a loc_simulate
     // 1D
@@ -425,6 +429,7 @@ static inline Tree make_tree(const loc_model *m)
 // ------------------------------------------------------------------------------------------------
 // kernels / launchers implemented in the other translation units
 // ------------------------------------------------------------------------------------------------
+int loc_launch_solve(loc_model *m);
 int loc_launch_sim1d(loc_model *m, int geom);
 int loc_launch_sim3d(loc_model *m, int geom);
 int loc_setup3d(loc_model *m);
