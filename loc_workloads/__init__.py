@@ -306,6 +306,99 @@ def build_octree(fields: dict, nroot: int, nlev: int, refine_frac) -> dict:
     return out
 
 
+# ---- the same recipe on torch (CUDA when there is one): full-size C4 / C5 only ---------------------------------
+# numpy needs minutes for the 512^3 / 1024^3 fields (complex128 FFTs, fancy indexing over 2e8 cells); the white noise still
+# comes from the seeded numpy generator, so the realisation does not depend on the machine beyond the rounding of the FFT.
+TORCH_FROM_NFINE = 512
+
+
+def _torch_device():
+    import torch
+    return torch.device("cuda", torch.cuda.current_device()) if torch.cuda.is_available() else torch.device("cpu")
+
+
+def gaussian_field_t(n: int, slope: float, gen: np.random.Generator, device):
+    """gaussian_field() with the FFTs and the filter on `device` in float32 / complex64; returns a torch tensor [z][y][x]"""
+    import torch
+    white = torch.from_numpy(gen.standard_normal((n, n, n), dtype=np.float32)).to(device)
+    fk = torch.fft.rfftn(white)
+    del white
+    kx = torch.fft.fftfreq(n, device=device) * n
+    kz = torch.fft.rfftfreq(n, device=device) * n
+    k2 = kx[:, None, None] ** 2 + kx[None, :, None] ** 2 + kz[None, None, :] ** 2
+    k2[0, 0, 0] = 1.0
+    fk *= k2 ** (slope / 4.0)
+    del k2
+    fk[0, 0, 0] = 0.0
+    f = torch.fft.irfftn(fk, s=(n, n, n))
+    del fk
+    f -= f.mean()
+    f /= f.std(unbiased=False)
+    return f
+
+
+def build_octree_t(fields: dict, nroot: int, nlev: int, refine_frac, device) -> dict:
+    """build_octree() on torch tensors (same rules, same array layout); returns numpy arrays"""
+    import torch
+    if np.isscalar(refine_frac):
+        refine_frac = [refine_frac] * (nlev - 1)
+
+    def coarsen(a, w=None):
+        n = a.shape[0] // 2
+        if w is None:
+            return a.reshape(n, 2, n, 2, n, 2).mean(dim=(1, 3, 5))
+        return (a * w).reshape(n, 2, n, 2, n, 2).sum(dim=(1, 3, 5)) / w.reshape(n, 2, n, 2, n, 2).sum(dim=(1, 3, 5))
+
+    pyr = [None] * nlev
+    cur = dict(fields)
+    for l in range(nlev - 1, -1, -1):
+        pyr[l] = cur
+        if l > 0:
+            d = cur["density"].double()
+            nxt = {"density": coarsen(d)}
+            for k in cur:
+                if k != "density":
+                    nxt[k] = coarsen(cur[k].double(), d if k in ("vx", "vy", "vz") else None)
+            del d
+            cur = nxt
+    r = torch.arange(nroot, device=device, dtype=torch.int32)
+    iz, iy, ix = torch.meshgrid(r, r, r, indexing="ij")
+    coords = [torch.stack([ix.reshape(-1), iy.reshape(-1), iz.reshape(-1)], dim=1)]
+    oct_ = torch.tensor([[cx, cy, cz] for cz in (0, 1) for cy in (0, 1) for cx in (0, 1)], dtype=torch.int32, device=device)
+    childs = []
+    for l in range(nlev):
+        c = coords[l]
+        nc = c.shape[0]
+        ch = torch.full((nc,), -1, dtype=torch.int32, device=device)
+        if l < nlev - 1:
+            nref = int(round(refine_frac[l] * nc)) if refine_frac[l] > 0 else 0
+            if nref > 0:
+                dens = pyr[l]["density"][c[:, 2].long(), c[:, 1].long(), c[:, 0].long()]
+                thr = torch.kthvalue(dens, nc - nref + 1).values
+                refined = torch.nonzero(dens >= thr).reshape(-1)[:nref]  # ties: the first nref in cell order
+                del dens
+                ch[refined] = 8 * torch.arange(refined.shape[0], dtype=torch.int32, device=device)
+                coords.append((2 * c[refined][:, None, :] + oct_[None, :, :]).reshape(-1, 3))
+            else:
+                coords.append(torch.zeros((0, 3), dtype=torch.int32, device=device))
+        childs.append(ch)
+    while len(coords) > 1 and coords[-1].shape[0] == 0:
+        coords.pop()
+    nlev_eff = len(coords)
+    childs = childs[:nlev_eff]
+    noff = np.zeros(nlev_eff + 1, np.int64)
+    for l in range(nlev_eff):
+        noff[l + 1] = noff[l] + coords[l].shape[0]
+    out = {"nlev": nlev_eff, "noff": noff, "child": torch.cat(childs).cpu().numpy(),
+           "level": np.concatenate([np.full(coords[l].shape[0], l, np.int8) for l in range(nlev_eff)])}
+    idx = [(coords[l][:, 2].long(), coords[l][:, 1].long(), coords[l][:, 0].long()) for l in range(nlev_eff)]
+    for k in fields:
+        out[k] = torch.cat([pyr[l][k][idx[l]].float() for l in range(nlev_eff)]).cpu().numpy()
+    del idx
+    out["coords"] = torch.cat(coords).cpu().numpy()
+    return out
+
+
 def cloud_config(which: int, nroot: int | None = None, nlev: int | None = None, nchannel: int | None = None,
                  nside: int | None = None, refine_frac=None, nlevel_species: int | None = None,
                  seed_config: int | None = None) -> OctreeModel:
@@ -324,19 +417,36 @@ def cloud_config(which: int, nroot: int | None = None, nlev: int | None = None, 
     frac = cfg["frac"] if refine_frac is None else refine_frac
     sc = seed_config if seed_config is not None else which
     nfine = nroot * 2 ** (nlev - 1)
-    g = gaussian_field(nfine, -11.0 / 3.0, rng(sc, 2))
     sln = cfg["sln"]
-    dens = (1e3 * np.exp(sln * g - 0.5 * sln * sln)).astype(np.float32)
-    del g
     s1 = cfg["vrms"] * KMS / math.sqrt(3.0)
-    fields = {"density": dens}
-    for k, st in (("vx", 3), ("vy", 4), ("vz", 5)):
-        fields[k] = np.clip(gaussian_field(nfine, -11.0 / 3.0, rng(sc, st)) * s1, -5 * s1, 5 * s1).astype(np.float32)
-    if which == 4:
-        fields["tkin"] = rng(sc, 6).uniform(10.0, 20.0, size=(nfine,) * 3).astype(np.float32)
+    if nfine >= TORCH_FROM_NFINE:
+        import torch
+        dev = _torch_device()
+        g = gaussian_field_t(nfine, -11.0 / 3.0, rng(sc, 2), dev)
+        fields = {"density": 1e3 * torch.exp(sln * g - 0.5 * sln * sln)}
+        del g
+        for k, st in (("vx", 3), ("vy", 4), ("vz", 5)):
+            fields[k] = torch.clamp(gaussian_field_t(nfine, -11.0 / 3.0, rng(sc, st), dev) * s1, -5 * s1, 5 * s1)
+        if which == 4:
+            fields["tkin"] = torch.from_numpy(rng(sc, 6).uniform(10.0, 20.0, size=(nfine,) * 3).astype(np.float32)).to(dev)
+        else:
+            fields["tkin"] = torch.full((nfine,) * 3, 10.0, dtype=torch.float32, device=dev)
+        tree = build_octree_t(fields, nroot, nlev, frac, dev)
+        del fields
+        if dev.type == "cuda":
+            torch.cuda.empty_cache()
     else:
-        fields["tkin"] = np.full((nfine,) * 3, 10.0, np.float32)
-    tree = build_octree(fields, nroot, nlev, frac)
+        g = gaussian_field(nfine, -11.0 / 3.0, rng(sc, 2))
+        dens = (1e3 * np.exp(sln * g - 0.5 * sln * sln)).astype(np.float32)
+        del g
+        fields = {"density": dens}
+        for k, st in (("vx", 3), ("vy", 4), ("vz", 5)):
+            fields[k] = np.clip(gaussian_field(nfine, -11.0 / 3.0, rng(sc, st)) * s1, -5 * s1, 5 * s1).astype(np.float32)
+        if which == 4:
+            fields["tkin"] = rng(sc, 6).uniform(10.0, 20.0, size=(nfine,) * 3).astype(np.float32)
+        else:
+            fields["tkin"] = np.full((nfine,) * 3, 10.0, np.float32)
+        tree = build_octree(fields, nroot, nlev, frac)
     ncell = int(tree["noff"][-1])
     sp = rotor_species(nlevel_species or 10, sc)
     sel = np.array([0, 1, 2], np.int32) if which == 5 else None
