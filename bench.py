@@ -11,6 +11,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import subprocess
 import sys
@@ -25,13 +26,15 @@ import numpy as np
 
 METRIC = "ray-cell-channel updates/sec per ALI iteration"
 UNIT = "updates/s"
-DEFAULT_WORKLOAD = "C4"
+VALUE_KIND = "active updates: channels within 5 sigma of the line centre x traced transitions x ray-cell steps (DESIGN.md 8.1)"
+DEFAULT_WORKLOAD = "C5"
 
 # ---- roofline constants -----------------------------------------------------------------------------
 N_SM = 148
 # DRAM bytes read + written by one launch of the dominant kernel, from the committed `ncu --set full` captures
 # (profiles/r1_v9_summary.md, profiles/r1_sim1d_C2.md); workloads without a capture report null
-NCU_TRAFFIC_BYTES = {"C2": 24.3e6, "C3": 19.09e9 + 7.88e9, "C4": 904.4e9 + 299.2e9}
+NCU_TRAFFIC_BYTES = {"C2": (24.3e6, "profiles/r1_sim1d_C2.md"), "C3": (19.09e9 + 7.88e9, "profiles/r1_v9_summary.md"),
+                     "C4": (904.4e9 + 299.2e9, "profiles/r1_v9_summary.md")}
 FP32_LANES_PER_SM_CLK = 128  # 4 sub-partitions x 1 warp instruction / clk
 MUFU_PER_SM_CLK = 16
 
@@ -106,10 +109,30 @@ class ClockSampler(threading.Thread):
 
 
 # ---- CPU oracle sample (cpu_baseline / --impl reference) --------------------------------------------------------------
-def oracle_sample(m, budget_updates=6e9):
+_KB_OVER_AMU = 1.380649e-16 / 1.66053906660e-24
+
+
+def active_channels_per_cell(m, d=None):
+    """the counting rule of the metric: number of channels with |v_c - v_0| <= 5 sigma for one ray
+    step through each cell, for propagation direction d (3D) or for mu = 1 (1D: an upper bound is not needed -- the 1D arm
+    counts per step, see oracle_sample).  float64 numpy; the library counts the same rule per step in float32."""
+    dv = 2.0 * m.band_half / m.nchannel
+    sig = np.sqrt(np.asarray(m.sigma, np.float64) ** 2 + (_KB_OVER_AMU / m.species.mass_amu if m.species.mass_amu > 0 else 0.0)
+                  * np.asarray(m.tkin, np.float64))
+    v0 = -(np.asarray(m.vx, np.float64) * d[0] + np.asarray(m.vy, np.float64) * d[1] + np.asarray(m.vz, np.float64) * d[2])
+    cc = v0 / dv + 0.5 * (m.nchannel - 1)
+    hw = 5.0 * sig / dv
+    return np.maximum(0, np.minimum(m.nchannel - 1, np.floor(cc + hw)) - np.maximum(0, np.ceil(cc - hw)) + 1)
+
+
+_GEOM_CACHE = {}
+
+
+def oracle_sample(m, budget_updates=6e9, keep=False):
     """Runs the float64 oracle, as it stands, on a bounded sample of the workload: the ray tracing (all channels) of as
-    many transitions / directions as fit the update budget, plus the solve over all cells.  Returns
-    (nominal updates done, seconds, threads, description)."""
+    many transitions of direction 0 as fit the update budget -- or, when even one transition of one direction is more than
+    twice the budget (C5), of every k-th line of the root lattice of direction 0 -- plus the solve over all cells.
+    Returns a dict: nominal / active updates done, seconds, threads, description (and the oracle's result with keep=True)."""
     import oracle as O
     ncores = os.cpu_count() or 1
     O.set_threads(ncores)
@@ -117,39 +140,65 @@ def oracle_sample(m, budget_updates=6e9):
     nch = m.nchannel
     dv = 2.0 * m.band_half / nch
     dens, tk, ab = (np.asarray(x, np.float64) for x in (m.density, m.tkin, m.abundance))
-    pops = O.lte(sp, dens, tk, ab)
     if hasattr(m, "child"):
-        r0 = O.sim_3d(sp, m, None, geom_only=True, dirs=m.dirs[0])
-        steps_dir = int(r0["visits"].sum())
-        nt = max(1, min(sp.ntrans, int(budget_updates // max(1, steps_dir * nch))))
-        sel = np.arange(nt, dtype=np.int32)
+        allsel = np.arange(sp.ntrans, dtype=np.int32) if getattr(m, "sel", None) is None else np.asarray(m.sel, np.int32)
+        key = id(m)
+        if key not in _GEOM_CACHE:  # the geometry pass is not part of the timed sample
+            _GEOM_CACHE[key] = int(O.sim_3d(sp, m, None, geom_only=True, dirs=m.dirs[0])["visits"].sum())
+        steps_dir = _GEOM_CACHE[key]
+        per_trans = max(1.0, float(steps_dir) * nch)
+        pops = O.lte(sp, dens, tk, ab)
+        if per_trans <= 2.0 * budget_updates:
+            nt, stride = max(1, min(len(allsel), int(budget_updates // per_trans))), 1
+            desc = f"direction 0 of {len(m.dirs)}, transitions {list(map(int, allsel[:nt]))}, all {nch} channels, all cells; then the solve"
+        else:
+            nt, stride = 1, int(math.ceil(per_trans / budget_updates))
+            desc = (f"direction 0 of {len(m.dirs)}, transition {int(allsel[0])}, every {stride}-th line of the root lattice (rays born in "
+                    f"refined regions not traced), all {nch} channels; then the solve over all cells")
+        sel = allsel[:nt]
         t0 = time.perf_counter()
-        r = O.sim_3d(sp, m, pops, sel, dirs=m.dirs[0])
+        r = O.sim_3d(sp, m, pops, sel, dirs=m.dirs[0], root_stride=stride)
         O.solve(sp, dens, tk, ab, r["veff"], sel, r["P"], r["LAM"], dv, m.t_bg, pops)
         dt = time.perf_counter() - t0
-        done = nominal_updates(steps_dir, nch, nt)
-        desc = f"direction 0 of {len(m.dirs)}, transitions 0..{nt - 1}, all {nch} channels, all cells; then the solve"
+        steps = int(r["visits"].sum())
+        act = float((r["visits"] * active_channels_per_cell(m, m.dirs[0])).sum()) * nt
         threads = ncores  # rays are distributed over OpenMP threads
     else:
+        pops = O.lte(sp, dens, tk, ab)
         sel = np.arange(sp.ntrans, dtype=np.int32)
+        nt = len(sel)
         nray = len(m.ray_p)
         steps_all = sum(2 * (len(m.r_out) - 1 - int(np.searchsorted(m.r_out, p, side="right"))) + 1 for p in m.ray_p)
         frac = min(1.0, budget_updates / 8 / max(1.0, nominal_updates(steps_all, nch, len(sel))))  # 1D oracle is serial
         if frac < 1.0:
             import copy
-            keep = np.arange(0, nray, max(1, int(round(1 / frac))))
+            kept = np.arange(0, nray, max(1, int(round(1 / frac))))
             ms = copy.copy(m)
-            ms.ray_p, ms.ray_w = m.ray_p[keep], m.ray_w[keep]
+            ms.ray_p, ms.ray_w = m.ray_p[kept], m.ray_w[kept]
         else:
-            keep, ms = np.arange(nray), m
+            kept, ms = np.arange(nray), m
         t0 = time.perf_counter()
         r = O.sim_1d(sp, ms, pops, sel)
         O.solve(sp, dens, tk, ab, r["veff"], sel, r["P"], r["LAM"], dv, m.t_bg, pops)
         dt = time.perf_counter() - t0
-        done = nominal_updates(int(r["visits"].sum()), nch, len(sel))
-        desc = f"{len(keep)} of {nray} rays, all {len(sel)} transitions, all {nch} channels; then the solve"
+        steps = int(r["visits"].sum())
+        # 1D: the Doppler shift of a step is -v_r mu with the entry cosine of the step (oracle's path table)
+        sig = np.sqrt(np.asarray(m.sigma, np.float64) ** 2 + (_KB_OVER_AMU / m.species.mass_amu if m.species.mass_amu > 0 else 0.0)
+                      * np.asarray(m.tkin, np.float64))
+        vr = np.asarray(m.vrad, np.float64)
+        act = 0.0
+        for p_ in ms.ray_p:
+            sh, _, mu = O.path_1d(m.r_out, float(p_))
+            cc = -vr[sh] * mu / dv + 0.5 * (nch - 1)
+            hw = 5.0 * sig[sh] / dv
+            act += float(np.maximum(0, np.minimum(nch - 1, np.floor(cc + hw)) - np.maximum(0, np.ceil(cc - hw)) + 1).sum())
+        act *= nt
+        desc = f"{len(kept)} of {nray} rays, all {len(sel)} transitions, all {nch} channels; then the solve"
         threads = 1  # the 1D ray loop of the oracle is serial
-    return done, dt, threads, desc
+    out = {"nominal": nominal_updates(steps, nch, nt), "active": act, "seconds": dt, "threads": threads, "desc": desc}
+    if keep:
+        out.update(result=r, sel=sel)
+    return out
 
 
 def run_reference(args):
@@ -159,19 +208,18 @@ def run_reference(args):
     m, desc = make_workload(args.workload)
     import oracle as O
     O.build()
-    times, done, threads, sdesc = [], 0.0, 1, ""
+    times, last = [], None
     for i in range(args.warmup + args.steps):
-        d, dt, threads, sdesc = oracle_sample(m, budget_updates=args.ref_budget)
+        last = oracle_sample(m, budget_updates=args.ref_budget)
         if i >= args.warmup:
-            times.append(dt)
-            done = d
+            times.append(last["seconds"])
     t = float(np.mean(times))
-    val = done / t
-    out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-           "warmup": args.warmup, "ms_per_step": 1e3 * t, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-           "dtype": "f64", "data": "synthetic",
-           "config": {"workload": desc, "sample": sdesc},
-           "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sdesc},
+    val = last["active"] / t
+    out = {"impl": "reference", "metric": METRIC, "value": val, "value_kind": VALUE_KIND, "unit": UNIT, "n_gpus": args.gpus,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic", "nominal_updates_per_s": last["nominal"] / t,
+           "config": {"workload": desc, "sample": last["desc"]},
+           "cpu_baseline": {"value": val, "unit": UNIT, "cores": last["threads"], "kind": "oracle", "sample": last["desc"]},
            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
            "gpu_launches": 0}
     print(json.dumps(out))
@@ -191,6 +239,57 @@ def max_over_ranks(values, device="cpu"):
 def whole_job_value(updates_per_rank_step: float, steps: int, world: int, seconds: float) -> float:
     """`value` of the JSON line: units all ranks processed / max-over-ranks time (weak scaling: every rank runs a replica)"""
     return world * updates_per_rank_step * steps / seconds
+
+
+# ---- full-size parity on a direction subset (SURVEY 8d parity protocol (b); DESIGN.md 7) -----------------------------------
+def parity_leg(g, m, dirs_idx, ntrans=1):
+    """The oracle traces directions `dirs_idx` of the FULL model for the first `ntrans` traced transitions from LTE
+    populations (its own, rounded to float32: the input of both sides); the library does the same with
+    loc_set_directions(those directions).  Compared per cell: visit counts and integer path sums bit-exact, SJ within 1e-4
+    relative, ESC within 1e-4 of (ESC + 3e-3) -- the rules of tests/parity.py and tests/test_gpu_3d.py.  Leaves the model
+    with the subset as its directions (call last)."""
+    import oracle as O
+    import torch
+    O.set_threads(os.cpu_count() or 1)
+    sp = O.OSpecies(m.species)
+    allsel = np.arange(sp.ntrans, dtype=np.int32) if getattr(m, "sel", None) is None else np.asarray(m.sel, np.int32)
+    sel = np.ascontiguousarray(allsel[:ntrans])
+    nch = m.nchannel
+    dv = 2.0 * m.band_half / nch
+    p64 = O.lte(sp, m.density, m.tkin, m.abundance)          # [ncell][NL]
+    p32 = np.ascontiguousarray(p64.T.astype(np.float32))     # level-major, float32: the common input
+    p64[...] = p32.T
+    is3d = hasattr(m, "child")
+    t0 = time.perf_counter()
+    if is3d:
+        dsub = np.ascontiguousarray(np.asarray(m.dirs, np.float64)[list(dirs_idx)])
+        ref = O.sim_3d(sp, m, p64, sel, dirs=dsub)
+        g.set_directions(dsub)
+    else:
+        ref = O.sim_1d(sp, m, p64, sel)
+    t_or = time.perf_counter() - t0
+    del p64
+    g.set_populations(p32)
+    g.simulate(sel, geometry_counters=True)
+    sj, esc = g.counters()
+    sj, esc = sj.cpu().numpy().astype(np.float64), esc.cpu().numpy().astype(np.float64)
+    vis, pz = g.geometry_counters()
+    vis = vis.cpu().numpy().astype(np.int64)
+    visits_equal = bool(np.array_equal(vis, ref["visits"]))
+    path_equal = bool(np.array_equal(pz.cpu().numpy().astype(np.int64), ref["pathz"])) if is3d else None
+    leaf = (np.asarray(m.child) < 0) if is3d else np.ones(len(m.density), bool)
+    cvel = 2.99792458e10
+    worst_sj, worst_esc = 0.0, 0.0
+    for k, t in enumerate(sel):
+        sj_o = cvel ** 3 * ref["P"][k] / (8.0 * np.pi * sp.freq(int(t)) ** 3 * dv * ref["veff"])
+        esc_o = 1.0 - ref["LAM"][k]
+        worst_sj = max(worst_sj, float((np.abs(sj[leaf, k] - sj_o[leaf]) / np.maximum(np.abs(sj_o[leaf]), 1e-300)).max()))
+        worst_esc = max(worst_esc, float((np.abs(esc[leaf, k] - esc_o[leaf]) / (np.abs(esc_o[leaf]) + 3e-3)).max()))
+    ok = visits_equal and (path_equal is not False) and worst_sj < 1e-4 and worst_esc < 1e-4
+    return {"workload": m.name, "directions": [int(d) for d in dirs_idx] if is3d else None, "transitions": [int(t) for t in sel],
+            "cells": int(leaf.sum()), "ray_cell_steps": int(ref["visits"].sum()), "visits_equal": visits_equal,
+            "path_sums_equal": path_equal, "max_rel_sj": worst_sj, "max_esc_err": worst_esc, "tol": 1e-4, "passed": bool(ok),
+            "oracle_seconds": t_or, "note": "per-cell counters of the first simulate from LTE; oracle float64, all channels, no cut-off"}
 
 
 # ---- own arm ------------------------------------------------------------------------------------------------------------
@@ -215,7 +314,9 @@ def roofline(stats_geom, nt, t_sim_s, hbm_gbs, sm_mhz, peak_kind):
         r = {"bound": "alu", "achieved": fp32 / t_sim_s / 1e12, "peak": N_SM * FP32_LANES_PER_SM_CLK * clk / 1e12,
              "unit": "Tinstr/s (FP32-pipe lane instructions)"}
     r["frac"] = t_roof / t_sim_s
-    r["traffic"] = NCU_TRAFFIC_BYTES.get(stats_geom.get("workload"))
+    tr = NCU_TRAFFIC_BYTES.get(stats_geom.get("workload"))
+    r["traffic"] = tr[0] if tr else None  # not measured in this run: from the committed ncu capture named next
+    r["traffic_from_profile"] = tr[1] if tr else None
     r.update({"kernel": "k_sim3d" if stats_geom.get("is3d") else "k_sim1d_w", "peak_source": peak_kind + " HBM copy; ALU peaks derived at sm_max clock",
               "algorithmic_bytes_per_launch": byt, "active_updates_per_launch": u_active, "hbm_gbs_achieved": byt / t_sim_s / 1e9,
               "hbm_frac": t_hbm / t_sim_s, "mufu_frac": t_mufu / t_sim_s, "fp32_frac": t_fp32 / t_sim_s,
@@ -266,21 +367,26 @@ def run_own(args):
     sampler = ClockSampler(local)
     sampler.start()
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    ev_all = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
     l0 = g.stats()["kernel_launches"]
     barrier()
+    ev_all[0].record()  # ONE pair around the K steps: the host synchronisation of every loc_solve (its scalar) is inside
     for k in range(args.steps):
         ev[k][0].record()
         g.simulate()
         ev[k][1].record()
         g.solve()
         ev[k][2].record()
+    ev_all[1].record()
     barrier()
     clocks = sampler.stop()
     launches = g.stats()["kernel_launches"] - l0
     t_sim = sum(e[0].elapsed_time(e[1]) for e in ev) * 1e-3
-    t_all = sum(e[0].elapsed_time(e[2]) for e in ev) * 1e-3
-    t_all, t_sim = max_over_ranks([t_all, t_sim], device=f"cuda:{local}")
-    value = whole_job_value(u_nom, args.steps, world, t_all)
+    t_solve = sum(e[1].elapsed_time(e[2]) for e in ev) * 1e-3
+    t_all = ev_all[0].elapsed_time(ev_all[1]) * 1e-3
+    t_all, t_sim, t_solve = max_over_ranks([t_all, t_sim, t_solve], device=f"cuda:{local}")
+    u_act = float(sg["active_channels"]) * nt
+    value = whole_job_value(u_act, args.steps, world, t_all)
 
     # ---- end to end: host buffers -> device -> one ALI iteration -> populations back to the host ----
     names = ["density", "tkin", "sigma", "abundance"] + (["vx", "vy", "vz"] if is3d else ["vx"])
@@ -314,7 +420,8 @@ def run_own(args):
     e1.record()
     barrier()
     (t_e2e,) = max_over_ranks([e0.elapsed_time(e1) * 1e-3], device=f"cuda:{local}")
-    e2e_val = whole_job_value(u_nom, n_e2e, world, t_e2e)
+    e2e_val = whole_job_value(u_act, n_e2e, world, t_e2e)
+    del host, host_pops, host_out  # 24 GB of pinned memory at C5: returned before the oracle runs
 
     # ---- S10: spectral cube of the first traced line along +z, one pixel per finest cell (C5: 1024 x 1024 x
     #      256 channels), and its line-area map; after the iterations above, timed apart from `value` ----
@@ -346,6 +453,12 @@ def run_own(args):
                     "cube_bytes": int(cube.numel() * 4), "w_mean_K_kms": float(wmap.mean())}
         del cube, wmap
 
+    parity = None
+    if rank == 0 and world == 1 and not args.no_parity:
+        import oracle as O
+        O.build()
+        parity = parity_leg(g, m, [int(x) for x in args.parity_dirs.split(",")], ntrans=args.parity_trans)
+
     if rank == 0:
         hbm, sm_max, kind = load_peaks()
         if map_info is not None:
@@ -355,18 +468,19 @@ def run_own(args):
         if world == 1 and not args.no_cpu:
             import oracle as O
             O.build()
-            done, dt, threads, sdesc = oracle_sample(m, budget_updates=args.ref_budget)
-            cpu = {"value": done / dt, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sdesc, "seconds": dt}
-        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            smp = oracle_sample(m, budget_updates=args.ref_budget)
+            cpu = {"value": smp["active"] / smp["seconds"], "unit": UNIT, "cores": smp["threads"], "kind": "oracle", "sample": smp["desc"],
+                   "seconds": smp["seconds"], "nominal_updates_per_s": smp["nominal"] / smp["seconds"]}
+        out = {"metric": METRIC, "value": value, "value_kind": VALUE_KIND, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
                "ms_per_step": 1e3 * t_all / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                "dtype": "f32", "data": "synthetic",
                "config": {"workload": desc, "cells": int(g.ncell), "ray_cell_steps_per_iteration": int(steps_per_iter),
                           "channels": int(m.nchannel), "transitions_traced": int(nt), "parallelism": "replicas" if world > 1 else "single GPU",
-                          "updates": "nominal = steps x channels x transitions (what the oracle evaluates); active = 5-sigma rule",
+                          "updates": "value = active updates (5-sigma rule) / s; nominal = steps x channels x transitions (what a code without a profile cut-off evaluates)",
                           "l2": "inputs larger than L2 (no flush)" if is3d and g.ncell > 1_000_000 else "working set fits L2 (model is small); no flush: the data is re-read from L2 by design",
                           "setup_ms_once": sg["setup_ms"], "input_generation_s": t_gen},
-               "active_updates_per_s": world * sg["active_channels"] * nt * args.steps / t_all,
-               "ms_simulate": 1e3 * t_sim / args.steps, "ms_solve": 1e3 * (t_all - t_sim) / args.steps,
+               "nominal_updates_per_s": whole_job_value(u_nom, args.steps, world, t_all),
+               "ms_simulate": 1e3 * t_sim / args.steps, "ms_solve": 1e3 * t_solve / args.steps,
                "clocks": clocks, "roofline": roof,
                "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
                "gpu_launches": int(launches)}
@@ -374,10 +488,14 @@ def run_own(args):
             out["cpu_baseline"] = cpu
         if map_info is not None:
             out["map"] = map_info
-        print(json.dumps(out))
+        if parity is not None:
+            out["parity"] = parity
+        print(json.dumps(out), flush=True)
     g.close()
     if world > 1:
         dist.destroy_process_group()
+    if parity is not None and not parity["passed"]:
+        raise SystemExit("bench.py: full-size parity against the oracle FAILED: " + json.dumps(parity))
 
 
 def main():
@@ -389,6 +507,9 @@ def main():
     ap.add_argument("--workload", default=os.environ.get("LOC_BENCH_WORKLOAD", DEFAULT_WORKLOAD))
     ap.add_argument("--ref-budget", type=float, default=6e9, help="nominal updates per oracle sample (about 10-30 s of CPU)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-parity", action="store_true", help="skip the full-size parity leg (oracle vs library on a direction subset)")
+    ap.add_argument("--parity-dirs", default="0", help="comma-separated direction indices of the parity leg (3D)")
+    ap.add_argument("--parity-trans", type=int, default=1, help="traced transitions compared in the parity leg")
     ap.add_argument("--no-map", action="store_true", help="skip the spectral-cube / line-area leg of the 3D workloads")
     args = ap.parse_args()
     if args.impl == "reference":

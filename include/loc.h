@@ -53,13 +53,18 @@ extern "C" {
 #define LOC_OPT_WINDOW_EPS_TAU 2 /* (1e-6) 1D kernel: X >= sqrt(2 ln(tau0 / eps_tau)), tau0 = largest line-centre optical
                                     depth of the step                                                                     */
 #define LOC_OPT_SPAN_XCLIP 3     /* (3.4) 3D kernel: a step whose 32-channel span does not reach X sigma, X^2 = xclip^2 +
-                                    2 ln max(1, tau0), takes two spans or the masked path                               */
+                                    2 ln max(1, tau0), takes two spans or the masked path (beyond X sigma the optical depth of
+                                    the step is < 3e-3: the 8 channels below and above the span are carried to first order)  */
+#define LOC_OPT_SPAN_XFULL 7     /* (4.8) 3D kernel: ... and the span with those 8 + 8 channels must reach X_f sigma, X_f^2 =
+                                    xfull^2 + 2 ln max(1, tau0): what lies beyond is dropped (optical depth < 1e-5)          */
 #define LOC_OPT_SIM3D_PARTS 4    /* (0 = automatic) 3D kernel: split the traced transitions over at least this many launches */
 #define LOC_OPT_SOLVER 5         /* (0 = automatic: float32 in registers for species of <= 12 levels whose transitions and
                                     collisional pairs all run from the higher to the lower level index, else float64)
                                     1 = float64 solver with the matrix in local memory, 2 = float64 solver with the matrix in
                                     shared memory (<= 16 levels): A/B measurements and reference runs                    */
 #define LOC_OPT_SOLVER_LOCAL LOC_OPT_SOLVER /* earlier name of the key */
+#define LOC_OPT_SIM3D_WARPS 6    /* (0 = automatic: one warp per set of four rays up to 4 traced transitions per launch, else two
+                                    warps that split the transitions) 1 = one warp where compiled (<= 6 transitions), 2 = two */
 
 typedef struct loc_model loc_model; /* opaque */
 

@@ -202,8 +202,10 @@ def line_area(TA, dv_cm_s):
     return np.asarray(TA, np.float64).sum(axis=-1) * (float(dv_cm_s) * 1e-5)
 
 
-def sim_3d(sp: OSpecies, m, pops, sel=None, ali=True, geom_only=False, dirs=None, off64=(25, 41)):
-    """m: loc_workloads.OctreeModel.  pops [ncell][NL] float64.  Returns dict of counters."""
+def sim_3d(sp: OSpecies, m, pops, sel=None, ali=True, geom_only=False, dirs=None, off64=(25, 41), root_stride=1):
+    """m: loc_workloads.OctreeModel.  pops [ncell][NL] float64.  Returns dict of counters.
+    root_stride > 1: a bounded TIMING sample for bench.py (every root_stride-th line of the root lattice only); its
+    counters are incomplete and must not be compared with anything."""
     G = OGrid(m)
     n = G.ncell
     sel = np.arange(sp.ntrans, dtype=np.int32) if sel is None else np.ascontiguousarray(sel, np.int32)
@@ -218,7 +220,7 @@ def sim_3d(sp: OSpecies, m, pops, sel=None, ali=True, geom_only=False, dirs=None
     lib().orc_sim_3d(sp.ref(), G.ref(), _p(tk), _p(sg), _p(vx), _p(vy), _p(vz), _p(pops), C.c_int(m.nchannel),
                      C.c_double(m.band_half), C.c_double(m.t_bg), C.c_int(len(dirs)), _p(dirs), C.c_int(nsel), _p(sel),
                      C.c_int(int(ali)), C.c_int(int(geom_only)), _p(off), _p(ABS), _p(P), _p(LAM), _p(visits), _p(pathz),
-                     _p(ledger))
+                     _p(ledger), C.c_int(int(root_stride)))
     lev = np.asarray(m.level, np.int64)
     veff = (m.root_cm / 2.0 ** lev) ** 3
     return dict(ABS=ABS, P=P, LAM=LAM, visits=visits, pathz=pathz, ledger=dict(zip(LEDGER, ledger)), veff=veff)

@@ -734,7 +734,8 @@ static void trace_line(const sim3_ctx *S, const orc_dir *D, int tag, int64_t bp,
 int orc_sim_3d(const orc_species *sp, const orc_grid *G, const double *tkin, const double *sigma_turb, const double *vx,
                const double *vy, const double *vz, const double *pops, int nch, double band_half, double tbg, int ndir,
                const double *dirs, int nsel, const int *sel, int ali, int geom_only, const int *off64 /* lattice offset in 1/64 root cell: {25,41} (R8) */,
-               double *ABS, double *P, double *LAM, int64_t *visits, int64_t *pathz, double *ledger)
+               double *ABS, double *P, double *LAM, int64_t *visits, int64_t *pathz, double *ledger,
+               int root_stride /* > 1: TIMING SAMPLE ONLY (bench.py): every root_stride-th line of the root lattice, no finer lattices */)
 {
     int64_t ncell = G->noff[G->nlev];
     sim3_ctx S;
@@ -754,7 +755,7 @@ int orc_sim_3d(const orc_species *sp, const orc_grid *G, const double *tkin, con
     for (int id = 0; id < ndir; id++) {
         orc_dir D;
         orc_setup_dir(dirs + 3 * id, G->nx, G->ny, G->nz, &D);
-        for (int tag = 0; tag < G->nlev; tag++) {
+        for (int tag = 0; tag < (root_stride > 1 ? 1 : G->nlev); tag++) {
             int64_t hk = ORC_H0 >> tag;
             int64_t np = D.W[1] / hk, nq = D.W[2] / hk;
             int64_t Op = off64[0] * (ORC_H0 / 64), Oq = off64[1] * (ORC_H0 / 64);
@@ -768,6 +769,7 @@ int orc_sim_3d(const orc_species *sp, const orc_grid *G, const double *tkin, con
                 for (int64_t ij = 0; ij < np * nq; ij++) {
                     int64_t i = ij % np, j = ij / np;
                     if (tag > 0 && !((i & 1) || (j & 1))) continue; /* belongs to a coarser lattice */
+                    if (root_stride > 1 && ij % root_stride) continue; /* bounded sample of the rays (no result is used) */
                     trace_line(&S, &D, tag, Op + i * hk, Oq + j * hk, N, phi, lled);
                 }
 #pragma omp critical

@@ -17,6 +17,8 @@ from . import build as _build
 LOC_OK, LOC_EINVAL, LOC_ESTATE, LOC_ENOMEM, LOC_ECUDA, LOC_ENONFINITE = 0, -1, -2, -3, -4, -5
 LOC_OPT_WINDOW_XMIN, LOC_OPT_WINDOW_EPS_TAU, LOC_OPT_SPAN_XCLIP, LOC_OPT_SIM3D_PARTS, LOC_OPT_SOLVER = 1, 2, 3, 4, 5
 LOC_OPT_SOLVER_LOCAL = LOC_OPT_SOLVER
+LOC_OPT_SIM3D_WARPS = 6
+LOC_OPT_SPAN_XFULL = 7
 LOC_GRID_SHELL, LOC_GRID_OCTREE = 1, 2
 
 SYMBOLS = ("loc_workspace_bytes", "loc_create_model", "loc_set_species", "loc_refresh_cells", "loc_set_directions", "loc_set_populations",

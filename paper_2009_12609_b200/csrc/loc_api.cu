@@ -264,6 +264,7 @@ extern "C" int loc_create_model(const loc_grid *g, const loc_cells *cells, int n
     m->ali = 1;
     m->eps_tau = 1e-6f;
     m->xclip = LOC_XCLIP;
+    m->xfull = LOC_XFULL;
     m->nsm = device_sm_count();
     m->ncell = (g->kind == LOC_GRID_SHELL) ? g->nshell : g->level_offset[g->nlevel];
     m->ws = (char *)workspace;
@@ -623,6 +624,14 @@ extern "C" int loc_set_option(loc_model *m, int key, double value)
     case LOC_OPT_SIM3D_PARTS:
         if (!(value >= 0.0 && value <= LOC_MAX_TRANS) || value != floor(value)) return fail(m, LOC_EINVAL, "LOC_OPT_SIM3D_PARTS must be an integer in [0, LOC_MAX_TRANS]");
         m->sim3d_parts = (int)value;
+        return LOC_OK;
+    case LOC_OPT_SPAN_XFULL:
+        if (!(value >= 1.0 && value <= 12.0)) return fail(m, LOC_EINVAL, "LOC_OPT_SPAN_XFULL must be in [1, 12]");
+        m->xfull = (float)value;
+        return LOC_OK;
+    case LOC_OPT_SIM3D_WARPS:
+        if (value != 0.0 && value != 1.0 && value != 2.0) return fail(m, LOC_EINVAL, "LOC_OPT_SIM3D_WARPS must be 0, 1 or 2");
+        m->sim3d_warps = (int)value;
         return LOC_OK;
     case LOC_OPT_SOLVER:
         if (value != 0.0 && value != 1.0 && value != 2.0) return fail(m, LOC_EINVAL, "LOC_OPT_SOLVER must be 0, 1 or 2");

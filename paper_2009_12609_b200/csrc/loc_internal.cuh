@@ -22,6 +22,7 @@
 
 #define LOC_LOG2E 1.4426950408889634f
 #define LOC_XCLIP 3.4f     // 3D kernel: the span reaches at least this many sigma to both sides of the line centre, or the step is masked (default of LOC_OPT_XCLIP)
+#define LOC_XFULL 4.8f     // 3D kernel: span + wing extension (or the pair of spans, or the masked window) reach at least this many sigma (default of LOC_OPT_SPAN_XFULL)
 #define LOC_THICK_TAU 0.05f   // line-centre optical depth of a step above which exp() is used instead of the series
 
 // ------------------------------------------------------------------------------------------------
@@ -110,8 +111,9 @@ struct loc_model {
     int ali;  // 1: accelerated lambda iteration (default), 0: plain lambda iteration (loc_set_ali)
     float *pops;  // registered [nlevel][ncell]
     // accuracy knobs (DESIGN 5.3), set through loc_set_option only
-    float xmin, eps_tau, xclip;
+    float xmin, eps_tau, xclip, xfull;
     int sim3d_parts;   // 0 = automatic split of the traced transitions over launches
+    int sim3d_warps;   // 0 = automatic, 1 = one warp per ray set (up to 6 transitions per launch), 2 = two warps
     int solver;        // loc_set_option(LOC_OPT_SOLVER): 0 = automatic, 1 = float64 local memory, 2 = float64 shared memory
     int nsm;           // multiprocessors of the model's device (queried once in loc_create_model)
     bool simulated;    // counters hold the result of a loc_simulate

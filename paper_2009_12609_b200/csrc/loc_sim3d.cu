@@ -51,12 +51,13 @@
 #define LOC_GROUPS 4  // rays per warp
 #define LOC_CHUNK 4   // records per group and prepare phase (LOC_TASK_ALIGN is a multiple)
 #define LOC_SPAN 32   // channels per pass: 8 lanes x one aligned float4
+#define LOC_EXT 4     // wing extension: channels below and above the span that are carried to first order in tau (one per lane)
 
 struct Sim3D {
     int nch, nchp, nsp, nslot;
     int slot0;  // first counter / coefficient slot handled by this launch (transitions may be split over launches)
     int geom;   // also accumulate the geometry counters (visits, path sums, active channels)
-    float dv, xmin, xclip, inv_ndir;
+    float dv, xmin, xclip, xfull, inv_ndir;
     const Dir3 *dirs;
     const uint16_t *task_dir;
     const long long *task_off;
@@ -81,10 +82,10 @@ struct Sim3D {
 //   +24  uint  opdz           opcode | level | dzeta (stream word)
 //   +28  float cc             line centre in channel units
 //   +32  float tm[4]          largest line-centre optical depth among the transitions of preparing lane 2 W + half
-//   +48  float ql, qh, qe     profile mass below / above the span (wing correction), and outside it (or -1), 1 pad word
-//   +64  float4 tp[NT]        (C0, Ce, c1, alpha) per transition (header comment)
-//   +64 + 16 NT   float U[NT4]    1 = series, 0 = exponential; NT4 = NT rounded up to 4
-//   then          float sc[NT4]   scale of the channel sums: w (series) or w / (kappa s) (exponential)
+//   +48  float -, -, qe       profile mass outside the span (or -1: the round sums phi itself), 1 pad word
+//   +64  float2 cf[NT]        (kappa s, c1) per transition: c1 = eps / kappa (exponential form) or eps s (series); the lowest
+//                             mantissa bit of c1 holds the form (1 = exponential): make_tcoef
+//   then float sc[NT4]        scale of the channel sums: w (series) or w / (kappa s) (exponential); NT4 = NT rounded up to 4
 #define LOC_WB_MASK 0x3ffu
 #define LOC_RS_WIDE 0x10000000u  // mode bits of a step, formed after the prepare phase (step_mode): two spans
 #define LOC_RS_SLOW 0x20000000u  //   masked multi-pass path
@@ -99,14 +100,13 @@ struct Lay {
     static constexpr int NT0 = (NT + 1) / 2;         // transitions of warp 0; warp 1 has the other NT - NT0
     static constexpr int TM = 32;                    // byte offset of tm[]
     static constexpr int QW = 48;                    // byte offset of (ql, qh)
-    static constexpr int TP = 64;                    // byte offset of tp[] in a record
-    static constexpr int UO = TP + 16 * NT;          // byte offset of U[]
-    static constexpr int SC = UO + 4 * NT4;          // byte offset of sc[]
-    static constexpr int RECB = SC + 4 * NT4;        // record bytes (multiple of 16)
-    // group stride: LOC_CHUNK records, padded so that the four groups start 8 banks apart (32-bit reads of the four
-    // groups in one instruction do not collide)
-    static constexpr int GW0 = LOC_CHUNK * RECB / 4;
-    static constexpr int GSB = 4 * (GW0 + ((8 + 32 - GW0 % 32) % 32));
+    static constexpr int CF = 64;                    // byte offset of cf[]: (kappa s, c1 | form bit) per transition
+    static constexpr int SC = CF + 8 * NT;           // byte offset of sc[]
+    static constexpr int RAW = (SC + 4 * NT4 + 15) & ~15;
+    // record stride = 32 (mod 128) bytes and group stride = 16 (mod 128): the 64-bit stores of the prepare phase (4 records
+    // x 2 lanes x 2 groups per half-warp) and the broadcast loads of the rounds are then free of bank conflicts
+    static constexpr int RECB = RAW + (32 + 128 - RAW % 128) % 128;
+    static constexpr int GSB = LOC_CHUNK * RECB + (16 + 128 - (LOC_CHUNK * RECB) % 128) % 128;
     // per-lane partial sums (a_t, b_t) of the round: [group][t][lane], rows of 10 float2 (8 used) = 80 bytes: the
     // reducing lanes of a group read 8 different rows with LDS.128 conflict free; then per warp one row of 8 floats:
     // the lanes' sums of phi.  Groups 16 banks apart.
@@ -217,13 +217,17 @@ __device__ __forceinline__ void wing_mass(float cc, float rs, float s0, float le
 // pair prepares NHW of them, from T0(half).
 template <int NT, int W>
 struct Own {
-    static constexpr int TB = W ? Lay<NT>::NT0 : 0;
-    static constexpr int NW = W ? NT - Lay<NT>::NT0 : Lay<NT>::NT0;
+    // W = 2: the CTA is ONE warp that owns every transition (small NT: no second warp repeating the stream fetch, the
+    // prepare phase and the barriers for one or two transitions; profiles/r2_sim3d.md)
+    static constexpr bool ONE = W == 2;
+    static constexpr int TB = ONE ? 0 : (W ? Lay<NT>::NT0 : 0);
+    static constexpr int NW = ONE ? NT : (W ? NT - Lay<NT>::NT0 : Lay<NT>::NT0);
     static constexpr int NHW = (NW + 1) / 2;
     static constexpr int NHR = NHW > 0 ? NHW : 1;  // array sizes
     // the warp with fewer transitions also prepares the record headers, keeps the statistics and the geometry counters
     static constexpr int HW = (NT - Lay<NT>::NT0 > 0 && NT - Lay<NT>::NT0 < Lay<NT>::NT0) ? 1 : 0;
-    static constexpr bool HEAD = W == HW;
+    static constexpr bool HEAD = ONE || W == HW;
+    static constexpr int TMI = ONE ? 0 : 2 * W;  // first of the warp's two slots of tm[]
 };
 
 // Cell data of one stream record as the prepare phase needs it: the kinematics and the (kappa, eps) pairs of the lane's
@@ -293,8 +297,7 @@ __device__ __forceinline__ unsigned prepare_record(const Sim3D &P, uint2 rec, co
             q1 = -2.0f * A * ky;
             q2 = -ky * ky;
             wb = (unsigned)iwb;
-            // qe = profile mass outside the span (-1: the round takes 1 - sum phi); ql, qh feed the wing correction
-            // (header comment) and vanish at the edges of the band, where no channels follow
+            // qe = profile mass outside the span (-1: the round takes 1 - sum phi)
             {
                 float Ql, Qh;
                 bool far;
@@ -304,8 +307,6 @@ __device__ __forceinline__ unsigned prepare_record(const Sim3D &P, uint2 rec, co
                 // 1 - sum phi any more: the round then takes the sum itself (DESIGN 5.3)
                 far = far && sigch >= 1.0f;
                 qe = far ? Ql + Qh : -1.0f;
-                ql = (iwb == 0 || !far) ? 0.0f : Ql;
-                qh = (iwb + LOC_SPAN >= P.nch || !far) ? 0.0f : Qh;
             }
             if (P.geom) nact = max(0, min(P.nch - 1, (int)floorf(cc + 5.0f * sigch)) - max(0, (int)ceilf(cc - 5.0f * sigch)) + 1);
         }
@@ -313,6 +314,7 @@ __device__ __forceinline__ unsigned prepare_record(const Sim3D &P, uint2 rec, co
         const unsigned coff = step ? rec.x * (unsigned)P.nsp + (unsigned)P.slot0 : rec.x;
         sts128u(rb + 16, make_uint4(coff, __float_as_uint(w), rec.y, __float_as_uint(cc)));
         sts128(rb + L::QW, make_float4(ql, qh, qe, 0.f));
+        if (O::ONE) sts64(rb + L::TM + 8, make_float2(0.f, 0.f));  // the slots of the absent second warp
     }
     // per transition, branch free: the exponential form from tau0 >= LOC_EXP_TAU (header comment); records that are not
     // steps have kappa = eps = s = w = 0 and get all-zero coefficients
@@ -328,17 +330,12 @@ __device__ __forceinline__ unsigned prepare_record(const Sim3D &P, uint2 rec, co
             tm = fmaxf(tm, tau0);
             const bool thick = tau0 >= LOC_EXP_TAU;
             const float rk = rcpf(ke.x);
-            float4 tp;
-            tp.x = thick ? 0.0f : ks;
-            tp.y = thick ? -ks * LOC_LOG2E : 0.0f;
-            tp.z = thick ? ke.y * rk : ke.y * s;   // source function in occupation-number units | eps s
-            tp.w = thick ? -1.0f : -ks;
-            sts128(rb + L::TP + 16 * t, tp);
-            sts32(rb + L::UO + 4 * t, thick ? 0.0f : 1.0f);
+            const float c1 = thick ? ke.y * rk : ke.y * s;  // source function in occupation-number units | eps s
+            sts64(rb + L::CF + 8 * t, make_float2(ks, __uint_as_float((__float_as_uint(c1) & ~1u) | (thick ? 1u : 0u))));
             sts32(rb + L::SC + 4 * t, thick ? wos * rk : w);  // the sums of the exponential form carry a factor kappa s
         }
     }
-    sts32(rb + L::TM + 4 * (2 * W + half), tm);
+    sts32(rb + L::TM + 4 * (O::TMI + half), tm);
     return flags;
 }
 
@@ -367,19 +364,25 @@ __device__ __forceinline__ unsigned step_mode(const Sim3D &P, unsigned rb, float
         const float4 tm = lds128(rb + L::TM);
         const float cc = lds32(rb + 28);
         const float tau0m = fmaxf(fmaxf(tm.x, tm.y), fmaxf(tm.z, tm.w));
-        float X2 = P.xclip * P.xclip;
-        if (tau0m > 1.0f) X2 = fmaf(1.3862944f, __log2f(tau0m), X2);  // 2 ln tau0m
+        const float lt = tau0m > 1.0f ? 1.3862944f * __log2f(tau0m) : 0.0f;  // 2 ln max(1, tau0m)
+        const float X2 = fmaf(P.xclip, P.xclip, lt);
         float need;  // X sigma in channels = sqrt(X2) * 0.8493218 / sqrt(-q2)
         asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(need) : "f"(X2 * 0.7213475f * rcpf(-h0.z)));
+        // ... and the span with its wing extension must reach X_f sigma, X_f^2 = xfull^2 + 2 ln max(1, tau0m)
+        float needf;
+        asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(needf) : "f"(fmaf(P.xfull, P.xfull, lt) * 0.7213475f * rcpf(-h0.z)));
         const int wb = (int)(wbop & LOC_WB_MASK);
-        const bool ok1 = P.nch >= LOC_SPAN && (wb == 0 || cc - (float)wb >= need) && (wb + LOC_SPAN >= P.nch || (float)(wb + LOC_SPAN - 1) - cc >= need);
+        const bool ok1 = P.nch >= LOC_SPAN && (wb == 0 || cc - (float)wb >= need) && (wb + LOC_SPAN >= P.nch || (float)(wb + LOC_SPAN - 1) - cc >= need) &&
+                         (wb - LOC_EXT <= 0 || cc - (float)(wb - LOC_EXT) >= needf) &&
+                         (wb + LOC_SPAN + LOC_EXT >= P.nch || (float)(wb + LOC_SPAN + LOC_EXT - 1) - cc >= needf);
         if (-h0.z > 0.7213475f) {
             // channels wider than the line (sigma < dv; -q2 = log2(e) / (2 sigch^2)): the exact masked path, which sums the
             // sampled profile itself and evaluates it from the distance to the line centre (DESIGN 5.3)
             flags |= LOC_RS_SLOW;
         } else if (!ok1) {
             const int ww = wide_start(P.nch, cc);
-            const bool ok2 = P.nch >= 2 * LOC_SPAN && (ww == 0 || cc - (float)ww >= need) && (ww + 2 * LOC_SPAN >= P.nch || (float)(ww + 2 * LOC_SPAN - 1) - cc >= need);
+            const float need2 = fmaxf(need, needf);  // a pair of spans has no extension
+            const bool ok2 = P.nch >= 2 * LOC_SPAN && (ww == 0 || cc - (float)ww >= need2) && (ww + 2 * LOC_SPAN >= P.nch || (float)(ww + 2 * LOC_SPAN - 1) - cc >= need2);
             flags |= ok2 ? LOC_RS_WIDE : LOC_RS_SLOW;
             if (ok2) {
                 float Ql, Qh;
@@ -392,13 +395,35 @@ __device__ __forceinline__ unsigned step_mode(const Sim3D &P, unsigned rb, float
     return flags;
 }
 
+// Coefficients of one (ray step, transition) for the unified per-channel factor (header comment), derived by every lane
+// from the record's pair cf = (kappa s, c1) -- c1 = eps / kappa (exponential form) or eps s (series), the form in the
+// lowest mantissa bit of c1 (one ulp) -- instead of being read as six floats: the kernel is bound by shared-memory
+// wavefronts (profiles/r2_sim3d.md), a 64-bit broadcast load is 2 of them where LDS.128 + LDS.32 were 5.
+struct TCoef {
+    float C0, Ce, c1, al, U, g, ks, es;  // g = unit of the channel sums relative to phi n: kappa s (exponential) or 1 (series)
+};
+__device__ __forceinline__ TCoef make_tcoef(float2 cf)
+{
+    TCoef c;
+    const bool thick = __float_as_uint(cf.y) & 1u;
+    c.ks = cf.x;
+    c.c1 = cf.y;
+    c.C0 = thick ? 0.0f : cf.x;
+    c.Ce = thick ? -LOC_LOG2E * cf.x : 0.0f;
+    c.al = thick ? -1.0f : -cf.x;
+    c.U = thick ? 0.0f : 1.0f;
+    c.g = thick ? cf.x : 1.0f;
+    c.es = cf.y * c.g;  // eps s: the first-order emission of the wing-extension channel
+    return c;
+}
+
 // Masked multi-pass round for one lane's ray step (rare: DESIGN 6.4): passes of 32 channels over the step's nominal
 // window [clo, chi], which is formed here from the record (the largest line-centre optical depth of ALL transitions sets
-// its width, DESIGN 5.3), for the warp's own transitions.  Adds the lane's partial sums to its slots of the `part` rows
-// (zeroed here) and returns the lane's sum of phi.  Scalar arithmetic, rolled over the transitions; same expressions as
-// the common round.
+// its width, DESIGN 5.3), for the warp's own transitions.  Leaves the lane's partial sums in its slots of the `part` rows:
+// (a_t, b_t - g_t sum phi), i.e. with the lane's sum of the sampled profile already folded into b (see the reduction).
+// Scalar arithmetic, rolled over the transitions; same expressions as the common round.
 template <int NT, int W>
-__device__ __forceinline__ float slow_round(const Sim3D &P, unsigned rb, unsigned sqg, unsigned pl, int l8, int nchp)
+__device__ __forceinline__ void slow_round(const Sim3D &P, unsigned rb, unsigned sqg, unsigned pl, int l8, int nchp)
 {
     typedef Lay<NT> L;
     typedef Own<NT, W> O;
@@ -416,8 +441,8 @@ __device__ __forceinline__ float slow_round(const Sim3D &P, unsigned rb, unsigne
         const float sigch = 0.8493218f * rcpf(ky);
         const float4 tm = lds128(rb + L::TM);
         const float tau0m = fmaxf(fmaxf(tm.x, tm.y), fmaxf(tm.z, tm.w));
-        float X2 = P.xmin * P.xmin;
-        // channels wider than the line: a handful of channels whatever the reach, and no wing correction on this path:
+        float X2 = fmaxf(P.xmin, P.xfull) * fmaxf(P.xmin, P.xfull);
+        // channels wider than the line: a handful of channels whatever the reach, and no analytic wing mass on this path:
         // reach 6.5 sigma at least, + 2 ln (dv/sigma)^2 (see loc_sim1d.cu)
         if (sigch < 1.0f) X2 = fmaf(-4.0f, __logf(sigch), fmaxf(X2, 42.25f));
         if (tau0m > 1.0f) X2 = fmaf(2.0f, __logf(tau0m), X2);
@@ -446,8 +471,7 @@ __device__ __forceinline__ float slow_round(const Sim3D &P, unsigned rb, unsigne
         if (inq) {
 #pragma unroll 1
             for (int t = O::TB; t < O::TB + O::NW; t++) {
-                const float4 tp = lds128(rb + L::TP + 16 * t);
-                const float U = lds32(rb + L::UO + 4 * t);
+                const TCoef tc = make_tcoef(lds64(rb + L::CF + 8 * t));
                 const unsigned sa = sqg + 4 * base + 4 * t * nchp;
                 const float4 n4 = lds128(sa);
                 float n[4] = {n4.x, n4.y, n4.z, n4.w};
@@ -455,10 +479,10 @@ __device__ __forceinline__ float slow_round(const Sim3D &P, unsigned rb, unsigne
 #pragma unroll
                 for (int k = 0; k < 4; k++) {
                     const float p = e[k];
-                    const float X = fmaf(tp.x, fmaf(tp.x, p * p * p * (1.0f / 6.0f), -0.5f * p * p), fmaf(U, p, 1.0f - ex2f(tp.y * p)));
+                    const float X = fmaf(tc.C0, fmaf(tc.C0, p * p * p * (1.0f / 6.0f), -0.5f * p * p), fmaf(tc.U, p, 1.0f - ex2f(tc.Ce * p)));
                     a = fmaf(n[k], X, a);
                     b += X;
-                    n[k] = fmaf(X, fmaf(tp.w, n[k], tp.z), n[k]);
+                    n[k] = fmaf(X, fmaf(tc.al, n[k], tc.c1), n[k]);
                 }
                 sts128(sa, make_float4(n[0], n[1], n[2], n[3]));
                 const float2 pv = lds64(pl + t * L::ROWB);
@@ -467,18 +491,26 @@ __device__ __forceinline__ float slow_round(const Sim3D &P, unsigned rb, unsigne
         }
         base += LOC_SPAN;
     }
-    return sphi;
+#pragma unroll 1
+    for (int t = O::TB; t < O::TB + O::NW; t++) {  // fold the lane's sum of phi into b (the round sums phi itself: qe = -1)
+        const TCoef tc = make_tcoef(lds64(rb + L::CF + 8 * t));
+        const float2 pv = lds64(pl + t * L::ROWB);
+        sts64(pl + t * L::ROWB, make_float2(pv.x, fmaf(-tc.g, sphi, pv.y)));
+    }
 }
 
 // The common round: one pass over the span for the warp's NW transitions, straight-line code.  `sq` = shared address of
-// the lane's quad in transition 0, `rowb` = bytes between the spectra of consecutive transitions, `pl` = the lane's slot
-// in row 0 of the group's partial sums.  Returns the lane's sum of phi.
-// ACC: second pass of a WIDE round, the partial sums are added to those of the first pass.
-// el, eh: wing correction of the lane (profile mass below / above the span for the lanes that own its first / last
-// channel, else 0): the incoming photons of the edge channel stand for those of the wing beyond it.
-template <int NT, int W, bool ACC>
-__device__ __forceinline__ float fast_round(unsigned rb, unsigned sq, int rowb, unsigned pl, const float4 h0, const f32x2 J01, const f32x2 J23, float el,
-                                            float eh)
+// the lane's quad in transition 0, `rowb` = bytes between the spectra of consecutive transitions.  The lane's partial
+// sums (a_t, b_t) are ADDED to ab[] (registers): a second pass of a WIDE round accumulates.
+// fold: 1 if the round sums the sampled profile itself for the escape fraction (no analytic wing mass: qe < 0), else 0:
+//       b_t -= g_t fold sum_lane(phi), so that sc_t sum_lanes(b_t) = w (sum phi f - sum phi) and the escape fraction is
+//       w + that (the reduction needs no separate sum of phi).
+// Wing extension (header comment): `se` = shared address (transition 0) of the lane's channel beyond the span, pe its
+// profile value, `ext` = the channel exists (inside the band, and the ray takes the extension in this pass); without it
+// se points at readable memory, pe = 0 and nothing is stored.
+template <int NT, int W>
+__device__ __forceinline__ void fast_round(unsigned rb, unsigned sq, int rowb, const float4 h0, const f32x2 J01, const f32x2 J23, unsigned se, float pe,
+                                           bool ext, float fold, float2 (&ab)[Own<NT, W>::NHR * 2])
 {
     typedef Lay<NT> L;
     typedef Own<NT, W> O;
@@ -490,7 +522,7 @@ __device__ __forceinline__ float fast_round(unsigned rb, unsigned sq, int rowb, 
     const f32x2 P01 = pk2(ex2f(y0), ex2f(y1)), P23 = pk2(ex2f(y2), ex2f(y3));
     float sa, sb;
     upk2(add2(P01, P23), sa, sb);
-    const float sphi = sa + sb;
+    const float sphif = (sa + sb) * fold;
     const f32x2 ONE2 = pk2(1.0f, 1.0f), MONE2 = pk2(-1.0f, -1.0f);
     const f32x2 K2 = pk2(-0.5f, -0.5f), K3 = pk2(1.0f / 6.0f, 1.0f / 6.0f);
     const f32x2 s01 = mul2(P01, P01), s23 = mul2(P23, P23);
@@ -498,19 +530,19 @@ __device__ __forceinline__ float fast_round(unsigned rb, unsigned sq, int rowb, 
     const f32x2 B3a = mul2(mul2(s01, P01), K3), B3b = mul2(mul2(s23, P23), K3);
     // three phases (all loads, arithmetic, all stores): the shared-memory accesses are ordered among themselves, the
     // arithmetic of the transitions in between is free to interleave
-    float4 tp[O::NHR * 2], n4[O::NHR * 2];  // tp = C0, Ce, c1, alpha
-    float Uv[O::NHR * 2];
+    float4 n4[O::NHR * 2];
+    float2 cf[O::NHR * 2];
+    float ne[O::NHR * 2];
 #pragma unroll
     for (int i = 0; i < O::NW; i++) {
-        tp[i] = lds128(rb + L::TP + 16 * (O::TB + i));
-        Uv[i] = lds32(rb + L::UO + 4 * (O::TB + i));
+        cf[i] = lds64(rb + L::CF + 8 * (O::TB + i));
         n4[i] = lds128(sq + (O::TB + i) * rowb);
+        ne[i] = lds32(se + (O::TB + i) * rowb);
     }
-    float2 ab[O::NHR * 2];
 #pragma unroll
     for (int i = 0; i < O::NW; i++) {
-        const f32x2 C0 = pk2(tp[i].x, tp[i].x), CE = pk2(tp[i].y, tp[i].y), C1 = pk2(tp[i].z, tp[i].z), AL = pk2(tp[i].w, tp[i].w),
-                    UU = pk2(Uv[i], Uv[i]);
+        const TCoef tc = make_tcoef(cf[i]);
+        const f32x2 C0 = pk2(tc.C0, tc.C0), CE = pk2(tc.Ce, tc.Ce), C1 = pk2(tc.c1, tc.c1), AL = pk2(tc.al, tc.al), UU = pk2(tc.U, tc.U);
         float z0, z1, z2, z3;
         upk2(mul2(CE, P01), z0, z1);
         upk2(mul2(CE, P23), z2, z3);
@@ -521,27 +553,29 @@ __device__ __forceinline__ float fast_round(unsigned rb, unsigned sq, int rowb, 
         float a0, a1, b0, b1;
         upk2(fma2(N01, X01, mul2(N23, X23)), a0, a1);
         upk2(add2(X01, X23), b0, b1);
-        // wing term in the units of the sum: phi n for the series, kappa s phi n for the exponential form (Ce = -kappa s log2 e)
-        ab[i] = make_float2(fmaf(fmaf(-0.6931472f, tp[i].y, Uv[i]), fmaf(el, n4[i].x, eh * n4[i].w), a0 + a1), b0 + b1);
-        if (ACC) {
-            const float2 pv = lds64(pl + (O::TB + i) * L::ROWB);
-            ab[i].x += pv.x;
-            ab[i].y += pv.y;
-        }
+        // the wing channel: absorbed-photon sum in the units of the span's sum (g phi n), photons to first order in tau:
+        // n' = n + phi (eps s - kappa s n)
+        const float pg = pe * tc.g;
+        ab[i].x += fmaf(pg, ne[i], a0 + a1);
+        ab[i].y += fmaf(-tc.g, sphif, b0 + b1);
+        ne[i] = fmaf(pe, fmaf(-tc.ks, ne[i], tc.es), ne[i]);
         upk2(fma2(X01, fma2(AL, N01, C1), N01), n4[i].x, n4[i].y);
         upk2(fma2(X23, fma2(AL, N23, C1), N23), n4[i].z, n4[i].w);
     }
 #pragma unroll
     for (int i = 0; i < O::NW; i++) {
         sts128(sq + (O::TB + i) * rowb, n4[i]);
-        sts64(pl + (O::TB + i) * L::ROWB, ab[i]);
+        if (ext) sts32(se + (O::TB + i) * rowb, ne[i]);
     }
-    return sphi;
 }
 
-__device__ __forceinline__ void cta_sync()  // both warps of the CTA
+template <int W>
+__device__ __forceinline__ void cta_sync()  // both warps of the CTA (one-warp CTAs: the warp)
 {
-    asm volatile("bar.sync 0, 64;" ::: "memory");
+    if (W == 2)
+        __syncwarp();
+    else
+        asm volatile("bar.sync 0, 64;" ::: "memory");
 }
 
 // One warp of the CTA.  NCHP_T: spectrum row length in floats when known at compile time (immediate offsets), 0 = P.nchp
@@ -560,13 +594,24 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
     const unsigned rec_g = tb + L::OFF_REC + grp * L::GSB;
     const unsigned part_g = tb + L::OFF_PART + grp * L::PGB;
     const unsigned pl = part_g + 8 * l8;                        // my slot in row 0
-    const unsigned prow = part_g + L::ROWB * (O::TB + l8);      // row of my transition (reducing lane)
-    const unsigned phi_g = part_g + L::PHI + 32 * W;
-    const unsigned sq_g = sm0 + 4u * grp * spec + 16 * l8;
+    const unsigned sq_r = sm0 + 4u * grp * spec;   // the ray's spectrum, channel 0 of transition 0
+    const unsigned sq_g = sq_r + 16 * l8;          // ... the lane's quad of a span that starts at channel 0
+    const int e0 = l8 < 4 ? l8 - LOC_EXT : l8 + LOC_SPAN - LOC_EXT;  // the lane's wing-extension channel, relative to the span start
+    const float je = (float)(e0 - 16);
+    // the lane that owns the totals of the warp's own-th transition after the butterfly reduction of a round (-1: none)
+    int own;
+    {
+        float dz[O::NHR * 2];
+#pragma unroll
+        for (int i = 0; i < O::NHR * 2; i++) dz[i] = 0.0f;
+        int ob = 0, onv = O::NW;
+        MultiReduce<O::NW, 4>::run(dz, lane, ob, onv);
+        own = onv >= 1 ? ob : -1;
+    }
     float *slots_warp = P.pool + (long long)blockIdx.x * LOC_GROUPS * P.nslot * spec;
     const float jb = (float)(4 * l8 - 16);
     const f32x2 J01 = pk2(jb, jb + 1.0f), J23 = pk2(jb + 2.0f, jb + 3.0f);
-    float2 *const cnt_l = P.cnt + O::TB + l8;
+    float2 *const cnt_o = P.cnt + O::TB + (own >= 0 ? own : 0);
     // the spectrum slots of the resident CTAs (donor spectra, DESIGN 6.3) are re-read by every ray born from them: keep
     // them in L2 against the streaming traffic of the step records, coefficients and counters
     unsigned long long pol_keep;
@@ -590,8 +635,8 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
     for (;;) {
         // ---- refill: groups whose task is exhausted take the next root ray from the queue (warp 0 asks, both read) ----
         const bool need = !done && off >= end;
-        if (W == 0 && need && l8 == 0) sts32u(tb + L::OFF_TASK + 4 * grp, atomicAdd(P.queue, 1u));
-        cta_sync();  // the previous chunk's records are free; the tasks are posted
+        if (W != 1 && need && l8 == 0) sts32u(tb + L::OFF_TASK + 4 * grp, atomicAdd(P.queue, 1u));
+        cta_sync<W>();  // the previous chunk's records are free; the tasks are posted
         if (need) {
             const long long task = lds32u(tb + L::OFF_TASK + 4 * grp);
             if (task >= P.ntask) {
@@ -621,7 +666,7 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
             myactive += nact;
         }
         load_cell<NT, W>(P, r1, half, cell);  // for the next chunk (NOP records load nothing)
-        cta_sync();  // the records of the chunk are complete
+        cta_sync<W>();  // the records of the chunk are complete
         // mode of record rj (the lanes of a pair agree), then the class of round rj: OR over the four groups
         float myqew;
         const unsigned myflags = step_mode<NT>(P, rec_g + rj * L::RECB, myqew);
@@ -673,51 +718,66 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
             const float4 h0 = lds128(rb);
             const unsigned wbop = __float_as_uint(h0.w);
             const float4 qw = lds128(rb + L::QW);
-            const float el = l8 == 0 ? qw.x : 0.0f, eh = l8 == 7 ? qw.y : 0.0f;
-            float sphi;
+            // photons emitted outside the updated channels escape (DESIGN 5.3): analytic mass of the wings for a common
+            // round (qe >= 0), else the round sums the sampled profile itself: w (1 - sum phi), folded into b (fast_round)
+            float qe = qw.z;
+            if (cls & LOC_RS_SLOW) qe = -1.0f;
+            else if (mode & LOC_RS_WIDE) qe = qew;
+            const float fold = qe < 0.0f ? 1.0f : 0.0f;
+            float2 ab[O::NHR * 2];
+#pragma unroll
+            for (int i = 0; i < O::NHR * 2; i++) ab[i] = make_float2(0.f, 0.f);
             if (cls & LOC_RS_SLOW) {
-                sphi = slow_round<NT, W>(P, rb, sq_g, pl, l8, nchp);
-            } else if (!(cls & LOC_RS_WIDE)) {
-                sphi = fast_round<NT, W, false>(rb, sq_g + 4u * (wbop & LOC_WB_MASK), rowb, pl, h0, J01, J23, el, eh);
+                slow_round<NT, W>(P, rb, sq_g, pl, l8, nchp);
+#pragma unroll
+                for (int i = 0; i < O::NW; i++) ab[i] = lds64(pl + (O::TB + i) * L::ROWB);
             } else {
-                // two passes: a WIDE ray over its pair of spans, the other rays over their span and then over nothing
-                const bool wide = mode & LOC_RS_WIDE;
-                const int wb = (int)(wbop & LOC_WB_MASK);
-                const int w1 = wide ? wide_start(P.nch, lds32(rb + 28)) : wb;
-                const float d1 = (float)(w1 - wb), d2 = d1 + (float)LOC_SPAN;
-                float4 ha = h0, hb = h0;  // the profile's quadratic, re-centred on the spans that start at w1 and w1 + 32
-                ha.x = fmaf(d1, fmaf(d1, h0.z, h0.y), h0.x);
-                ha.y = fmaf(2.0f * d1, h0.z, h0.y);
-                hb.x = wide ? fmaf(d2, fmaf(d2, h0.z, h0.y), h0.x) : -INFINITY;
-                hb.y = fmaf(2.0f * d2, h0.z, h0.y);
-                sphi = fast_round<NT, W, false>(rb, sq_g + 4u * w1, rowb, pl, ha, J01, J23, wide ? 0.0f : el, wide ? 0.0f : eh);
-                sphi += fast_round<NT, W, true>(rb, sq_g + 4u * (wide ? w1 + LOC_SPAN : w1), rowb, pl, hb, J01, J23, 0.0f, 0.0f);
+                // wing extension: the lane's channel among the LOC_EXT below / above the span, if inside the band (records that
+                // are not steps have phi = 0 and all-zero coefficients)
+                const int wb0 = (int)(wbop & LOC_WB_MASK);
+                const int ce = wb0 + e0;
+                const bool ext = ce >= 0 && ce < P.nch;
+                const unsigned se = ext ? sq_r + 4u * ce : sq_g + 4u * wb0;
+                const float pe = ext ? ex2f(fmaf(je, fmaf(je, h0.z, h0.y), h0.x)) : 0.0f;
+                if (!(cls & LOC_RS_WIDE)) {
+                    fast_round<NT, W>(rb, sq_g + 4u * wb0, rowb, h0, J01, J23, se, pe, ext, fold, ab);
+                } else {
+                    // two passes: a WIDE ray over its pair of spans, the other rays over their span and then over nothing
+                    const bool wide = mode & LOC_RS_WIDE;
+                    const int w1 = wide ? wide_start(P.nch, lds32(rb + 28)) : wb0;
+                    const float d1 = (float)(w1 - wb0), d2 = d1 + (float)LOC_SPAN;
+                    float4 ha = h0, hb = h0;  // the profile's quadratic, re-centred on the spans that start at w1 and w1 + 32
+                    ha.x = fmaf(d1, fmaf(d1, h0.z, h0.y), h0.x);
+                    ha.y = fmaf(2.0f * d1, h0.z, h0.y);
+                    hb.x = wide ? fmaf(d2, fmaf(d2, h0.z, h0.y), h0.x) : -INFINITY;
+                    hb.y = fmaf(2.0f * d2, h0.z, h0.y);
+                    // (a ray of the round that is not WIDE itself keeps its wing extension in the first pass)
+                    fast_round<NT, W>(rb, sq_g + 4u * w1, rowb, ha, J01, J23, wide ? sq_g + 4u * w1 : se, wide ? 0.0f : pe, ext && !wide, fold, ab);
+                    fast_round<NT, W>(rb, sq_g + 4u * (wide ? w1 + LOC_SPAN : w1), rowb, hb, J01, J23, sq_g + 4u * w1, 0.0f, false, fold, ab);
+                }
             }
-            sts32(phi_g + 4 * l8, sphi);
-            __syncwarp();
-            // ---- reduction over the 8 lanes of each group: lane i adds up the row of the warp's i-th transition and
-            //      issues the two float atomics of (cell, transition) as one 64-bit RED ----
+            // ---- reduction over the 8 lanes of each group in registers (halving butterfly: about 2 NW shuffles for the NW
+            //      pairs): lane `own` ends up with the totals (A, B) of the warp's own-th transition and issues the two float
+            //      atomics of (cell, transition) as one 64-bit RED ----
+            float va[O::NHR * 2], vb[O::NHR * 2];
+#pragma unroll
+            for (int i = 0; i < O::NW; i++) {
+                va[i] = ab[i].x;
+                vb[i] = ab[i].y;
+            }
+            {
+                int b0 = 0, n0 = O::NW, b1 = 0, n1 = O::NW;
+                MultiReduce<O::NW, 4>::run(va, lane, b0, n0);
+                MultiReduce<O::NW, 4>::run(vb, lane, b1, n1);
+            }
             const bool step = wbop & LOC_RS_STEP;
             const uint4 h1 = lds128u(rb + 16);  // coff, w, opdz, cc
-            if (step && l8 < O::NW) {
-                const float4 f0 = lds128(phi_g), f1 = lds128(phi_g + 16);
-                const float4 a0 = lds128(prow), a1 = lds128(prow + 16), a2 = lds128(prow + 32), a3 = lds128(prow + 48);
-                const float sc = lds32(rb + L::SC + 4 * (O::TB + l8));
-                float fa, fb;
-                upk2(add2(add2(pk2(f0.x, f0.y), pk2(f0.z, f0.w)), add2(pk2(f1.x, f1.y), pk2(f1.z, f1.w))), fa, fb);
+            if (step && own >= 0) {
+                const float sc = lds32(rb + L::SC + 4 * (O::TB + own));
                 const float w = __uint_as_float(h1.y);
-                // photons emitted outside the updated channels escape (DESIGN 5.3): analytic mass of the wings for a common
-                // round, 1 - sum phi otherwise
-                float qe = qw.z;
-                if (cls & LOC_RS_SLOW) qe = -1.0f;
-                else if (mode & LOC_RS_WIDE) qe = qew;
-                const float wesc = qe < 0.0f ? fmaf(-w, fa + fb, w) : w * qe;
-                const f32x2 s01 = add2(add2(pk2(a0.x, a0.y), pk2(a0.z, a0.w)), add2(pk2(a1.x, a1.y), pk2(a1.z, a1.w)));
-                const f32x2 s23 = add2(add2(pk2(a2.x, a2.y), pk2(a2.z, a2.w)), add2(pk2(a3.x, a3.y), pk2(a3.z, a3.w)));
-                float A, B;
-                upk2(add2(s01, s23), A, B);
-                float2 *cn = cnt_l + h1.x;
-                asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(cn), "f"(A * sc), "f"(fmaf(B, sc, wesc)) : "memory");
+                const float wesc = qe < 0.0f ? w : w * qe;
+                float2 *cn = cnt_o + h1.x;
+                asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(cn), "f"(va[0] * sc), "f"(fmaf(vb[0], sc, wesc)) : "memory");
             }
             if (O::HEAD && P.geom && step && l8 == 0) {
                 const unsigned cellidx = (h1.x - (unsigned)P.slot0) / (unsigned)P.nsp;
@@ -741,30 +801,35 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
     }
 }
 
-template <int NT, int NCHP_T>
-__global__ void __maxnreg__(128) k_sim3d(Sim3D P)
+template <int NT, int NCHP_T, bool ONE>
+__global__ void __maxnreg__(ONE ? 152 : 128) k_sim3d(Sim3D P)
 {
     extern __shared__ __align__(16) float smem[];  // [4][NT][nchp] spectra, then the tables of Lay<NT>
-    if (threadIdx.x < 32)
+    if (ONE)
+        run_warp<NT, NCHP_T, 2>(P, smem);
+    else if (threadIdx.x < 32)
         run_warp<NT, NCHP_T, 0>(P, smem);
     else
         run_warp<NT, NCHP_T, 1>(P, smem);
 }
 
-template <int NT, int NCHP_T>
+#define LOC_ONE_WARP_MAXNT 6  // one-warp CTAs are compiled up to this many transitions (the round keeps them all in registers)
+
+template <int NT, int NCHP_T, bool ONE>
 static int launch3d_t(loc_model *m, Sim3D &P, size_t smem)
 {
-    auto kern = k_sim3d<NT, NCHP_T>;
+    auto kern = k_sim3d<NT, NCHP_T, ONE>;
+    const int nthr = ONE ? 32 : 64;
     LOC_CUDA_CHECK(m, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int bps = 0;
-    LOC_CUDA_CHECK(m, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kern, 64, smem));
+    LOC_CUDA_CHECK(m, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kern, nthr, smem));
     if (bps < 1) bps = 1;
     long long blocks = (long long)m->nsm * bps;
     blocks = std::min<long long>(blocks, (m->ntask + LOC_GROUPS - 1) / LOC_GROUPS);
     blocks = std::min<long long>(blocks, m->max_warps);
     if (blocks < 1) blocks = 1;
     LOC_CUDA_CHECK(m, cudaMemsetAsync(m->d_queue, 0, sizeof(unsigned int), m->stream));
-    kern<<<(unsigned)blocks, 64, smem, m->stream>>>(P);
+    kern<<<(unsigned)blocks, nthr, smem, m->stream>>>(P);
     m->launches++;
     LOC_CUDA_CHECK(m, cudaGetLastError());
     return LOC_OK;
@@ -780,9 +845,17 @@ static int launch3d(loc_model *m, Sim3D &P)
         snprintf(m->err, sizeof(m->err), "nchannel * ntrans too large for the shared-memory spectra (%zu bytes per warp)", smem);
         return LOC_EINVAL;
     }
-    if (P.nchp == 128) return launch3d_t<NT, 128>(m, P, smem);
-    if (P.nchp == 256) return launch3d_t<NT, 256>(m, P, smem);
-    return launch3d_t<NT, 0>(m, P, smem);
+    // one warp per ray set for few transitions (loc_set_option(LOC_OPT_SIM3D_WARPS): 0 = automatic: up to 4 transitions)
+    if constexpr (NT <= LOC_ONE_WARP_MAXNT) {
+        if (m->sim3d_warps == 1 || (m->sim3d_warps == 0 && NT <= 4)) {
+            if (P.nchp == 128) return launch3d_t<NT, 128, true>(m, P, smem);
+            if (P.nchp == 256) return launch3d_t<NT, 256, true>(m, P, smem);
+            return launch3d_t<NT, 0, true>(m, P, smem);
+        }
+    }
+    if (P.nchp == 128) return launch3d_t<NT, 128, false>(m, P, smem);
+    if (P.nchp == 256) return launch3d_t<NT, 256, false>(m, P, smem);
+    return launch3d_t<NT, 0, false>(m, P, smem);
 }
 
 int loc_launch_sim3d(loc_model *m, int geom)
@@ -795,6 +868,7 @@ int loc_launch_sim3d(loc_model *m, int geom)
     P.dv = (float)m->dv;
     P.xmin = m->xmin;
     P.xclip = m->xclip;
+    P.xfull = m->xfull;
     P.inv_ndir = 1.0f / (float)m->ndir;
     P.dirs = m->d_dirs;
     P.task_dir = m->d_task_dir;

@@ -75,6 +75,15 @@ def test_nine_transitions_256_channels_split_launches():
     assert launches_3 == launches_auto + 1
 
 
+@pytest.mark.parametrize("nls,warps", [(4, 1), (4, 2), (2, 1), (2, 2), (6, 1), (7, 1), (7, 2), (5, 2)])
+def test_one_and_two_warp_ray_sets(nls, warps):
+    """loc_set_option(LOC_OPT_SIM3D_WARPS): one warp per set of four rays carrying all transitions (the default up to 4
+    traced transitions) and two warps splitting them give the oracle's counters alike; thick cells, 3 levels, 128 channels"""
+    from paper_2009_12609_b200 import binding as B
+    m = small(which=4, nroot=4, nlev=3, nside=1, nch=128, frac=0.4, nls=nls, seed=7, dens=15.0)
+    _first_simulate_3d(m, options=((B.LOC_OPT_SIM3D_WARPS, warps),))
+
+
 def test_C5_shape_three_of_nine_transitions_256_channels():
     """C5's shape: root + 2 levels, 3 of 9 transitions traced (R23), 256 channels over +-8 km/s, sigma_ln = 2, 2 km/s rms;
     first-simulate counters and 3 ALI iterations"""
