@@ -344,6 +344,9 @@ def run_own(args):
     sel = None if getattr(m, "sel", None) is None else m.sel
     nt = len(m.species.upper) if sel is None else len(sel)
     g = LocModel(m, device=f"cuda:{local}", ntrans_sim=nt)
+    for kv in args.option:  # loc_set_option(key, value) for A/B measurements; recorded in config.options
+        k, v = kv.split("=")
+        g.set_option(int(k), float(v))
     g.init_lte()
     # one untimed pass with the geometry counters: step and active-channel counts of this workload
     g.simulate(sel, geometry_counters=True)
@@ -478,7 +481,7 @@ def run_own(args):
                           "channels": int(m.nchannel), "transitions_traced": int(nt), "parallelism": "replicas" if world > 1 else "single GPU",
                           "updates": "value = active updates (5-sigma rule) / s; nominal = steps x channels x transitions (what a code without a profile cut-off evaluates)",
                           "l2": "inputs larger than L2 (no flush)" if is3d and g.ncell > 1_000_000 else "working set fits L2 (model is small); no flush: the data is re-read from L2 by design",
-                          "setup_ms_once": sg["setup_ms"], "input_generation_s": t_gen},
+                          "setup_ms_once": sg["setup_ms"], "input_generation_s": t_gen, "options": args.option},
                "nominal_updates_per_s": whole_job_value(u_nom, args.steps, world, t_all),
                "ms_simulate": 1e3 * t_sim / args.steps, "ms_solve": 1e3 * t_solve / args.steps,
                "clocks": clocks, "roofline": roof,
@@ -510,6 +513,7 @@ def main():
     ap.add_argument("--no-parity", action="store_true", help="skip the full-size parity leg (oracle vs library on a direction subset)")
     ap.add_argument("--parity-dirs", default="0", help="comma-separated direction indices of the parity leg (3D)")
     ap.add_argument("--parity-trans", type=int, default=1, help="traced transitions compared in the parity leg")
+    ap.add_argument("--option", action="append", default=[], metavar="KEY=VALUE", help="loc_set_option before the run (A/B measurements)")
     ap.add_argument("--no-map", action="store_true", help="skip the spectral-cube / line-area leg of the 3D workloads")
     args = ap.parse_args()
     if args.impl == "reference":

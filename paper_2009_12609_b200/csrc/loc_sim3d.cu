@@ -51,6 +51,7 @@
 #define LOC_GROUPS 4  // rays per warp
 #define LOC_CHUNK 4   // records per group and prepare phase (LOC_TASK_ALIGN is a multiple)
 #define LOC_SPAN 32   // channels per pass: 8 lanes x one aligned float4
+#define LOC_RAY_SKEW 8  // floats between the end of a ray's spectrum and the start of the next ray's, in shared memory
 #define LOC_EXT 4     // wing extension: channels below and above the span that are carried to first order in tau (one per lane)
 
 struct Sim3D {
@@ -208,8 +209,11 @@ __device__ __forceinline__ void sts32u(unsigned a, unsigned v)
 __device__ __forceinline__ void wing_mass(float cc, float rs, float s0, float len, float &Ql, float &Qh, bool &far)
 {
     const float xl = (cc - (s0 - 0.5f)) * rs, xh = ((s0 + len - 0.5f) - cc) * rs;
-    Ql = 0.3989422804f * ex2f(-0.7213475f * xl * xl) * rcpf(xl + rcpf(xl + 2.0f * rcpf(xl + 3.0f * rcpf(xl + 4.0f * rcpf(xl)))));
-    Qh = 0.3989422804f * ex2f(-0.7213475f * xh * xh) * rcpf(xh + rcpf(xh + 2.0f * rcpf(xh + 3.0f * rcpf(xh + 4.0f * rcpf(xh)))));
+    // the continued fraction written as one rational function: x + 1/(x + 2/(x + 3/(x + 4/x))) = x (u^2 + 10 u + 15) / (u^2 + 9 u + 8),
+    // u = x^2: one reciprocal per side instead of a chain of five
+    const float ul = xl * xl, uh = xh * xh;
+    Ql = 0.3989422804f * ex2f(-0.7213475f * ul) * fmaf(ul, ul + 9.0f, 8.0f) * rcpf(xl * fmaf(ul, ul + 10.0f, 15.0f));
+    Qh = 0.3989422804f * ex2f(-0.7213475f * uh) * fmaf(uh, uh + 9.0f, 8.0f) * rcpf(xh * fmaf(uh, uh + 10.0f, 15.0f));
     far = xl >= 3.0f && xh >= 3.0f;
 }
 
@@ -587,14 +591,16 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
     const int lane = threadIdx.x & 31, grp = lane >> 3, l8 = lane & 7, rj = l8 >> 1, half = l8 & 1;
     const int nchp = NCHP_T ? NCHP_T : P.nchp;
     const int spec = NT * nchp;                // floats per ray spectrum
+    const int specs = spec + LOC_RAY_SKEW;     // ... and between the rays' spectra in shared memory: the rays start 8 banks apart, so
+                                               // that the 32-bit accesses of the wing extension of rays with the same span do not collide
     const int rowb = 4 * nchp;
     float *sn_all = smem;
     const unsigned sm0 = (unsigned)__cvta_generic_to_shared(smem);
-    const unsigned tb = sm0 + 4u * LOC_GROUPS * spec;
+    const unsigned tb = sm0 + 4u * LOC_GROUPS * specs;
     const unsigned rec_g = tb + L::OFF_REC + grp * L::GSB;
     const unsigned part_g = tb + L::OFF_PART + grp * L::PGB;
     const unsigned pl = part_g + 8 * l8;                        // my slot in row 0
-    const unsigned sq_r = sm0 + 4u * grp * spec;   // the ray's spectrum, channel 0 of transition 0
+    const unsigned sq_r = sm0 + 4u * grp * specs;   // the ray's spectrum, channel 0 of transition 0
     const unsigned sq_g = sq_r + 16 * l8;          // ... the lane's quad of a span that starts at channel 0
     const int e0 = l8 < 4 ? l8 - LOC_EXT : l8 + LOC_SPAN - LOC_EXT;  // the lane's wing-extension channel, relative to the span start
     const float je = (float)(e0 - 16);
@@ -689,7 +695,7 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
                     cm &= ~(0xffu << (8 * g));
                     const uint4 gh = lds128u(tb + L::OFF_REC + g * L::GSB + r * L::RECB + 16);
                     const unsigned gop = gh.z >> 24, gx = gh.x;
-                    float *gs = sn_all + g * spec + row0;
+                    float *gs = sn_all + g * specs + row0;
                     float *slot = slots_warp + ((long long)g * P.nslot + gx) * spec + row0;
                     if (gop == LOC_OP_BG) {
                         for (int t = 0; t < O::NW; t++) {
@@ -835,7 +841,7 @@ static int launch3d_t(loc_model *m, Sim3D &P, size_t smem)
     return LOC_OK;
 }
 
-static size_t spectra_bytes(int nt, int nchp) { return sizeof(float) * LOC_GROUPS * (size_t)nt * nchp; }
+static size_t spectra_bytes(int nt, int nchp) { return sizeof(float) * LOC_GROUPS * ((size_t)nt * nchp + LOC_RAY_SKEW); }
 
 template <int NT>
 static int launch3d(loc_model *m, Sim3D &P)
