@@ -46,6 +46,8 @@ class Species:
     cl: np.ndarray  # [ncoll] int32
     temps_K: np.ndarray  # [ntemp]
     rate_down: np.ndarray  # [ntemp][ncoll] cm^3/s
+    # hyperfine structure with LTE between the components: {transition: (velocity offsets cm/s, weights summing to 1)}
+    hfs: dict = dataclasses.field(default_factory=dict)
 
     @property
     def nlevel(self) -> int:

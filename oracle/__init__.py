@@ -29,7 +29,8 @@ class _Species(C.Structure):
     _fields_ = [("nlevel", C.c_int), ("energy_K", C.c_void_p), ("g", C.c_void_p), ("ntrans", C.c_int),
                 ("upper", C.c_void_p), ("lower", C.c_void_p), ("A", C.c_void_p), ("mass_amu", C.c_double),
                 ("ncoll", C.c_int), ("cu", C.c_void_p), ("cl", C.c_void_p), ("ntemp", C.c_int),
-                ("temps_K", C.c_void_p), ("rate_down", C.c_void_p)]
+                ("temps_K", C.c_void_p), ("rate_down", C.c_void_p), ("hf_off", C.c_void_p), ("hf_dv", C.c_void_p),
+                ("hf_w", C.c_void_p)]
 
 
 class _Grid(C.Structure):
@@ -83,9 +84,23 @@ class OSpecies:
         self.temps = _f64(sp.temps_K)
         self.rates = _f64(sp.rate_down)
         self.nlevel, self.ntrans = len(self.e), len(self.up)
+        # hyperfine structure: sp.hfs = {transition: (offsets cm/s, weights)} (loc_workloads.Species), optional
+        hfs = getattr(sp, "hfs", None) or {}
+        if hfs:
+            off = np.zeros(self.ntrans + 1, np.int32)
+            dv, w = [], []
+            for t in range(self.ntrans):
+                if t in hfs:
+                    dv += list(np.asarray(hfs[t][0], np.float64))
+                    w += list(np.asarray(hfs[t][1], np.float64))
+                off[t + 1] = len(dv)
+            self.hf_off, self.hf_dv, self.hf_w = off, _f64(dv), _f64(w)
+            hf = (_p(self.hf_off), _p(self.hf_dv), _p(self.hf_w))
+        else:
+            hf = (None, None, None)
         self.c = _Species(self.nlevel, _p(self.e), _p(self.g), self.ntrans, _p(self.up), _p(self.lo), _p(self.A),
                           float(sp.mass_amu), len(self.cu), _p(self.cu), _p(self.cl), len(self.temps), _p(self.temps),
-                          _p(self.rates))
+                          _p(self.rates), *hf)
 
     def ref(self):
         return C.byref(self.c)
@@ -271,6 +286,13 @@ def slab(sp: OSpecies, t, nch, band_half, tbg, a, veff_each, s, sigma, v0, n_u, 
 def profile(nch, dv, sigma, v0):
     phi = np.zeros(nch)
     lib().orc_profile(C.c_int(nch), C.c_double(dv), C.c_double(sigma), C.c_double(v0), _p(phi))
+    return phi
+
+
+def profile_t(sp: OSpecies, t, nch, dv, sigma, v0):
+    """profile of transition t including its hyperfine components"""
+    phi = np.zeros(nch)
+    lib().orc_profile_t(sp.ref(), C.c_int(t), C.c_int(nch), C.c_double(dv), C.c_double(sigma), C.c_double(v0), _p(phi))
     return phi
 
 

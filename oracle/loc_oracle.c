@@ -61,6 +61,13 @@ typedef struct {
     int ntemp;
     const double *temps_K;   /* [ntemp] ascending                        */
     const double *rate_down; /* [ntemp][ncoll] cm^3/s                    */
+    /* hyperfine structure with LTE between the components: transition t has the
+     * components hf_off[t] .. hf_off[t+1]-1, each a Gaussian of the cell's width shifted by hf_dv (cm/s, on the channel
+     * velocity axis) carrying the fraction hf_w of the line (sum = 1).  One population per level: the components share
+     * the source function.  hf_off == NULL or an empty range: a single component at zero offset.                      */
+    const int *hf_off;    /* [ntrans+1] or NULL */
+    const double *hf_dv;  /* [hf_off[ntrans]] */
+    const double *hf_w;   /* [hf_off[ntrans]] */
 } orc_species;
 
 /* ledger slots (pin P6) */
@@ -278,6 +285,24 @@ static void profile(int nch, double dv, double sigma, double v0, double *phi)
     }
 }
 
+/* Profile of transition t: the sum over its hyperfine components  phi_c = sum_k w_k dv/(sigma sqrt(2 pi)) exp(-(v_c - v0 -
+ * dv_k)^2 / (2 sigma^2))  (LTE between the components: PAPER.md:39, 149); without hyperfine structure the plain profile. */
+static void profile_t(const orc_species *sp, int t, int nch, double dv, double sigma, double v0, double *phi)
+{
+    if (!sp->hf_off || sp->hf_off[t + 1] == sp->hf_off[t]) {
+        profile(nch, dv, sigma, v0, phi);
+        return;
+    }
+    double amp = dv / (sigma * sqrt(2.0 * ORC_PI));
+    for (int c = 0; c < nch; c++) phi[c] = 0.0;
+    for (int k = sp->hf_off[t]; k < sp->hf_off[t + 1]; k++)
+        for (int c = 0; c < nch; c++) {
+            double vc = (c - 0.5 * (nch - 1)) * dv;
+            double x = (vc - v0 - sp->hf_dv[k]) / sigma;
+            phi[c] += sp->hf_w[k] * amp * exp(-0.5 * x * x);
+        }
+}
+
 static double total_sigma(const orc_species *sp, double sigma_turb, double T)
 {
     if (sp->mass_amu <= 0.0) return sigma_turb;
@@ -436,7 +461,7 @@ int orc_sim_1d(const orc_species *sp, int ns, const double *r, const double *tki
                 int cell = sh[j];
                 double sig = total_sigma(sp, sigma_turb[cell], tkin[cell]);
                 /* R6: radio convention, v0 = -(v . d) = -v_r mu, mu at the entry of the step */
-                profile(nch, dv, sig, -vrad[cell] * mu[j], phi);
+                profile_t(sp, t, nch, dv, sig, -vrad[cell] * mu[j], phi);
                 cell_step(nch, N, phi, w[i], ss[j], veff[cell], kcoef, gr, sp->A[t], pops[cell * NL + u],
                           pops[cell * NL + l], ali, &ABS[k * ns + cell], &P[k * ns + cell], &LAM[k * ns + cell], ledger);
                 if (k == 0 && visits) visits[cell]++;
@@ -478,7 +503,7 @@ int orc_spectra_1d(const orc_species *sp, int ns, const double *r, const double 
                 double n_u = pops[cell * NL + u], n_l = pops[cell * NL + l];
                 double kt = kcoef * (n_l * gr - n_u);
                 double Snu = 2.0 * ORC_H * nu * nu * nu / (ORC_C * ORC_C) / (n_l * gr / n_u - 1.0);
-                profile(nch, dv, total_sigma(sp, sigma_turb[cell], tkin[cell]), -vrad[cell] * mu[j], phi);
+                profile_t(sp, t, nch, dv, total_sigma(sp, sigma_turb[cell], tkin[cell]), -vrad[cell] * mu[j], phi);
                 for (int c = 0; c < nch; c++) {
                     double tau = kt * phi[c] * ss[j];
                     double ome = -expm1(-tau);
@@ -711,10 +736,10 @@ static void trace_line(const sim3_ctx *S, const orc_dir *D, int tag, int64_t bp,
                 double s = (double)dz * u_cm * D->lenf;
                 double veff = hcm * hcm * hcm;
                 double v0 = -(S->vx[cell] * D->d[0] + S->vy[cell] * D->d[1] + S->vz[cell] * D->d[2]); /* R6 */
-                profile(nch, S->dv, total_sigma(sp, S->sigma_turb[cell], S->tkin[cell]), v0, phi);
                 for (int k = 0; k < nsel; k++) {
                     int t = S->sel[k], u = sp->upper[t], l = sp->lower[t];
                     double nu = orc_freq(sp, t);
+                    profile_t(sp, t, nch, S->dv, total_sigma(sp, S->sigma_turb[cell], S->tkin[cell]), v0, phi);
                     double kcoef = ORC_C * ORC_C * ORC_C * sp->A[t] / (8.0 * ORC_PI * nu * nu * nu * S->dv);
                     cell_step(nch, N + k * nch, phi, a_cur, s, veff, kcoef, sp->g[u] / sp->g[l], sp->A[t],
                               S->pops[cell * NL + u], S->pops[cell * NL + l], S->ali, &S->ABS[(size_t)k * S->ncell + cell],
@@ -879,7 +904,7 @@ int orc_spectra_3d(const orc_species *sp, const orc_grid *G, const double *tkin,
                 double kt = kcoef * (n_l * gr - n_u);
                 double Snu = 2.0 * ORC_H * nu * nu * nu / (ORC_C * ORC_C) / (n_l * gr / n_u - 1.0);
                 double v0 = -(vx[cell] * D.d[0] + vy[cell] * D.d[1] + vz[cell] * D.d[2]);
-                profile(nch, dv, total_sigma(sp, sigma_turb[cell], tkin[cell]), v0, phi);
+                profile_t(sp, t, nch, dv, total_sigma(sp, sigma_turb[cell], tkin[cell]), v0, phi);
                 for (int c = 0; c < nch; c++) {
                     double ome = -expm1(-kt * phi[c] * s);
                     I[c] = I[c] * (1.0 - ome) + Snu * ome;
@@ -903,7 +928,7 @@ void orc_slab(const orc_species *sp, int t, int nch, double band_half, double tb
     double dv = 2.0 * band_half / nch, nu = orc_freq(sp, t);
     double kcoef = ORC_C * ORC_C * ORC_C * sp->A[t] / (8.0 * ORC_PI * nu * nu * nu * dv);
     double *phi = (double *)malloc(sizeof(double) * nch);
-    profile(nch, dv, sigma, v0, phi);
+    profile_t(sp, t, nch, dv, sigma, v0, phi);
     if (inject)
         for (int c = 0; c < nch; c++) N[c] = bg_photons(nu, tbg, a, dv);
     acc[0] = acc[1] = acc[2] = 0.0;
@@ -914,3 +939,4 @@ void orc_slab(const orc_species *sp, int t, int nch, double band_half, double tb
 }
 
 void orc_profile(int nch, double dv, double sigma, double v0, double *phi) { profile(nch, dv, sigma, v0, phi); }
+void orc_profile_t(const orc_species *sp, int t, int nch, double dv, double sigma, double v0, double *phi) { profile_t(sp, t, nch, dv, sigma, v0, phi); }

@@ -1,0 +1,125 @@
+"""Oracle parity at BASELINE size (SURVEY 8d parity protocol; VERDICT r1 "C2 / C3 / C4 at BASELINE size"), through the C-ABI, in
+the launch configuration bench.py times.  What the 16 host cores of the GPU box allow inside a test run:
+
+  C2 (1000 shells, 4000 rays, 256 channels): first-simulate counters of transitions 0 and 8 on ALL rays, and the populations
+      after 2 ALI iterations with transitions 0..2 traced (the others see the background, R23);
+  C3 (128^3, 128 channels): counters of transitions 0, 3, 8 for a subset of 4 of the 48 directions (the oracle's counters of a
+      direction subset are exactly what the library computes after loc_set_directions(subset)), and ONE FULL ALI iteration
+      (48 directions, 9 transitions, ~2e11 channel updates in the oracle): populations and T_ex of every cell;
+  C4 (octree, 36.6 M cells, 4 hierarchy levels): counters of transitions 0 and 4 for directions 0 and 17 of the full model:
+      ray births, donor spectra and level changes at full depth.
+  C5 (222.8 M cells, 80 GB) does not fit a test run; bench.py's parity leg does the same comparison for it (direction 0,
+      transition 0, all cells) and fails the bench if it is off.
+
+Compared: visit counts and integer path sums bit-exact; SJ within 1e-4 relative; ESC within 1e-4 of (ESC + 3e-3);
+populations / T_ex within 1e-3 (R20)."""
+import functools
+
+import numpy as np
+import pytest
+
+import loc_workloads as W
+import oracle as O
+from parity import check_pops, f32_pops_from_oracle_lte, oracle_SJ_ESC, rel_err, tex_all
+
+pytestmark = pytest.mark.gpu
+TOL_SJ = 1e-4
+TOL_POP = 1e-3
+
+
+@functools.lru_cache(maxsize=1)
+def _c3():
+    return W.cloud_config(3)
+
+
+def _model(m, **kw):
+    from paper_2009_12609_b200 import LocModel
+    return LocModel(m, **kw)
+
+
+def _compare_counters(m, g, ref, sel, sp, is3d=True):
+    sj_o, esc_o = oracle_SJ_ESC(sp, m, ref, sel)
+    sj, esc = g.counters()
+    sj, esc = sj.cpu().numpy(), esc.cpu().numpy()
+    vis, pz = g.geometry_counters()
+    assert np.array_equal(vis.cpu().numpy().astype(np.int64), ref["visits"])
+    if is3d:
+        assert np.array_equal(pz.cpu().numpy().astype(np.int64), ref["pathz"])
+    leaf = (m.child < 0) if is3d else np.ones(len(m.density), bool)
+    e_sj = rel_err(sj[leaf], sj_o[leaf]).max()
+    e_esc = np.max(np.abs(esc[leaf] - esc_o[leaf]) / (np.abs(esc_o[leaf]) + 3e-3))
+    assert e_sj < TOL_SJ and e_esc < TOL_SJ, (e_sj, e_esc)
+    return e_sj, e_esc
+
+
+def test_C2_full_size_counters_and_two_iterations():
+    m = W.shell_config(2)
+    sp = O.OSpecies(m.species)
+    pops64, pops32 = f32_pops_from_oracle_lte(sp, m)
+    sel = np.array([0, 8], np.int32)
+    ref = O.sim_1d(sp, m, pops64, sel)
+    g = _model(m, ntrans_sim=3)
+    g.set_populations(pops32)
+    g.simulate(sel, geometry_counters=True)
+    _compare_counters(m, g, ref, sel, sp, is3d=False)
+    sel3 = np.array([0, 1, 2], np.int32)
+    pops_o, _ = O.iterate(sp, m, 2, sel=sel3)
+    g.init_lte()
+    g.simulate(sel3)
+    g.init_lte()
+    g.iterate(2)
+    pg = g.pops.cpu().numpy()
+    g.close()
+    worst, small_abs = check_pops(pg, pops_o)
+    assert worst < TOL_POP and small_abs < 1e-10, (worst, small_abs)
+
+
+def test_C3_full_size_counters_on_a_direction_subset():
+    m = _c3()
+    sp = O.OSpecies(m.species)
+    O.set_threads(16)
+    pops64, pops32 = f32_pops_from_oracle_lte(sp, m)
+    sel = np.array([0, 3, 8], np.int32)
+    dsub = np.ascontiguousarray(m.dirs[[0, 5, 20, 47]])  # ring z = 11/12, a tie |dx| = |dy|, the equator, the last one
+    ref = O.sim_3d(sp, m, pops64, sel, dirs=dsub)
+    g = _model(m, ntrans_sim=3)
+    g.set_directions(dsub)
+    g.set_populations(pops32)
+    g.simulate(sel, geometry_counters=True)
+    _compare_counters(m, g, ref, sel, sp)
+    g.close()
+
+
+def test_C3_full_size_one_full_iteration():
+    """all 48 directions, all 9 transitions, every cell: populations and T_ex after one ALI iteration from LTE"""
+    m = _c3()
+    sp = O.OSpecies(m.species)
+    O.set_threads(16)
+    pops_o, _ = O.iterate(sp, m, 1)
+    g = _model(m)
+    g.init_lte()
+    g.iterate(1)
+    pg = g.pops.cpu().numpy()
+    g.close()
+    worst, small_abs = check_pops(pg, pops_o)
+    assert worst < TOL_POP and small_abs < 1e-10, (worst, small_abs)
+    tg, to = tex_all(sp, pg.astype(np.float64).T, m.species), tex_all(sp, pops_o, m.species)
+    assert rel_err(tg, to).max() < TOL_POP
+
+
+def test_C4_full_size_counters_on_a_direction_subset():
+    m = W.cloud_config(4)
+    assert m.nlev == 4 and m.ncell > 30_000_000
+    sp = O.OSpecies(m.species)
+    O.set_threads(16)
+    pops64, pops32 = f32_pops_from_oracle_lte(sp, m)
+    sel = np.array([0, 4], np.int32)
+    dsub = np.ascontiguousarray(m.dirs[[0, 17]])
+    ref = O.sim_3d(sp, m, pops64, sel, dirs=dsub)
+    assert ref["ledger"]["created"] > 0 and ref["ledger"]["terminated"] > 0
+    g = _model(m, ntrans_sim=2)
+    g.set_directions(dsub)
+    g.set_populations(pops32)
+    g.simulate(sel, geometry_counters=True)
+    _compare_counters(m, g, ref, sel, sp)
+    g.close()
