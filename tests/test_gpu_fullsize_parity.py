@@ -103,8 +103,13 @@ def test_C3_full_size_one_full_iteration():
     g.close()
     worst, small_abs = check_pops(pg, pops_o)
     assert worst < TOL_POP and small_abs < 1e-10, (worst, small_abs)
+    # T_ex of the transitions whose two levels hold >= 1e-10 of the molecules (R20): in the thinnest cells of the log-normal
+    # field the high levels hold 1e-40 of them -- float32 denormals in the population buffer, a few significant bits
     tg, to = tex_all(sp, pg.astype(np.float64).T, m.species), tex_all(sp, pops_o, m.species)
-    assert rel_err(tg, to).max() < TOL_POP
+    frac = pops_o / pops_o.sum(axis=1, keepdims=True)
+    ok = (frac[:, m.species.upper] >= 1e-10) & (frac[:, m.species.lower] >= 1e-10)
+    assert ok[:, :3].all() and ok.mean() > 0.5
+    assert rel_err(tg, to)[ok].max() < TOL_POP
 
 
 def test_C4_full_size_counters_on_a_direction_subset():
