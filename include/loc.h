@@ -45,6 +45,7 @@ extern "C" {
 #define LOC_MAX_LEVELS 32 /* energy levels of the species                           */
 #define LOC_MAX_TREE_LEVELS 6
 #define LOC_MAX_DIRECTIONS 65535 /* ray directions of one model (loc_set_directions)                    */
+#define LOC_MAX_HFS 8            /* hyperfine components of one transition (loc_set_hyperfine)          */
 
 /* Keys of loc_set_option.  The library reads NO environment variables: every knob that can change a result or a launch
  * configuration is an argument of this call (defaults in parentheses; DESIGN.md 5.3 derives them).                    */
@@ -112,6 +113,9 @@ typedef struct {
                                 channel updates per traced transition (DESIGN 8), independent of the kernel's window */
     int64_t setup_steps;     /* octree: ray-cell steps in the precomputed step stream (all directions)      */
     double setup_ms;         /* octree: device time of the last path set-up (loc_set_directions), ms        */
+    int64_t active_updates;  /* the same count summed over the traced transitions: = active_channels x ntrans_sim without
+                                hyperfine structure; with it a transition's active channels are those within 5 sigma of
+                                any of its components, and active_channels = active_updates / ntrans_sim               */
 } loc_stats;
 
 /* Bytes of device workspace loc_create_model needs for this grid and these limits.
@@ -134,6 +138,18 @@ int loc_create_model(const loc_grid *grid, const loc_cells *cells, int nchannel,
 int loc_set_species(loc_model *m, int nlevel, const double *energy_K, const double *g, int ntrans, const int *upper,
                     const int *lower, const double *einstein_A, double mass_amu, int ncoll, const int *cu, const int *cl,
                     int ntemp, const double *temps_K, const double *rate_down);
+
+/* Hyperfine structure with LTE between the components ("in the case of hyperfine spectra, assuming LTE
+ * distribution between the hyperfine components"; PAPER.md:149 NH3(1,1), PAPER.md:388 HCN J = 1-0): transition `trans`
+ * of the species consists of ncomp components; component k is a Gaussian of the cell's line width centred dv_cm_s[k] away
+ * from the line centre on the channel velocity axis (positive = higher channel velocity) and carries the fraction
+ * weight[k] of the line (weights > 0, sum 1 within 1e-6).  The levels keep ONE population each, so the components share
+ * the source function; profile, optical depth and both counters of the transition use
+ *     phi_c = sum_k weight[k] dv / (sigma sqrt(2 pi)) exp(-(v_c - v_0 - dv_cm_s[k])^2 / (2 sigma^2)).
+ * Host arrays, copied.  ncomp = 0 (or 1 with zero offset) removes the structure; ncomp <= LOC_MAX_HFS.  Call after
+ * loc_set_species (which clears all hyperfine structure).  Steps of a model with any hyperfine transition take the
+ * kernels' general (masked-window) path.                                                                          */
+int loc_set_hyperfine(loc_model *m, int trans, int ncomp, const double *dv_cm_s, const double *weight);
 
 /* Re-read the caller's cell arrays (same device pointers as given to loc_create_model) after their content has been
  * changed from outside, and rebuild the derived per-cell kinematics record (velocity, total line width).     */

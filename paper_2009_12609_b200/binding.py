@@ -20,11 +20,12 @@ LOC_OPT_SOLVER_LOCAL = LOC_OPT_SOLVER
 LOC_OPT_SIM3D_WARPS = 6
 LOC_OPT_SPAN_XFULL = 7
 LOC_GRID_SHELL, LOC_GRID_OCTREE = 1, 2
+LOC_MAX_HFS = 8
 
 SYMBOLS = ("loc_workspace_bytes", "loc_create_model", "loc_set_species", "loc_refresh_cells", "loc_set_directions", "loc_set_populations",
            "loc_init_lte", "loc_simulate", "loc_get_counters", "loc_solve", "loc_iterate", "loc_set_ali",
            "loc_set_option", "loc_iterate_until", "loc_spectra", "loc_spectra_map", "loc_line_area", "loc_tex",
-           "loc_get_stats", "loc_destroy_model", "loc_last_error")
+           "loc_get_stats", "loc_destroy_model", "loc_last_error", "loc_set_hyperfine")
 
 
 class LocError(RuntimeError):
@@ -47,7 +48,7 @@ class loc_cells(C.Structure):
 class loc_stats(C.Structure):
     _fields_ = [("ncell", C.c_int64), ("steps", C.c_int64), ("ntrans_sim", C.c_int), ("nchannel", C.c_int),
                 ("kernel_launches", C.c_int64), ("counter_stride", C.c_int), ("active_channels", C.c_int64), ("setup_steps", C.c_int64),
-                ("setup_ms", C.c_double)]
+                ("setup_ms", C.c_double), ("active_updates", C.c_int64)]
 
 
 _lib = None
@@ -83,6 +84,7 @@ def lib():
         L.loc_solve.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.loc_iterate.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double)]
         L.loc_set_ali.argtypes = [C.c_void_p, C.c_int]
+        L.loc_set_hyperfine.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
         L.loc_iterate_until.argtypes = [C.c_void_p, C.c_int, C.c_double, C.POINTER(C.c_int), C.POINTER(C.c_double)]
         L.loc_spectra.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
         L.loc_set_option.argtypes = [C.c_void_p, C.c_int, C.c_double]
@@ -212,6 +214,13 @@ def loc_tex(h, trans: int, dev_tex) -> None:
 
 def loc_line_area(h, dev_cube, npix: int, dev_w) -> None:
     _check(lib().loc_line_area(h, _dp(dev_cube), int(npix), _dp(dev_w)), h)
+
+
+def loc_set_hyperfine(h, trans: int, dv_cm_s, weight) -> None:
+    dv = np.ascontiguousarray(dv_cm_s, np.float64)
+    w = np.ascontiguousarray(weight, np.float64)
+    assert dv.shape == w.shape and dv.ndim == 1
+    _check(lib().loc_set_hyperfine(h, int(trans), len(dv), dv.ctypes.data_as(C.c_void_p), w.ctypes.data_as(C.c_void_p)), h)
 
 
 def loc_set_ali(h, ali: bool) -> None:

@@ -464,9 +464,57 @@ extern "C" int loc_set_species(loc_model *m, int nlevel, const double *energy_K,
     }
     LOC_CUDA_CHECK(m, cudaStreamSynchronize(st));  // bg vector goes out of scope
     m->have_species = true;
+    memset(m->h_hfs_nc, 0, sizeof(m->h_hfs_nc));  // a new species has no hyperfine structure until loc_set_hyperfine
     m->selh.nsel = 0;
     m->coef_valid = false;
     return build_selection(m, 0, nullptr);
+}
+
+static void fill_hfs_slot(const loc_model *m, int t, int k, HfsTab &H)
+{
+    const int nc = m->h_hfs_nc[t];
+    H.nc[k] = nc > 0 ? nc : 1;
+    for (int c = 0; c < LOC_MAX_HFS; c++) {
+        H.dch[k][c] = (nc > 0 && c < nc) ? (float)(m->h_hfs_dv[t][c] / m->dv) : 0.0f;
+        H.w[k][c] = (nc > 0) ? (c < nc ? (float)m->h_hfs_w[t][c] : 0.0f) : (c == 0 ? 1.0f : 0.0f);
+    }
+    for (int c = 0; c < H.nc[k]; c++) {
+        H.lo = std::min(H.lo, H.dch[k][c]);
+        H.hi = std::max(H.hi, H.dch[k][c]);
+        if (H.dch[k][c] != 0.0f || H.nc[k] > 1) H.any = 1;
+    }
+}
+
+void loc_fill_hfs(const loc_model *m, HfsTab &H)
+{
+    memset(&H, 0, sizeof(H));
+    for (int k = 0; k < m->selh.nsel; k++) fill_hfs_slot(m, m->selh.sel[k], k, H);
+}
+
+void loc_fill_hfs_one(const loc_model *m, int trans, HfsTab &H)
+{
+    memset(&H, 0, sizeof(H));
+    fill_hfs_slot(m, trans, 0, H);
+}
+
+extern "C" int loc_set_hyperfine(loc_model *m, int trans, int ncomp, const double *dv_cm_s, const double *weight)
+{
+    if (!m) return LOC_EINVAL;
+    if (!m->have_species) return fail(m, LOC_ESTATE, "loc_set_species must be called before loc_set_hyperfine");
+    if (trans < 0 || trans >= m->ntrans) return fail(m, LOC_EINVAL, "loc_set_hyperfine: transition index out of range");
+    if (ncomp < 0 || ncomp > LOC_MAX_HFS || (ncomp > 0 && (!dv_cm_s || !weight))) return fail(m, LOC_EINVAL, "loc_set_hyperfine: ncomp must be in [0, LOC_MAX_HFS]");
+    double sum = 0.0;
+    for (int k = 0; k < ncomp; k++) {
+        if (!(weight[k] > 0.0) || !(fabs(dv_cm_s[k]) <= 2.0 * m->band_half)) return fail(m, LOC_EINVAL, "loc_set_hyperfine: weights must be > 0 and offsets within the band width");
+        sum += weight[k];
+    }
+    if (ncomp > 0 && fabs(sum - 1.0) > 1e-6) return fail(m, LOC_EINVAL, "loc_set_hyperfine: the weights must sum to 1");
+    m->h_hfs_nc[trans] = ncomp;
+    for (int k = 0; k < ncomp; k++) {
+        m->h_hfs_dv[trans][k] = dv_cm_s[k];
+        m->h_hfs_w[trans][k] = weight[k];
+    }
+    return LOC_OK;
 }
 
 extern "C" int loc_set_directions(loc_model *m, int ndir, const double *dir)
@@ -721,7 +769,8 @@ extern "C" int loc_get_stats(loc_model *m, loc_stats *out)
     LOC_CUDA_CHECK(m, cudaStreamSynchronize(m->stream));
     out->ncell = m->ncell;
     out->steps = (m->kind == LOC_GRID_SHELL) ? m->steps1d : (int64_t)steps[0];
-    out->active_channels = (int64_t)steps[1];
+    out->active_updates = (int64_t)steps[1];
+    out->active_channels = m->selh.nsel > 0 ? (int64_t)steps[1] / m->selh.nsel : 0;
     out->ntrans_sim = m->selh.nsel;
     out->nchannel = m->nch;
     out->kernel_launches = m->launches;

@@ -52,6 +52,15 @@ struct Selection {
     double ck[LOC_MAX_TRANS];    // c^3 A / (8 pi nu^3 dv)
 };
 
+// hyperfine structure of the traced transitions (loc_set_hyperfine), slot by slot as in Selection: kernel parameter
+struct HfsTab {
+    int any;                                 // some traced transition has more than one component (or a shifted one)
+    int nc[LOC_MAX_TRANS];                   // components of the slot's transition (>= 1)
+    float dch[LOC_MAX_TRANS][LOC_MAX_HFS];   // offsets of the components in CHANNELS (dv_k / dv)
+    float w[LOC_MAX_TRANS][LOC_MAX_HFS];     // weights
+    float lo, hi;                            // smallest / largest offset over all traced transitions, channels
+};
+
 // per-direction data of the integer ray lattice (DESIGN 6.3).  Working frame: axis 0 = main axis (zeta), 1 = p, 2 = q;
 // axes with a negative direction component are mirrored so that every ray moves towards +zeta, +p, +q.
 struct Dir3 {
@@ -107,6 +116,9 @@ struct loc_model {
     float *d_rates_f;           // [64][66] dense float32 rate table of k_solve_f (ntemp > 1)
     bool rates_f_valid;
     Selection selh;
+    int h_hfs_nc[LOC_MAX_LEVELS * (LOC_MAX_LEVELS - 1) / 2];              // hyperfine components per species transition (0 = none)
+    double h_hfs_dv[LOC_MAX_LEVELS * (LOC_MAX_LEVELS - 1) / 2][LOC_MAX_HFS];
+    double h_hfs_w[LOC_MAX_LEVELS * (LOC_MAX_LEVELS - 1) / 2][LOC_MAX_HFS];
     bool coef_valid;
     int ali;  // 1: accelerated lambda iteration (default), 0: plain lambda iteration (loc_set_ali)
     float *pops;  // registered [nlevel][ncell]
@@ -432,6 +444,8 @@ static inline Tree make_tree(const loc_model *m)
 // kernels / launchers implemented in the other translation units
 // ------------------------------------------------------------------------------------------------
 int loc_launch_solve(loc_model *m);
+void loc_fill_hfs(const loc_model *m, HfsTab &H);                       // table of the current selection
+void loc_fill_hfs_one(const loc_model *m, int trans, HfsTab &H);        // slot 0 = species transition `trans` (spectra)
 int loc_launch_sim1d(loc_model *m, int geom);
 int loc_launch_sim3d(loc_model *m, int geom);
 int loc_setup3d(loc_model *m);

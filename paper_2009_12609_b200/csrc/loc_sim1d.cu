@@ -22,6 +22,7 @@ struct Sim1D {
     uint32_t *visits;
     unsigned long long *nactive;
     Selection S;
+    HfsTab H;
 };
 
 __device__ __forceinline__ void seg1d(const Sim1D &P, int j, int nin, int k0, long long off, int &k, float &s, float &mu, float &w)
@@ -70,10 +71,14 @@ __device__ __forceinline__ void load_step1d(const Sim1D &P, int j, int nin, int 
     if (lane < NT) S.ke = __ldg(P.coef + (long long)S.k * P.nsp + lane);
 }
 
-template <int NT, bool GEOM>
+// HFS: some traced transition has hyperfine structure (loc_set_hyperfine): every transition then gets its own profile, the
+// sum over its components, evaluated over ONE window that covers the components of all transitions; the sum of the sampled
+// profile is folded into the escape sum transition by transition (b_t -= g_t sum phi_t), and with GEOM the active channels
+// are counted per transition (within 5 sigma of any of its components).
+template <int NT, bool GEOM, bool HFS>
 __global__ void __launch_bounds__(LOC_1D_WARPS * 32) k_sim1d_w(Sim1D P, int nray)
 {
-    constexpr int NV = 2 * NT + 1;
+    constexpr int NV = HFS ? 2 * NT : 2 * NT + 1;
     extern __shared__ __align__(16) float s_w[];  // per warp: [NT][nchp] spectra, then NT TParam
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int slot = blockIdx.x * LOC_1D_WARPS + warp;
@@ -119,8 +124,8 @@ __global__ void __launch_bounds__(LOC_1D_WARPS * 32) k_sim1d_w(Sim1D P, int nray
         if (tau0m > P.eps_tau) X = fmaxf(X, sqrtf(2.0f * __logf(tau0m / P.eps_tau)));
         const float cc = v0 * inv_dv + chalf;
         const float hw = X * sig * inv_dv;
-        const int c_lo = max(0, (int)ceilf(cc - hw)), c_hi = min(P.nch - 1, (int)floorf(cc + hw));
-        if (GEOM) {
+        const int c_lo = max(0, (int)ceilf(cc + (HFS ? P.H.lo : 0.0f) - hw)), c_hi = min(P.nch - 1, (int)floorf(cc + (HFS ? P.H.hi : 0.0f) + hw));
+        if (GEOM && !HFS) {
             const float h5 = 5.0f * sig * inv_dv;
             nact += (unsigned long long)max(0, min(P.nch - 1, (int)floorf(cc + h5)) - max(0, (int)ceilf(cc - h5)) + 1);
         }
@@ -129,6 +134,37 @@ __global__ void __launch_bounds__(LOC_1D_WARPS * 32) k_sim1d_w(Sim1D P, int nray
         float v[NV];
 #pragma unroll
         for (int i = 0; i < NV; i++) v[i] = 0.f;
+        if (HFS) {
+            const float kyc = ky * P.dv;  // per channel
+            for (int cb = (c_lo & ~3) + 4 * lane; cb <= c_hi; cb += 128) {
+#pragma unroll
+                for (int t = 0; t < NT; t++) {
+                    float phi[4] = {0.f, 0.f, 0.f, 0.f};
+                    bool act[4] = {false, false, false, false};
+                    for (int q = 0; q < P.H.nc[t]; q++) {
+                        const float wq = P.H.w[t][q], dq = P.H.dch[t][q];
+#pragma unroll
+                        for (int i = 0; i < 4; i++) {
+                            const int c = cb + i;
+                            const float y = ((float)c - cc - dq) * kyc;
+                            const bool in = c >= c_lo && c <= c_hi;
+                            phi[i] = in ? fmaf(wq, ex2f(fmaf(-y, y, lamp)), phi[i]) : phi[i];
+                            act[i] |= in && y * y <= 18.033688f;  // |v - v0 - dv_q| <= 5 sigma
+                        }
+                    }
+                    if (GEOM) nact += (unsigned long long)((int)act[0] + (int)act[1] + (int)act[2] + (int)act[3]);
+                    const TParam tp = stp[t];
+                    float4 n4 = *reinterpret_cast<float4 *>(sn + t * nchp + cb);
+                    f32x2 n01 = pk2(n4.x, n4.y), n23 = pk2(n4.z, n4.w);
+                    channel_update4(n01, n23, pk2(phi[0], phi[1]), pk2(phi[2], phi[3]), tp, v[t], v[NT + t]);
+                    // photons emitted outside the window escape: w (1 - sum phi_t), as -g_t sum phi_t in the units of b_t
+                    v[NT + t] = fmaf(tp.thick ? tp.c0 * (1.0f / LOC_LOG2E) : -1.0f, (phi[0] + phi[1]) + (phi[2] + phi[3]), v[NT + t]);
+                    upk2(n01, n4.x, n4.y);
+                    upk2(n23, n4.z, n4.w);
+                    *reinterpret_cast<float4 *>(sn + t * nchp + cb) = n4;
+                }
+            }
+        } else
         for (int cb = (c_lo & ~3) + 4 * lane; cb <= c_hi; cb += 128) {
             float phi[4];
 #pragma unroll
@@ -152,8 +188,11 @@ __global__ void __launch_bounds__(LOC_1D_WARPS * 32) k_sim1d_w(Sim1D P, int nray
         }
         int owner;
         const float tot = warp_multi_reduce<NV>(v, lane, owner);
-        const unsigned mphi = __ballot_sync(0xffffffffu, owner == 2 * NT);
-        const float sphi = __shfl_sync(0xffffffffu, tot, __ffs(mphi) - 1);
+        float sphi = 0.0f;  // (HFS: already folded into the escape sums)
+        if (!HFS) {
+            const unsigned mphi = __ballot_sync(0xffffffffu, owner == 2 * NT);
+            sphi = __shfl_sync(0xffffffffu, tot, __ffs(mphi) - 1);
+        }
         if (owner >= 0 && owner < 2 * NT) {
             const int t = owner < NT ? owner : owner - NT;
             float2 *cn = P.cnt + (long long)cur.k * P.nsp + t;
@@ -165,7 +204,14 @@ __global__ void __launch_bounds__(LOC_1D_WARPS * 32) k_sim1d_w(Sim1D P, int nray
         if (GEOM && lane == 0) atomicAdd(&P.visits[cur.k], 1u);
         cur = nxt;
     }
-    if (GEOM && lane == 0 && nact) atomicAdd(P.nactive, nact);
+    if (GEOM) {  // active updates of the ray, summed over the traced transitions (loc_stats.active_updates)
+        if (HFS) {
+            for (int o = 16; o >= 1; o >>= 1) nact += __shfl_xor_sync(0xffffffffu, nact, o);
+        } else {
+            nact *= NT;
+        }
+        if (lane == 0 && nact) atomicAdd(P.nactive, nact);
+    }
 }
 
 template <int NT>
@@ -179,13 +225,19 @@ static int launch1d(loc_model *m, const Sim1D &P, int geom)
         return LOC_EINVAL;
     }
     const int blocks = (m->nray + LOC_1D_WARPS - 1) / LOC_1D_WARPS;
-    if (geom) {
-        LOC_CUDA_CHECK(m, cudaFuncSetAttribute(k_sim1d_w<NT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_w));
-        k_sim1d_w<NT, true><<<blocks, LOC_1D_WARPS * 32, smem_w, m->stream>>>(P, m->nray);
+#define LOC_L1(G, HF)                                                                                                             \
+    do {                                                                                                                          \
+        LOC_CUDA_CHECK(m, cudaFuncSetAttribute(k_sim1d_w<NT, G, HF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_w)); \
+        k_sim1d_w<NT, G, HF><<<blocks, LOC_1D_WARPS * 32, smem_w, m->stream>>>(P, m->nray);                                    \
+    } while (0)
+    if (P.H.any) {
+        if (geom) LOC_L1(true, true);
+        else LOC_L1(false, true);
     } else {
-        LOC_CUDA_CHECK(m, cudaFuncSetAttribute(k_sim1d_w<NT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_w));
-        k_sim1d_w<NT, false><<<blocks, LOC_1D_WARPS * 32, smem_w, m->stream>>>(P, m->nray);
+        if (geom) LOC_L1(true, false);
+        else LOC_L1(false, false);
     }
+#undef LOC_L1
     m->launches++;
     LOC_CUDA_CHECK(m, cudaGetLastError());
     return LOC_OK;
@@ -212,6 +264,7 @@ int loc_launch_sim1d(loc_model *m, int geom)
     P.visits = m->visits;
     P.nactive = m->d_steps + 1;
     P.S = m->selh;
+    loc_fill_hfs(m, P.H);
     switch (m->selh.nsel) {
 #define C1(N) \
     case N:   \

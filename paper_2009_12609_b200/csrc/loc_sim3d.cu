@@ -59,6 +59,10 @@ struct Sim3D {
     int slot0;  // first counter / coefficient slot handled by this launch (transitions may be split over launches)
     int geom;   // also accumulate the geometry counters (visits, path sums, active channels)
     float dv, xmin, xclip, xfull, inv_ndir;
+    int nsel_all;  // traced transitions of the whole selection (this launch may hold a part)
+    int geomact;   // count the active channel-transitions of the masked rounds (hyperfine structure: every part of a split launch)
+    unsigned long long *nactive;
+    HfsTab H;      // hyperfine structure of the selection's slots
     const Dir3 *dirs;
     const uint16_t *task_dir;
     const long long *task_off;
@@ -379,9 +383,10 @@ __device__ __forceinline__ unsigned step_mode(const Sim3D &P, unsigned rb, float
         const bool ok1 = P.nch >= LOC_SPAN && (wb == 0 || cc - (float)wb >= need) && (wb + LOC_SPAN >= P.nch || (float)(wb + LOC_SPAN - 1) - cc >= need) &&
                          (wb - LOC_EXT <= 0 || cc - (float)(wb - LOC_EXT) >= needf) &&
                          (wb + LOC_SPAN + LOC_EXT >= P.nch || (float)(wb + LOC_SPAN + LOC_EXT - 1) - cc >= needf);
-        if (-h0.z > 0.7213475f) {
+        if (-h0.z > 0.7213475f || P.H.any) {
             // channels wider than the line (sigma < dv; -q2 = log2(e) / (2 sigch^2)): the exact masked path, which sums the
-            // sampled profile itself and evaluates it from the distance to the line centre (DESIGN 5.3)
+            // sampled profile itself and evaluates it from the distance to the line centre (DESIGN 5.3); so do all steps of a
+            // model with hyperfine structure (a profile per transition, components spread over the band)
             flags |= LOC_RS_SLOW;
         } else if (!ok1) {
             const int ww = wide_start(P.nch, cc);
@@ -427,13 +432,14 @@ __device__ __forceinline__ TCoef make_tcoef(float2 cf)
 // (a_t, b_t - g_t sum phi), i.e. with the lane's sum of the sampled profile already folded into b (see the reduction).
 // Scalar arithmetic, rolled over the transitions; same expressions as the common round.
 template <int NT, int W>
-__device__ __forceinline__ void slow_round(const Sim3D &P, unsigned rb, unsigned sqg, unsigned pl, int l8, int nchp)
+__device__ __forceinline__ unsigned slow_round(const Sim3D &P, unsigned rb, unsigned sqg, unsigned pl, int l8, int nchp)
 {
     typedef Lay<NT> L;
     typedef Own<NT, W> O;
     const float4 h0 = lds128(rb);
     const uint4 h1 = lds128u(rb + 16);
     const unsigned wbop = __float_as_uint(h0.w);
+    const bool hfs = P.H.any;  // hyperfine structure: a profile per transition, summed over its components (loc_set_hyperfine)
     int clo = 1, chi = 0;
     // the profile from the distance to the line centre: log2 phi(c) = lamp - ((c - cc) ky)^2.  (The quadratic around the
     // middle of the span that the common round uses cancels badly when the span is clamped far from the line AND the
@@ -452,12 +458,13 @@ __device__ __forceinline__ void slow_round(const Sim3D &P, unsigned rb, unsigned
         if (tau0m > 1.0f) X2 = fmaf(2.0f, __logf(tau0m), X2);
         const float X = sqrtf(X2);
         const float cc = __uint_as_float(h1.w), hw = X * sigch;
-        clo = max(0, (int)ceilf(cc - hw));
-        chi = min(P.nch - 1, (int)floorf(cc + hw));
+        clo = max(0, (int)ceilf(cc + P.H.lo - hw));  // (lo = hi = 0 without hyperfine structure: one window for all components)
+        chi = min(P.nch - 1, (int)floorf(cc + P.H.hi + hw));
     }
 #pragma unroll 1
     for (int t = O::TB; t < O::TB + O::NW; t++) sts64(pl + t * L::ROWB, make_float2(0.f, 0.f));
     float sphi = 0.f;
+    unsigned nact = 0;
     int base = clo & ~3;
     while (__any_sync(0xffffffffu, base <= chi)) {
         const int cb = base + 4 * l8;
@@ -476,6 +483,27 @@ __device__ __forceinline__ void slow_round(const Sim3D &P, unsigned rb, unsigned
 #pragma unroll 1
             for (int t = O::TB; t < O::TB + O::NW; t++) {
                 const TCoef tc = make_tcoef(lds64(rb + L::CF + 8 * t));
+                float fold = 0.0f;
+                if (hfs) {  // the transition's own profile over the same channels; its sum is folded into b here
+                    const int slot = P.slot0 + t;
+                    bool act[4] = {false, false, false, false};
+#pragma unroll
+                    for (int k = 0; k < 4; k++) e[k] = 0.0f;
+                    for (int q = 0; q < P.H.nc[slot]; q++) {
+                        const float wq = P.H.w[slot][q], dq = P.H.dch[slot][q];
+#pragma unroll
+                        for (int k = 0; k < 4; k++) {
+                            const int c = cb + k;
+                            const float y = ((float)c - ccc - dq) * kyc;
+                            if (c >= clo && c <= chi) {
+                                e[k] = fmaf(wq, ex2f(fmaf(-y, y, lamp)), e[k]);
+                                act[k] |= y * y <= 18.033688f;  // within 5 sigma of the component (the metric's counting rule)
+                            }
+                        }
+                    }
+                    fold = tc.g * ((e[0] + e[1]) + (e[2] + e[3]));
+                    if (P.geomact) nact += (unsigned)act[0] + (unsigned)act[1] + (unsigned)act[2] + (unsigned)act[3];
+                }
                 const unsigned sa = sqg + 4 * base + 4 * t * nchp;
                 const float4 n4 = lds128(sa);
                 float n[4] = {n4.x, n4.y, n4.z, n4.w};
@@ -490,17 +518,20 @@ __device__ __forceinline__ void slow_round(const Sim3D &P, unsigned rb, unsigned
                 }
                 sts128(sa, make_float4(n[0], n[1], n[2], n[3]));
                 const float2 pv = lds64(pl + t * L::ROWB);
-                sts64(pl + t * L::ROWB, make_float2(pv.x + a, pv.y + b));
+                sts64(pl + t * L::ROWB, make_float2(pv.x + a, pv.y + b - fold));
             }
         }
         base += LOC_SPAN;
     }
+    if (!hfs) {
 #pragma unroll 1
-    for (int t = O::TB; t < O::TB + O::NW; t++) {  // fold the lane's sum of phi into b (the round sums phi itself: qe = -1)
-        const TCoef tc = make_tcoef(lds64(rb + L::CF + 8 * t));
-        const float2 pv = lds64(pl + t * L::ROWB);
-        sts64(pl + t * L::ROWB, make_float2(pv.x, fmaf(-tc.g, sphi, pv.y)));
+        for (int t = O::TB; t < O::TB + O::NW; t++) {  // fold the lane's sum of phi into b (the round sums phi itself: qe = -1)
+            const TCoef tc = make_tcoef(lds64(rb + L::CF + 8 * t));
+            const float2 pv = lds64(pl + t * L::ROWB);
+            sts64(pl + t * L::ROWB, make_float2(pv.x, fmaf(-tc.g, sphi, pv.y)));
+        }
     }
+    return nact;
 }
 
 // The common round: one pass over the span for the warp's NW transitions, straight-line code.  `sq` = shared address of
@@ -629,7 +660,7 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
     bool done = false, fresh = false;
     float4 dir = make_float4(0.f, 0.f, 0.f, 0.f);  // (d0, d1, d2, sf) of the group's ray
     unsigned mysteps = 0;
-    unsigned long long myactive = 0;
+    unsigned long long myactive = 0, hfsact = 0;
     // software pipeline over chunks: r0 = records of this chunk, r1 / r2 = of the next two (r2 in flight), `cell` = cell
     // data of r0's record, loaded during the previous chunk's rounds
     uint2 r0 = NOPREC, r1 = NOPREC, r2 = NOPREC;
@@ -734,7 +765,7 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
 #pragma unroll
             for (int i = 0; i < O::NHR * 2; i++) ab[i] = make_float2(0.f, 0.f);
             if (cls & LOC_RS_SLOW) {
-                slow_round<NT, W>(P, rb, sq_g, pl, l8, nchp);
+                hfsact += slow_round<NT, W>(P, rb, sq_g, pl, l8, nchp);
 #pragma unroll
                 for (int i = 0; i < O::NW; i++) ab[i] = lds64(pl + (O::TB + i) * L::ROWB);
             } else {
@@ -803,7 +834,12 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
             myactive += __shfl_xor_sync(0xffffffffu, myactive, o);
         }
         if (lane == 0 && ms) atomicAdd(P.nsteps, ms);
-        if (P.geom && lane == 0 && myactive) atomicAdd(P.nsteps + 1, myactive);
+        // active updates = active channels of the steps x traced transitions (loc_stats.active_updates) ...
+        if (P.geom && !P.H.any && lane == 0 && myactive) atomicAdd(P.nactive, myactive * (unsigned long long)P.nsel_all);
+    }
+    if (P.geomact && P.H.any) {  // ... with hyperfine structure counted transition by transition in the masked round (every warp its own)
+        for (int o = 16; o >= 1; o >>= 1) hfsact += __shfl_xor_sync(0xffffffffu, hfsact, o);
+        if (lane == 0 && hfsact) atomicAdd(P.nactive, hfsact);
     }
 }
 
@@ -887,9 +923,12 @@ int loc_launch_sim3d(loc_model *m, int geom)
     P.visits = m->visits;
     P.pathz = m->pathz;
     P.nsteps = m->d_steps;
+    P.nactive = m->d_steps + 1;
     P.queue = m->d_queue;
     P.pool = m->spec_pool;
     P.S = m->selh;
+    P.nsel_all = m->selh.nsel;
+    loc_fill_hfs(m, P.H);
     if ((long long)m->ncell * P.nsp >= (1ll << 32)) {
         snprintf(m->err, sizeof(m->err), "ncell * ntrans exceeds the 32-bit counter offsets of the 3D kernel");
         return LOC_EINVAL;
@@ -909,6 +948,7 @@ int loc_launch_sim3d(loc_model *m, int geom)
         int rc = LOC_EINVAL;
         // the step / active-channel statistics are taken by the first part only
         P.geom = geom && part == 0;
+        P.geomact = geom && (part == 0 || P.H.any);
         unsigned long long *keep = P.nsteps;
         if (part > 0) P.nsteps = m->d_steps + 2;  // scratch slot
         switch (n) {

@@ -30,6 +30,9 @@ struct SpecCommon {
     const float *pop_u, *pop_l;
     const float4 *kin;
     float *out;
+    // hyperfine structure of the transition (loc_set_hyperfine): nc components at dch channels from the line centre
+    int nc;
+    float dch[LOC_MAX_HFS], wgt[LOC_MAX_HFS], lo, hi;
 };
 
 // one cell step of a line of sight: all lanes of the warp, channels of the window split over the lanes
@@ -49,12 +52,21 @@ __device__ __forceinline__ void spectrum_step(const SpecCommon &C, float *D, int
     const float inv_dv = __fdividef(1.0f, C.dv);
     const float cc = fmaf(v0, inv_dv, 0.5f * (float)(C.nch - 1));
     const float hw = X * sig * inv_dv;
-    const int clo = max(0, (int)ceilf(cc - hw)), chi = min(C.nch - 1, (int)floorf(cc + hw));
+    const int clo = max(0, (int)ceilf(cc + C.lo - hw)), chi = min(C.nch - 1, (int)floorf(cc + C.hi + hw));
     const float ky = C.dv * 0.8493218f * inv_sig, lamp = __log2f(amp);
     const bool thick = tau0 >= 0.03f;
     for (int c = clo + lane; c <= chi; c += 32) {
-        const float y = ((float)c - cc) * ky;
-        const float phi = ex2f(fmaf(-y, y, lamp));
+        float phi;
+        if (C.nc == 1 && C.dch[0] == 0.0f) {
+            const float y = ((float)c - cc) * ky;
+            phi = ex2f(fmaf(-y, y, lamp));
+        } else {  // sum over the hyperfine components (LTE between them, one source function)
+            phi = 0.0f;
+            for (int q = 0; q < C.nc; q++) {
+                const float y = ((float)c - cc - C.dch[q]) * ky;
+                phi = fmaf(C.wgt[q], ex2f(fmaf(-y, y, lamp)), phi);
+            }
+        }
         const float tau = ks * phi;
         float Xc;
         if (thick)
@@ -180,6 +192,15 @@ static void spec_common(loc_model *m, int trans, SpecCommon &C)
     C.pop_u = m->pops + (int64_t)u * m->ncell;
     C.pop_l = m->pops + (int64_t)l * m->ncell;
     C.kin = m->kin;
+    HfsTab H;
+    loc_fill_hfs_one(m, trans, H);
+    C.nc = H.nc[0];
+    for (int q = 0; q < LOC_MAX_HFS; q++) {
+        C.dch[q] = H.dch[0][q];
+        C.wgt[q] = H.w[0][q];
+    }
+    C.lo = H.lo;
+    C.hi = H.hi;
 }
 
 static int launch_spectra3d(loc_model *m, int trans, const double *dir, int nx, int ny, const double *o, const double *ex, const double *ey,

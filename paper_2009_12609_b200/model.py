@@ -69,6 +69,8 @@ class LocModel:
         self.h = B.loc_create_model(self.grid, self.cells, self.nch, m.band_half, m.t_bg, self.nlevel, nts, ndir_max,
                                     self.workspace, sptr)
         B.loc_set_species(self.h, sp)
+        for t, (dvk, wk) in sorted((getattr(sp, "hfs", None) or {}).items()):
+            B.loc_set_hyperfine(self.h, t, dvk, wk)
         if self.is3d:
             B.loc_set_directions(self.h, m.dirs)
         self.pops = torch.empty((self.nlevel, self.ncell), dtype=torch.float32, device=self.dev)
