@@ -56,6 +56,11 @@ def make_workload(name: str):
         return W.shell_config(1), "C1: 1D, 64 log shells, 64 rays, 64 channels, 5-level rotor (4 transitions)"
     if name == "C2":
         return W.shell_config(2), "C2: 1D, 1000 log shells, 4000 rays, 256 channels, 10-level rotor (9 transitions)"
+    if name == "C2H":  # C2 with a three-component hyperfine structure on J = 1-0 (LTE between the components)
+        m = W.shell_config(2)
+        m.species.hfs = {0: (np.array([-1.0e5, 0.05e5, 0.7e5]), np.array([0.2, 0.5, 0.3]))}
+        m.name = "C2H"
+        return m, "C2H: C2 with hyperfine structure on J = 1-0: components at -1.0, +0.05, +0.7 km/s with weights 0.2, 0.5, 0.3"
     if name == "C3":
         return W.cloud_config(3), "C3: Cartesian 128^3, 48 directions, 128 channels, 10-level rotor (9 transitions)"
     if name == "C4":
@@ -110,6 +115,20 @@ class ClockSampler(threading.Thread):
 
 # ---- CPU oracle sample (cpu_baseline / --impl reference) --------------------------------------------------------------
 _KB_OVER_AMU = 1.380649e-16 / 1.66053906660e-24
+
+
+def _union_count(cc, hw, nch, offs):
+    """channels of [0, nch) within hw of any of the centres cc + offs (offs ascending; arrays over steps)"""
+    tot = 0.0
+    prev_hi = None
+    for o in offs:
+        lo = np.maximum(0, np.ceil(cc + o - hw))
+        hi = np.minimum(nch - 1, np.floor(cc + o + hw))
+        if prev_hi is not None:
+            lo = np.maximum(lo, prev_hi + 1)
+        tot += float(np.maximum(0, hi - lo + 1).sum())
+        prev_hi = hi if prev_hi is None else np.maximum(prev_hi, hi)
+    return tot
 
 
 def active_channels_per_cell(m, d=None):
@@ -187,12 +206,14 @@ def oracle_sample(m, budget_updates=6e9, keep=False):
                       * np.asarray(m.tkin, np.float64))
         vr = np.asarray(m.vrad, np.float64)
         act = 0.0
+        hfs = getattr(m.species, "hfs", None) or {}
         for p_ in ms.ray_p:
             sh, _, mu = O.path_1d(m.r_out, float(p_))
             cc = -vr[sh] * mu / dv + 0.5 * (nch - 1)
             hw = 5.0 * sig[sh] / dv
-            act += float(np.maximum(0, np.minimum(nch - 1, np.floor(cc + hw)) - np.maximum(0, np.ceil(cc - hw)) + 1).sum())
-        act *= nt
+            for t in sel:  # a transition's active channels: within 5 sigma of any of its hyperfine components
+                offs = np.sort(np.asarray(hfs[int(t)][0], np.float64) / dv) if int(t) in hfs else np.zeros(1)
+                act += _union_count(cc, hw, nch, offs)
         desc = f"{len(kept)} of {nray} rays, all {len(sel)} transitions, all {nch} channels; then the solve"
         threads = 1  # the 1D ray loop of the oracle is serial
     out = {"nominal": nominal_updates(steps, nch, nt), "active": act, "seconds": dt, "threads": threads, "desc": desc}
@@ -296,8 +317,8 @@ def parity_leg(g, m, dirs_idx, ntrans=1):
 def roofline(stats_geom, nt, t_sim_s, hbm_gbs, sm_mhz, peak_kind):
     """T_roof = max(bytes / HBM, MUFU ops / MUFU rate, FP32 instructions / issue rate) for the simulation
     kernel; `achieved`/`peak` are quoted for the binding resource."""
-    steps, act = stats_geom["steps"], stats_geom["active_channels"]
-    u_active = float(act) * nt
+    steps = stats_geom["steps"]
+    u_active = float(stats_geom["active_updates"])
     byt = float(steps) * (8 + 16 + 24 * nt)
     mufu = u_active * (1.0 + 1.0 / nt)
     fp32 = u_active * (8.0 + 4.0 / nt)
@@ -388,7 +409,7 @@ def run_own(args):
     t_solve = sum(e[1].elapsed_time(e[2]) for e in ev) * 1e-3
     t_all = ev_all[0].elapsed_time(ev_all[1]) * 1e-3
     t_all, t_sim, t_solve = max_over_ranks([t_all, t_sim, t_solve], device=f"cuda:{local}")
-    u_act = float(sg["active_channels"]) * nt
+    u_act = float(sg["active_updates"])
     value = whole_job_value(u_act, args.steps, world, t_all)
 
     # ---- end to end: host buffers -> device -> one ALI iteration -> populations back to the host ----

@@ -35,7 +35,9 @@ struct SpecCommon {
     float dch[LOC_MAX_HFS], wgt[LOC_MAX_HFS], lo, hi;
 };
 
-// one cell step of a line of sight: all lanes of the warp, channels of the window split over the lanes
+// one cell step of a line of sight: the LPL lanes that carry it split the channels of the window (lane l owns the channels
+// c = l mod LPL throughout, so the lanes of a line of sight never touch each other's channels: no synchronisation)
+template <int LPL>
 __device__ __forceinline__ void spectrum_step(const SpecCommon &C, float *D, int lane, long long cell, float s, float v0, float sig)
 {
     const double nu_ = (double)__ldg(C.pop_u + cell), nl_ = (double)__ldg(C.pop_l + cell);
@@ -55,7 +57,7 @@ __device__ __forceinline__ void spectrum_step(const SpecCommon &C, float *D, int
     const int clo = max(0, (int)ceilf(cc + C.lo - hw)), chi = min(C.nch - 1, (int)floorf(cc + C.hi + hw));
     const float ky = C.dv * 0.8493218f * inv_sig, lamp = __log2f(amp);
     const bool thick = tau0 >= 0.03f;
-    for (int c = clo + lane; c <= chi; c += 32) {
+    for (int c = clo + ((lane - clo) & (LPL - 1)); c <= chi; c += LPL) {
         float phi;
         if (C.nc == 1 && C.dch[0] == 0.0f) {
             const float y = ((float)c - cc) * ky;
@@ -90,15 +92,19 @@ struct Spec3D {
     double o[2], ex[2], ey[2];
 };
 
+// Octree: a quarter-warp per line of sight, four neighbouring pixels per warp (round 1 gave a whole warp to each: all 32
+// lanes repeated the 64-bit lattice walk and the ~40 channels of a step's window left the second trip over the lanes
+// mostly idle: C5 cube 143 ms).  The four walks of a warp diverge only where their cells differ in refinement.
+#define LOC_SPEC_LPL 8
 __global__ void __launch_bounds__(32 * LOC_SPEC_WARPS) k_spectra3d(Spec3D P)
 {
     extern __shared__ __align__(16) float smem[];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const long long pix = (long long)blockIdx.x * LOC_SPEC_WARPS + warp;
+    constexpr int LPW = 32 / LOC_SPEC_LPL;  // lines of sight per warp
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, grp = lane / LOC_SPEC_LPL, l = lane % LOC_SPEC_LPL;
+    const long long pix = ((long long)blockIdx.x * LOC_SPEC_WARPS + warp) * LPW + grp;
     if (pix >= (long long)P.nx * P.ny) return;
-    float *Dc = smem + warp * P.C.nchp;
-    for (int c = lane; c < P.C.nchp; c += 32) Dc[c] = 0.f;
-    __syncwarp();
+    float *Dc = smem + (warp * LPW + grp) * P.C.nchp;
+    for (int c = l; c < P.C.nchp; c += LOC_SPEC_LPL) Dc[c] = 0.f;
     const int ix = (int)(pix % P.nx), iy = (int)(pix / P.nx);
     const long long bp = (long long)floor(__dadd_rn(__dadd_rn(P.o[0], __dmul_rn((double)ix, P.ex[0])), __dmul_rn((double)iy, P.ey[0])));
     const long long bq = (long long)floor(__dadd_rn(__dadd_rn(P.o[1], __dmul_rn((double)ix, P.ex[1])), __dmul_rn((double)iy, P.ey[1])));
@@ -120,12 +126,11 @@ __global__ void __launch_bounds__(32 * LOC_SPEC_WARPS) k_spectra3d(Spec3D P)
         const long long cell = L.cell[L.level];
         const float4 k = __ldg(P.C.kin + cell);
         const float v0 = -(k.x * D.d[0] + k.y * D.d[1] + k.z * D.d[2]);  // DESIGN R6
-        spectrum_step(P.C, Dc, lane, cell, (float)(znext - zeta) * D.sf, v0, k.w);
+        spectrum_step<LOC_SPEC_LPL>(P.C, Dc, l, cell, (float)(znext - zeta) * D.sf, v0, k.w);
         zeta = znext;
     }
-    __syncwarp();
     float *o = P.C.out + pix * P.C.nch;
-    for (int c = lane; c < P.C.nch; c += 32) o[c] = P.C.tk_per_occ * Dc[c];
+    for (int c = l; c < P.C.nch; c += LOC_SPEC_LPL) o[c] = P.C.tk_per_occ * Dc[c];
 }
 
 struct Spec1D {
@@ -168,7 +173,7 @@ __global__ void __launch_bounds__(32 * LOC_SPEC_WARPS) k_spectra1d(Spec1D P)
                 mu = sqrt(1.0 - b2 / (ri * ri));
             }
             const float4 kk = __ldg(P.C.kin + k);
-            spectrum_step(P.C, Dc, lane, k, (float)s, -kk.x * (float)mu, kk.w);
+            spectrum_step<32>(P.C, Dc, lane, k, (float)s, -kk.x * (float)mu, kk.w);
         }
     }
     __syncwarp();
@@ -223,9 +228,11 @@ static int launch_spectra3d(loc_model *m, int trans, const double *dir, int nx, 
         P.ex[i] = ex[i];
         P.ey[i] = ey[i];
     }
-    const size_t smem = sizeof(float) * LOC_SPEC_WARPS * P.C.nchp;
+    constexpr int PPB = LOC_SPEC_WARPS * (32 / LOC_SPEC_LPL);  // pixels per block
+    const size_t smem = sizeof(float) * PPB * P.C.nchp;
     const long long npix = (long long)nx * ny;
-    k_spectra3d<<<(unsigned)((npix + LOC_SPEC_WARPS - 1) / LOC_SPEC_WARPS), 32 * LOC_SPEC_WARPS, smem, m->stream>>>(P);
+    if (smem > 48 * 1024) LOC_CUDA_CHECK(m, cudaFuncSetAttribute(k_spectra3d, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_spectra3d<<<(unsigned)((npix + PPB - 1) / PPB), 32 * LOC_SPEC_WARPS, smem, m->stream>>>(P);
     m->launches++;
     LOC_CUDA_CHECK(m, cudaGetLastError());
     return LOC_OK;
