@@ -388,7 +388,7 @@ __global__ void __launch_bounds__(LOC_SOLVE_F_THREADS) k_solve_f(int64_t n, cons
                 f = (T - Q.temps[j]) / (Q.temps[j + 1] - Q.temps[j]);
             }
         }
-        const float nit = __fdividef(-1.0f, T);  // (approximate reciprocals throughout: 1 ulp, against a tolerance of 1e-3)
+        const float nit = -1.0f / T;
         float R[NL][NL];
 #pragma unroll
         for (int u = 1; u < NL; u++) {
@@ -420,7 +420,7 @@ __global__ void __launch_bounds__(LOC_SOLVE_F_THREADS) k_solve_f(int64_t n, cons
             float sm = 0.0f;
 #pragma unroll
             for (int c = 0; c < q; c++) sm += R[q][c];
-            const float inv = sm > 0.0f ? __fdividef(1.0f, sm) : 0.0f;
+            const float inv = sm > 0.0f ? 1.0f / sm : 0.0f;
 #pragma unroll
             for (int r = 0; r < q; r++) {
                 const float rq = R[r][q] * inv;
@@ -441,13 +441,12 @@ __global__ void __launch_bounds__(LOC_SOLVE_F_THREADS) k_solve_f(int64_t n, cons
             x[q] = sm;
             tot += sm;
         }
-        const float sc = __fdividef(ntot, tot);
-        const float floor_n = 1e-10f * ntot;
+        const float sc = ntot / tot;
 #pragma unroll
         for (int l = 0; l < NL; l++) {
             const float nw = x[l] * sc;
             const float old = pops[(int64_t)l * n + i];
-            if (ntot > 0.0f && (nw >= floor_n || old >= floor_n)) rel = fmaxf(rel, __fdividef(fabsf(nw - old), fmaxf(nw, 1e-37f)));
+            if (ntot > 0.0f && (nw >= 1e-10f * ntot || old >= 1e-10f * ntot)) rel = fmaxf(rel, fabsf(nw - old) / fmaxf(nw, 1e-37f));
             if (!isfinite(nw)) rel = INFINITY;  // see k_solve
             pops[(int64_t)l * n + i] = nw;
             col[l * TH] = nw;
