@@ -360,7 +360,7 @@ __device__ __forceinline__ int wide_start(int nch, float cc)
 // sum  sum phi f(tau) ~ 1 / tau0  as LOC_XCLIP sigma for a thin line (DESIGN 5.3).  If the centred 32-channel span reaches
 // that far on both sides (or to the edge of the band) the step is a common round; else, if two adjacent spans do, a WIDE
 // round (two passes); else a masked round over its exact window.  Returns the record's flags with the mode bits.
-template <int NT>
+template <int NT, bool HFS>
 __device__ __forceinline__ unsigned step_mode(const Sim3D &P, unsigned rb, float &qe_wide)
 {
     qe_wide = -1.0f;  // profile mass outside the pair of spans of a WIDE step (-1: the round takes 1 - sum phi)
@@ -383,7 +383,7 @@ __device__ __forceinline__ unsigned step_mode(const Sim3D &P, unsigned rb, float
         const bool ok1 = P.nch >= LOC_SPAN && (wb == 0 || cc - (float)wb >= need) && (wb + LOC_SPAN >= P.nch || (float)(wb + LOC_SPAN - 1) - cc >= need) &&
                          (wb - LOC_EXT <= 0 || cc - (float)(wb - LOC_EXT) >= needf) &&
                          (wb + LOC_SPAN + LOC_EXT >= P.nch || (float)(wb + LOC_SPAN + LOC_EXT - 1) - cc >= needf);
-        if (-h0.z > 0.7213475f || P.H.any) {
+        if (-h0.z > 0.7213475f || HFS) {
             // channels wider than the line (sigma < dv; -q2 = log2(e) / (2 sigch^2)): the exact masked path, which sums the
             // sampled profile itself and evaluates it from the distance to the line centre (DESIGN 5.3); so do all steps of a
             // model with hyperfine structure (a profile per transition, components spread over the band)
@@ -431,7 +431,9 @@ __device__ __forceinline__ TCoef make_tcoef(float2 cf)
 // its width, DESIGN 5.3), for the warp's own transitions.  Leaves the lane's partial sums in its slots of the `part` rows:
 // (a_t, b_t - g_t sum phi), i.e. with the lane's sum of the sampled profile already folded into b (see the reduction).
 // Scalar arithmetic, rolled over the transitions; same expressions as the common round.
-template <int NT, int W>
+// HFS: the model has hyperfine structure (a template parameter: the kernels of models without it carry none of that code --
+// the instruction-fetch stalls of the common round grow with the size of the loop body, profiles/r2_sim3d.md)
+template <int NT, int W, bool HFS>
 __device__ __forceinline__ unsigned slow_round(const Sim3D &P, unsigned rb, unsigned sqg, unsigned pl, int l8, int nchp)
 {
     typedef Lay<NT> L;
@@ -439,7 +441,7 @@ __device__ __forceinline__ unsigned slow_round(const Sim3D &P, unsigned rb, unsi
     const float4 h0 = lds128(rb);
     const uint4 h1 = lds128u(rb + 16);
     const unsigned wbop = __float_as_uint(h0.w);
-    const bool hfs = P.H.any;  // hyperfine structure: a profile per transition, summed over its components (loc_set_hyperfine)
+    constexpr bool hfs = HFS;  // hyperfine structure: a profile per transition, summed over its components (loc_set_hyperfine)
     int clo = 1, chi = 0;
     // the profile from the distance to the line centre: log2 phi(c) = lamp - ((c - cc) ky)^2.  (The quadratic around the
     // middle of the span that the common round uses cancels badly when the span is clamped far from the line AND the
@@ -614,7 +616,7 @@ __device__ __forceinline__ void cta_sync()  // both warps of the CTA (one-warp C
 }
 
 // One warp of the CTA.  NCHP_T: spectrum row length in floats when known at compile time (immediate offsets), 0 = P.nchp
-template <int NT, int NCHP_T, int W>
+template <int NT, int NCHP_T, int W, bool HFS>
 __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
 {
     typedef Lay<NT> L;
@@ -706,7 +708,7 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
         cta_sync<W>();  // the records of the chunk are complete
         // mode of record rj (the lanes of a pair agree), then the class of round rj: OR over the four groups
         float myqew;
-        const unsigned myflags = step_mode<NT>(P, rec_g + rj * L::RECB, myqew);
+        const unsigned myflags = step_mode<NT, HFS>(P, rec_g + rj * L::RECB, myqew);
         unsigned orflags = myflags | __shfl_xor_sync(0xffffffffu, myflags, 8);
         orflags |= __shfl_xor_sync(0xffffffffu, orflags, 16);
 
@@ -765,7 +767,7 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
 #pragma unroll
             for (int i = 0; i < O::NHR * 2; i++) ab[i] = make_float2(0.f, 0.f);
             if (cls & LOC_RS_SLOW) {
-                hfsact += slow_round<NT, W>(P, rb, sq_g, pl, l8, nchp);
+                hfsact += slow_round<NT, W, HFS>(P, rb, sq_g, pl, l8, nchp);
 #pragma unroll
                 for (int i = 0; i < O::NW; i++) ab[i] = lds64(pl + (O::TB + i) * L::ROWB);
             } else {
@@ -835,32 +837,32 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
         }
         if (lane == 0 && ms) atomicAdd(P.nsteps, ms);
         // active updates = active channels of the steps x traced transitions (loc_stats.active_updates) ...
-        if (P.geom && !P.H.any && lane == 0 && myactive) atomicAdd(P.nactive, myactive * (unsigned long long)P.nsel_all);
+        if (P.geom && !HFS && lane == 0 && myactive) atomicAdd(P.nactive, myactive * (unsigned long long)P.nsel_all);
     }
-    if (P.geomact && P.H.any) {  // ... with hyperfine structure counted transition by transition in the masked round (every warp its own)
+    if (HFS && P.geomact) {  // ... with hyperfine structure counted transition by transition in the masked round (every warp its own)
         for (int o = 16; o >= 1; o >>= 1) hfsact += __shfl_xor_sync(0xffffffffu, hfsact, o);
         if (lane == 0 && hfsact) atomicAdd(P.nactive, hfsact);
     }
 }
 
-template <int NT, int NCHP_T, bool ONE>
+template <int NT, int NCHP_T, bool ONE, bool HFS>
 __global__ void __maxnreg__(ONE ? 152 : 128) k_sim3d(Sim3D P)
 {
     extern __shared__ __align__(16) float smem[];  // [4][NT][nchp] spectra, then the tables of Lay<NT>
     if (ONE)
-        run_warp<NT, NCHP_T, 2>(P, smem);
+        run_warp<NT, NCHP_T, 2, HFS>(P, smem);
     else if (threadIdx.x < 32)
-        run_warp<NT, NCHP_T, 0>(P, smem);
+        run_warp<NT, NCHP_T, 0, HFS>(P, smem);
     else
-        run_warp<NT, NCHP_T, 1>(P, smem);
+        run_warp<NT, NCHP_T, 1, HFS>(P, smem);
 }
 
 #define LOC_ONE_WARP_MAXNT 6  // one-warp CTAs are compiled up to this many transitions (the round keeps them all in registers)
 
-template <int NT, int NCHP_T, bool ONE>
+template <int NT, int NCHP_T, bool ONE, bool HFS = false>
 static int launch3d_t(loc_model *m, Sim3D &P, size_t smem)
 {
-    auto kern = k_sim3d<NT, NCHP_T, ONE>;
+    auto kern = k_sim3d<NT, NCHP_T, ONE, HFS>;
     const int nthr = ONE ? 32 : 64;
     LOC_CUDA_CHECK(m, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int bps = 0;
@@ -887,6 +889,7 @@ static int launch3d(loc_model *m, Sim3D &P)
         snprintf(m->err, sizeof(m->err), "nchannel * ntrans too large for the shared-memory spectra (%zu bytes per warp)", smem);
         return LOC_EINVAL;
     }
+    if (P.H.any) return launch3d_t<NT, 0, false, true>(m, P, smem);  // hyperfine structure: every step takes the masked round
     // one warp per ray set for few transitions (loc_set_option(LOC_OPT_SIM3D_WARPS): 0 = automatic: up to 4 transitions)
     if constexpr (NT <= LOC_ONE_WARP_MAXNT) {
         if (m->sim3d_warps == 1 || (m->sim3d_warps == 0 && NT <= 4)) {

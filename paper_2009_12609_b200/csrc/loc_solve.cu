@@ -347,17 +347,30 @@ __global__ void __launch_bounds__(LOC_SOLVE_F_THREADS) k_solve_f(int64_t n, cons
         __syncthreads();
     }
     const int64_t i = blockIdx.x * (int64_t)TH + tid;
-    bool act = i < n;
-    if (act && child && child[i] >= 0) act = false;  // refined cell: no gas of its own
+    const bool inr = i < n;
+    // every global load of the cell is issued here, before anything depends on one (profiles/r2_solve.md: with the loads
+    // behind the leaf test and the old populations read at the end, 7.5 issue slots per instruction waited on the long
+    // scoreboard): leaf flag, counter record, density / temperature / abundance, old populations
+    const int64_t ic = inr ? i : 0;
+    const int32_t chd = child ? __ldg(child + ic) : -1;
+    const float4 *rec = reinterpret_cast<const float4 *>(cnt + ic * Q.nsp);
+    float4 recv[LOC_MAX_TRANS / 2];
+#pragma unroll
+    for (int h = 0; h < LOC_MAX_TRANS / 2; h++)
+        if (2 * h < Q.nsp) recv[h] = __ldg(rec + h);  // (SJ, ESC) of slots 2h, 2h + 1
+    const float dens = __ldg(density + ic), T = __ldg(tkin + ic), abun = __ldg(abundance + ic);
+    float oldp[NL];
+#pragma unroll
+    for (int l = 0; l < NL; l++) oldp[l] = pops[(int64_t)l * n + ic];
+    const bool act = inr && chd < 0;  // refined cell: no gas of its own
     float rel = 0.0f;
     if (act) {
-        // ---- the cell's counter record -> its scratch column (two slots per 128-bit load) ----
-        const float4 *rec = reinterpret_cast<const float4 *>(cnt + i * Q.nsp);
+        // ---- the cell's counter record -> its scratch column ----
         const float4 *crec = reinterpret_cast<const float4 *>(coef + i * Q.nsp);
 #pragma unroll
         for (int h = 0; h < LOC_MAX_TRANS / 2; h++) {
             if (2 * h < Q.nsp) {
-                float4 v = __ldg(rec + h);  // (SJ, ESC) of slots 2h, 2h + 1
+                float4 v = recv[h];
                 if (!ali) {  // plain lambda iteration: see k_solve
                     const float4 ke = crec[h];
                     if (ke.x != 0.0f) v.x += (1.0f - v.y) * (ke.y / ke.x);
@@ -371,8 +384,7 @@ __global__ void __launch_bounds__(LOC_SOLVE_F_THREADS) k_solve_f(int64_t n, cons
                 col[(4 * h + 3) * TH] = v.w;
             }
         }
-        const float dens = density[i], T = tkin[i];
-        const float ntot = dens * abundance[i];
+        const float ntot = dens * abun;
         // collisions: linear interpolation in T, clamped
         int j = 0;
         float f = 0.0f;
@@ -445,7 +457,7 @@ __global__ void __launch_bounds__(LOC_SOLVE_F_THREADS) k_solve_f(int64_t n, cons
 #pragma unroll
         for (int l = 0; l < NL; l++) {
             const float nw = x[l] * sc;
-            const float old = pops[(int64_t)l * n + i];
+            const float old = oldp[l];
             if (ntot > 0.0f && (nw >= 1e-10f * ntot || old >= 1e-10f * ntot)) rel = fmaxf(rel, fabsf(nw - old) / fmaxf(nw, 1e-37f));
             if (!isfinite(nw)) rel = INFINITY;  // see k_solve
             pops[(int64_t)l * n + i] = nw;
