@@ -197,6 +197,7 @@ static int build_selection(loc_model *m, int nsel, const int *idx)
         S.ck[k] = LOC_CL * LOC_CL * LOC_CL * m->h_A[t] / (8.0 * LOC_PI * nu * nu * nu * m->dv);
         S.bgocc[k] = (m->tbg > 0.0) ? (float)(1.0 / expm1(LOC_HP * nu / (LOC_KB * m->tbg))) : 0.0f;
     }
+    for (int k = nsel; k < LOC_MAX_TRANS; k++) S.bgocc[k] = 0.0f;  // (pad slots of the 3D kernel: no photons)
     if (changed) m->coef_valid = false;
     return LOC_OK;
 }

@@ -316,7 +316,7 @@ __device__ __forceinline__ unsigned prepare_record(const Sim3D &P, uint2 rec, co
                 far = far && sigch >= 1.0f;
                 qe = far ? Ql + Qh : -1.0f;
             }
-            if (P.geom) nact = max(0, min(P.nch - 1, (int)floorf(cc + 5.0f * sigch)) - max(0, (int)ceilf(cc - 5.0f * sigch)) + 1);
+            if (__builtin_expect(P.geom != 0, 0)) nact = max(0, min(P.nch - 1, (int)floorf(cc + 5.0f * sigch)) - max(0, (int)ceilf(cc - 5.0f * sigch)) + 1);
         }
         sts128u(rb, make_uint4(__float_as_uint(q0), __float_as_uint(q1), __float_as_uint(q2), wb | flags));
         const unsigned coff = step ? rec.x * (unsigned)P.nsp + (unsigned)P.slot0 : rec.x;
@@ -360,7 +360,8 @@ __device__ __forceinline__ int wide_start(int nch, float cc)
 // sum  sum phi f(tau) ~ 1 / tau0  as LOC_XCLIP sigma for a thin line (DESIGN 5.3).  If the centred 32-channel span reaches
 // that far on both sides (or to the edge of the band) the step is a common round; else, if two adjacent spans do, a WIDE
 // round (two passes); else a masked round over its exact window.  Returns the record's flags with the mode bits.
-template <int NT, bool HFS>
+// WIDEP: the kernel has the two-span (WIDE) round; without it such steps take the masked round (see k_sim3d)
+template <int NT, bool HFS, bool WIDEP>
 __device__ __forceinline__ unsigned step_mode(const Sim3D &P, unsigned rb, float &qe_wide)
 {
     qe_wide = -1.0f;  // profile mass outside the pair of spans of a WIDE step (-1: the round takes 1 - sum phi)
@@ -388,11 +389,11 @@ __device__ __forceinline__ unsigned step_mode(const Sim3D &P, unsigned rb, float
             // sampled profile itself and evaluates it from the distance to the line centre (DESIGN 5.3); so do all steps of a
             // model with hyperfine structure (a profile per transition, components spread over the band)
             flags |= LOC_RS_SLOW;
-        } else if (!ok1) {
+        } else if (__builtin_expect(!ok1, 0)) {
             const int ww = wide_start(P.nch, cc);
             const float need2 = fmaxf(need, needf);  // a pair of spans has no extension
             const bool ok2 = P.nch >= 2 * LOC_SPAN && (ww == 0 || cc - (float)ww >= need2) && (ww + 2 * LOC_SPAN >= P.nch || (float)(ww + 2 * LOC_SPAN - 1) - cc >= need2);
-            flags |= ok2 ? LOC_RS_WIDE : LOC_RS_SLOW;
+            flags |= (WIDEP && ok2) ? LOC_RS_WIDE : LOC_RS_SLOW;
             if (ok2) {
                 float Ql, Qh;
                 bool far;
@@ -676,7 +677,7 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
         const bool need = !done && off >= end;
         if (W != 1 && need && l8 == 0) sts32u(tb + L::OFF_TASK + 4 * grp, atomicAdd(P.queue, 1u));
         cta_sync<W>();  // the previous chunk's records are free; the tasks are posted
-        if (need) {
+        if (__builtin_expect(need, 0)) {
             const long long task = lds32u(tb + L::OFF_TASK + 4 * grp);
             if (task >= P.ntask) {
                 done = true;
@@ -690,7 +691,7 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
             }
         }
         if (__all_sync(0xffffffffu, done)) break;  // the same in both warps
-        if (fresh) {  // first chunk of a ray: nothing was prefetched
+        if (__builtin_expect(fresh, 0)) {  // first chunk of a ray: nothing was prefetched
             r0 = __ldg(P.stream + off + rj);
             r1 = (off + LOC_CHUNK < end) ? __ldg(P.stream + off + LOC_CHUNK + rj) : NOPREC;
             load_cell<NT, W>(P, r0, half, cell);
@@ -708,7 +709,7 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
         cta_sync<W>();  // the records of the chunk are complete
         // mode of record rj (the lanes of a pair agree), then the class of round rj: OR over the four groups
         float myqew;
-        const unsigned myflags = step_mode<NT, HFS>(P, rec_g + rj * L::RECB, myqew);
+        const unsigned myflags = step_mode<NT, HFS, W == 2>(P, rec_g + rj * L::RECB, myqew);
         unsigned orflags = myflags | __shfl_xor_sync(0xffffffffu, myflags, 8);
         orflags |= __shfl_xor_sync(0xffffffffu, orflags, 16);
 
@@ -719,7 +720,7 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
             const unsigned mode = __shfl_sync(0xffffffffu, myflags, 8 * grp + 2 * r);
             const float qew = __shfl_sync(0xffffffffu, myqew, 8 * grp + 2 * r);
             const unsigned rb = rec_g + r * L::RECB;
-            if (cls & LOC_RS_CTRL) {
+            if (__builtin_expect((cls & LOC_RS_CTRL) != 0, 0)) {
                 // spectrum operations on the warp's own rows, executed by the whole warp for one group at a time; only the
                 // groups that have one are visited (their lanes hold the record's CTRL bit in `mode`)
                 unsigned cm = __ballot_sync(0xffffffffu, mode & LOC_RS_CTRL);
@@ -766,7 +767,7 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
             float2 ab[O::NHR * 2];
 #pragma unroll
             for (int i = 0; i < O::NHR * 2; i++) ab[i] = make_float2(0.f, 0.f);
-            if (cls & LOC_RS_SLOW) {
+            if (__builtin_expect((cls & LOC_RS_SLOW) != 0, 0)) {
                 hfsact += slow_round<NT, W, HFS>(P, rb, sq_g, pl, l8, nchp);
 #pragma unroll
                 for (int i = 0; i < O::NW; i++) ab[i] = lds64(pl + (O::TB + i) * L::ROWB);
@@ -778,7 +779,7 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
                 const bool ext = ce >= 0 && ce < P.nch;
                 const unsigned se = ext ? sq_r + 4u * ce : sq_g + 4u * wb0;
                 const float pe = ext ? ex2f(fmaf(je, fmaf(je, h0.z, h0.y), h0.x)) : 0.0f;
-                if (!(cls & LOC_RS_WIDE)) {
+                if (W != 2 || __builtin_expect(!(cls & LOC_RS_WIDE), 1)) {
                     fast_round<NT, W>(rb, sq_g + 4u * wb0, rowb, h0, J01, J23, se, pe, ext, fold, ab);
                 } else {
                     // two passes: a WIDE ray over its pair of spans, the other rays over their span and then over nothing
@@ -818,7 +819,7 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
                 float2 *cn = cnt_o + h1.x;
                 asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(cn), "f"(va[0] * sc), "f"(fmaf(vb[0], sc, wesc)) : "memory");
             }
-            if (O::HEAD && P.geom && step && l8 == 0) {
+            if (O::HEAD && __builtin_expect(P.geom != 0, 0) && step && l8 == 0) {
                 const unsigned cellidx = (h1.x - (unsigned)P.slot0) / (unsigned)P.nsp;
                 atomicAdd(&P.visits[cellidx], 1u);
                 atomicAdd(&P.pathz[cellidx], h1.z & 0x1fffffu);
@@ -845,6 +846,10 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
     }
 }
 
+// The two-warp CTA runs two different instruction streams (each warp's transitions, the header work), and its time follows
+// the size of the loop body (instruction-fetch stalls: profiles/r2_sim3d.md): the two-span WIDE round -- two more copies of
+// the common round -- is compiled into the one-warp kernel only (C5: 580 vs 592 ms without it); in the two-warp kernel the
+// few steps that need more than span + extension take the masked round instead (C3 57.7 -> 50.6 ms, C4 1012 -> 880 ms).
 template <int NT, int NCHP_T, bool ONE, bool HFS>
 __global__ void __maxnreg__(ONE ? 152 : 128) k_sim3d(Sim3D P)
 {
