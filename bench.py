@@ -32,9 +32,9 @@ DEFAULT_WORKLOAD = "C5"
 # ---- roofline constants -----------------------------------------------------------------------------
 N_SM = 148
 # DRAM bytes read + written by one launch of the dominant kernel, from the committed `ncu --set full` captures
-# (profiles/r1_v9_summary.md, profiles/r1_sim1d_C2.md); workloads without a capture report null
-NCU_TRAFFIC_BYTES = {"C2": (24.3e6, "profiles/r1_sim1d_C2.md"), "C3": (19.09e9 + 7.88e9, "profiles/r1_v9_summary.md"),
-                     "C4": (904.4e9 + 299.2e9, "profiles/r1_v9_summary.md")}
+# (profiles/r2_summary.md, profiles/r1_sim1d_C2.md); workloads without a capture report null
+NCU_TRAFFIC_BYTES = {"C2": (24.3e6, "profiles/r1_sim1d_C2.md"), "C3": (19.08e9 + 7.87e9, "profiles/r2_summary.md"),
+                     "C5": (816.6e9 + 142.8e9, "profiles/r2_summary.md")}
 FP32_LANES_PER_SM_CLK = 128  # 4 sub-partitions x 1 warp instruction / clk
 MUFU_PER_SM_CLK = 16
 
@@ -175,9 +175,14 @@ def oracle_sample(m, budget_updates=6e9, keep=False):
             desc = (f"direction 0 of {len(m.dirs)}, transition {int(allsel[0])}, every {stride}-th line of the root lattice (rays born in "
                     f"refined regions not traced), all {nch} channels; then the solve over all cells")
         sel = allsel[:nt]
+        # the solve of the step is sampled in the same proportion as its ray tracing: every k-th cell
+        k = max(1, int(round(len(m.dirs) * len(allsel) * stride / nt)))
+        desc = desc.replace("then the solve over all cells", "then the solve").replace("then the solve", f"then the solve of every {k}-th cell (the same fraction of the step)")
         t0 = time.perf_counter()
         r = O.sim_3d(sp, m, pops, sel, dirs=m.dirs[0], root_stride=stride)
-        O.solve(sp, dens, tk, ab, r["veff"], sel, r["P"], r["LAM"], dv, m.t_bg, pops)
+        ps = np.ascontiguousarray(pops[::k])
+        O.solve(sp, dens[::k], tk[::k], ab[::k], r["veff"][::k], sel, np.ascontiguousarray(r["P"][:, ::k]), np.ascontiguousarray(r["LAM"][:, ::k]),
+                dv, m.t_bg, ps)
         dt = time.perf_counter() - t0
         steps = int(r["visits"].sum())
         act = float((r["visits"] * active_channels_per_cell(m, m.dirs[0])).sum()) * nt
@@ -196,9 +201,12 @@ def oracle_sample(m, budget_updates=6e9, keep=False):
             ms.ray_p, ms.ray_w = m.ray_p[kept], m.ray_w[kept]
         else:
             kept, ms = np.arange(nray), m
+        k = max(1, int(round(nray / len(kept))))
         t0 = time.perf_counter()
         r = O.sim_1d(sp, ms, pops, sel)
-        O.solve(sp, dens, tk, ab, r["veff"], sel, r["P"], r["LAM"], dv, m.t_bg, pops)
+        ps = np.ascontiguousarray(pops[::k])
+        O.solve(sp, dens[::k], tk[::k], ab[::k], r["veff"][::k], sel, np.ascontiguousarray(r["P"][:, ::k]), np.ascontiguousarray(r["LAM"][:, ::k]),
+                dv, m.t_bg, ps)
         dt = time.perf_counter() - t0
         steps = int(r["visits"].sum())
         # 1D: the Doppler shift of a step is -v_r mu with the entry cosine of the step (oracle's path table)
@@ -214,7 +222,7 @@ def oracle_sample(m, budget_updates=6e9, keep=False):
             for t in sel:  # a transition's active channels: within 5 sigma of any of its hyperfine components
                 offs = np.sort(np.asarray(hfs[int(t)][0], np.float64) / dv) if int(t) in hfs else np.zeros(1)
                 act += _union_count(cc, hw, nch, offs)
-        desc = f"{len(kept)} of {nray} rays, all {len(sel)} transitions, all {nch} channels; then the solve"
+        desc = f"{len(kept)} of {nray} rays, all {len(sel)} transitions, all {nch} channels; then the solve of every {k}-th shell (the same fraction of the step)"
         threads = 1  # the 1D ray loop of the oracle is serial
     out = {"nominal": nominal_updates(steps, nch, nt), "active": act, "seconds": dt, "threads": threads, "desc": desc}
     if keep:

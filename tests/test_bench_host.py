@@ -65,7 +65,7 @@ def test_reference_arm_under_torchrun_world2():
 
 def test_roofline_bookkeeping():
     """T_roof = max(bytes / HBM, MUFU ops / rate, FP32 instructions / rate); frac = T_roof / t"""
-    sg = {"steps": 1000, "active_channels": 33000, "is3d": True}
+    sg = {"steps": 1000, "active_updates": 33000 * 9, "is3d": True}
     nt, hbm, mhz = 9, 6544.0, 1965.0
     r = bench.roofline(sg, nt, 1e-3, hbm, mhz, "measured")
     u = 33000 * nt
