@@ -288,3 +288,32 @@ def test_set_directions_invalid_arguments_keep_the_old_directions():
     g.simulate()  # an invalid ARGUMENT leaves the old directions in place
     assert lib.loc_set_directions(g.h, 13, many.ctypes.data_as(C.c_void_p)) == B.LOC_EINVAL  # more than ndir_max
     g.close()
+
+
+@pytest.mark.parametrize("case", ["octree", "C3", "1d"])
+def test_counters_reproducible_run_to_run(case):
+    """compute-sanitizer is closed on the GPU pool (profiles/r2_sanitizer.md), so a race between the lanes / warps that share a
+    ray's spectra in shared memory is looked for by its symptom: two simulations from the same populations must give the same
+    counters up to the order of the float32 atomic additions (observed ~1e-6; a lost or doubled update of a spectrum is
+    orders of magnitude above that), and identical integer visit counts.  Thick octree with births, full-size C3, and 1D."""
+    if case == "octree":
+        m = small(which=4, nroot=6, nlev=3, nside=2, nch=128, frac=0.45, nls=10, seed=13, dens=20.0)
+    elif case == "C3":
+        m = W.cloud_config(3)
+    else:
+        m = W.shell_config(2, ns=400, nchannel=256, nsub=2)
+    g = _model(m)
+    g.init_lte()
+    g.iterate(2)  # populations away from LTE
+    out = []
+    for _ in range(3):
+        g.simulate(geometry_counters=True)
+        sj, esc = g.counters()
+        vis, _ = g.geometry_counters()
+        out.append((sj.cpu().numpy().astype(np.float64), esc.cpu().numpy().astype(np.float64), vis.cpu().numpy().copy()))
+    g.close()
+    leaf = _leaf(m)
+    for k in (1, 2):
+        assert np.array_equal(out[k][2], out[0][2])
+        assert rel_err(out[k][0][leaf], out[0][0][leaf]).max() < 2e-5
+        assert np.max(np.abs(out[k][1][leaf] - out[0][1][leaf])) < 2e-5
