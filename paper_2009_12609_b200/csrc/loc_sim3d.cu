@@ -851,7 +851,7 @@ __device__ __forceinline__ void run_warp(const Sim3D &P, float *smem)
 // the common round -- is compiled into the one-warp kernel only (C5: 580 vs 592 ms without it); in the two-warp kernel the
 // few steps that need more than span + extension take the masked round instead (C3 57.7 -> 50.6 ms, C4 1012 -> 880 ms).
 template <int NT, int NCHP_T, bool ONE, bool HFS>
-__global__ void __maxnreg__(ONE ? 152 : 128) k_sim3d(Sim3D P)
+__global__ void __maxnreg__(128) k_sim3d(Sim3D P)
 {
     extern __shared__ __align__(16) float smem[];  // [4][NT][nchp] spectra, then the tables of Lay<NT>
     if (ONE)
