@@ -49,6 +49,7 @@ def lib():
         _lib.orc_planck.argtypes = [C.c_double, C.c_double]
         _lib.orc_freq.restype = C.c_double
         _lib.orc_solve.restype = C.c_double
+        _lib.orc_solve_sub.restype = C.c_double
         _lib.orc_tex.restype = C.c_double
     return _lib
 
@@ -158,6 +159,17 @@ def solve(sp: OSpecies, density, tkin, abundance, veff, sel, P, LAM, dv, tbg, po
     assert pops.dtype == np.float64 and pops.flags.c_contiguous
     return lib().orc_solve(sp.ref(), C.c_int64(n), _p(d), _p(t), _p(a), _p(v), C.c_int(len(sel)), _p(sel), _p(P), _p(LAM),
                            C.c_double(dv), C.c_double(tbg), C.c_int(int(ali)), _p(pops))
+
+
+def solve_sub(sp: OSpecies, density, tkin, abundance, veff, sel, P, LAM, dv, tbg, pops, nsub):
+    """O9 with nsub sub-iterations between two ray passes (R26); nsub = 1 is solve()."""
+    n = len(density)
+    d, t, a, v = _f64(density), _f64(tkin), _f64(abundance), _f64(veff)
+    sel = np.ascontiguousarray(sel, np.int32)
+    P, LAM = _f64(P), _f64(LAM)
+    assert pops.dtype == np.float64 and pops.flags.c_contiguous
+    return lib().orc_solve_sub(sp.ref(), C.c_int64(n), _p(d), _p(t), _p(a), _p(v), C.c_int(len(sel)), _p(sel), _p(P), _p(LAM),
+                               C.c_double(dv), C.c_double(tbg), C.c_int(int(nsub)), _p(pops))
 
 
 def tex(sp: OSpecies, t, n_u, n_l):
@@ -296,8 +308,9 @@ def profile_t(sp: OSpecies, t, nch, dv, sigma, v0):
     return phi
 
 
-def iterate(sp: OSpecies, m, niter, sel=None, ali=True, pops=None, history=False):
-    """O10: niter x (simulate all selected transitions from the old populations; solve) from LTE (O3)."""
+def iterate(sp: OSpecies, m, niter, sel=None, ali=True, pops=None, history=False, nsub=1):
+    """O10: niter x (simulate all selected transitions from the old populations; solve) from LTE (O3).
+    nsub > 1: sub-iterations of the solve between the ray passes (solve_sub; ALI only)."""
     is3d = hasattr(m, "child")
     dens, tk, ab = _f64(m.density), _f64(m.tkin), _f64(m.abundance)
     if pops is None:
@@ -308,5 +321,9 @@ def iterate(sp: OSpecies, m, niter, sel=None, ali=True, pops=None, history=False
     for _ in range(niter):
         r = sim_3d(sp, m, pops, sel_arr, ali) if is3d else sim_1d(sp, m, pops, sel_arr, ali)
         last = r
-        changes.append(solve(sp, dens, tk, ab, r["veff"], sel_arr, r["P"], r["LAM"], dv, m.t_bg, pops, ali))
+        if nsub > 1:
+            assert ali
+            changes.append(solve_sub(sp, dens, tk, ab, r["veff"], sel_arr, r["P"], r["LAM"], dv, m.t_bg, pops, nsub))
+        else:
+            changes.append(solve(sp, dens, tk, ab, r["veff"], sel_arr, r["P"], r["LAM"], dv, m.t_bg, pops, ali))
     return (pops, changes, last) if history else (pops, changes[-1] if changes else 0.0)

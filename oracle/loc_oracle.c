@@ -26,6 +26,7 @@
  * layered model with partial refinement (every level's leaves == the uniform
  * Cartesian grid of that resolution), the thick closed form of orc_spectra_1d,
  * 90-degree rotation / z-mirror of the direction set in 3D.
+ * Hyperfine structure (profile_t): tests/test_oracle_pins_hfs.py; sub-iterations (orc_solve_sub): tests/test_oracle_subiter.py.
  * Parity unpinned: none of the functions below.  One READING stays constrained
  * by invariants only (blackbody enclosure P4, ledger P6): at a SIDE-face birth
  * the donor is the line that entered the level-(tag-1) ancestor through its
@@ -248,6 +249,86 @@ double orc_solve(const orc_species *sp, int64_t ncell, const double *density, co
         }
         build_rates(sp, density[c], tkin[c], S, beta, R);
         solve_ge(NL, R, ntot, x);
+        for (int i = 0; i < NL; i++) {
+            double old = pops[c * NL + i];
+            if (x[i] / ntot >= 1e-10 || old / ntot >= 1e-10) {
+                double rel = fabs(x[i] - old) / fmax(fabs(x[i]), 1e-300);
+                if (rel > maxrel) maxrel = rel;
+            }
+            pops[c * NL + i] = x[i];
+        }
+    }
+    free(slot);
+    return maxrel;
+}
+
+/* Sub-iterations of the solve between two ray passes ("some form of sub-iterations, where level
+ * populations are updated more frequently in optically thick regions" -- the paper gives no formula: DESIGN.md R26).
+ * The ray pass measured, per cell and traced transition, the escape probability beta0 = 1 - LAM and the external field P with
+ * the OLD populations.  A one-zone model of the cell carries both to other populations: tau_eff is defined by
+ * E(tau_eff) = beta0, E(tau) = (1 - e^-tau)/tau; new populations change the line opacity by r = k_new / k_old
+ * (k = n_l g_u/g_l - n_u), and then beta = E(tau_eff r), P = P0 beta / beta0 (the external photons meet the same escape
+ * probability on their way in).  Sub-iteration 1 is the plain ALI solve (r = 1); each further one re-solves with (beta, P) of
+ * the previous solution.  At the ALI fixed point r = 1, so the fixed point is unchanged.  nsub = 1 == orc_solve.         */
+static double e_of_tau(double t) { return (fabs(t) < 1e-6) ? 1.0 - t / 2.0 + t * t / 6.0 : -expm1(-t) / t; }
+static double inv_e(double beta) /* tau >= 0 with E(tau) = beta, by bisection (E is decreasing) */
+{
+    if (!(beta < 1.0)) return 0.0;
+    if (!(beta > 0.0)) return 1e300;
+    double lo = 0.0, hi = 2.0 / beta + 1.0;
+    for (int i = 0; i < 200; i++) {
+        double mid = 0.5 * (lo + hi);
+        if (e_of_tau(mid) > beta) lo = mid; else hi = mid;
+    }
+    return 0.5 * (lo + hi);
+}
+double orc_solve_sub(const orc_species *sp, int64_t ncell, const double *density, const double *tkin,
+                     const double *abundance, const double *veff, int nsel, const int *sel, const double *P,
+                     const double *LAM, double dv, double tbg, int nsub, double *pops /* in/out [ncell][NL] */)
+{
+    int NL = sp->nlevel, NT = sp->ntrans;
+    double maxrel = 0.0;
+    int *slot = (int *)malloc(sizeof(int) * NT);
+    for (int t = 0; t < NT; t++) slot[t] = -1;
+    for (int k = 0; k < nsel; k++) slot[sel[k]] = k;
+#pragma omp parallel for reduction(max : maxrel) schedule(static)
+    for (int64_t c = 0; c < ncell; c++) {
+        double S0[64], S[64], beta0[64], beta[64], teff[64], k0[64], R[32 * 32], x[32];
+        double ntot = density[c] * abundance[c];
+        if (ntot <= 0.0) {
+            for (int i = 0; i < NL; i++) pops[c * NL + i] = 0.0;
+            continue;
+        }
+        for (int t = 0; t < NT; t++) {
+            int u = sp->upper[t], l = sp->lower[t];
+            double nu = orc_freq(sp, t);
+            double gr = sp->g[u] / sp->g[l];
+            k0[t] = pops[c * NL + l] * gr - pops[c * NL + u];
+            if (slot[t] >= 0) {
+                double coef = gr * ORC_C * ORC_C * ORC_C * sp->A[t] / (8.0 * ORC_PI * nu * nu * nu * dv);
+                S0[t] = coef * P[(size_t)slot[t] * ncell + c] / veff[c];
+                beta0[t] = 1.0 - LAM[(size_t)slot[t] * ncell + c];
+                teff[t] = inv_e(beta0[t]);
+            } else {
+                S0[t] = (tbg > 0.0) ? gr * sp->A[t] / expm1(ORC_H * nu / (ORC_K * tbg)) : 0.0;
+                beta0[t] = 1.0;
+                teff[t] = 0.0;
+            }
+            S[t] = S0[t];
+            beta[t] = beta0[t];
+        }
+        for (int it = 0; it < nsub; it++) {
+            build_rates(sp, density[c], tkin[c], S, beta, R);
+            solve_ge(NL, R, ntot, x);
+            for (int t = 0; t < NT; t++) {
+                if (slot[t] < 0 || !(beta0[t] > 0.0) || k0[t] == 0.0) continue;
+                int u = sp->upper[t], l = sp->lower[t];
+                double r = (x[l] * sp->g[u] / sp->g[l] - x[u]) / k0[t];
+                if (!(r > 0.0)) r = 1.0; /* inverted or vanishing line: keep the measured values */
+                beta[t] = e_of_tau(teff[t] * r);
+                S[t] = S0[t] * beta[t] / beta0[t];
+            }
+        }
         for (int i = 0; i < NL; i++) {
             double old = pops[c * NL + i];
             if (x[i] / ntot >= 1e-10 || old / ntot >= 1e-10) {
