@@ -34,7 +34,7 @@ N_SM = 148
 # DRAM bytes read + written by one launch of the dominant kernel, from the committed `ncu --set full` captures
 # (profiles/r2_summary.md, profiles/r1_sim1d_C2.md); workloads without a capture report null
 NCU_TRAFFIC_BYTES = {"C2": (24.3e6, "profiles/r1_sim1d_C2.md"), "C3": (19.08e9 + 7.87e9, "profiles/r2_summary.md"),
-                     "C5": (816.6e9 + 142.8e9, "profiles/r2_summary.md")}
+                     "C4": (904.1e9 + 298.6e9, "profiles/r2_summary.md"), "C5": (816.6e9 + 142.8e9, "profiles/r2_summary.md")}
 FP32_LANES_PER_SM_CLK = 128  # 4 sub-partitions x 1 warp instruction / clk
 MUFU_PER_SM_CLK = 16
 
