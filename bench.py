@@ -434,26 +434,39 @@ def run_own(args):
     d2h = host_out.numel() * 4
     from paper_2009_12609_b200 import binding as B
 
+    # the caller's side of the public API, pipelined as a user would: the device-to-host read of step k's result runs on a
+    # second stream (its own copy engine) while step k + 1's inputs come in; every step still copies all its inputs from
+    # pinned host memory and its result back, and the timed region ends only when the last result has arrived
+    side = torch.cuda.Stream(device=local)
+    out_dev = torch.empty_like(g.pops)
+
     def e2e_step():
         g.update_cells(**host)
         g.pops.copy_(host_pops, non_blocking=True)
         B.loc_set_populations(g.h, g.pops)
         g.iterate(1)
-        host_out.copy_(g.pops, non_blocking=True)
-        torch.cuda.current_stream().synchronize()
+        torch.cuda.current_stream().wait_stream(side)  # (the previous result has left out_dev)
+        out_dev.copy_(g.pops, non_blocking=True)
+        done = torch.cuda.Event()
+        done.record()
+        side.wait_event(done)
+        with torch.cuda.stream(side):
+            host_out.copy_(out_dev, non_blocking=True)
 
     e2e_step()
+    torch.cuda.current_stream().wait_stream(side)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     n_e2e = max(1, min(args.steps, 5))
     barrier()
     e0.record()
     for _ in range(n_e2e):
         e2e_step()
+    torch.cuda.current_stream().wait_stream(side)  # the last result is on the host before the clock stops
     e1.record()
     barrier()
     (t_e2e,) = max_over_ranks([e0.elapsed_time(e1) * 1e-3], device=f"cuda:{local}")
     e2e_val = whole_job_value(u_act, n_e2e, world, t_e2e)
-    del host, host_pops, host_out  # 24 GB of pinned memory at C5: returned before the oracle runs
+    del host, host_pops, host_out, out_dev  # 24 GB of pinned memory at C5: returned before the oracle runs
 
     # ---- S10: spectral cube of the first traced line along +z, one pixel per finest cell (C5: 1024 x 1024 x
     #      256 channels), and its line-area map; after the iterations above, timed apart from `value` ----
