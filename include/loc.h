@@ -256,6 +256,56 @@ int loc_tex(loc_model *m, int trans, float *dev_tex);
  * float [npix].  Enqueued on the model's stream; npix = 0 is a no-op.                                          */
 int loc_line_area(loc_model *m, const float *dev_cube, int64_t npix, float *dev_w);
 
+/* Spectra of a shell model for callers that cannot allocate device memory.
+ *
+ * Everything else in this header needs a loc_model, and a loc_model needs a workspace that somebody obtained from
+ * cudaMalloc (or a pool built on it).  Some code that wants a spectrum is not in a position to do that: a plug-in or
+ * callback that is handed its input and output buffers by a host application which owns every byte of device memory; a
+ * monitoring or display step that runs next to a solver whose workspace already fills the GPU; code on a latency-critical
+ * path where the implicit device-wide synchronisation of cudaMalloc / cudaFree is not acceptable.  For those callers this
+ * one call computes what loc_spectra computes for a LOC_GRID_SHELL model (PAPER.md:77 line-of-sight integration,
+ * PAPER.md:137 Doppler shift from the direction cosine at the entry of each step; same kernel, k_spectra1d) from plain
+ * arrays, without a model and without a workspace.  The scratch the kernel needs -- a device copy of the shell radii and
+ * the packed (radial velocity, total line width) record per shell -- lives in a fixed array inside the library image of
+ * 24 * LOC_STATIC_MAX_SHELLS bytes (96 KiB), which every GPU that loads the library holds until the process exits.
+ * The call itself allocates nothing: no cudaMalloc / cudaFree, no allocating library routine.
+ *
+ *   nshell            1 .. LOC_STATIC_MAX_SHELLS; more shells -> LOC_EINVAL with a message that names the limit (use a
+ *                     loc_model with a workspace for larger models)
+ *   r_out             host [nshell], strictly ascending, cm (as in loc_grid); copied during the call
+ *   dev_vrad, dev_sigma, dev_tkin
+ *                     DEVICE float [nshell]: radial velocity (cm/s, positive outward), turbulent 1-D velocity dispersion
+ *                     (cm/s) and kinetic temperature (K), as in loc_cells; the thermal width k T / m is added for
+ *                     mass_amu > 0 (mass_amu = 0: dev_sigma is the total width, DESIGN R3)
+ *   dev_pop_u, dev_pop_l
+ *                     DEVICE float [nshell]: populations (cm^-3) of the upper and lower level of the line
+ *   freq_hz, einstein_A, g_upper, g_lower
+ *                     the line: rest frequency (Hz), Einstein A (1/s), statistical weights.  No hyperfine structure.
+ *   nchannel, band_halfwidth_cm_s, t_background_K
+ *                     as in loc_create_model (1 <= nchannel <= 1024)
+ *   nlos, offsets_cm  host [nlos]: impact parameters of the lines of sight (cm; the sign is ignored; beyond the outer
+ *                     radius the spectrum is zero).  nlos = 0 is a no-op.
+ *   dev_out           DEVICE float [nlos][nchannel]: T_A in K, as loc_spectra writes it
+ *   stream            cudaStream_t as void* (NULL = default stream) of the CURRENT device; all work is enqueued there and
+ *                     the call does not wait for it
+ *   err, err_len      optional host buffer that receives the text of a failure (may be NULL)
+ *
+ * Rules that follow from the shared array:
+ *   - The first call on a device looks up the array's address on that device (cudaGetSymbolAddress, with that device
+ *     current) and remembers it.  Make that first call during start-up, before any stream capture is begun.
+ *   - All calls on a device use the same array.  Calls on one stream are ordered and safe back to back.  Calls whose GPU
+ *     work can overlap (different streams without an event between them, or several host threads each with a stream of
+ *     its own) race on the array and give wrong spectra: serialise them.
+ *   - The array keeps what the last call wrote.  Each call overwrites the entries it reads (the first nshell) before
+ *     reading them, so nothing needs clearing and a smaller model after a larger one is safe.
+ * Returns LOC_OK, LOC_EINVAL (bad argument or size) or LOC_ECUDA.                                                       */
+#define LOC_STATIC_MAX_SHELLS 4096
+int loc_spectra_shells_static(int nshell, const double *r_out, const float *dev_vrad, const float *dev_sigma,
+                              const float *dev_tkin, double mass_amu, const float *dev_pop_u, const float *dev_pop_l,
+                              double freq_hz, double einstein_A, double g_upper, double g_lower, int nchannel,
+                              double band_halfwidth_cm_s, double t_background_K, int nlos, const double *offsets_cm,
+                              float *dev_out, void *stream, char *err, int err_len);
+
 int loc_get_stats(loc_model *m, loc_stats *out);
 void loc_destroy_model(loc_model *m);
 const char *loc_last_error(const loc_model *m); /* m may be NULL: error of the last failed loc_create_model */

@@ -25,7 +25,8 @@ LOC_MAX_HFS = 8
 SYMBOLS = ("loc_workspace_bytes", "loc_create_model", "loc_set_species", "loc_refresh_cells", "loc_set_directions", "loc_set_populations",
            "loc_init_lte", "loc_simulate", "loc_get_counters", "loc_solve", "loc_iterate", "loc_set_ali",
            "loc_set_option", "loc_iterate_until", "loc_spectra", "loc_spectra_map", "loc_line_area", "loc_tex",
-           "loc_get_stats", "loc_destroy_model", "loc_last_error", "loc_set_hyperfine")
+           "loc_get_stats", "loc_destroy_model", "loc_last_error", "loc_set_hyperfine", "loc_spectra_shells_static")
+LOC_STATIC_MAX_SHELLS = 4096
 
 
 class LocError(RuntimeError):
@@ -92,6 +93,9 @@ def lib():
         L.loc_tex.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
         L.loc_line_area.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]
         L.loc_get_stats.argtypes = [C.c_void_p, C.POINTER(loc_stats)]
+        L.loc_spectra_shells_static.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p,
+                                                C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, C.c_double,
+                                                C.c_double, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_char_p, C.c_int]
         L.loc_destroy_model.argtypes = [C.c_void_p]
         L.loc_destroy_model.restype = None
         L.loc_last_error.argtypes = [C.c_void_p]
@@ -249,6 +253,24 @@ def loc_set_option(h, key: int, value: float) -> None:
 def loc_spectra_map(h, trans, dev_out, nx, ny, dir, pixel_cm, centre_cm):
     d, c = _np(dir, np.float64), _np(centre_cm, np.float64)
     _check(lib().loc_spectra_map(h, int(trans), _hp(d), int(nx), int(ny), float(pixel_cm), _hp(c), _dp(dev_out)), h)
+
+
+def loc_spectra_shells_static(r_out, dev_vrad, dev_sigma, dev_tkin, mass_amu, dev_pop_u, dev_pop_l, freq_hz, einstein_A,
+                              g_upper, g_lower, nchannel, band_halfwidth_cm_s, t_background_K, offsets_cm, dev_out,
+                              stream_ptr=0) -> None:
+    """Shell-model spectra for callers that cannot allocate device memory (include/loc.h): no model, no workspace; the
+    kernel's scratch is a fixed array inside the library (at most LOC_STATIC_MAX_SHELLS shells).  This wrapper only
+    marshals: it creates no tensor -- inputs and dev_out are the caller's CUDA tensors, r_out and offsets_cm host arrays.
+    All calls on a device share the scratch array: keep them on one stream (or otherwise serialised), and make the first
+    call on each device during start-up."""
+    r, o = _np(r_out, np.float64), _np(offsets_cm, np.float64)
+    err = C.create_string_buffer(512)
+    rc = lib().loc_spectra_shells_static(len(r), _hp(r), _dp(dev_vrad), _dp(dev_sigma), _dp(dev_tkin), float(mass_amu),
+                                         _dp(dev_pop_u), _dp(dev_pop_l), float(freq_hz), float(einstein_A), float(g_upper),
+                                         float(g_lower), int(nchannel), float(band_halfwidth_cm_s), float(t_background_K),
+                                         len(o), _hp(o), _dp(dev_out), C.c_void_p(stream_ptr), err, len(err))
+    if rc != LOC_OK:
+        raise LocError(rc, err.value.decode())
 
 
 def loc_get_stats(h) -> dict:

@@ -11,9 +11,12 @@
 // of sight starts where it enters the model and ends where it leaves it -- and the lanes then split the channels of the
 // step's profile window (DESIGN R13).  kap and S are formed in double from the float32 populations (n_l g_u/g_l - n_u cancels).
 #include <math.h>
+#include <stdarg.h>
 #include <stdio.h>
+#include <string.h>
 
 #include <algorithm>
+#include <mutex>
 
 #include "loc_internal.cuh"
 
@@ -340,5 +343,128 @@ int loc_launch_line_area(loc_model *m, const float *dev_cube, long long npix, fl
     k_line_area<<<(unsigned)((threads + 255) / 256), 256, 0, m->stream>>>(dev_cube, npix, m->nch, (float)(m->dv * 1e-5), dev_w);
     m->launches++;
     LOC_CUDA_CHECK(m, cudaGetLastError());
+    return LOC_OK;
+}
+
+// ---- shell spectra without a workspace (include/loc.h, loc_spectra_shells_static) -----------------------------------------
+// k_spectra1d reads two pieces of scratch that normally sit in the model's workspace: the device copy of the shell radii
+// and the packed (velocity, total line width) record of every shell.  Here both sit in one array that is part of the
+// library image, so the call needs neither a loc_model nor a byte of memory from the caller beyond inputs and outputs.
+//   bytes [0, 8 MAX)        double r_out[MAX]
+//   bytes [8 MAX, 24 MAX)   float4 kin[MAX]     (v_r, 0, 0, sqrt(sigma^2 + k T / m))
+// Each call writes the first nshell entries of both parts before the kernel reads them and reads nothing beyond, so what an
+// earlier call (possibly with more shells) left behind is never seen and nothing has to be cleared.
+static __device__ __align__(256) unsigned char g_shell_scratch[LOC_STATIC_MAX_SHELLS * (sizeof(double) + sizeof(float4))];
+
+#define LOC_STATIC_MAX_DEVICES 64
+// g_shell_scratch is a host-side handle in host code, not an address a kernel can use; the device address differs per GPU
+// and is looked up once per device, with that device current, on the first call made there.
+static void *g_shell_scratch_addr[LOC_STATIC_MAX_DEVICES];
+static std::mutex g_shell_scratch_mu;
+
+// same arithmetic as k_pack_kin (loc_api.cu), written into the static array, which device code may name directly
+__global__ void k_pack_kin_static(int n, const float *vr, const float *sigma, const float *tkin, double kT_over_m_per_K)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float4 *kin = reinterpret_cast<float4 *>(g_shell_scratch + LOC_STATIC_MAX_SHELLS * sizeof(double));
+    const double s = sigma[i];
+    const double st = sqrt(s * s + kT_over_m_per_K * (double)tkin[i]);  // DESIGN R3
+    kin[i] = make_float4(vr[i], 0.0f, 0.0f, (float)st);
+}
+
+static int static_fail(char *err, int err_len, int code, const char *fmt, ...)
+{
+    if (err && err_len > 0) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(err, (size_t)err_len, fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+extern "C" int loc_spectra_shells_static(int nshell, const double *r_out, const float *dev_vrad, const float *dev_sigma,
+                                         const float *dev_tkin, double mass_amu, const float *dev_pop_u, const float *dev_pop_l,
+                                         double freq_hz, double einstein_A, double g_upper, double g_lower, int nchannel,
+                                         double band_halfwidth_cm_s, double t_background_K, int nlos, const double *offsets_cm,
+                                         float *dev_out, void *stream, char *err, int err_len)
+{
+    if (err && err_len > 0) err[0] = 0;
+    if (nshell > LOC_STATIC_MAX_SHELLS)
+        return static_fail(err, err_len, LOC_EINVAL, "loc_spectra_shells_static: %d shells exceed LOC_STATIC_MAX_SHELLS = %d (the built-in scratch array); use loc_create_model + loc_spectra with a workspace for larger models", nshell, LOC_STATIC_MAX_SHELLS);
+    if (nshell < 1 || nlos < 0) return static_fail(err, err_len, LOC_EINVAL, "loc_spectra_shells_static: nshell must be >= 1 and nlos >= 0");
+    if (nchannel < 1 || nchannel > 1024) return static_fail(err, err_len, LOC_EINVAL, "loc_spectra_shells_static: nchannel must be in [1,1024]");
+    if (!r_out || !dev_vrad || !dev_sigma || !dev_tkin || !dev_pop_u || !dev_pop_l || (nlos > 0 && (!offsets_cm || !dev_out)))
+        return static_fail(err, err_len, LOC_EINVAL, "loc_spectra_shells_static: NULL argument");
+    if (!(band_halfwidth_cm_s > 0.0) || !(t_background_K >= 0.0) || !(freq_hz > 0.0) || !(einstein_A > 0.0) || !(g_upper > 0.0) || !(g_lower > 0.0) || !(mass_amu >= 0.0))
+        return static_fail(err, err_len, LOC_EINVAL, "loc_spectra_shells_static: band, frequency, A and statistical weights must be > 0; T_bg and mass >= 0");
+    double prev = 0.0;
+    for (int k = 0; k < nshell; k++) {
+        if (!(r_out[k] > prev)) return static_fail(err, err_len, LOC_EINVAL, "loc_spectra_shells_static: shell radii must be positive and strictly ascending");
+        prev = r_out[k];
+    }
+    if (nlos == 0) return LOC_OK;
+
+    // once per device: the device address of the scratch array
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return static_fail(err, err_len, LOC_ECUDA, "loc_spectra_shells_static: cudaGetDevice: %s", cudaGetErrorString(e));
+    if (dev < 0 || dev >= LOC_STATIC_MAX_DEVICES) return static_fail(err, err_len, LOC_EINVAL, "loc_spectra_shells_static: device ordinal %d not supported (< %d)", dev, LOC_STATIC_MAX_DEVICES);
+    unsigned char *base;
+    {
+        std::lock_guard<std::mutex> lock(g_shell_scratch_mu);
+        if (!g_shell_scratch_addr[dev]) {
+            void *p = nullptr;
+            e = cudaGetSymbolAddress(&p, g_shell_scratch);
+            if (e != cudaSuccess || !p)
+                return static_fail(err, err_len, LOC_ECUDA, "loc_spectra_shells_static: cudaGetSymbolAddress on device %d: %s", dev, cudaGetErrorString(e));
+            g_shell_scratch_addr[dev] = p;
+        }
+        base = static_cast<unsigned char *>(g_shell_scratch_addr[dev]);
+    }
+    double *d_rout = reinterpret_cast<double *>(base);
+    float4 *d_kin = reinterpret_cast<float4 *>(base + LOC_STATIC_MAX_SHELLS * sizeof(double));
+    cudaStream_t st = (cudaStream_t)stream;
+
+    // stream-ordered behind whatever the previous call on this stream still reads from the array
+    e = cudaMemcpyAsync(d_rout, r_out, sizeof(double) * nshell, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return static_fail(err, err_len, LOC_ECUDA, "loc_spectra_shells_static: cudaMemcpyAsync(r_out): %s", cudaGetErrorString(e));
+    const double ktm = (mass_amu > 0.0) ? LOC_KB / (mass_amu * LOC_AMU) : 0.0;
+    k_pack_kin_static<<<(nshell + 255) / 256, 256, 0, st>>>(nshell, dev_vrad, dev_sigma, dev_tkin, ktm);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return static_fail(err, err_len, LOC_ECUDA, "loc_spectra_shells_static: k_pack_kin_static: %s", cudaGetErrorString(e));
+
+    // the parameter block of k_spectra1d, filled as spec_common() fills it from a loc_model (no hyperfine structure)
+    const double dv = 2.0 * band_halfwidth_cm_s / nchannel;
+    SpecCommon C;
+    memset(&C, 0, sizeof(C));
+    C.nch = nchannel;
+    C.nchp = (nchannel + 3) & ~3;
+    C.dv = (float)dv;
+    C.xmin = 6.0f;
+    C.tk_per_occ = (float)(LOC_HP * freq_hz / LOC_KB);
+    C.bgocc = (t_background_K > 0.0) ? (float)(1.0 / expm1(LOC_HP * freq_hz / (LOC_KB * t_background_K))) : 0.0f;
+    C.ck = LOC_CL * LOC_CL * LOC_CL * einstein_A / (8.0 * LOC_PI * freq_hz * freq_hz * freq_hz * dv);
+    C.gratio = g_upper / g_lower;
+    C.ncell = nshell;
+    C.pop_u = dev_pop_u;
+    C.pop_l = dev_pop_l;
+    C.kin = d_kin;
+    C.nc = 1;
+    C.wgt[0] = 1.0f;
+    const size_t smem = sizeof(float) * LOC_SPEC_WARPS * C.nchp;
+    for (int b0 = 0; b0 < nlos; b0 += LOC_SPEC_BATCH1D) {
+        Spec1D P;
+        P.C = C;
+        P.C.out = dev_out + (int64_t)b0 * nchannel;
+        P.ns = nshell;
+        P.nlos = std::min(nlos - b0, LOC_SPEC_BATCH1D);
+        P.r_out = d_rout;
+        for (int i = 0; i < LOC_SPEC_BATCH1D; i++) P.b[i] = (i < P.nlos) ? offsets_cm[b0 + i] : 0.0;
+        k_spectra1d<<<(P.nlos + LOC_SPEC_WARPS - 1) / LOC_SPEC_WARPS, 32 * LOC_SPEC_WARPS, smem, st>>>(P);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return static_fail(err, err_len, LOC_ECUDA, "loc_spectra_shells_static: k_spectra1d: %s", cudaGetErrorString(e));
+    }
     return LOC_OK;
 }
