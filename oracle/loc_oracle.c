@@ -25,7 +25,9 @@
  * 1D path (mu r_entry = ray abscissa), the donor spectrum at ray births on a
  * layered model with partial refinement (every level's leaves == the uniform
  * Cartesian grid of that resolution), the thick closed form of orc_spectra_1d,
- * 90-degree rotation / z-mirror of the direction set in 3D.
+ * 90-degree rotation / z-mirror of the direction set in 3D; since round 3 the
+ * side entry and side exit of a map's lines of sight (orc_spectra_3d: path
+ * inside the uniform model from the lattice definition by integer search).
  * Hyperfine structure (profile_t): tests/test_oracle_pins_hfs.py; sub-iterations (orc_solve_sub): tests/test_oracle_subiter.py.
  * Parity unpinned: none of the functions below.  One READING stays constrained
  * by invariants only (blackbody enclosure P4, ledger P6): at a SIDE-face birth

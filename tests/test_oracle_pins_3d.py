@@ -246,6 +246,93 @@ def test_spectra_3d_uniform_slab_closed_form():
     assert np.all(TA == 0.0)
 
 
+def _first_zeta_with_shift_at_least(T, D):
+    """smallest zeta >= 0 with floor(zeta 2^32 / T) >= D, found by SEARCH from the lattice definition of the transverse
+    shift (R7), in Python integers -- not by the oracle's rounding formula"""
+    if D <= 0:
+        return 0
+    z = (D * T) >> 32
+    while ((z << 32) // T) < D:
+        z += 1
+    while z > 0 and (((z - 1) << 32) // T) >= D:
+        z -= 1
+    return z
+
+
+def test_spectra_3d_side_entry_and_exit_closed_form():
+    """Pin of the map's side entry / side exit (VERDICT r2 "parity unpinned", oracle/loc_oracle.c orc_spectra_3d; PAPER.md:123
+    "simple tracing of individual rays through an octree").  On the uniform model a line of sight is a
+    homogeneous slab whatever cells it crosses, so T_A follows from the length of the line INSIDE the model alone:
+        path = (zeta_out - zeta_in) * (root_cm / 2^20) * lenf,
+    zeta_in  = first zeta at which both transverse coordinates b + shift(zeta) are >= 0        (entry through a side face),
+    zeta_out = first zeta at which one of them reaches the extent W, or the depth W_0          (exit through a side face),
+    both found here by search in Python integers.  A line whose transverse coordinates are never inside together gives 0.
+    Shifting the entry by 50 000 units, or following lines past the side face, changes the path by > 1e-2 of its length."""
+    sp_ = W.rotor_species(3, 4)
+    root_cm, nroot = 1.0e17, 4
+    dens, tk, sig, ab, tbg = 3.0e3, 12.0, 2.0e4, 1e-6, 2.73
+    nch, band = 48, 1.5e5
+    m = W.uniform_octree(nroot, 3, root_cm, dens, tk, sig, (0.0, 0.0, 0.0), ab, sp_, W.healpix_dirs(1), nch, band, tbg)
+    os_ = O.OSpecies(sp_)
+    pops = O.lte(os_, m.density, m.tkin, m.abundance)
+    t = 1
+    u, l = sp_.upper[t], sp_.lower[t]
+    nu = (sp_.energy_K[u] - sp_.energy_K[l]) * _K / _H
+    dv = 2 * band / nch
+    sigma = math.sqrt(sig ** 2 + _K * tk / (sp_.mass_amu * 1.66053906660e-24))
+    v = (np.arange(nch) - (nch - 1) / 2) * dv
+    phi = dv / (sigma * math.sqrt(2 * math.pi)) * np.exp(-v ** 2 / (2 * sigma ** 2))
+    n_u, n_l = pops[-1, u], pops[-1, l]
+    gr = sp_.g[u] / sp_.g[l]
+    kap = _C ** 3 * sp_.einstein_A[t] / (8 * math.pi * nu ** 3 * dv) * (n_l * gr - n_u)
+    S_occ, bg_occ = 1.0 / (n_l * gr / n_u - 1.0), 1.0 / math.expm1(_H * nu / (_K * tbg))
+    Wd = nroot * H0
+    # (direction, start (bp, bq) on the upstream face in the working frame, what happens)
+    cases = [
+        ((0.5, 0.2, 1.0), (-7 * H0 // 10, 3 * H0 // 10), "enters through the p side, leaves through the back"),
+        ((0.5, 0.2, 1.0), (32 * H0 // 10 + 12345, 3 * H0 // 10), "enters through the front, leaves through the p side"),
+        ((0.5, 0.4, 1.0), (29 * H0 // 10, -4 * H0 // 10 - 77), "enters through the q side, leaves through the p side"),
+        ((-0.5, 0.4, -1.0), (29 * H0 // 10, -4 * H0 // 10 - 77), "the same with mirrored axes"),
+        ((0.3, 1.0, -0.45), (-11 * H0 // 10 + 5, -2 * H0 // 10), "main axis y; both transverse coordinates start outside"),
+        ((0.5, 0.4, 1.0), (-19 * H0 // 10, 39 * H0 // 10), "q has left before p enters: never inside"),
+        ((0.0, 0.4, 1.0), (-5, 3 * H0 // 10), "zero slope in p and p outside: never inside"),
+    ]
+    seen_paths = []
+    for d, (bp, bq), what in cases:
+        d = np.array(d, float)
+        d /= np.linalg.norm(d)
+        a = np.abs(d)
+        ma = int(np.argmax(a >= a.max()))
+        T = []
+        for ax in ((ma + 1) % 3, (ma + 2) % 3):
+            S = int(np.rint(a[ax] / a[ma] * 2 ** 20))
+            T.append(0 if S == 0 else (2 ** 52 + S // 2) // S)
+        sl = [0.0 if T_ == 0 else 2.0 ** 32 / T_ for T_ in T]
+        lenf = math.sqrt(1.0 + sl[0] ** 2 + sl[1] ** 2)
+        zin, zout = 0, Wd
+        for b, T_ in ((bp, T[0]), (bq, T[1])):
+            if T_ == 0:
+                if b < 0 or b >= Wd:
+                    zin, zout = 0, 0
+                continue
+            zin = max(zin, _first_zeta_with_shift_at_least(T_, -b))
+            zout = min(zout, _first_zeta_with_shift_at_least(T_, Wd - b))
+        inside = max(0, zout - zin)
+        seen_paths.append(inside)
+        TA = O.spectra_3d(os_, m, pops, t, d, 1, 1, np.array([bp, bq, 0, 0, 0, 0], np.int64))[0, 0]
+        expect = _H * nu / _K * (S_occ - bg_occ) * -np.expm1(-kap * phi * inside * (root_cm / H0) * lenf)
+        if inside == 0:
+            assert np.all(TA == 0.0), what
+        else:
+            assert np.max(np.abs(TA - expect)) < 1e-9 * np.max(np.abs(expect)), what
+            # the pin has teeth: one unit of zeta more or less is already outside the bound
+            other = _H * nu / _K * (S_occ - bg_occ) * -np.expm1(-kap * phi * (inside + 1) * (root_cm / H0) * lenf)
+            assert np.max(np.abs(other - expect)) > 1e-8 * np.max(np.abs(expect))
+    # the cases are what they claim: partial paths well inside (0, W), and two misses
+    assert sorted(p_ == 0 for p_ in seen_paths) == [False] * 5 + [True] * 2
+    assert all(H0 // 2 < p_ < Wd - H0 // 2 for p_ in seen_paths if p_)
+
+
 def test_spectra_3d_thin_limit_column_density():
     """P2 for the map: tau << 1, T_bg = 0: integral T_A dv = (h c^3 A / 8 pi k nu^2) N_u, with the upper-level column
     N_u summed here, pixel by pixel, over the cells of the column (x, y fixed) of an octree with two refinement levels:
