@@ -13,7 +13,8 @@
  *
  * Every channel is evaluated (no profile cut-off), every sum is a plain loop.
  * The optional OpenMP pragmas only distribute whole rays over threads and add
- * to the counters with atomic double adds; the arithmetic per ray is serial.
+ * to the counters with atomic double adds (3D) or into per-thread counters that
+ * are summed in thread order (1D, round 3); the arithmetic per ray is serial.
  *
  * Pins (tests/test_oracle_*.py): slab closed form, optically thin limit, LTE
  * limit, blackbody enclosure, two-level closed form, photon ledger, path
@@ -37,6 +38,9 @@
  * (Absolute T_ex profiles of the paper's figures are not reproducible: their
  * inputs are not available.)
  */
+#ifdef _OPENMP
+#include <omp.h>
+#endif
 #include <math.h>
 #include <stdint.h>
 #include <stdlib.h>
@@ -527,40 +531,81 @@ int orc_sim_1d(const orc_species *sp, int ns, const double *r, const double *tki
     memset(LAM, 0, sizeof(double) * nsel * ns);
     if (visits) memset(visits, 0, sizeof(int64_t) * ns);
     if (ledger) memset(ledger, 0, sizeof(double) * LG_N);
-    int *sh = (int *)malloc(sizeof(int) * 2 * ns);
-    double *ss = (double *)malloc(sizeof(double) * 2 * ns), *mu = (double *)malloc(sizeof(double) * 2 * ns);
-    double *phi = (double *)malloc(sizeof(double) * nch), *N = (double *)malloc(sizeof(double) * nch);
-    for (int i = 0; i < nray; i++) {
-        int nseg = ray_path_1d(ns, r, p[i], sh, ss, mu);
-        for (int k = 0; k < nsel; k++) {
-            int t = sel[k], u = sp->upper[t], l = sp->lower[t];
-            double nu = orc_freq(sp, t);
-            double kcoef = ORC_C * ORC_C * ORC_C * sp->A[t] / (8.0 * ORC_PI * nu * nu * nu * dv);
-            double gr = sp->g[u] / sp->g[l];
-            double n0 = bg_photons(nu, tbg, w[i], dv); /* Eq. 1, a = W_i */
-            for (int c = 0; c < nch; c++) N[c] = n0;
-            if (ledger) ledger[LG_INJECTED] += n0 * nch;
-            for (int j = 0; j < nseg; j++) {
-                int cell = sh[j];
-                double sig = total_sigma(sp, sigma_turb[cell], tkin[cell]);
-                /* R6: radio convention, v0 = -(v . d) = -v_r mu, mu at the entry of the step */
-                profile_t(sp, t, nch, dv, sig, -vrad[cell] * mu[j], phi);
-                cell_step(nch, N, phi, w[i], ss[j], veff[cell], kcoef, gr, sp->A[t], pops[cell * NL + u],
-                          pops[cell * NL + l], ali, &ABS[k * ns + cell], &P[k * ns + cell], &LAM[k * ns + cell], ledger);
-                if (k == 0 && visits) visits[cell]++;
-            }
-            for (int c = 0; c < nch; c++) {
-                if (ledger) ledger[LG_ESCAPED] += N[c];
-                if (nout) nout[((size_t)i * nsel + k) * nch + c] = N[c];
+    /* Whole rays are dealt out to the threads in turn (schedule(static, 1): ray i goes to thread i mod T -- the rays
+     * differ in length by the number of shells they cross, and dealing balances that); every thread adds into counters of
+     * its own, and the threads' counters are added up in thread order afterwards.  The arithmetic per ray is serial and in
+     * the paper's order; with one thread the sums are those of the plain loop over rays, bit for bit; with T threads only
+     * the order in which the rays' contributions to a shell are added differs (rounding, ~1e-16 relative).             */
+    int nthr = 1;
+#ifdef _OPENMP
+    nthr = omp_get_max_threads();
+    if (nthr > nray) nthr = nray;
+    if (nthr < 1) nthr = 1;
+#endif
+    size_t ncnt = (size_t)nsel * ns;
+    double *tacc = (double *)calloc((size_t)nthr * 3 * ncnt, sizeof(double));
+    double *tled = (double *)calloc((size_t)nthr * LG_N, sizeof(double));
+    int64_t *tvis = (int64_t *)calloc((size_t)nthr * ns, sizeof(int64_t));
+#pragma omp parallel num_threads(nthr)
+    {
+        int tid = 0;
+#ifdef _OPENMP
+        tid = omp_get_thread_num();
+#endif
+        double *tABS = tacc + (size_t)tid * 3 * ncnt, *tP = tABS + ncnt, *tLAM = tP + ncnt;
+        double *led = ledger ? tled + (size_t)tid * LG_N : NULL;
+        int64_t *vis = tvis + (size_t)tid * ns;
+        int *sh = (int *)malloc(sizeof(int) * 2 * ns);
+        double *ss = (double *)malloc(sizeof(double) * 2 * ns), *mu = (double *)malloc(sizeof(double) * 2 * ns);
+        double *phi = (double *)malloc(sizeof(double) * nch), *N = (double *)malloc(sizeof(double) * nch);
+#pragma omp for schedule(static, 1)
+        for (int i = 0; i < nray; i++) {
+            int nseg = ray_path_1d(ns, r, p[i], sh, ss, mu);
+            for (int k = 0; k < nsel; k++) {
+                int t = sel[k], u = sp->upper[t], l = sp->lower[t];
+                double nu = orc_freq(sp, t);
+                double kcoef = ORC_C * ORC_C * ORC_C * sp->A[t] / (8.0 * ORC_PI * nu * nu * nu * dv);
+                double gr = sp->g[u] / sp->g[l];
+                double n0 = bg_photons(nu, tbg, w[i], dv); /* Eq. 1, a = W_i */
+                for (int c = 0; c < nch; c++) N[c] = n0;
+                if (led) led[LG_INJECTED] += n0 * nch;
+                for (int j = 0; j < nseg; j++) {
+                    int cell = sh[j];
+                    double sig = total_sigma(sp, sigma_turb[cell], tkin[cell]);
+                    /* R6: radio convention, v0 = -(v . d) = -v_r mu, mu at the entry of the step */
+                    profile_t(sp, t, nch, dv, sig, -vrad[cell] * mu[j], phi);
+                    cell_step(nch, N, phi, w[i], ss[j], veff[cell], kcoef, gr, sp->A[t], pops[cell * NL + u],
+                              pops[cell * NL + l], ali, &tABS[k * ns + cell], &tP[k * ns + cell], &tLAM[k * ns + cell], led);
+                    if (k == 0) vis[cell]++;
+                }
+                for (int c = 0; c < nch; c++) {
+                    if (led) led[LG_ESCAPED] += N[c];
+                    if (nout) nout[((size_t)i * nsel + k) * nch + c] = N[c];
+                }
             }
         }
+        free(sh);
+        free(ss);
+        free(mu);
+        free(phi);
+        free(N);
     }
+    for (int tid = 0; tid < nthr; tid++) { /* fixed order: thread 0 (rays 0, T, 2T, ...), then thread 1, and so on */
+        const double *tABS = tacc + (size_t)tid * 3 * ncnt, *tP = tABS + ncnt, *tLAM = tP + ncnt;
+        for (size_t q = 0; q < ncnt; q++) {
+            ABS[q] += tABS[q];
+            P[q] += tP[q];
+            LAM[q] += tLAM[q];
+        }
+        if (visits)
+            for (int c = 0; c < ns; c++) visits[c] += tvis[(size_t)tid * ns + c];
+        if (ledger)
+            for (int q = 0; q < LG_N; q++) ledger[q] += tled[(size_t)tid * LG_N + q];
+    }
+    free(tacc);
+    free(tled);
+    free(tvis);
     free(veff);
-    free(sh);
-    free(ss);
-    free(mu);
-    free(phi);
-    free(N);
     return 0;
 }
 
