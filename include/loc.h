@@ -213,9 +213,13 @@ int loc_iterate(loc_model *m, int niter, double *max_rel_change);
 int loc_set_ali(loc_model *m, int ali);
 
 /* Accuracy / launch knobs (keys LOC_OPT_* above).  LOC_EINVAL for an unknown key or a value outside the key's range.
- * Channel widths: the kernels need no minimum resolution of the line profile -- with channels wider than the line
- * (dv > sigma) the sampled profile of PAPER.md:73 is no longer normalised, and the kernels then sum the sampled values
- * themselves instead of using the analytic wing mass, and widen the window by 2 ln (dv/sigma)^2.     */
+ * Channel widths: loc_simulate and loc_spectra need no minimum resolution of the line profile -- with channels wider than
+ * the line (dv > sigma) the sampled profile of PAPER.md:73 is no longer normalised, and the kernels then sum the sampled
+ * values themselves instead of using the analytic wing mass, and widen the window by 2 ln (dv/sigma)^2.
+ * ITERATION is another matter: for dv > 2 sigma the sampled profile can sum to more than 1, the method's own LAMBDA*
+ * then exceeds 1 (ESC < 0) and the accelerated rate equations leave the physical range -- in the float64
+ * oracle just as in the kernels.  loc_solve / loc_iterate* are defined for dv <= 2 sigma in every cell; beyond that their
+ * result is unspecified (it may be LOC_ENONFINITE).  The counters of a single loc_simulate stay well defined.          */
 int loc_set_option(loc_model *m, int key, double value);
 
 /* Convergence-controlled iteration ("repeated until the level populations converge"):

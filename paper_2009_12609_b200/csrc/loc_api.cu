@@ -11,7 +11,7 @@
 
 #include "loc_internal.cuh"
 
-static char g_create_err[512] = "";
+static thread_local char g_create_err[512] = "";  // per thread: loc_create_model has no model to carry its error text
 
 // ------------------------------------------------------------------------------------------------
 // workspace carving
@@ -42,7 +42,10 @@ static int device_sm_count()
     }
     return nsm;
 }
-static int max_resident_ctas() { return device_sm_count() * 16; }  // upper bound used to size the per-CTA spectrum slots
+// upper bound used to size the per-CTA spectrum slots of k_sim3d: 32 CTAs per multiprocessor is the hardware's limit, so the
+// launch (occupancy query x multiprocessors) is never clamped by the pool whatever a kernel variant's register / shared-
+// memory use allows (round 2 sized it for 16: right for today's 128-register one-warp CTAs, a silent cap for leaner ones)
+static int max_resident_ctas() { return device_sm_count() * 32; }
 
 // lays out the workspace; with dry=true only sizes are computed
 static int64_t carve(loc_model *m, Carver &c, const loc_grid *g, int nch, int nlevel, int ntrans, int ndir_max)
@@ -405,7 +408,7 @@ extern "C" int loc_set_species(loc_model *m, int nlevel, const double *energy_K,
     }
     for (int k = 0; k < ncoll; k++)
         if (cu[k] < 0 || cu[k] >= nlevel || cl[k] < 0 || cl[k] >= nlevel || cu[k] == cl[k]) return fail(m, LOC_EINVAL, "bad collisional pair");
-    for (int j = 1; j < ntemp; j++)
+    for (int j = 1; temps_K && j < ntemp; j++)
         if (!(temps_K[j] > temps_K[j - 1])) return fail(m, LOC_EINVAL, "collision temperatures must ascend");
     m->nlevel = nlevel;
     m->ntrans = ntrans;
@@ -415,21 +418,27 @@ extern "C" int loc_set_species(loc_model *m, int nlevel, const double *energy_K,
     memcpy(m->h_g, g, sizeof(double) * nlevel);
     free(m->h_upper); free(m->h_lower); free(m->h_A); free(m->h_freq);
     free(m->h_cu); free(m->h_cl); free(m->h_temps); free(m->h_rates);
-    m->h_cu = (int *)malloc(sizeof(int) * std::max(ncoll, 1));
-    m->h_cl = (int *)malloc(sizeof(int) * std::max(ncoll, 1));
-    m->h_temps = (double *)malloc(sizeof(double) * ntemp);
-    m->h_rates = (double *)malloc(sizeof(double) * ntemp * std::max(ncoll, 1));
+    m->have_species = false;
+    m->simulated = false;  // counters traced for the previous species say nothing about this one
+    m->h_cu = (int *)calloc(std::max(ncoll, 1), sizeof(int));
+    m->h_cl = (int *)calloc(std::max(ncoll, 1), sizeof(int));
+    m->h_temps = (double *)calloc(ntemp, sizeof(double));
+    m->h_rates = (double *)calloc((size_t)ntemp * std::max(ncoll, 1), sizeof(double));
+    m->h_upper = (int *)calloc(ntrans, sizeof(int));
+    m->h_lower = (int *)calloc(ntrans, sizeof(int));
+    m->h_A = (double *)calloc(ntrans, sizeof(double));
+    m->h_freq = (double *)calloc(ntrans, sizeof(double));
+    if (!m->h_cu || !m->h_cl || !m->h_temps || !m->h_rates || !m->h_upper || !m->h_lower || !m->h_A || !m->h_freq)
+        return fail(m, LOC_ENOMEM, "loc_set_species: host allocation failed");
+    // a species without collisions may still carry a temperature grid (ntemp > 1): the solvers interpolate on it
+    if (temps_K) memcpy(m->h_temps, temps_K, sizeof(double) * ntemp);
+    else for (int j = 0; j < ntemp; j++) m->h_temps[j] = 1.0 + j;
     if (ncoll) {
         memcpy(m->h_cu, cu, sizeof(int) * ncoll);
         memcpy(m->h_cl, cl, sizeof(int) * ncoll);
-        memcpy(m->h_temps, temps_K, sizeof(double) * ntemp);
         memcpy(m->h_rates, rate_down, sizeof(double) * ntemp * ncoll);
     }
     m->rates_f_valid = false;
-    m->h_upper = (int *)malloc(sizeof(int) * ntrans);
-    m->h_lower = (int *)malloc(sizeof(int) * ntrans);
-    m->h_A = (double *)malloc(sizeof(double) * ntrans);
-    m->h_freq = (double *)malloc(sizeof(double) * ntrans);
     std::vector<double> bg(ntrans);
     for (int t = 0; t < ntrans; t++) {
         m->h_upper[t] = upper[t];
@@ -452,10 +461,10 @@ extern "C" int loc_set_species(loc_model *m, int nlevel, const double *energy_K,
     LOC_CUDA_CHECK(m, cudaMemcpyAsync((void *)sp.A, A, sizeof(double) * ntrans, cudaMemcpyHostToDevice, st));
     LOC_CUDA_CHECK(m, cudaMemcpyAsync((void *)sp.freq, m->h_freq, sizeof(double) * ntrans, cudaMemcpyHostToDevice, st));
     LOC_CUDA_CHECK(m, cudaMemcpyAsync((void *)sp.bgocc, bg.data(), sizeof(double) * ntrans, cudaMemcpyHostToDevice, st));
+    LOC_CUDA_CHECK(m, cudaMemcpyAsync((void *)sp.temps, m->h_temps, sizeof(double) * ntemp, cudaMemcpyHostToDevice, st));
     if (ncoll) {
         LOC_CUDA_CHECK(m, cudaMemcpyAsync((void *)sp.cu, cu, sizeof(int) * ncoll, cudaMemcpyHostToDevice, st));
         LOC_CUDA_CHECK(m, cudaMemcpyAsync((void *)sp.cl, cl, sizeof(int) * ncoll, cudaMemcpyHostToDevice, st));
-        LOC_CUDA_CHECK(m, cudaMemcpyAsync((void *)sp.temps, temps_K, sizeof(double) * ntemp, cudaMemcpyHostToDevice, st));
         LOC_CUDA_CHECK(m, cudaMemcpyAsync((void *)sp.rates, rate_down, sizeof(double) * ntemp * ncoll, cudaMemcpyHostToDevice, st));
     }
     m->have_species = true;
@@ -510,6 +519,7 @@ extern "C" int loc_set_hyperfine(loc_model *m, int trans, int ncomp, const doubl
         sum += weight[k];
     }
     if (ncomp > 0 && fabs(sum - 1.0) > 1e-6) return fail(m, LOC_EINVAL, "loc_set_hyperfine: the weights must sum to 1");
+    m->simulated = false;  // the counters were traced with the old profile
     m->h_hfs_nc[trans] = ncomp;
     for (int k = 0; k < ncomp; k++) {
         m->h_hfs_dv[trans][k] = dv_cm_s[k];

@@ -160,7 +160,6 @@ struct loc_model {
     double setup_ms;
     // stats
     int64_t launches;
-    int64_t last_steps;
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -230,32 +229,12 @@ __device__ __forceinline__ TParam make_tparam(float2 ke, float s, float w, float
     return p;
 }
 
-// One channel, one transition (Eq. 3 and the two sums of Eq. 2 / PAPER.md:81 in occupation-number units).
+// One channel, one transition (Eq. 3 and the two sums of Eq. 2 / PAPER.md:81 in occupation-number units):
 //   n      photon occupation number in the channel, updated
 //   phi    fraction of the profile in the channel (0 for inactive lanes)
 //   accA  += n_in * phi * f(tau)        (thick: n_in (1-e^-tau), rescaled by 1/(kap s) afterwards)
 //   accB  += phi * f(tau)               (thick: (1-e^-tau))
-__device__ __forceinline__ void channel_update(float &n, float phi, const TParam &p, float &accA, float &accB)
-{
-    if (p.thick) {
-        float e = ex2f(phi * p.c0);
-        float om = 1.0f - e;
-        accA = fmaf(n, om, accA);
-        accB += om;
-        n = fmaf(om, p.c1 - n, n);
-    } else {
-        float tau = phi * p.c0;
-        float P = fmaf(tau, fmaf(tau, fmaf(tau, -1.0f / 24.0f, 1.0f / 6.0f), -0.5f), 1.0f);  // (1-e^-tau)/tau
-        float q = phi * P;
-        float om = tau * P;
-        accA = fmaf(n, q, accA);
-        accB += q;
-        n = fmaf(p.c1, q, fmaf(-n, om, n));
-    }
-}
-
-// channel_update for a quad of channels in packed pairs (same operations per element as channel_update, so the same
-// results; half the issue slots).  n01 / n23 and phi01 / phi23 hold channels (0, 1) / (2, 3); acc += the quad's sums.
+// The same for a quad of channels in packed pairs (half the issue slots).  n01 / n23 and phi01 / phi23 hold channels (0, 1) / (2, 3); acc += the quad's sums.
 __device__ __forceinline__ void channel_update4(f32x2 &n01, f32x2 &n23, f32x2 phi01, f32x2 phi23, const TParam &p, float &accA, float &accB)
 {
     const f32x2 C0 = pk2(p.c0, p.c0), C1 = pk2(p.c1, p.c1);

@@ -9,8 +9,8 @@
 //      per-shell path lengths of the 1D model that the paper pre-calculates -- they are computed once
 //      and kept in HBM (B200: 180 GB) instead of being recomputed by one idle-lane-surrounded work item per step
 //      (the paper's stated bottleneck).
-//  (2) RADIATIVE KERNEL (every ALI iteration): one warp per root-ray task, lanes over the velocity channels of the
-//      local profile window.  It streams the records, evaluates the Doppler-shifted profile, optical depths, Eq. 3 and
+//  (2) RADIATIVE KERNEL (every ALI iteration): a quarter-warp per root-ray task, four tasks per CTA of one or two warps
+//      (loc_sim3d.cu), lanes over the velocity channels of the local profile window.  It streams the records, evaluates the Doppler-shifted profile, optical depths, Eq. 3 and
 //      the two per-cell sums (Eq. 2 first term and the escape fraction) for all traced transitions at once.
 #include <stdio.h>
 

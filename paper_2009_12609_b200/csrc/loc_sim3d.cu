@@ -14,8 +14,9 @@
 //     transition, conflict free for any span position (a quarter-warp is one shared-memory phase);
 //   * the per-channel arithmetic is done on packed pairs (fma.rn.f32x2) and is ONE straight-line expression for both
 //     regimes of the optical depth (below): no masks, no selects, no branches per transition;
-//   * the sums over a lane's 4 channels are free, and the cross-lane reduction goes through shared memory: lane t of
-//     the group adds up the 8 partial sums of transition t and issues ONE 64-bit RED for the cell's (SJ, ESC) pair;
+//   * the sums over a lane's 4 channels are free, and the cross-lane reduction is a halving butterfly in registers
+//     (warp_multi_reduce): lane t of the group ends up with the total of transition t and issues ONE 64-bit RED for
+//     the cell's (SJ, ESC) pair;
 //   * all per-step scalar work (record decode, Doppler shift, window, per-transition coefficients, scale of the sums,
 //     counter offset) is done in a "prepare" phase, two lanes of each warp per record for 4 records x 4 rays at once,
 //     from cell data prefetched into registers one chunk ahead, and left in one shared-memory record per (ray, round):

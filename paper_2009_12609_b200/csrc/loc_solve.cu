@@ -490,11 +490,13 @@ __global__ void __launch_bounds__(LOC_SOLVE_F_THREADS) k_solve_f(int64_t n, cons
 // ------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------
-// dense pair tables of k_solve_f from the species and the current selection; false = the species does not fit them
-static bool fill_solve_f(loc_model *m, SolveF &Q)
+// dense pair tables of k_solve_f from the species and the current selection.  Returns 1 = filled, 0 = the species does not
+// fit them (the float64 kernels take over), LOC_ECUDA = the upload of the dense rate table failed (reported, never hidden
+// behind the fallback).
+static int fill_solve_f(loc_model *m, SolveF &Q)
 {
     const int NL = m->nlevel;
-    if (NL < 2 || NL > LOC_SOLVE_F_MAXNL) return false;
+    if (NL < 2 || NL > LOC_SOLVE_F_MAXNL) return 0;
     memset(&Q, 0, sizeof(Q));
     const int np = NL * (NL - 1) / 2;
     for (int u = 1; u < NL; u++)
@@ -506,11 +508,11 @@ static bool fill_solve_f(loc_model *m, SolveF &Q)
         }
     for (int t = 0; t < m->ntrans; t++) {
         const int u = m->h_upper[t], l = m->h_lower[t];
-        if (u <= l) return false;
+        if (u <= l) return 0;
         const int p = u * (u - 1) / 2 + l;
-        if (Q.A[p] != 0.0f) return false;  // two transitions between the same levels
+        if (Q.A[p] != 0.0f) return 0;  // two transitions between the same levels
         Q.A[p] = (float)m->h_A[t];
-        if (Q.A[p] == 0.0f) return false;  // below the float32 range
+        if (Q.A[p] == 0.0f) return 0;  // below the float32 range
         Q.bg[p] = (m->tbg > 0.0) ? (float)(1.0 / expm1(LOC_HP * m->h_freq[t] / (LOC_KB * m->tbg))) : 0.0f;
         for (int k = 0; k < m->selh.nsel; k++)
             if (m->selh.sel[k] == t) Q.slot[p] = k;
@@ -518,7 +520,7 @@ static bool fill_solve_f(loc_model *m, SolveF &Q)
     std::vector<float> dense((size_t)m->ntemp * np, 0.0f);
     for (int k = 0; k < m->ncoll; k++) {
         const int u = m->h_cu[k], l = m->h_cl[k];
-        if (u <= l) return false;
+        if (u <= l) return 0;
         const int p = u * (u - 1) / 2 + l;
         for (int j = 0; j < m->ntemp; j++) dense[(size_t)j * np + p] += (float)m->h_rates[(size_t)j * m->ncoll + k];
     }
@@ -527,11 +529,11 @@ static bool fill_solve_f(loc_model *m, SolveF &Q)
         for (int p = 0; p < np; p++) Q.gd[p] = dense[p];
     } else {
         for (int j = 0; j < m->ntemp; j++) Q.temps[j] = (float)m->h_temps[j];
-        // the dense table lives in the workspace; rewritten only when the species changes (loc_set_species clears the flag)
+        // the dense table lives in the workspace; rewritten only when the species changes (loc_set_species clears the flag).
+        // The first solve after loc_set_species therefore waits once for the stream (`dense` goes out of scope).
         if (!m->rates_f_valid) {
-            if (cudaMemcpyAsync(m->d_rates_f, dense.data(), sizeof(float) * dense.size(), cudaMemcpyHostToDevice, m->stream) != cudaSuccess ||
-                cudaStreamSynchronize(m->stream) != cudaSuccess)  // `dense` goes out of scope
-                return false;
+            LOC_CUDA_CHECK(m, cudaMemcpyAsync(m->d_rates_f, dense.data(), sizeof(float) * dense.size(), cudaMemcpyHostToDevice, m->stream));
+            LOC_CUDA_CHECK(m, cudaStreamSynchronize(m->stream));
             m->rates_f_valid = true;
         }
         Q.rates = m->d_rates_f;
@@ -545,7 +547,7 @@ static bool fill_solve_f(loc_model *m, SolveF &Q)
         Q.ck[k] = (float)m->selh.ck[k];
         Q.gratio[k] = m->selh.gratio[k];
     }
-    return true;
+    return 1;
 }
 
 template <int NL>
@@ -574,7 +576,9 @@ int loc_launch_solve(loc_model *m)
     // memory, else float64 in local memory), 1 = force the local-memory kernel, 2 = the shared-memory kernel (A/B runs)
     if (m->solver == 0) {
         SolveF Q;
-        if (fill_solve_f(m, Q)) {
+        const int fits = fill_solve_f(m, Q);
+        if (fits < 0) return fits;
+        if (fits) {
             int rc = LOC_EINVAL;
             switch (m->nlevel) {
 #define LOC_SF(N)                          \

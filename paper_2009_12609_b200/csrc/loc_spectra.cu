@@ -2,12 +2,13 @@
 // transitions by a final line-of-sight integration through the model", "simple tracing of individual rays
 // through an octree", PAPER.md:203 pixel = smallest cell).
 //
-// One warp per line of sight (map pixel).  The pixel's spectrum lives in shared memory as the EXCESS photon occupation
+// Octree maps: a quarter-warp per line of sight (map pixel), four neighbouring pixels per warp; shell models: one warp per
+// line of sight.  The pixel's spectrum lives in shared memory as the EXCESS photon occupation
 // number over the background, D_c = n_c - n_bg, so that the output T_A(c) = (h nu / k) D_c (= (c^2/2k nu^2)(I_c - B_nu(T_bg)))
 // carries no cancellation:
 //     D_c <- D_c + X_c (S - n_bg - D_c),   X_c = 1 - exp(-tau_c),   tau_c = kap s phi_c,   S = n_u / (n_l g_u/g_l - n_u)
 // (the formal solution I <- I e^-tau + S_nu (1 - e^-tau) in occupation-number units, DESIGN 5.2).  The path is walked by all
-// lanes in lock step with the integer lattice arithmetic of the path builder (DESIGN R7) -- no births, no wrap-around: a line
+// lanes of a line of sight in lock step with the integer lattice arithmetic of the path builder (DESIGN R7) -- no births, no wrap-around: a line
 // of sight starts where it enters the model and ends where it leaves it -- and the lanes then split the channels of the
 // step's profile window (DESIGN R13).  kap and S are formed in double from the float32 populations (n_l g_u/g_l - n_u cancels).
 #include <math.h>

@@ -44,7 +44,8 @@ def test_spectra_1d(ns, nch):
 
 
 @pytest.mark.parametrize("cfg", [dict(nroot=4, nlev=3, nch=32, frac=0.35), dict(nroot=6, nlev=1, nch=45, frac=0.0),
-                                 dict(nroot=3, nlev=4, nch=64, frac=0.5)])
+                                 dict(nroot=3, nlev=4, nch=64, frac=0.5),
+                                 dict(nroot=4, nlev=3, nch=256, frac=0.38)])  # C5's band: 256 channels on a 3-level octree
 def test_spectra_3d(cfg):
     from paper_2009_12609_b200 import LocModel
     m = W.cloud_config(4, nroot=cfg["nroot"], nlev=cfg["nlev"], nchannel=cfg["nch"], nside=1, refine_frac=cfg["frac"],
