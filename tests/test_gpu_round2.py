@@ -270,6 +270,44 @@ def test_options_and_error_paths():
     g.close()
 
 
+def test_state_guards_after_species_or_profile_change_and_no_collisions():
+    """(a) loc_set_hyperfine / loc_set_species after a loc_simulate invalidate the counters -- loc_solve then
+    returns LOC_ESTATE instead of solving on counters traced with another profile / species; (b) a species WITHOUT
+    collisional pairs but WITH a temperature grid (ncoll = 0, ntemp > 1: legal) solves to finite populations (round 2 read
+    uninitialised temperatures there) and gives what the oracle gives."""
+    from paper_2009_12609_b200 import binding as B
+    lib = B.lib()
+    m = W.shell_config(1, ns=12, nchannel=32)
+    g = _model(m)
+    g.init_lte()
+    g.simulate()
+    assert lib.loc_solve(g.h, None) == B.LOC_OK
+    g.simulate()
+    B.loc_set_hyperfine(g.h, 0, [-0.3e5, 0.2e5], [0.4, 0.6])
+    assert lib.loc_solve(g.h, None) == B.LOC_ESTATE
+    g.simulate()
+    assert lib.loc_solve(g.h, None) == B.LOC_OK
+    B.loc_set_species(g.h, m.species)
+    B.loc_set_populations(g.h, g.pops)
+    assert lib.loc_solve(g.h, None) == B.LOC_ESTATE
+    g.close()
+    # (b) radiative-only species on a 3-node temperature grid
+    m = W.shell_config(1, ns=12, nchannel=32)
+    s = m.species
+    s.cu, s.cl = np.zeros(0, np.int32), np.zeros(0, np.int32)
+    s.temps_K = np.array([8.0, 12.0, 18.0])
+    s.rate_down = np.zeros((3, 0))
+    sp = O.OSpecies(s)
+    pops_o, _ = O.iterate(sp, m, 2)
+    g = _model(m)
+    g.init_lte()
+    g.iterate(2)
+    pg = g.pops.cpu().numpy()
+    g.close()
+    assert np.all(np.isfinite(pg))
+    assert check_pops(pg, pops_o)[0] < TOL_POP
+
+
 def test_set_directions_invalid_arguments_keep_the_old_directions():
     """an invalid ARGUMENT (not a unit vector, more directions than ndir_max) is rejected before anything is touched: the
     model keeps its directions and step stream.  (A failure INSIDE the path set-up -- LOC_ENOMEM / LOC_ECUDA -- leaves the
