@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the LOC hot path (one ALI iteration = loc_simulate + loc_solve) on synthetic clouds.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C1|C2|C3|C4|C5] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C1|C2|C2H|C3|C3H|C4|C5] [--impl reference]
 
 One "step" is one pass of the whole hot path (ray tracing of all directions / rays for all traced transitions, then
 the per-cell statistical-equilibrium solve) over one synthetic model.  Prints ONE JSON line (rank 0).
@@ -28,6 +28,7 @@ METRIC = "ray-cell-channel updates/sec per ALI iteration"
 UNIT = "updates/s"
 VALUE_KIND = "active updates: channels within 5 sigma of the line centre x traced transitions x ray-cell steps (DESIGN.md 8.1)"
 DEFAULT_WORKLOAD = "C5"
+CONFIG_ITERATIONS = {"C1": 20, "C2": 50, "C2H": 50, "C3": 10, "C3H": 10, "C4": 10, "C5": 5}  # BASELINE.json configs: ALI iterations of a run
 
 # ---- roofline constants -----------------------------------------------------------------------------
 N_SM = 148
@@ -61,6 +62,11 @@ def make_workload(name: str):
         m.species.hfs = {0: (np.array([-1.0e5, 0.05e5, 0.7e5]), np.array([0.2, 0.5, 0.3]))}
         m.name = "C2H"
         return m, "C2H: C2 with hyperfine structure on J = 1-0: components at -1.0, +0.05, +0.7 km/s with weights 0.2, 0.5, 0.3"
+    if name == "C3H":  # the cost of the masked (hyperfine) path of k_sim3d on record at C3 size
+        m = W.cloud_config(3)
+        m.species.hfs = {0: (np.array([-1.0e5, 0.05e5, 0.7e5]), np.array([0.2, 0.5, 0.3]))}
+        m.name = "C3H"
+        return m, "C3H: C3 with hyperfine structure on J = 1-0 (components at -1.0, +0.05, +0.7 km/s, weights 0.2, 0.5, 0.3): every step takes the masked round"
     if name == "C3":
         return W.cloud_config(3), "C3: Cartesian 128^3, 48 directions, 128 channels, 10-level rotor (9 transitions)"
     if name == "C4":
@@ -271,7 +277,21 @@ def whole_job_value(updates_per_rank_step: float, steps: int, world: int, second
 
 
 # ---- full-size parity on a direction subset (SURVEY 8d parity protocol (b)) -----------------------------------
-def parity_leg(g, m, dirs_idx, ntrans=1):
+def default_parity_dirs(dirs):
+    """direction 0 plus the first axis-aligned direction whose main component is negative (zero slopes: the T = 0 branches of
+    the lattice arithmetic; mirrored main axis)"""
+    d = np.asarray(dirs, np.float64)
+    out = [0]
+    for i in range(len(d)):
+        a = np.abs(d[i])
+        k = int(np.argmax(a))
+        if d[i, k] < 0 and np.all(np.rint(np.delete(a, k) / a[k] * 2 ** 20) == 0) and i not in out:
+            out.append(i)
+            break
+    return out
+
+
+def parity_leg(g, m, dirs_idx, ntrans=1, map_patch=0):
     """The oracle traces directions `dirs_idx` of the FULL model for the first `ntrans` traced transitions from LTE
     populations (its own, rounded to float32: the input of both sides); the library does the same with
     loc_set_directions(those directions).  Compared per cell: visit counts and integer path sums bit-exact, SJ within 1e-4
@@ -289,36 +309,72 @@ def parity_leg(g, m, dirs_idx, ntrans=1):
     p32 = np.ascontiguousarray(p64.T.astype(np.float32))     # level-major, float32: the common input
     p64[...] = p32.T
     is3d = hasattr(m, "child")
-    t0 = time.perf_counter()
+    leaf = (np.asarray(m.child) < 0) if is3d else np.ones(len(m.density), bool)
+    # the library first: all compared transitions in one pass over the direction subset
     if is3d:
         dsub = np.ascontiguousarray(np.asarray(m.dirs, np.float64)[list(dirs_idx)])
-        ref = O.sim_3d(sp, m, p64, sel, dirs=dsub)
         g.set_directions(dsub)
-    else:
-        ref = O.sim_1d(sp, m, p64, sel)
-    t_or = time.perf_counter() - t0
-    del p64
     g.set_populations(p32)
     g.simulate(sel, geometry_counters=True)
     sj, esc = g.counters()
-    sj, esc = sj.cpu().numpy().astype(np.float64), esc.cpu().numpy().astype(np.float64)
+    sj, esc = sj.cpu().numpy(), esc.cpu().numpy()
     vis, pz = g.geometry_counters()
-    vis = vis.cpu().numpy().astype(np.int64)
-    visits_equal = bool(np.array_equal(vis, ref["visits"]))
-    path_equal = bool(np.array_equal(pz.cpu().numpy().astype(np.int64), ref["pathz"])) if is3d else None
-    leaf = (np.asarray(m.child) < 0) if is3d else np.ones(len(m.density), bool)
+    vis, pz = vis.cpu().numpy().astype(np.int64), pz.cpu().numpy().astype(np.int64)
+    # the oracle keeps one donor spectrum [transitions][channels] of float64 per refined cell while it traces a direction
+    # (C5: 25.8 M refined cells x 256 channels = 53 GB per transition), so the transitions go through it in groups that keep
+    # that store below ~60 GB: one at a time on C5, all at once on the small workloads
+    nref = int((~leaf).sum()) if is3d else 0
+    per_trans = max(1, nref) * nch * 8
+    group = int(max(1, min(len(sel), 60e9 // per_trans)))
     cvel = 2.99792458e10
-    worst_sj, worst_esc = 0.0, 0.0
-    for k, t in enumerate(sel):
-        sj_o = cvel ** 3 * ref["P"][k] / (8.0 * np.pi * sp.freq(int(t)) ** 3 * dv * ref["veff"])
-        esc_o = 1.0 - ref["LAM"][k]
-        worst_sj = max(worst_sj, float((np.abs(sj[leaf, k] - sj_o[leaf]) / np.maximum(np.abs(sj_o[leaf]), 1e-300)).max()))
-        worst_esc = max(worst_esc, float((np.abs(esc[leaf, k] - esc_o[leaf]) / (np.abs(esc_o[leaf]) + 3e-3)).max()))
+    worst_sj, worst_esc, t_or, nsteps_ref = 0.0, 0.0, 0.0, 0
+    visits_equal, path_equal = True, (True if is3d else None)
+    for k0 in range(0, len(sel), group):
+        sub = np.ascontiguousarray(sel[k0:k0 + group])
+        t0 = time.perf_counter()
+        ref = O.sim_3d(sp, m, p64, sub, dirs=dsub) if is3d else O.sim_1d(sp, m, p64, sub)
+        t_or += time.perf_counter() - t0
+        if k0 == 0:
+            nsteps_ref = int(ref["visits"].sum())
+            visits_equal = bool(np.array_equal(vis, ref["visits"]))
+            if is3d:
+                path_equal = bool(np.array_equal(pz, ref["pathz"]))
+        for j, t in enumerate(sub):
+            k = k0 + j
+            sj_o = cvel ** 3 * ref["P"][j] / (8.0 * np.pi * sp.freq(int(t)) ** 3 * dv * ref["veff"])
+            esc_o = 1.0 - ref["LAM"][j]
+            worst_sj = max(worst_sj, float((np.abs(sj[leaf, k] - sj_o[leaf]) / np.maximum(np.abs(sj_o[leaf]), 1e-300)).max()))
+            worst_esc = max(worst_esc, float((np.abs(esc[leaf, k] - esc_o[leaf]) / (np.abs(esc_o[leaf]) + 3e-3)).max()))
+        del ref
+    del sj, esc, vis, pz
     ok = visits_equal and (path_equal is not False) and worst_sj < 1e-4 and worst_esc < 1e-4
-    return {"workload": m.name, "directions": [int(d) for d in dirs_idx] if is3d else None, "transitions": [int(t) for t in sel],
-            "cells": int(leaf.sum()), "ray_cell_steps": int(ref["visits"].sum()), "visits_equal": visits_equal,
+    map_par = None
+    if is3d and map_patch > 0:
+        # S10 at full size: the cube bench.py times (one pixel per finest cell along +z), computed in full by the
+        # library from the same float32 LTE populations; its corner patch (two map edges) against orc_spectra_3d, channel by
+        # channel at the tolerance of tests/test_gpu_spectra.py
+        nfine, pix = int(m.nx) << (int(m.nlev) - 1), (1 << 20) >> (int(m.nlev) - 1)
+        npt = min(int(map_patch), nfine)
+        ix0, iy0 = 0, nfine - npt
+        zdir = np.array([0.0, 0.0, 1.0])
+        tm = int(sel[0])
+        cube = g.spectra(tm, nfine, nfine, dir=zdir, aff=np.array([pix // 2, pix // 2, pix, 0, 0, pix], np.int64))
+        ta = cube[iy0:iy0 + npt, ix0:ix0 + npt, :].cpu().numpy().astype(np.float64)
+        del cube
+        t1 = time.perf_counter()
+        rm = O.spectra_3d(sp, m, p64, tm, zdir, npt, npt, np.array([pix // 2 + ix0 * pix, pix // 2 + iy0 * pix, pix, 0, 0, pix], np.int64))
+        tol = 1e-3 * np.abs(rm) + 2e-5 * np.max(np.abs(rm))
+        worst = float(np.max(np.abs(ta - rm) / tol))
+        map_par = {"pixels": [npt, npt], "origin": [ix0, iy0], "of_map": [nfine, nfine], "channels": int(nch), "transition": tm,
+                   "peak_K": float(np.max(np.abs(rm))), "max_err_over_tol": worst, "tol": "1e-3 |T_A| + 2e-5 max|T_A| per channel",
+                   "passed": bool(worst <= 1.0 and np.max(np.abs(rm)) > 0), "oracle_seconds": time.perf_counter() - t1}
+        ok = ok and map_par["passed"]
+    del p64
+    return {"map": map_par, "workload": m.name, "directions": [int(d) for d in dirs_idx] if is3d else None, "transitions": [int(t) for t in sel],
+            "cells": int(leaf.sum()), "ray_cell_steps": nsteps_ref, "visits_equal": visits_equal,
             "path_sums_equal": path_equal, "max_rel_sj": worst_sj, "max_esc_err": worst_esc, "tol": 1e-4, "passed": bool(ok),
-            "oracle_seconds": t_or, "note": "per-cell counters of the first simulate from LTE; oracle float64, all channels, no cut-off"}
+            "oracle_seconds": t_or, "oracle_transitions_per_pass": group,
+            "note": "per-cell counters of the first simulate from LTE; oracle float64, all channels, no cut-off"}
 
 
 # ---- own arm ------------------------------------------------------------------------------------------------------------
@@ -370,6 +426,13 @@ def run_own(args):
     m, desc = make_workload(args.workload)
     t_gen = time.perf_counter() - t_gen
     is3d = hasattr(m, "child")
+    # fingerprint of the realisation (the C4/C5 inputs come from a float32 torch FFT whose rounding depends on the
+    # backend): numbers of two runs are on the same model only if this matches
+    import hashlib
+    hh = hashlib.blake2b(digest_size=8)
+    for a in ([m.child] if is3d else [m.r_out]) + [m.density]:
+        hh.update(np.ascontiguousarray(a).view(np.uint8).reshape(-1))
+    input_hash = hh.hexdigest()
     sel = None if getattr(m, "sel", None) is None else m.sel
     nt = len(m.species.upper) if sel is None else len(sel)
     g = LocModel(m, device=f"cuda:{local}", ntrans_sim=nt)
@@ -419,6 +482,9 @@ def run_own(args):
     t_all, t_sim, t_solve = max_over_ranks([t_all, t_sim, t_solve], device=f"cuda:{local}")
     u_act = float(sg["active_updates"])
     value = whole_job_value(u_act, args.steps, world, t_all)
+    # the same throughput with the one-off path set-up (loc_set_directions) spread over the ALI iterations the config names
+    n_cfg = CONFIG_ITERATIONS.get(args.workload, args.steps)
+    value_setup = world * u_act * n_cfg / (1e-3 * sg["setup_ms"] + n_cfg * t_all / args.steps)
 
     # ---- end to end: host buffers -> device -> one ALI iteration -> populations back to the host ----
     names = ["density", "tkin", "sigma", "abundance"] + (["vx", "vy", "vz"] if is3d else ["vx"])
@@ -467,6 +533,8 @@ def run_own(args):
     (t_e2e,) = max_over_ranks([e0.elapsed_time(e1) * 1e-3], device=f"cuda:{local}")
     e2e_val = whole_job_value(u_act, n_e2e, world, t_e2e)
     del host, host_pops, host_out, out_dev  # 24 GB of pinned memory at C5: returned before the oracle runs
+    if hasattr(torch._C, "_host_emptyCache"):
+        torch._C._host_emptyCache()  # (torch caches freed pinned blocks; the oracle legs need the host memory)
 
     # ---- S10: spectral cube of the first traced line along +z, one pixel per finest cell (C5: 1024 x 1024 x
     #      256 channels), and its line-area map; after the iterations above, timed apart from `value` ----
@@ -492,22 +560,40 @@ def run_own(args):
         barrier()
         t_map, t_area = max_over_ranks([me[0].elapsed_time(me[1]) * 1e-3 / nrep, me[1].elapsed_time(me[2]) * 1e-3 / nrep],
                                        device=f"cuda:{local}")
+        # roofline of k_spectra3d (DESIGN 8.2).  Along +z a pixel of the finest grid crosses every leaf of
+        # its column once: steps = sum over leaves of 4^(finest level - level).  Per step and active channel (the 5-sigma rule of
+        # the metric) the kernel needs two ex2 (profile, 1 - e^-tau) on the MUFU pipe: 16 per SM and clock.
+        lvl = np.asarray(m.level, np.int64)
+        leafm = np.asarray(m.child) < 0
+        cover = np.left_shift(1, 2 * (int(m.nlev) - 1 - lvl[leafm]))
+        act = active_channels_per_cell(m, zdir)[leafm]
+        map_steps = int(cover.sum())
+        map_active = float((cover * act).sum())
+        del lvl, leafm, cover, act
         area_bytes = float(nfine) * nfine * (4 * m.nchannel + 4)
         map_info = {"pixels": [nfine, nfine], "channels": int(m.nchannel), "transition": t0, "ms_spectra": 1e3 * t_map,
                     "ms_line_area": 1e3 * t_area, "line_area_gbs": area_bytes / t_area / 1e9,
-                    "cube_bytes": int(cube.numel() * 4), "w_mean_K_kms": float(wmap.mean())}
+                    "cube_bytes": int(cube.numel() * 4), "w_mean_K_kms": float(wmap.mean()),
+                    "los_steps": map_steps, "active_updates": map_active}
         del cube, wmap
 
     parity = None
     if rank == 0 and world == 1 and not args.no_parity:
         import oracle as O
         O.build()
-        parity = parity_leg(g, m, [int(x) for x in args.parity_dirs.split(",")], ntrans=args.parity_trans)
+        pdirs = [int(x) for x in args.parity_dirs.split(",")] if args.parity_dirs else (default_parity_dirs(m.dirs) if is3d else [0])
+        parity = parity_leg(g, m, pdirs, ntrans=min(args.parity_trans, nt), map_patch=args.parity_map)
 
     if rank == 0:
         hbm, sm_max, kind = load_peaks()
         if map_info is not None:
             map_info["line_area_hbm_frac"] = map_info["line_area_gbs"] / hbm
+            mufu_peak = N_SM * MUFU_PER_SM_CLK * sm_max * 1e6  # ex2 per second
+            mufu_ach = 2.0 * map_info["active_updates"] / (1e-3 * map_info["ms_spectra"])
+            map_info["roofline"] = {"kernel": "k_spectra3d", "bound": "alu", "resource": "MUFU ex2: 2 per active channel and step",
+                                    "achieved": mufu_ach / 1e12, "peak": mufu_peak / 1e12, "unit": "Tex2/s", "frac": mufu_ach / mufu_peak,
+                                    "hbm_frac_of_cube_write": map_info["cube_bytes"] / (1e-3 * map_info["ms_spectra"]) / 1e9 / hbm,
+                                    "traffic": None}
         roof = roofline(sg, nt, t_sim / args.steps, hbm, sm_max, kind)
         cpu = None
         if world == 1 and not args.no_cpu:
@@ -523,7 +609,9 @@ def run_own(args):
                           "channels": int(m.nchannel), "transitions_traced": int(nt), "parallelism": "replicas" if world > 1 else "single GPU",
                           "updates": "value = active updates (5-sigma rule) / s; nominal = steps x channels x transitions (what a code without a profile cut-off evaluates)",
                           "l2": "inputs larger than L2 (no flush)" if is3d and g.ncell > 1_000_000 else "working set fits L2 (model is small); no flush: the data is re-read from L2 by design",
-                          "setup_ms_once": sg["setup_ms"], "input_generation_s": t_gen, "options": args.option},
+                          "setup_ms_once": sg["setup_ms"], "input_generation_s": t_gen, "options": args.option,
+                          "input_hash": input_hash, "iterations_of_config": n_cfg},
+               "value_incl_setup": value_setup,
                "nominal_updates_per_s": whole_job_value(u_nom, args.steps, world, t_all),
                "ms_simulate": 1e3 * t_sim / args.steps, "ms_solve": 1e3 * t_solve / args.steps,
                "clocks": clocks, "roofline": roof,
@@ -549,12 +637,15 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="own", choices=["own", "reference"])
-    ap.add_argument("--workload", default=os.environ.get("LOC_BENCH_WORKLOAD", DEFAULT_WORKLOAD))
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD)
     ap.add_argument("--ref-budget", type=float, default=6e9, help="nominal updates per oracle sample (about 10-30 s of CPU)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-parity", action="store_true", help="skip the full-size parity leg (oracle vs library on a direction subset)")
-    ap.add_argument("--parity-dirs", default="0", help="comma-separated direction indices of the parity leg (3D)")
-    ap.add_argument("--parity-trans", type=int, default=1, help="traced transitions compared in the parity leg")
+    ap.add_argument("--parity-dirs", default=None,
+                    help="comma-separated direction indices of the parity leg (3D); default: direction 0 plus the first direction "
+                         "with zero slopes and a negative main component (axis-aligned, mirrored main axis)")
+    ap.add_argument("--parity-trans", type=int, default=3, help="traced transitions compared in the parity leg (at most those traced)")
+    ap.add_argument("--parity-map", type=int, default=64, help="edge of the corner patch of the spectral cube compared with the oracle (0 = none)")
     ap.add_argument("--option", action="append", default=[], metavar="KEY=VALUE", help="loc_set_option before the run (A/B measurements)")
     ap.add_argument("--no-map", action="store_true", help="skip the spectral-cube / line-area leg of the 3D workloads")
     args = ap.parse_args()
